@@ -1,0 +1,129 @@
+/*
+ * foldcp_trimul.h -- C ABI of the B200-native (sm_100a) triangle multiplicative update.
+ *
+ * The operation (forward pass, one pair tensor, batch 1):
+ *   PAPER.md section 3.3, Eq. 2-3:
+ *       outgoing  o_nm = sum_k a_nk (.) b_mk        incoming  o_nm = sum_k a_kn (.) b_km
+ *   "a, b are projections of the pair representation z in R^{BxNxNxD} ... structurally a batched
+ *   matrix multiplication with element-wise gating"; line 132: the variants "differ only in which
+ *   operand is transposed".  The LayerNorms, gates and output projection around the contraction
+ *   are those of BASELINE.json's north_star (AF3 supplementary Alg. 12/13):
+ *
+ *       z'  = LayerNorm(z; ln_in_gamma, ln_in_beta, ln_eps)        over c_z, biased variance
+ *       a   = M (.) sigmoid(W_ga z' + b_ga) (.) (W_a z' + b_a)     [N,N,c_hidden]
+ *       b   = M (.) sigmoid(W_gb z' + b_gb) (.) (W_b z' + b_b)
+ *       o   = Eq. 2 (direction = FOLDCP_OUTGOING) or Eq. 3 (FOLDCP_INCOMING), per channel
+ *       out = [M (.)] sigmoid(W_g z' + b_g) (.) (W_o LayerNorm(o; ln_out_*) + b_o)   [N,N,c_z]
+ *
+ *   `out` is the UPDATE only: the paper's "z_nm +=" residual add belongs to the caller
+ *   (reading A1).
+ *
+ * Memory: every tensor pointer below is a DEVICE pointer owned by the caller and must stay valid
+ * until the work enqueued on `stream` has finished.  The params struct itself is HOST memory and
+ * is only read during the call.  The library never allocates, frees or synchronises inside
+ * foldcp_trimul(): it enqueues kernels on `stream` and returns.  Same inputs give bitwise
+ * identical outputs (no atomics, no split-K).  No exceptions cross this boundary; every failure
+ * is a status code and, when detected on the host, leaves `out` untouched.
+ */
+#ifndef FOLDCP_TRIMUL_H_
+#define FOLDCP_TRIMUL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  FOLDCP_OK = 0,
+  FOLDCP_ERR_INVALID_ARG = 1, /* NULL pointer, N <= 0, bad direction / dtype, struct_size mismatch */
+  FOLDCP_ERR_UNSUPPORTED = 2, /* c_z or c_hidden != 128; bf16 mode with N not a multiple of 8      */
+  FOLDCP_ERR_ALIGNMENT = 3,   /* a tensor pointer is not 16-byte aligned                           */
+  FOLDCP_ERR_WORKSPACE = 4,   /* workspace NULL or smaller than foldcp_trimul_workspace_bytes()    */
+  FOLDCP_ERR_ALIAS = 5,       /* out overlaps z or the workspace                                   */
+  FOLDCP_ERR_ARCH = 6,        /* current device is not compute capability 10.x (sm_100)           */
+  FOLDCP_ERR_CUDA = 7         /* launch / tensor-map failure (cudaGetLastError is preserved)       */
+} foldcp_status_t;
+
+typedef enum { FOLDCP_OUTGOING = 0, FOLDCP_INCOMING = 1 } foldcp_direction_t;
+
+/* dtype of z, mask, out and of the six weight matrices.  FOLDCP_F32 is the exact mode
+ * (plain fp32 FFMA arithmetic, tolerance 1e-5 relative); FOLDCP_BF16 is the tensor-core mode
+ * (bf16 operands, fp32 accumulation in tensor memory). */
+typedef enum { FOLDCP_F32 = 0, FOLDCP_BF16 = 1 } foldcp_dtype_t;
+
+typedef struct {
+  uint32_t struct_size; /* = sizeof(foldcp_trimul_params); ABI versioning                          */
+  int32_t dtype;        /* foldcp_dtype_t                                                          */
+  float ln_eps;         /* LayerNorm epsilon (inside the sqrt); 1e-5 in every BASELINE config      */
+  int32_t mask_output;  /* 1: out_ij *= M_ij (north_star's epilogue); 0: mask only a and b (AF3)   */
+  const float* ln_in_gamma;  /* [c_z]      fp32 in both modes                                      */
+  const float* ln_in_beta;   /* [c_z]                                                              */
+  const void* w_a;           /* [c_hidden][c_z] row-major (= torch Linear.weight), dtype above     */
+  const void* w_a_gate;      /* [c_hidden][c_z]                                                    */
+  const void* w_b;           /* [c_hidden][c_z]                                                    */
+  const void* w_b_gate;      /* [c_hidden][c_z]                                                    */
+  const float* b_a;          /* [c_hidden] fp32; each bias may be NULL (= no bias, AF3 LinearNoBias) */
+  const float* b_a_gate;
+  const float* b_b;
+  const float* b_b_gate;
+  const void* w_g;           /* [c_z][c_z]   output gate                                           */
+  const float* b_g;          /* [c_z] or NULL                                                      */
+  const float* ln_out_gamma; /* [c_hidden] fp32                                                    */
+  const float* ln_out_beta;  /* [c_hidden]                                                         */
+  const void* w_o;           /* [c_z][c_hidden]   output projection                                */
+  const float* b_o;          /* [c_z] or NULL                                                      */
+  void* workspace;           /* caller-owned device scratch, 256-byte aligned                      */
+  size_t workspace_bytes;    /* >= foldcp_trimul_workspace_bytes(N, c_z, c_hidden, dtype)          */
+} foldcp_trimul_params;
+
+/*
+ * One forward triangle multiplicative update, enqueued on `stream`.
+ *
+ *   z      [N][N][c_z]  device, dtype = params->dtype, channel fastest
+ *   mask   [N][N]       device, same dtype, PAIR mask multiplied as-is (not thresholded);
+ *                       NULL = all ones
+ *   params host struct (see above)
+ *   N, c_z, c_hidden    N >= 1; c_z = c_hidden = 128 (anything else: FOLDCP_ERR_UNSUPPORTED);
+ *                       bf16 mode needs N % 8 == 0 (16-byte TMA row stride) -- pad and mask
+ *   direction           foldcp_direction_t
+ *   out    [N][N][c_z]  device, dtype = params->dtype; must not overlap z or the workspace
+ *   stream              cudaStream_t (as void*); NULL = the legacy default stream
+ *
+ * Returns a foldcp_status_t.  Asynchronous: returns after enqueueing.
+ */
+int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
+                  int c_z, int c_hidden, int direction, void* out, void* stream);
+
+/* Bytes of device scratch foldcp_trimul needs for this problem (a, b and o, channel-major);
+ * 0 if the shape / dtype is unsupported.  Monotone in N. */
+size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
+
+/* Stage-level entry points (same conventions; used by the tests, the benchmark's per-kernel
+ * roofline and by callers that keep a / b / o).  All tensors are device pointers.
+ *
+ *   foldcp_trimul_project : step a1+a2 -- LayerNorm + gated projections + mask
+ *        a, b  [c_hidden][N][N]  channel-major ("[channel][row][col]" of the pair index), dtype
+ *   foldcp_trimul_contract: step a4 -- Eq. 2 / Eq. 3 per channel
+ *        o     [c_hidden][N][N]  channel-major, dtype
+ *   foldcp_trimul_finalize: step a3+a5 -- LayerNorm(o) + output projection + sigmoid gate + mask
+ */
+int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_params* params,
+                          int N, int c_z, int c_hidden, void* a, void* b, void* stream);
+int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
+                           int direction, void* o, void* stream);
+int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
+                           const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
+                           void* out, void* stream);
+
+/* Number of kernels one foldcp_trimul call launches for this dtype (for launch accounting). */
+int foldcp_trimul_launches_per_call(int dtype);
+
+const char* foldcp_status_string(int status);
+int foldcp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FOLDCP_TRIMUL_H_ */

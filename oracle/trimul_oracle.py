@@ -1,0 +1,154 @@
+"""fp64 CPU oracle of the triangle multiplicative update (outgoing / incoming).
+
+TEST INFRASTRUCTURE -- NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / `--impl reference` legs may import this package.  It shares no
+code with the CUDA path (paper_2603_14806_b200/csrc) and never imports it.
+
+What it computes (plain definition, written out; numpy fp64 throughout):
+
+  PAPER.md lines 117-130, section 3.3, Eq. 2-3 (Eq. 2 is printed twice -- extraction
+  duplicate):
+      outgoing:  o_nm = sum_k a_nk (.) b_mk          incoming:  o_nm = sum_k a_kn (.) b_km
+  "where a, b are projections of the pair representation z in R^{B x N x N x D}.  This
+  operation is structurally a batched matrix multiplication with element-wise gating";
+  PAPER.md line 132: "The outgoing and incoming variants differ only in which operand is
+  transposed".  The paper's equations leave out the LayerNorms, the gates and the output
+  projection; BASELINE.json's north_star (= AF3 supplementary Alg. 12/13) fixes them:
+
+      z'   = LayerNorm(z)                                  (over c_z, biased variance)
+      a    = M * sigmoid(W_ga z' + b_ga) * (W_a z' + b_a)   (pair mask M applied)
+      b    = M * sigmoid(W_gb z' + b_gb) * (W_b z' + b_b)
+      g    = sigmoid(W_g z' + b_g)
+      o    = contraction above (per channel, no residual add: DESIGN.md reading A1)
+      out  = [M *] g * (W_o LayerNorm(o) + b_o)             (LayerNorm over c_hidden)
+
+Readings of the paper taken here are listed in DESIGN.md ("Readings"): A1 update only (no
+`+=` residual), A6 eps inside the sqrt / biased variance, A7 pair mask multiplied after
+gating, A8 `mask_output` flag.
+
+A library primitive (numpy matmul) serves as the dense-contraction step; there is no
+blocking, fusion or reordering beyond the definition.  Pins: tests/test_oracle_pins.py
+(brute-force index loops from oracle/brute_force.py on tiny shapes, closed forms S1-S4,
+invariants I1/I1'/I2/I3/I6/S8, N=1) -- every function below is pinned there.
+"""
+from __future__ import annotations
+
+from typing import Dict, Optional
+
+import numpy as np
+
+OUTGOING = 0
+INCOMING = 1
+
+_F = np.float64
+
+
+def sigmoid(x: np.ndarray) -> np.ndarray:
+    """1 / (1 + exp(-x)), evaluated without overflow for either sign of x."""
+    x = np.asarray(x, dtype=_F)
+    e = np.exp(-np.abs(x))
+    return np.where(x >= 0, 1.0 / (1.0 + e), e / (1.0 + e))
+
+
+def layer_norm(x: np.ndarray, gamma: np.ndarray, beta: np.ndarray, eps: float) -> np.ndarray:
+    """LayerNorm over the last axis: (x - mean) / sqrt(var + eps) * gamma + beta, var = biased
+    (divide by the channel count).  north_star "LayerNorm"; reading A6."""
+    x = np.asarray(x, dtype=_F)
+    mu = x.mean(axis=-1, keepdims=True)
+    var = ((x - mu) ** 2).mean(axis=-1, keepdims=True)
+    return (x - mu) / np.sqrt(var + eps) * np.asarray(gamma, _F) + np.asarray(beta, _F)
+
+
+def _linear(x: np.ndarray, w: np.ndarray, b: Optional[np.ndarray]) -> np.ndarray:
+    """torch.nn.Linear convention: y = x W^T + b, W is [out_features, in_features]."""
+    y = x @ np.asarray(w, _F).T
+    if b is not None:
+        y = y + np.asarray(b, _F)
+    return y
+
+
+def gated_projection(zp: np.ndarray, mask: Optional[np.ndarray], w: np.ndarray,
+                     b: Optional[np.ndarray], w_gate: np.ndarray,
+                     b_gate: Optional[np.ndarray]) -> np.ndarray:
+    """a = M * sigmoid(W_g z' + b_g) * (W z' + b)   (north_star; PAPER.md line 130
+    "projections of the pair representation ... with element-wise gating")."""
+    out = sigmoid(_linear(zp, w_gate, b_gate)) * _linear(zp, w, b)
+    if mask is not None:
+        out = np.asarray(mask, _F)[..., None] * out
+    return out
+
+
+def contraction(a: np.ndarray, b: np.ndarray, direction: int) -> np.ndarray:
+    """PAPER.md Eq. 2-3 (lines 121-128).  a, b are [N, N, c]; returns o [N, N, c].
+
+    outgoing: o[i, j, c] = sum_k a[i, k, c] * b[j, k, c]   -> per channel  A_c  B_c^T
+    incoming: o[i, j, c] = sum_k a[k, i, c] * b[k, j, c]   -> per channel  A_c^T B_c
+    """
+    A = np.transpose(a, (2, 0, 1))      # [c, row, col]
+    B = np.transpose(b, (2, 0, 1))
+    if direction == OUTGOING:
+        O = A @ np.transpose(B, (0, 2, 1))
+    elif direction == INCOMING:
+        O = np.transpose(A, (0, 2, 1)) @ B
+    else:
+        raise ValueError("direction must be 0 (outgoing) or 1 (incoming)")
+    return np.transpose(O, (1, 2, 0))
+
+
+def output_stage(o: np.ndarray, zp: np.ndarray, mask: Optional[np.ndarray],
+                 p: Dict[str, np.ndarray], eps: float, mask_output: bool) -> np.ndarray:
+    """out = [M *] sigmoid(W_g z' + b_g) * (W_o LayerNorm(o) + b_o)   (north_star)."""
+    g = sigmoid(_linear(zp, p["w_g"], p.get("b_g")))
+    y = _linear(layer_norm(o, p["ln_out_gamma"], p["ln_out_beta"], eps), p["w_o"], p.get("b_o"))
+    out = g * y
+    if mask_output and mask is not None:
+        out = np.asarray(mask, _F)[..., None] * out
+    return out
+
+
+def trimul(z: np.ndarray, mask: Optional[np.ndarray], p: Dict[str, np.ndarray], direction: int,
+           eps: float = 1e-5, mask_output: bool = True) -> np.ndarray:
+    """Full op on z[N, N, c_z], pair mask M[N, N] (None = all ones) -> out[N, N, c_z] (fp64).
+
+    `p` maps the names of paper_2603_14806_b200.synth.make_params to arrays; any bias may be
+    absent / None (AF3's LinearNoBias).
+    """
+    z = np.asarray(z, _F)
+    zp = layer_norm(z, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    a = gated_projection(zp, mask, p["w_a"], p.get("b_a"), p["w_a_gate"], p.get("b_a_gate"))
+    b = gated_projection(zp, mask, p["w_b"], p.get("b_b"), p["w_b_gate"], p.get("b_b_gate"))
+    o = contraction(a, b, direction)
+    return output_stage(o, zp, mask, p, eps, mask_output)
+
+
+def trimul_subgrid(z_a: np.ndarray, mask_a: Optional[np.ndarray],
+                   z_b: np.ndarray, mask_b: Optional[np.ndarray],
+                   z_ij: np.ndarray, mask_ij: Optional[np.ndarray],
+                   p: Dict[str, np.ndarray], eps: float = 1e-5,
+                   mask_output: bool = True) -> np.ndarray:
+    """Exact out[I x J] (full sums over k) from only the slices of z the definition touches.
+
+    For index sets I, J the caller passes, in (row, k) order:
+        outgoing:  z_a = z[I, :, :]            z_b = z[J, :, :]            (a_ik, b_jk)
+        incoming:  z_a = z[:, I, :] swapped    z_b = z[:, J, :] swapped    (a_ki, b_kj)
+    to [|I|, N, c_z] / [|J|, N, c_z] (and the matching pair-mask slices), plus
+    z_ij = z[I][:, J] ([|I|, |J|, c_z]) for the output gate.  With the slices in that order
+    both directions are the same formula  o_ij = sum_k a'_ik * b'_jk  -- PAPER.md line 132:
+    the variants "differ only in which operand is transposed".
+    """
+    zpa = layer_norm(z_a, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    zpb = layer_norm(z_b, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    a = gated_projection(zpa, mask_a, p["w_a"], p.get("b_a"), p["w_a_gate"], p.get("b_a_gate"))
+    b = gated_projection(zpb, mask_b, p["w_b"], p.get("b_b"), p["w_b_gate"], p.get("b_b_gate"))
+    A = np.transpose(a, (2, 0, 1))                    # [c, |I|, N]
+    B = np.transpose(b, (2, 0, 1))                    # [c, |J|, N]
+    o = np.transpose(A @ np.transpose(B, (0, 2, 1)), (1, 2, 0))   # [|I|, |J|, c]
+    zp_ij = layer_norm(z_ij, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    return output_stage(o, zp_ij, mask_ij, p, eps, mask_output)
+
+
+def flops(N: int, c_z: int, c_hidden: int) -> float:
+    """Counted FLOPs of one call: contraction 2 c N^3 + five
+    projections 2 N^2 c_z (4c + c_z) + output projection 2 N^2 c c_z."""
+    return 2.0 * c_hidden * N ** 3 + 2.0 * N * N * c_z * (4 * c_hidden + c_z) \
+        + 2.0 * N * N * c_hidden * c_z

@@ -1,0 +1,400 @@
+"""Pins of the fp64 oracle against things other than itself (run with -m "not gpu").
+
+Each test is chosen so that a plausible mistake in oracle/trimul_oracle.py (dropped term,
+wrong sign or index, transposed operand, mask in the wrong place, unbiased variance, ...)
+fails at least one of them.  Names follow SURVEY.md section 8(c).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import brute_force
+from oracle import trimul_oracle as orc
+
+OUT, INC = orc.OUTGOING, orc.INCOMING
+
+
+def rand_params(rng, c_z, c, bias=True):
+    p = {
+        "ln_in_gamma": 1 + 0.1 * rng.standard_normal(c_z), "ln_in_beta": 0.1 * rng.standard_normal(c_z),
+        "w_a": rng.standard_normal((c, c_z)) / math.sqrt(c_z),
+        "w_a_gate": rng.standard_normal((c, c_z)) / math.sqrt(c_z),
+        "w_b": rng.standard_normal((c, c_z)) / math.sqrt(c_z),
+        "w_b_gate": rng.standard_normal((c, c_z)) / math.sqrt(c_z),
+        "w_g": rng.standard_normal((c_z, c_z)) / math.sqrt(c_z),
+        "ln_out_gamma": 1 + 0.1 * rng.standard_normal(c), "ln_out_beta": 0.1 * rng.standard_normal(c),
+        "w_o": rng.standard_normal((c_z, c)) / math.sqrt(c),
+    }
+    if bias:
+        for k, n in (("b_a", c), ("b_a_gate", c), ("b_b", c), ("b_b_gate", c), ("b_g", c_z), ("b_o", c_z)):
+            p[k] = 0.3 * rng.standard_normal(n)
+    return p
+
+
+def swap_ab(p):
+    q = dict(p)
+    for x, y in (("w_a", "w_b"), ("w_a_gate", "w_b_gate"), ("b_a", "b_b"), ("b_a_gate", "b_b_gate")):
+        if x in p:
+            q[x], q[y] = p[y], p[x]
+    return q
+
+
+def tolist(p):
+    return {k: np.asarray(v).tolist() for k, v in p.items()}
+
+
+def relerr(x, y):
+    return np.linalg.norm(x - y) / max(np.linalg.norm(y), 1e-300)
+
+
+# ----------------------------------------------------------------------------------------
+# brute force (pure-Python scalar loops) on tiny shapes, both directions, general pair mask
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,c_z,c", [(1, 4, 3), (2, 4, 3), (3, 8, 8), (5, 4, 8), (8, 8, 3)])
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("mask_output", [True, False])
+def test_brute_force(N, c_z, c, direction, mask_output):
+    rng = np.random.default_rng(100 * N + 10 * c_z + c + direction)
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)       # general, non-symmetric pair mask
+    p = rand_params(rng, c_z, c)
+    got = orc.trimul(z, M, p, direction, mask_output=mask_output)
+    ref = np.array(brute_force.trimul_brute(z.tolist(), M.tolist(), tolist(p), direction,
+                                            mask_output=mask_output))
+    assert got.shape == (N, N, c_z)
+    assert relerr(got, ref) < 1e-12
+
+
+def test_brute_force_no_bias_no_mask_soft_mask():
+    rng = np.random.default_rng(7)
+    N, c_z, c = 4, 8, 4
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c, bias=False)
+    for direction in (OUT, INC):
+        got = orc.trimul(z, None, p, direction)
+        ref = np.array(brute_force.trimul_brute(z.tolist(), None, tolist(p), direction))
+        assert relerr(got, ref) < 1e-12
+        Ms = rng.random((N, N))                              # soft (non 0/1) mask: multiplied as-is (A22)
+        got = orc.trimul(z, Ms, p, direction)
+        ref = np.array(brute_force.trimul_brute(z.tolist(), Ms.tolist(), tolist(p), direction))
+        assert relerr(got, ref) < 1e-12
+
+
+def test_none_bias_equals_zero_bias_bitwise():
+    rng = np.random.default_rng(8)
+    N, c_z, c = 5, 8, 8
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c, bias=False)
+    pz = dict(p)
+    for k, n in (("b_a", c), ("b_a_gate", c), ("b_b", c), ("b_b_gate", c), ("b_g", c_z), ("b_o", c_z)):
+        pz[k] = np.zeros(n)
+    for d in (OUT, INC):
+        assert np.array_equal(orc.trimul(z, None, p, d), orc.trimul(z, None, pz, d))
+
+
+# ----------------------------------------------------------------------------------------
+# contraction alone: Eq. 2-3 against scalar loops, I1' (swapped layouts), library matmul (S5)
+# ----------------------------------------------------------------------------------------
+def test_contraction_definition_loops():
+    rng = np.random.default_rng(1)
+    N, c = 6, 5
+    a = rng.standard_normal((N, N, c))
+    b = rng.standard_normal((N, N, c))
+    o_out = np.zeros((N, N, c))
+    o_in = np.zeros((N, N, c))
+    for i in range(N):
+        for j in range(N):
+            for k in range(N):
+                o_out[i, j] += a[i, k] * b[j, k]
+                o_in[i, j] += a[k, i] * b[k, j]
+    assert np.allclose(orc.contraction(a, b, OUT), o_out, rtol=0, atol=1e-13)
+    assert np.allclose(orc.contraction(a, b, INC), o_in, rtol=0, atol=1e-13)
+    # a wrong reading (transposing only one operand) must NOT pass
+    assert not np.allclose(orc.contraction(a, b, OUT), o_in, atol=1e-3)
+
+
+def test_I1prime_contraction_swapped_layouts():
+    rng = np.random.default_rng(2)
+    N, c = 7, 4
+    a = rng.standard_normal((N, N, c))
+    b = rng.standard_normal((N, N, c))
+    aT, bT = np.transpose(a, (1, 0, 2)), np.transpose(b, (1, 0, 2))
+    assert np.allclose(orc.contraction(a, b, INC), orc.contraction(aT, bT, OUT), rtol=0, atol=1e-13)
+
+
+def test_S5_reduces_to_dense_matmul():
+    """Gates saturated (sigmoid(+40) == 1 in fp64): a, b are affine maps of z' and each channel of
+    o is a textbook dense matrix product; checked through gamma_out-scaled pre-LN quantities."""
+    rng = np.random.default_rng(3)
+    N, c_z, c = 9, 8, 6
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c)
+    for k in ("w_a_gate", "w_b_gate"):
+        p[k] = np.zeros_like(p[k])
+    p["b_a_gate"] = np.full(c, 40.0)
+    p["b_b_gate"] = np.full(c, 40.0)
+    zp = orc.layer_norm(z, p["ln_in_gamma"], p["ln_in_beta"], 1e-5)
+    a = orc.gated_projection(zp, None, p["w_a"], p["b_a"], p["w_a_gate"], p["b_a_gate"])
+    b = orc.gated_projection(zp, None, p["w_b"], p["b_b"], p["w_b_gate"], p["b_b_gate"])
+    assert np.allclose(a, zp @ p["w_a"].T + p["b_a"], rtol=1e-15, atol=1e-15)
+    for ch in range(c):
+        A, B = a[:, :, ch], b[:, :, ch]
+        assert np.allclose(orc.contraction(a, b, OUT)[:, :, ch], np.einsum("ik,jk->ij", A, B), atol=1e-12)
+        assert np.allclose(orc.contraction(a, b, INC)[:, :, ch], np.einsum("ki,kj->ij", A, B), atol=1e-12)
+
+
+# ----------------------------------------------------------------------------------------
+# invariants
+# ----------------------------------------------------------------------------------------
+def test_I1_direction_identity_needs_ab_swap():
+    """incoming(z, M; theta) = T(outgoing(Tz, TM; theta with a<->b swapped)); the naive form of
+    north_star (no swap) is false for distinct a/b parameters (reading A10)."""
+    rng = np.random.default_rng(4)
+    N, c_z, c = 6, 8, 5
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)
+    p = rand_params(rng, c_z, c)
+    zT, MT = np.transpose(z, (1, 0, 2)), M.T
+    inc = orc.trimul(z, M, p, INC)
+    good = np.transpose(orc.trimul(zT, MT, swap_ab(p), OUT), (1, 0, 2))
+    naive = np.transpose(orc.trimul(zT, MT, p, OUT), (1, 0, 2))
+    assert relerr(good, inc) < 1e-12
+    assert relerr(naive, inc) > 1e-2
+    # with identical a and b parameter sets the naive form holds too
+    q = dict(p)
+    q["w_b"], q["w_b_gate"], q["b_b"], q["b_b_gate"] = p["w_a"], p["w_a_gate"], p["b_a"], p["b_a_gate"]
+    assert relerr(np.transpose(orc.trimul(zT, MT, q, OUT), (1, 0, 2)), orc.trimul(z, M, q, INC)) < 1e-12
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_I2_token_permutation_equivariance(direction):
+    rng = np.random.default_rng(5)
+    N, c_z, c = 7, 8, 4
+    z = rng.standard_normal((N, N, c_z))
+    m = (rng.random(N) > 0.25).astype(np.float64)
+    M = np.outer(m, m)
+    p = rand_params(rng, c_z, c)
+    pi = rng.permutation(N)
+    lhs = orc.trimul(z[pi][:, pi], M[pi][:, pi], p, direction)
+    rhs = orc.trimul(z, M, p, direction)[pi][:, pi]
+    assert relerr(lhs, rhs) < 1e-12
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_I3_masked_tokens_contribute_nothing(direction):
+    """Zero contribution from masked tokens: garbage (large, finite) under the mask leaves out
+    bitwise unchanged everywhere (mask_output) / on valid pairs (no output mask)."""
+    rng = np.random.default_rng(6)
+    N, c_z, c = 8, 8, 6
+    z = rng.standard_normal((N, N, c_z))
+    m = np.ones(N)
+    m[[2, 5]] = 0.0
+    M = np.outer(m, m)
+    p = rand_params(rng, c_z, c)
+    z2 = z.copy()
+    z2[M == 0] = 100.0 * rng.standard_normal((int((M == 0).sum()), c_z))
+    assert np.array_equal(orc.trimul(z, M, p, direction), orc.trimul(z2, M, p, direction))
+    o1 = orc.trimul(z, M, p, direction, mask_output=False)
+    o2 = orc.trimul(z2, M, p, direction, mask_output=False)
+    assert np.array_equal(o1[M == 1], o2[M == 1])
+    # and the masked output is exactly zero on masked pairs, non-zero without the output mask (A8/A20)
+    assert np.all(orc.trimul(z, M, p, direction)[M == 0] == 0.0)
+    assert np.all(np.abs(o1[M == 0]).max(axis=-1) > 0)
+    # removing masked tokens altogether gives the same values on the kept block
+    keep = np.where(m == 1)[0]
+    small = orc.trimul(z[keep][:, keep], None, p, direction)
+    assert relerr(small, orc.trimul(z, M, p, direction)[keep][:, keep]) < 1e-12
+
+
+def test_I6_input_layernorm_shift_and_scale():
+    rng = np.random.default_rng(9)
+    N, c_z, c = 5, 8, 4
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c)
+    ref = orc.trimul(z, None, p, OUT)
+    shift = rng.standard_normal((N, N, 1))
+    assert relerr(orc.trimul(z + shift, None, p, OUT), ref) < 1e-12
+    # scaling by s changes out only through eps: with eps=0 exactly invariant, with 1e-5 nearly
+    assert relerr(orc.trimul(3.0 * z, None, p, OUT, eps=0.0), orc.trimul(z, None, p, OUT, eps=0.0)) < 1e-12
+    assert relerr(orc.trimul(3.0 * z, None, p, OUT), ref) < 1e-4
+
+
+def test_layer_norm_biased_variance_and_eps_inside_sqrt():
+    x = np.array([[1.0, 2.0, 3.0, 6.0]])
+    g = np.array([1.0, 2.0, 1.0, 1.0])
+    b = np.array([0.0, 0.5, 0.0, 0.0])
+    mu, var = 3.0, (4 + 1 + 0 + 9) / 4.0          # biased: 3.5 (unbiased would be 14/3)
+    want = (x - mu) / math.sqrt(var + 0.25) * g + b
+    assert np.allclose(orc.layer_norm(x, g, b, 0.25), want, rtol=1e-15)
+    # degenerate constant row -> beta (A20), finite thanks to eps
+    assert np.allclose(orc.layer_norm(np.full((1, 4), 7.0), g, b, 1e-5), b)
+
+
+def test_sigmoid_values_and_stability():
+    assert orc.sigmoid(np.array(0.0)) == 0.5
+    assert np.isclose(orc.sigmoid(np.array(math.log(3.0))), 0.75, rtol=1e-15)
+    assert np.isclose(orc.sigmoid(np.array(-math.log(3.0))), 0.25, rtol=1e-15)
+    with np.errstate(over="raise"):
+        v = orc.sigmoid(np.array([-800.0, 800.0]))
+    assert v[0] >= 0 and v[0] < 1e-300 and v[1] == 1.0
+
+
+# ----------------------------------------------------------------------------------------
+# closed forms
+# ----------------------------------------------------------------------------------------
+def _one_pair(zv, p, eps=1e-5):
+    """Hand computation for a single feature vector (used by S1)."""
+    mu = zv.mean()
+    var = ((zv - mu) ** 2).mean()
+    zp = (zv - mu) / math.sqrt(var + eps) * p["ln_in_gamma"] + p["ln_in_beta"]
+    sg = lambda x: 1 / (1 + np.exp(-x))
+    alpha = sg(p["w_a_gate"] @ zp + p["b_a_gate"]) * (p["w_a"] @ zp + p["b_a"])
+    beta = sg(p["w_b_gate"] @ zp + p["b_b_gate"]) * (p["w_b"] @ zp + p["b_b"])
+    g = sg(p["w_g"] @ zp + p["b_g"])
+    return alpha, beta, g
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_S1_constant_z(direction):
+    rng = np.random.default_rng(10)
+    N, c_z, c = 6, 8, 5
+    zv = rng.standard_normal(c_z)
+    z = np.broadcast_to(zv, (N, N, c_z)).copy()
+    p = rand_params(rng, c_z, c)
+    alpha, beta, g = _one_pair(zv, p)
+    o = N * alpha * beta
+    mu, var = o.mean(), ((o - o.mean()) ** 2).mean()
+    on = (o - mu) / math.sqrt(var + 1e-5) * p["ln_out_gamma"] + p["ln_out_beta"]
+    want = g * (p["w_o"] @ on + p["b_o"])
+    got = orc.trimul(z, None, p, direction)
+    assert np.allclose(got, np.broadcast_to(want, got.shape), rtol=1e-12, atol=1e-13)
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_S2_zero_weights_token_mask(direction):
+    """All six W = 0, biases != 0, token mask m: o_ij = m_i m_j (sum_k m_k) alpha*beta."""
+    rng = np.random.default_rng(11)
+    N, c_z, c = 7, 8, 4
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c)
+    for k in ("w_a", "w_a_gate", "w_b", "w_b_gate", "w_g"):
+        p[k] = np.zeros_like(p[k])
+    m = np.array([1, 1, 0, 1, 0, 1, 1.0])
+    M = np.outer(m, m)
+    sg = lambda x: 1 / (1 + np.exp(-x))
+    alpha = sg(p["b_a_gate"]) * p["b_a"]
+    beta = sg(p["b_b_gate"]) * p["b_b"]
+    g = sg(p["b_g"])
+    want = np.zeros((N, N, c_z))
+    for i in range(N):
+        for j in range(N):
+            o = m[i] * m[j] * m.sum() * alpha * beta
+            mu, var = o.mean(), ((o - o.mean()) ** 2).mean()
+            on = (o - mu) / math.sqrt(var + 1e-5) * p["ln_out_gamma"] + p["ln_out_beta"]
+            want[i, j] = M[i, j] * g * (p["w_o"] @ on + p["b_o"])
+    assert np.allclose(orc.trimul(z, M, p, direction), want, rtol=1e-12, atol=1e-14)
+
+
+def test_S3_S4_output_stage_isolated():
+    rng = np.random.default_rng(12)
+    N, c_z, c = 5, 8, 6
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)
+    p = rand_params(rng, c_z, c)
+    # S3: gamma_out = 0 -> out_ij = M_ij g_ij * (W_o beta_out + b_o), independent of the contraction
+    q = dict(p)
+    q["ln_out_gamma"] = np.zeros(c)
+    zp = orc.layer_norm(z, p["ln_in_gamma"], p["ln_in_beta"], 1e-5)
+    g = 1 / (1 + np.exp(-(zp @ p["w_g"].T + p["b_g"])))
+    want = M[..., None] * g * (p["w_o"] @ p["ln_out_beta"] + p["b_o"])
+    for d in (OUT, INC):
+        assert np.allclose(orc.trimul(z, M, q, d), want, rtol=1e-12, atol=1e-14)
+    # S4: W_o = 0, b_o = 0 -> out == 0 exactly
+    q = dict(p)
+    q["w_o"] = np.zeros_like(p["w_o"])
+    q["b_o"] = np.zeros(c_z)
+    assert np.all(orc.trimul(z, M, q, OUT) == 0.0)
+
+
+def test_S8_symmetric_input_directions_coincide():
+    rng = np.random.default_rng(13)
+    N, c_z, c = 6, 8, 5
+    z = rng.standard_normal((N, N, c_z))
+    z = z + np.transpose(z, (1, 0, 2))
+    m = (rng.random(N) > 0.2).astype(np.float64)
+    M = np.outer(m, m)
+    p = rand_params(rng, c_z, c)
+    assert relerr(orc.trimul(z, M, p, OUT), orc.trimul(z, M, p, INC)) < 1e-13
+
+
+def test_N1_single_token():
+    rng = np.random.default_rng(14)
+    c_z, c = 8, 4
+    zv = rng.standard_normal(c_z)
+    p = rand_params(rng, c_z, c)
+    alpha, beta, g = _one_pair(zv, p)
+    o = alpha * beta
+    mu, var = o.mean(), ((o - o.mean()) ** 2).mean()
+    on = (o - mu) / math.sqrt(var + 1e-5) * p["ln_out_gamma"] + p["ln_out_beta"]
+    want = g * (p["w_o"] @ on + p["b_o"])
+    for d in (OUT, INC):
+        assert np.allclose(orc.trimul(zv[None, None], None, p, d)[0, 0], want, rtol=1e-12)
+
+
+def test_output_ln_scale_invariance_loose():
+    rng = np.random.default_rng(15)
+    N, c_z, c = 6, 8, 5
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c)
+    ref = orc.trimul(z, None, p, OUT)
+    for s in (0.5, 2.0):
+        q = dict(p)
+        q["w_a"], q["b_a"] = s * p["w_a"], s * p["b_a"]
+        assert relerr(orc.trimul(z, None, q, OUT), ref) < 1e-4
+
+
+# ----------------------------------------------------------------------------------------
+# sub-grid oracle == full oracle on the sampled pairs
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("mask_output", [True, False])
+def test_subgrid_matches_full(direction, mask_output):
+    rng = np.random.default_rng(16)
+    N, c_z, c = 11, 8, 6
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)
+    p = rand_params(rng, c_z, c)
+    I = np.array([0, 3, 10, 4])
+    J = np.array([10, 1, 2])
+    if direction == OUT:
+        za, ma, zb, mb = z[I], M[I], z[J], M[J]
+    else:
+        za, ma = np.transpose(z[:, I], (1, 0, 2)), M[:, I].T
+        zb, mb = np.transpose(z[:, J], (1, 0, 2)), M[:, J].T
+    got = orc.trimul_subgrid(za, ma, zb, mb, z[I][:, J], M[I][:, J], p, mask_output=mask_output)
+    full = orc.trimul(z, M, p, direction, mask_output=mask_output)
+    assert relerr(got, full[I][:, J]) < 1e-12
+
+
+def test_flop_count_matches_baseline_md():
+    # 17.592 + 2.749 + 0.550 = 20.891 TFLOP at N=4096, c=c_z=128
+    assert abs(orc.flops(4096, 128, 128) / 1e12 - 20.891) < 1e-3
+    assert abs(orc.flops(64, 128, 128) / 1e9 - 0.872) < 1e-3
+
+
+def test_golden_worked_example():
+    """Stored tiny worked example (written by tests/golden/make_trimul_golden.py from the scalar
+    brute force; the paper prints no numerical example of its own)."""
+    import json
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "trimul_n3.json")
+    with open(path) as f:
+        doc = json.load(f)
+    p = {k: np.array(v) for k, v in doc["params"].items()}
+    z, M = np.array(doc["z"]), np.array(doc["mask"])
+    for d in (OUT, INC):
+        for mo in (True, False):
+            want = np.array(doc["out"][f"dir{d}_maskout{int(mo)}"])
+            got = orc.trimul(z, M, p, d, eps=doc["eps"], mask_output=mo)
+            assert np.allclose(got, want, rtol=1e-12, atol=1e-14)
