@@ -1,0 +1,214 @@
+"""ctypes binding of libfoldcp_trimul.so -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI (include/foldcp_trimul.h);
+PyTorch is used for device memory and streams.  There is NO CPU fallback: if the shared library
+is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Dict, Optional
+
+import torch
+
+OUTGOING = 0
+INCOMING = 1
+F32 = 0
+BF16 = 1
+
+_LIB_NAME = "libfoldcp_trimul.so"
+_lib = None
+
+EXPORTS = (
+    "foldcp_trimul", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
+    "foldcp_trimul_contract", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
+    "foldcp_status_string", "foldcp_version",
+)
+
+
+class FoldcpError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        super().__init__(f"{what}: status {status} ({status_string(status)})")
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32), ("dtype", ctypes.c_int32),
+        ("ln_eps", ctypes.c_float), ("mask_output", ctypes.c_int32),
+        ("ln_in_gamma", ctypes.c_void_p), ("ln_in_beta", ctypes.c_void_p),
+        ("w_a", ctypes.c_void_p), ("w_a_gate", ctypes.c_void_p),
+        ("w_b", ctypes.c_void_p), ("w_b_gate", ctypes.c_void_p),
+        ("b_a", ctypes.c_void_p), ("b_a_gate", ctypes.c_void_p),
+        ("b_b", ctypes.c_void_p), ("b_b_gate", ctypes.c_void_p),
+        ("w_g", ctypes.c_void_p), ("b_g", ctypes.c_void_p),
+        ("ln_out_gamma", ctypes.c_void_p), ("ln_out_beta", ctypes.c_void_p),
+        ("w_o", ctypes.c_void_p), ("b_o", ctypes.c_void_p),
+        ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
+    ]
+
+
+def lib_path() -> str:
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), _LIB_NAME)
+
+
+def load() -> ctypes.CDLL:
+    """Load the shared library (raises if it has not been built: no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise RuntimeError(
+            f"{path} is missing: build it with `python -m paper_2603_14806_b200.build` "
+            "(there is no CPU fallback)")
+    lib = ctypes.CDLL(path)
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    lib.foldcp_trimul.restype = ci
+    lib.foldcp_trimul.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_workspace_bytes.restype = ctypes.c_size_t
+    lib.foldcp_trimul_workspace_bytes.argtypes = [ci, ci, ci, ci]
+    lib.foldcp_trimul_project.restype = ci
+    lib.foldcp_trimul_project.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp, vp]
+    lib.foldcp_trimul_contract.restype = ci
+    lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_finalize.restype = ci
+    lib.foldcp_trimul_finalize.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_launches_per_call.restype = ci
+    lib.foldcp_trimul_launches_per_call.argtypes = [ci]
+    lib.foldcp_status_string.restype = ctypes.c_char_p
+    lib.foldcp_status_string.argtypes = [ci]
+    lib.foldcp_version.restype = ci
+    lib.foldcp_version.argtypes = []
+    _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load().foldcp_status_string(int(status)).decode()
+
+
+def version() -> int:
+    return load().foldcp_version()
+
+
+def dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.bfloat16:
+        return BF16
+    raise TypeError(f"unsupported dtype {t.dtype}: z must be float32 or bfloat16")
+
+
+def workspace_bytes(N: int, c_z: int = 128, c_hidden: int = 128, dtype: int = BF16) -> int:
+    return int(load().foldcp_trimul_workspace_bytes(N, c_z, c_hidden, dtype))
+
+
+def launches_per_call(dtype: int = BF16) -> int:
+    return int(load().foldcp_trimul_launches_per_call(dtype))
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def make_params(p: Dict[str, Optional[torch.Tensor]], dtype: int, eps: float = 1e-5,
+                mask_output: bool = True, workspace: Optional[torch.Tensor] = None) -> _Params:
+    """Fill the C struct from a dict of device tensors (names of synth.make_params)."""
+    s = _Params()
+    s.struct_size = ctypes.sizeof(_Params)
+    s.dtype = dtype
+    s.ln_eps = eps
+    s.mask_output = 1 if mask_output else 0
+    for name in ("ln_in_gamma", "ln_in_beta", "w_a", "w_a_gate", "w_b", "w_b_gate", "b_a",
+                 "b_a_gate", "b_b", "b_b_gate", "w_g", "b_g", "ln_out_gamma", "ln_out_beta",
+                 "w_o", "b_o"):
+        t = p.get(name)
+        if t is not None:
+            assert t.is_contiguous(), name
+        setattr(s, name, _ptr(t))
+    if workspace is not None:
+        s.workspace = workspace.data_ptr()
+        s.workspace_bytes = workspace.numel() * workspace.element_size()
+    return s
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def trimul(z: torch.Tensor, mask: Optional[torch.Tensor], p: Dict[str, torch.Tensor],
+           direction: int, out: Optional[torch.Tensor] = None,
+           workspace: Optional[torch.Tensor] = None, eps: float = 1e-5,
+           mask_output: bool = True) -> torch.Tensor:
+    """One forward triangle multiplicative update on the current CUDA stream (asynchronous).
+
+    z [N, N, c_z] and mask [N, N] (or None) are CUDA tensors of the same dtype (fp32 / bf16).
+    `workspace` (uint8, >= workspace_bytes(N)) and `out` are allocated here if not given.
+    """
+    lib = load()
+    if not z.is_cuda:
+        raise ValueError("z must be a CUDA tensor (no CPU fallback)")
+    assert z.dim() == 3 and z.shape[0] == z.shape[1] and z.is_contiguous()
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = p["w_a"].shape[0]
+    dt = dtype_code(z)
+    if mask is not None:
+        assert mask.dtype == z.dtype and mask.is_contiguous() and mask.shape == (N, N)
+    if workspace is None:
+        workspace = torch.empty(max(workspace_bytes(N, c_z, c_hidden, dt), 1), dtype=torch.uint8,
+                                device=z.device)
+    if out is None:
+        out = torch.empty_like(z)
+    s = make_params(p, dt, eps, mask_output, workspace)
+    st = lib.foldcp_trimul(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
+                           int(direction), out.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul")
+    return out
+
+
+def project(z, mask, p, eps: float = 1e-5):
+    """Stage a1+a2: returns (a, b), each [c_hidden, N, N] channel-major."""
+    lib = load()
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = p["w_a"].shape[0]
+    a = torch.empty(c_hidden, N, N, dtype=z.dtype, device=z.device)
+    b = torch.empty_like(a)
+    s = make_params(p, dtype_code(z), eps)
+    st = lib.foldcp_trimul_project(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
+                                   a.data_ptr(), b.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_project")
+    return a, b
+
+
+def contract(a: torch.Tensor, b: torch.Tensor, direction: int,
+             o: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Stage a4 (Eq. 2-3): a, b [c, N, N] channel-major -> o [c, N, N]."""
+    lib = load()
+    c, N = a.shape[0], a.shape[1]
+    if o is None:
+        o = torch.empty_like(a)
+    st = lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, c, dtype_code(a),
+                                    int(direction), o.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_contract")
+    return o
+
+
+def finalize(o, z, mask, p, eps: float = 1e-5, mask_output: bool = True,
+             out: Optional[torch.Tensor] = None):
+    """Stage a3+a5: LayerNorm(o) + output projection + sigmoid gate + mask -> out [N, N, c_z]."""
+    lib = load()
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = o.shape[0]
+    if out is None:
+        out = torch.empty_like(z)
+    s = make_params(p, dtype_code(z), eps, mask_output)
+    st = lib.foldcp_trimul_finalize(o.data_ptr(), z.data_ptr(), _ptr(mask), ctypes.byref(s), N,
+                                    c_z, c_hidden, out.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_finalize")
+    return out

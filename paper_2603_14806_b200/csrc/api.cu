@@ -1,0 +1,252 @@
+// C-ABI boundary of libfoldcp_trimul (include/foldcp_trimul.h): argument validation, workspace
+// carving, stage dispatch.  Never allocates, frees or synchronises; enqueues on the caller's
+// stream and returns a status code.
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+
+#include "common.h"
+
+// default implementation of the three bf16 stages: bit0 K1, bit1 K2, bit2 K3 on tcgen05
+#ifndef FOLDCP_DEFAULT_TC_STAGES
+#define FOLDCP_DEFAULT_TC_STAGES 2
+#endif
+
+namespace foldcp {
+
+// ----------------------------------------------------------------------------- device info
+bool get_device_info(DeviceInfo* info) {
+  constexpr int kMaxDev = 64;
+  static DeviceInfo cache[kMaxDev];
+  static bool valid[kMaxDev] = {};
+  static std::mutex mu;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!valid[dev]) {
+    DeviceInfo d;
+    if (cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev) !=
+            cudaSuccess ||
+        cudaDeviceGetAttribute(&d.cc_minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess)
+      return false;
+    cache[dev] = d;
+    valid[dev] = true;
+  }
+  *info = cache[dev];
+  return true;
+}
+
+// ----------------------------------------------------------------------------- tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) !=
+            cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int rank,
+                      const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
+                      bool swizzle128) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return FOLDCP_ERR_CUDA;
+  cuuint64_t d[5], s[4];
+  cuuint32_t b[5], e[5];
+  for (int i = 0; i < rank; ++i) {
+    d[i] = dims[i];
+    b[i] = box[i];
+    e[i] = 1;
+    if (i + 1 < rank) s[i] = strides_bytes[i];
+  }
+  const CUtensorMapDataType dt =
+      elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  const CUresult r =
+      fn(map, dt, static_cast<cuuint32_t>(rank), const_cast<void*>(base), d, s, b, e,
+         CU_TENSOR_MAP_INTERLEAVE_NONE,
+         swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? FOLDCP_OK : FOLDCP_ERR_CUDA;
+}
+
+// ----------------------------------------------------------------------------- validation
+namespace {
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+inline size_t elem_bytes(int dtype) { return dtype == FOLDCP_F32 ? 4 : 2; }
+
+inline bool overlaps(const void* p, size_t pn, const void* q, size_t qn) {
+  const uintptr_t a = reinterpret_cast<uintptr_t>(p), b = reinterpret_cast<uintptr_t>(q);
+  return a < b + qn && b < a + pn;
+}
+
+int check_shape(int N, int c_z, int c_hidden, int dtype) {
+  if (dtype != FOLDCP_F32 && dtype != FOLDCP_BF16) return FOLDCP_ERR_INVALID_ARG;
+  if (N <= 0 || c_z <= 0 || c_hidden <= 0) return FOLDCP_ERR_INVALID_ARG;
+  if (c_z != kChannels || c_hidden != kChannels) return FOLDCP_ERR_UNSUPPORTED;
+  if (dtype == FOLDCP_BF16 && (N % 8) != 0) return FOLDCP_ERR_UNSUPPORTED;
+  if (N > 32768) return FOLDCP_ERR_UNSUPPORTED;   // a/b/o alone would exceed 180 GB
+  return FOLDCP_OK;
+}
+
+int check_params(const foldcp_trimul_params* p) {
+  if (!p) return FOLDCP_ERR_INVALID_ARG;
+  if (p->struct_size != sizeof(foldcp_trimul_params)) return FOLDCP_ERR_INVALID_ARG;
+  if (p->dtype != FOLDCP_F32 && p->dtype != FOLDCP_BF16) return FOLDCP_ERR_INVALID_ARG;
+  if (!(p->ln_eps >= 0.0f)) return FOLDCP_ERR_INVALID_ARG;
+  const void* required[] = {p->ln_in_gamma, p->ln_in_beta, p->w_a, p->w_a_gate, p->w_b,
+                            p->w_b_gate, p->w_g, p->ln_out_gamma, p->ln_out_beta, p->w_o};
+  for (const void* q : required)
+    if (!q) return FOLDCP_ERR_INVALID_ARG;
+  const void* all[] = {p->ln_in_gamma, p->ln_in_beta, p->w_a, p->w_a_gate, p->w_b, p->w_b_gate,
+                       p->b_a, p->b_a_gate, p->b_b, p->b_b_gate, p->w_g, p->b_g,
+                       p->ln_out_gamma, p->ln_out_beta, p->w_o, p->b_o};
+  for (const void* q : all)
+    if (q && !aligned16(q)) return FOLDCP_ERR_ALIGNMENT;
+  return FOLDCP_OK;
+}
+
+int check_arch() {
+  DeviceInfo d;
+  if (!get_device_info(&d)) return FOLDCP_ERR_CUDA;
+  return d.cc_major == 10 ? FOLDCP_OK : FOLDCP_ERR_ARCH;
+}
+
+bool force_simt() {
+  static const bool v = [] {
+    const char* e = getenv("FOLDCP_FORCE_SIMT");
+    return e && e[0] == '1';
+  }();
+  return v;
+}
+
+// which implementation runs a bf16 stage: bit0 = K1 tcgen05, bit1 = K2 tcgen05, bit2 = K3 tcgen05
+int bf16_stage_mask() {
+  static const int v = [] {
+    if (force_simt()) return 0;
+    const char* e = getenv("FOLDCP_TC_STAGES");
+    return e ? atoi(e) : FOLDCP_DEFAULT_TC_STAGES;
+  }();
+  return v;
+}
+
+}  // namespace
+}  // namespace foldcp
+
+using namespace foldcp;
+
+extern "C" {
+
+size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype) {
+  if (check_shape(N, c_z, c_hidden, dtype) != FOLDCP_OK) return 0;
+  return 3 * static_cast<size_t>(kChannels) * N * N * elem_bytes(dtype);
+}
+
+int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_params* params,
+                          int N, int c_z, int c_hidden, void* a, void* b, void* stream) {
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (!z || !a || !b) return FOLDCP_ERR_INVALID_ARG;
+  if (!aligned16(z) || !aligned16(a) || !aligned16(b) || (mask && !aligned16(mask)))
+    return FOLDCP_ERR_ALIGNMENT;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 1))
+    return launch_k1_project_bf16(z, mask, params, N, a, b, s);
+  return launch_simt_project(z, mask, params, N, a, b, s);
+}
+
+int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
+                           int direction, void* o, void* stream) {
+  int st = check_shape(N, kChannels, c_hidden, dtype);
+  if (st != FOLDCP_OK) return st;
+  if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
+  if (!a || !b || !o) return FOLDCP_ERR_INVALID_ARG;
+  if (!aligned16(a) || !aligned16(b) || !aligned16(o)) return FOLDCP_ERR_ALIGNMENT;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
+    return launch_k2_contract_bf16(a, b, o, N, direction, s);
+  return launch_simt_contract(a, b, o, N, dtype, direction, s);
+}
+
+int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
+                           const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
+                           void* out, void* stream) {
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (!o || !z || !out) return FOLDCP_ERR_INVALID_ARG;
+  if (!aligned16(o) || !aligned16(z) || !aligned16(out) || (mask && !aligned16(mask)))
+    return FOLDCP_ERR_ALIGNMENT;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 4))
+    return launch_k3_finalize_bf16(o, z, mask, params, N, out, s);
+  return launch_simt_finalize(o, z, mask, params, N, out, s);
+}
+
+int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
+                  int c_z, int c_hidden, int direction, void* out, void* stream) {
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
+  if (!z || !out) return FOLDCP_ERR_INVALID_ARG;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (!aligned16(z) || !aligned16(out) || (mask && !aligned16(mask))) return FOLDCP_ERR_ALIGNMENT;
+  const size_t need = foldcp_trimul_workspace_bytes(N, c_z, c_hidden, params->dtype);
+  if (!params->workspace || params->workspace_bytes < need) return FOLDCP_ERR_WORKSPACE;
+  if ((reinterpret_cast<uintptr_t>(params->workspace) & 255u) != 0) return FOLDCP_ERR_ALIGNMENT;
+  const size_t tensor_bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
+  if (overlaps(out, tensor_bytes, z, tensor_bytes) ||
+      overlaps(out, tensor_bytes, params->workspace, need) ||
+      overlaps(z, tensor_bytes, params->workspace, need))
+    return FOLDCP_ERR_ALIAS;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+
+  uint8_t* ws = static_cast<uint8_t*>(params->workspace);
+  void* a = ws;
+  void* b = ws + need / 3;
+  void* o = ws + 2 * (need / 3);
+  if ((st = foldcp_trimul_project(z, mask, params, N, c_z, c_hidden, a, b, stream)) != FOLDCP_OK)
+    return st;
+  if ((st = foldcp_trimul_contract(a, b, N, c_hidden, params->dtype, direction, o, stream)) !=
+      FOLDCP_OK)
+    return st;
+  return foldcp_trimul_finalize(o, z, mask, params, N, c_z, c_hidden, out, stream);
+}
+
+int foldcp_trimul_launches_per_call(int dtype) {
+  (void)dtype;
+  return 3;
+}
+
+const char* foldcp_status_string(int status) {
+  switch (status) {
+    case FOLDCP_OK: return "ok";
+    case FOLDCP_ERR_INVALID_ARG: return "invalid argument";
+    case FOLDCP_ERR_UNSUPPORTED: return "unsupported shape";
+    case FOLDCP_ERR_ALIGNMENT: return "misaligned pointer";
+    case FOLDCP_ERR_WORKSPACE: return "workspace missing or too small";
+    case FOLDCP_ERR_ALIAS: return "out overlaps an input or the workspace";
+    case FOLDCP_ERR_ARCH: return "device is not sm_100";
+    case FOLDCP_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+int foldcp_version(void) { return 100; }
+
+}  // extern "C"

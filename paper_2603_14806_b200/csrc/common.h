@@ -1,0 +1,53 @@
+// Host-side helpers shared by the translation units of libfoldcp_trimul: status plumbing,
+// tensor-map (TMA descriptor) encoding through the driver entry point, launch-config helpers.
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/foldcp_trimul.h"
+
+namespace foldcp {
+
+constexpr int kChannels = 128;  // c_z = c_hidden = 128 is the only supported channel count (A13)
+
+struct DeviceInfo {
+  int sm_count;
+  int cc_major;
+  int cc_minor;
+};
+
+// cached per device ordinal; returns false on CUDA error
+bool get_device_info(DeviceInfo* info);
+
+// Encode a tiled tensor map over a row-major tensor whose innermost dimension is dims[0].
+//   elem_bytes: 2 (bf16) or 4 (f32); rank 2..4; strides_bytes[i] = byte stride of dims[i+1]
+//   swizzle128: CU_TENSOR_MAP_SWIZZLE_128B (inner box must be 128 bytes) or none
+// Returns FOLDCP_OK or FOLDCP_ERR_CUDA.
+int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int rank,
+                      const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
+                      bool swizzle128);
+
+// ----- stage launchers (device pointers; return foldcp_status_t) -----
+int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
+                            cudaStream_t stream);
+
+int launch_simt_project(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
+                        void* a, void* b, cudaStream_t stream);
+int launch_simt_contract(const void* a, const void* b, void* o, int N, int dtype, int direction,
+                         cudaStream_t stream);
+int launch_simt_finalize(const void* o, const void* z, const void* mask,
+                         const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
+
+int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
+                           void* a, void* b, cudaStream_t stream);
+int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
+                            const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
+
+inline int check_launch() {
+  return cudaPeekAtLastError() == cudaSuccess ? FOLDCP_OK : FOLDCP_ERR_CUDA;
+}
+
+}  // namespace foldcp

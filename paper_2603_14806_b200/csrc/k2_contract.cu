@@ -1,0 +1,345 @@
+// K2 -- the triangle contraction (Eq. 2-3):
+//
+//   outgoing  o[c][i][j] = sum_k a[c][i][k] * b[c][j][k]      O_c = A_c  B_c^T   (operands K-major)
+//   incoming  o[c][i][j] = sum_k a[c][k][i] * b[c][k][j]      O_c = A_c^T B_c    (operands MN-major)
+//
+// a, b, o are channel-major bf16 [c][N][N]; c independent N x N x N GEMMs with fp32 accumulation.
+// "The outgoing and incoming variants differ only in which operand is transposed" (PAPER.md line
+// 132): here that is literally one bit per operand in the tcgen05 instruction descriptor plus the
+// TMA box coordinates -- the data is never moved.
+//
+// Kernel shape (persistent, warp-specialised, one CTA per SM, optionally CTA pairs):
+//   warp 0      TMA producer   : 64x64 bf16 boxes (128-byte swizzle) -> smem ring of kStages
+//   warp 1      MMA issuer     : one elected thread, tcgen05.mma kind::f16, D in tensor memory
+//   warp 2      TMEM allocator : 512 columns = two 128 x 256 fp32 accumulators (double buffer)
+//   warps 4-7   epilogue       : tcgen05.ld -> bf16 -> swizzled smem -> TMA store, overlapped
+//                                with the next tile's main loop through the second accumulator
+// kCtaGroup = 2 pairs two SMs on one 256 x 256 tile (cta_group::2): each CTA stages its own 128
+// rows of A and 128 of the 256 B rows, halving per-SM shared-memory operand traffic.
+#include "common.h"
+#include "ptx.cuh"
+
+namespace foldcp {
+namespace {
+
+constexpr int kBlockK = 64;        // k elements per pipeline stage (= one 128-byte swizzle row)
+constexpr int kBoxBytes = 64 * 64 * 2;  // one TMA box: 64 x 64 bf16
+constexpr int kTileN = 256;
+constexpr int kUmmaK = 16;
+constexpr int kThreads = 256;
+constexpr int kEpiBufBytes = 128 * 64 * 2;  // 128 rows x 64 bf16 columns
+constexpr int kAccumCols = 256;
+
+template <int kCtaGroup>
+struct Cfg {
+  static constexpr int kTileM = 128 * kCtaGroup;
+  static constexpr int kABytes = 2 * kBoxBytes;                  // 128 x 64 per CTA
+  static constexpr int kBBoxes = (kTileN / kCtaGroup) / 64;      // 4 or 2
+  static constexpr int kBBytes = kBBoxes * kBoxBytes;
+  static constexpr int kStageBytes = kABytes + kBBytes;          // 48 KB or 32 KB
+  static constexpr int kStages = kCtaGroup == 1 ? 4 : 6;
+  static constexpr int kBarBytes = 1024;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kEpiBufBytes + kBarBytes + 1024;
+};
+
+struct K2Params {
+  int N;
+  int tiles_m;
+  int tiles_n;
+  int num_tiles;   // channels * tiles_m * tiles_n
+  int num_kb;      // ceil(N / 64)
+};
+
+template <int kCtaGroup, bool kIncoming>
+__global__ void __launch_bounds__(kThreads, 1)
+k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
+                   const __grid_constant__ CUtensorMap tmap_b,
+                   const __grid_constant__ CUtensorMap tmap_o, const K2Params prm) {
+  using C = Cfg<kCtaGroup>;
+  extern __shared__ uint8_t smem_raw[];
+  // 128-byte swizzle needs 1024-byte aligned tiles
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t stage_base = smem_base;
+  const uint32_t epi_base = smem_base + C::kStages * C::kStageBytes;
+  const uint32_t bar_base = epi_base + 2 * kEpiBufBytes;
+  // barrier layout (8 bytes each)
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (C::kStages + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 2 + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * C::kStages + 4);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const uint32_t cta_rank = (kCtaGroup == 2) ? ptx::cluster_ctarank() : 0u;
+  const bool is_leader = cta_rank == 0;
+  const int group_id = blockIdx.x / kCtaGroup;
+  const int num_groups = gridDim.x / kCtaGroup;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmap_a);
+    ptx::prefetch_tmap(&tmap_b);
+    ptx::prefetch_tmap(&tmap_o);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < C::kStages; ++s) {
+      ptx::mbar_init(full_bar(s), 1);
+      ptx::mbar_init(empty_bar(s), 1);
+    }
+    for (int s = 0; s < 2; ++s) {
+      ptx::mbar_init(tfull_bar(s), 1);
+      ptx::mbar_init(tempty_bar(s), 4 * kCtaGroup);   // one arrival per epilogue warp per CTA
+    }
+    ptx::fence_mbar_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc<kCtaGroup>(tmem_slot, 512);
+  }
+  ptx::tc_fence_before();
+  if constexpr (kCtaGroup == 2) {
+    ptx::cluster_sync();
+  } else {
+    __syncthreads();
+  }
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int tiles_per_ch = prm.tiles_m * prm.tiles_n;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (ptx::elect_one()) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int t = group_id; t < prm.num_tiles; t += num_groups) {
+        const int ch = t / tiles_per_ch;
+        const int r = t - ch * tiles_per_ch;
+        const int m0 = (r / prm.tiles_n) * C::kTileM + static_cast<int>(cta_rank) * 128;
+        const int n0 = (r % prm.tiles_n) * kTileN + static_cast<int>(cta_rank) * (kTileN / kCtaGroup);
+        for (int kb = 0; kb < prm.num_kb; ++kb) {
+          ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+          const uint32_t sa = stage_base + stage * C::kStageBytes;
+          const uint32_t sb = sa + C::kABytes;
+          const int k0 = kb * kBlockK;
+          uint32_t bar = full_bar(stage);
+          if constexpr (kCtaGroup == 2) {
+            if (is_leader) ptx::mbar_arrive_expect_tx(bar, 2 * C::kStageBytes);
+            bar = ptx::mapa(bar, 0);
+          } else {
+            ptx::mbar_arrive_expect_tx(bar, C::kStageBytes);
+          }
+#pragma unroll
+          for (int bx = 0; bx < 2; ++bx) {
+            const int mn = m0 + 64 * bx;
+            const int c0 = kIncoming ? mn : k0;   // innermost tensor coordinate (column)
+            const int c1 = kIncoming ? k0 : mn;   // row
+            if constexpr (kCtaGroup == 2) {
+              ptx::tma_load_3d_2sm(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch);
+            } else {
+              ptx::tma_load_3d(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch);
+            }
+          }
+#pragma unroll
+          for (int bx = 0; bx < C::kBBoxes; ++bx) {
+            const int mn = n0 + 64 * bx;
+            const int c0 = kIncoming ? mn : k0;
+            const int c1 = kIncoming ? k0 : mn;
+            if constexpr (kCtaGroup == 2) {
+              ptx::tma_load_3d_2sm(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch);
+            } else {
+              ptx::tma_load_3d(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch);
+            }
+          }
+          if (++stage == C::kStages) {
+            stage = 0;
+            phase ^= 1u;
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (leader CTA only) =====================
+    if (is_leader && ptx::elect_one()) {
+      constexpr uint32_t idesc =
+          ptx::make_idesc_bf16(C::kTileM, kTileN, kIncoming ? 1 : 0, kIncoming ? 1 : 0);
+      // K-major : rows of 128 B, 8-row atoms 1024 B apart (SBO); one UMMA_K = 32 B along the row
+      // MN-major: 64-element MN groups kBoxBytes apart (LBO), 8-k atoms 1024 B apart (SBO);
+      //           one UMMA_K = two 8-k atoms = 2048 B
+      constexpr uint32_t lbo = kIncoming ? kBoxBytes : 16;
+      constexpr uint32_t sbo = 1024;
+      constexpr uint32_t kstep = kIncoming ? 2048 : 32;
+      int stage = 0;
+      uint32_t phase = 0;
+      int it = 0;
+      for (int t = group_id; t < prm.num_tiles; t += num_groups, ++it) {
+        const int as = it & 1;
+        const uint32_t aphase = (it >> 1) & 1;
+        ptx::mbar_wait_cluster(tempty_bar(as), aphase ^ 1u);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + as * kAccumCols;
+        for (int kb = 0; kb < prm.num_kb; ++kb) {
+          ptx::mbar_wait(full_bar(stage), phase);
+          ptx::tc_fence_after();
+          const uint32_t sa = stage_base + stage * C::kStageBytes;
+          const uint32_t sb = sa + C::kABytes;
+#pragma unroll
+          for (int k = 0; k < kBlockK / kUmmaK; ++k) {
+            const uint64_t da = ptx::make_smem_desc_sw128(sa + k * kstep, lbo, sbo);
+            const uint64_t db = ptx::make_smem_desc_sw128(sb + k * kstep, lbo, sbo);
+            ptx::umma_bf16<kCtaGroup>(d_tmem, da, db, idesc, (kb | k) != 0 ? 1u : 0u);
+          }
+          ptx::umma_commit<kCtaGroup>(empty_bar(stage));   // smem slot free once these MMAs retire
+          if (++stage == C::kStages) {
+            stage = 0;
+            phase ^= 1u;
+          }
+        }
+        ptx::umma_commit<kCtaGroup>(tfull_bar(as));        // accumulator ready for the epilogue
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue: TMEM -> bf16 -> smem -> TMA store =====================
+    const int q = warp - 4;                 // TMEM lane quadrant this warp may read
+    const int row = q * 32 + lane;          // row of the CTA's 128-row tile
+    const bool store_thread = (warp == 4 && lane == 0);
+    int it = 0;
+    int chunk_ctr = 0;
+    for (int t = group_id; t < prm.num_tiles; t += num_groups, ++it) {
+      const int ch = t / tiles_per_ch;
+      const int r = t - ch * tiles_per_ch;
+      const int m0 = (r / prm.tiles_n) * C::kTileM + static_cast<int>(cta_rank) * 128;
+      const int n0 = (r % prm.tiles_n) * kTileN;
+      const int as = it & 1;
+      const uint32_t aphase = (it >> 1) & 1;
+      ptx::mbar_wait(tfull_bar(as), aphase);
+      ptx::tc_fence_after();
+#pragma unroll 1
+      for (int j = 0; j < kAccumCols / 64; ++j, ++chunk_ctr) {
+        const uint32_t buf = epi_base + (chunk_ctr & 1) * kEpiBufBytes;
+        // the store issued two chunks ago read this buffer: wait until it has been drained
+        if (store_thread) ptx::tma_store_wait_read<1>();
+        ptx::named_bar_sync(1, 128);
+        uint32_t v0[32], v1[32];
+        const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) +
+                               as * kAccumCols + j * 64;
+        ptx::tmem_ld_32x32(taddr, v0);
+        ptx::tmem_ld_32x32(taddr + 32, v1);
+        ptx::tmem_ld_wait();
+        if (j == kAccumCols / 64 - 1) {
+          // accumulator fully read: hand it back to the MMA issuer (in the leader CTA)
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) {
+            if constexpr (kCtaGroup == 2) {
+              ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(as), 0));
+            } else {
+              ptx::mbar_arrive(tempty_bar(as));
+            }
+          }
+        }
+        const uint32_t row_addr = buf + row * 128;
+#pragma unroll
+        for (int cchunk = 0; cchunk < 8; ++cchunk) {
+          const uint32_t* src = (cchunk < 4) ? &v0[cchunk * 8] : &v1[(cchunk - 4) * 8];
+          const uint32_t p0 = ptx::pack_bf16x2(__uint_as_float(src[0]), __uint_as_float(src[1]));
+          const uint32_t p1 = ptx::pack_bf16x2(__uint_as_float(src[2]), __uint_as_float(src[3]));
+          const uint32_t p2 = ptx::pack_bf16x2(__uint_as_float(src[4]), __uint_as_float(src[5]));
+          const uint32_t p3 = ptx::pack_bf16x2(__uint_as_float(src[6]), __uint_as_float(src[7]));
+          const uint32_t dst = row_addr + ((cchunk ^ (row & 7)) << 4);
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(p0), "r"(p1),
+                       "r"(p2), "r"(p3)
+                       : "memory");
+        }
+        ptx::fence_proxy_async_smem();
+        ptx::named_bar_sync(1, 128);
+        if (store_thread) {
+          ptx::tma_store_3d(&tmap_o, buf, n0 + j * 64, m0, ch);
+          ptx::tma_store_commit();
+        }
+      }
+    }
+    if (store_thread) ptx::tma_store_wait<0>();
+  }
+
+  // ===================== teardown =====================
+  ptx::tc_fence_before();
+  if constexpr (kCtaGroup == 2) {
+    ptx::cluster_sync();
+  } else {
+    __syncthreads();
+  }
+  if (warp == 2) {
+    ptx::tmem_dealloc<kCtaGroup>(tmem_base, 512);
+  }
+}
+
+template <int kCtaGroup, bool kIncoming>
+int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& to,
+                   const K2Params& prm, int sm_count, cudaStream_t stream) {
+  using C = Cfg<kCtaGroup>;
+  auto kern = k2_contract_kernel<kCtaGroup, kIncoming>;
+  static bool attr_set = false;   // per template instance
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes) !=
+        cudaSuccess)
+      return FOLDCP_ERR_CUDA;
+    attr_set = true;
+  }
+  int groups = sm_count / kCtaGroup;
+  if (groups > prm.num_tiles) groups = prm.num_tiles;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(groups * kCtaGroup);
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = C::kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = kCtaGroup;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, kern, ta, tb, to, prm) != cudaSuccess) return FOLDCP_ERR_CUDA;
+  return FOLDCP_OK;
+}
+
+int g_k2_cta_group = 2;   // FOLDCP_K2_CTA_GROUP=1 selects the single-CTA variant (debug / A-B test)
+
+}  // namespace
+
+int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
+                            cudaStream_t stream) {
+  DeviceInfo dev;
+  if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
+  static const int cta_group = [] {
+    const char* e = getenv("FOLDCP_K2_CTA_GROUP");
+    return (e && e[0] == '1') ? 1 : g_k2_cta_group;
+  }();
+  const uint64_t n = static_cast<uint64_t>(N);
+  const uint64_t dims[3] = {n, n, static_cast<uint64_t>(kChannels)};
+  const uint64_t strides[2] = {n * 2, n * n * 2};
+  const uint32_t box_ld[3] = {64, 64, 1};
+  const uint32_t box_st[3] = {64, 128, 1};
+  CUtensorMap ta, tb, to;
+  int st;
+  if ((st = encode_tensor_map(&ta, a, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
+  if ((st = encode_tensor_map(&tb, b, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
+  if ((st = encode_tensor_map(&to, o, 2, 3, dims, strides, box_st, true)) != FOLDCP_OK) return st;
+  K2Params prm;
+  prm.N = N;
+  const int tile_m = 128 * cta_group;
+  prm.tiles_m = (N + tile_m - 1) / tile_m;
+  prm.tiles_n = (N + kTileN - 1) / kTileN;
+  prm.num_tiles = kChannels * prm.tiles_m * prm.tiles_n;
+  prm.num_kb = (N + kBlockK - 1) / kBlockK;
+  const bool inc = direction == FOLDCP_INCOMING;
+  if (cta_group == 2) {
+    return inc ? launch_variant<2, true>(ta, tb, to, prm, dev.sm_count, stream)
+               : launch_variant<2, false>(ta, tb, to, prm, dev.sm_count, stream);
+  }
+  return inc ? launch_variant<1, true>(ta, tb, to, prm, dev.sm_count, stream)
+             : launch_variant<1, false>(ta, tb, to, prm, dev.sm_count, stream);
+}
+
+}  // namespace foldcp
