@@ -160,3 +160,15 @@ def make_inputs(cfg: Config, direction: int, device="cpu", N: Optional[int] = No
     M = pair_mask(m, cfg.dtype, device)
     p = make_params(cfg.seed * 2 + int(direction), cfg.c_z, cfg.c_hidden, cfg.dtype, device)
     return z, M, p
+
+
+def make_z_slices(seed: int, rows: int, N: int, c_z: int = 128, dtype: str = "bf16"):
+    """The slices of a z ~ N(0,1) pair tensor that a rows x rows sub-grid evaluation touches:
+    (z_a [rows, N, c_z], z_b [rows, N, c_z], z_ij [rows, rows, c_z]) -- same distribution as make_z,
+    drawn directly so the bounded CPU-baseline sample never materialises the N x N tensor."""
+    td = _tdtype(dtype)
+    g = _gen(seed, "z", "cpu")
+    za = torch.randn(rows, N, c_z, generator=g, dtype=torch.float32).to(td)
+    zb = torch.randn(rows, N, c_z, generator=g, dtype=torch.float32).to(td)
+    zij = torch.randn(rows, rows, c_z, generator=g, dtype=torch.float32).to(td)
+    return za, zb, zij

@@ -1,0 +1,110 @@
+"""C-ABI checks that need no GPU: the library builds/loads, exports every symbol the header
+declares, and rejects bad arguments on the host before touching the device."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2603_14806_b200 import binding as B
+from paper_2603_14806_b200 import build as builder
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    builder.build()
+    return B.load()
+
+
+def test_exports_match_header(lib):
+    hdr = open(os.path.join(ROOT, "include", "foldcp_trimul.h")).read()
+    declared = set(re.findall(r"\b(foldcp_[a-z_]+)\s*\(", hdr))
+    assert declared == set(B.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_version_and_strings(lib):
+    assert B.version() >= 100
+    assert B.status_string(0) == "ok"
+    assert "workspace" in B.status_string(4)
+    assert B.status_string(99) == "unknown status"
+
+
+def test_workspace_bytes(lib):
+    assert B.workspace_bytes(4096, 128, 128, B.BF16) == 3 * 128 * 4096 * 4096 * 2   # 12 GiB
+    assert B.workspace_bytes(8192, 128, 128, B.BF16) == 48 * 2 ** 30
+    assert B.workspace_bytes(64, 128, 128, B.F32) == 3 * 128 * 64 * 64 * 4
+    assert B.workspace_bytes(12, 128, 128, B.BF16) == 0      # N % 8 != 0 in bf16
+    assert B.workspace_bytes(12, 128, 128, B.F32) > 0
+    assert B.workspace_bytes(64, 64, 128, B.BF16) == 0       # c_z != 128
+    assert B.workspace_bytes(64, 128, 64, B.BF16) == 0
+    assert B.workspace_bytes(0, 128, 128, B.BF16) == 0
+    assert B.workspace_bytes(64, 128, 128, 7) == 0
+    prev = 0
+    for n in (8, 64, 512, 2048, 4096, 8192):                 # monotone in N
+        cur = B.workspace_bytes(n)
+        assert cur > prev
+        prev = cur
+
+
+def _params(lib, dtype=B.BF16, ws=0x10000, ws_bytes=1 << 40):
+    s = B._Params()
+    s.struct_size = ctypes.sizeof(B._Params)
+    s.dtype = dtype
+    s.ln_eps = 1e-5
+    s.mask_output = 1
+    fake = 0x1000    # never dereferenced: all of these calls must fail on the host first
+    for i, (name, _) in enumerate(B._Params._fields_[4:20]):
+        setattr(s, name, fake + 0x100 * i)
+    s.workspace = ws
+    s.workspace_bytes = ws_bytes
+    return s
+
+
+def _call(lib, s, z=0x100000, mask=None, N=64, c_z=128, c=128, direction=0, out=0x900000):
+    return lib.foldcp_trimul(z, mask, ctypes.byref(s) if s is not None else None, N, c_z, c,
+                             direction, out, None)
+
+
+def test_host_side_rejections(lib):
+    INVALID, UNSUPPORTED, ALIGN, WS, ALIAS = 1, 2, 3, 4, 5
+    assert _call(lib, None) == INVALID
+    s = _params(lib)
+    assert _call(lib, s, z=None) == INVALID
+    assert _call(lib, s, out=None) == INVALID
+    assert _call(lib, s, N=0) == INVALID
+    assert _call(lib, s, N=-4) == INVALID
+    assert _call(lib, s, direction=2) == INVALID
+    assert _call(lib, s, N=12) == UNSUPPORTED
+    assert _call(lib, s, c_z=64) == UNSUPPORTED
+    assert _call(lib, s, c=64) == UNSUPPORTED
+    assert _call(lib, s, z=0x100002) == ALIGN
+    assert _call(lib, s, out=0x900008) == ALIGN
+    assert _call(lib, s, mask=0x500004) == ALIGN
+    bad = _params(lib); bad.struct_size -= 4
+    assert _call(lib, bad) == INVALID
+    bad = _params(lib); bad.dtype = 7
+    assert _call(lib, bad) == INVALID
+    for name in ("ln_in_gamma", "w_a", "w_b_gate", "w_g", "ln_out_beta", "w_o"):
+        bad = _params(lib); setattr(bad, name, None)
+        assert _call(lib, bad) == INVALID, name
+    bad = _params(lib); bad.w_a = 0x1002
+    assert _call(lib, bad) == ALIGN
+    need = B.workspace_bytes(64)
+    assert _call(lib, _params(lib, ws=None)) == WS
+    assert _call(lib, _params(lib, ws_bytes=need - 1)) == WS
+    # aliasing: out == z, out inside the workspace, z inside the workspace
+    big = 0x40000000
+    assert _call(lib, _params(lib, ws=big, ws_bytes=need), z=0x100000, out=0x100000) == ALIAS
+    assert _call(lib, _params(lib, ws=big, ws_bytes=need), out=big + 4096) == ALIAS
+    assert _call(lib, _params(lib, ws=big, ws_bytes=need), z=big + 256) == ALIAS
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    monkeypatch.setattr(B, "_lib", None)
+    monkeypatch.setattr(B, "lib_path", lambda: str(tmp_path / "nope.so"))
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        B.load()

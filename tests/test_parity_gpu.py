@@ -1,0 +1,129 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the fp64 oracle, element by
+element on the same seeded inputs.  Small sizes use the full oracle; BASELINE.json's large configs
+use the sub-grid oracle (exact full-k sums on sampled rows x columns)."""
+import numpy as np
+import pytest
+import torch
+
+import parity_util as U
+from paper_2603_14806_b200 import binding as B
+from paper_2603_14806_b200 import synth
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+OUT, INC = B.OUTGOING, B.INCOMING
+
+
+def to_dev(p):
+    return {k: v.to(DEV) for k, v in p.items()}
+
+
+def run_full(cfg, direction, N=None, mask_output=True, mask_kind=None):
+    z, M, p = synth.make_inputs(cfg, direction, "cpu", N=N)
+    if mask_kind is not None:
+        M = synth.pair_mask(synth.make_token_mask(mask_kind, z.shape[0], cfg.seed), cfg.dtype)
+    ref = U.oracle_full(z, M, p, direction, mask_output=mask_output)
+    out = B.trimul(z.to(DEV), M.to(DEV), to_dev(p), direction, mask_output=mask_output)
+    torch.cuda.synchronize()
+    return U.assert_parity(U.np64(out), ref, cfg.dtype, f"cfg{cfg.index} N={z.shape[0]} dir={direction}")
+
+
+# ---------------------------------------------------------------- BASELINE configs 0 and 1 (full oracle)
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_config0_fp32_n64(direction):
+    e = run_full(synth.CONFIGS[0], direction)
+    assert e["rel_fro"] < 1e-5
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("mask_output", [True, False])
+def test_config1_bf16_n512(direction, mask_output):
+    run_full(synth.CONFIGS[1], direction, mask_output=mask_output)
+
+
+# ---------------------------------------------------------------- ragged / tiny / odd sizes (full oracle)
+@pytest.mark.parametrize("N", [8, 72, 136, 328])
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_bf16_ragged_sizes(N, direction):
+    # 328 = 2 full 128-tiles + a 72 tail, not a multiple of the 64-wide k block either
+    run_full(synth.CONFIGS[1], direction, N=N, mask_kind="scatter")
+
+
+@pytest.mark.parametrize("N", [1, 5, 12, 67])
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_fp32_odd_sizes(N, direction):
+    run_full(synth.CONFIGS[0], direction, N=N, mask_kind="tail" if N >= 10 else "ones")
+
+
+# ---------------------------------------------------------------- stage-level parity
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("N", [64, 328, 520])
+def test_contract_stage_bf16(direction, N):
+    from oracle import trimul_oracle as orc
+    g = torch.Generator().manual_seed(N + direction)
+    a = torch.randn(128, N, N, generator=g).to(torch.bfloat16)
+    b = torch.randn(128, N, N, generator=g).to(torch.bfloat16)
+    o = B.contract(a.to(DEV), b.to(DEV), direction)
+    torch.cuda.synchronize()
+    ref = orc.contraction(np.transpose(U.np64(a), (1, 2, 0)), np.transpose(U.np64(b), (1, 2, 0)), direction)
+    got = np.transpose(U.np64(o), (1, 2, 0))
+    # only the final bf16 rounding of o (2^-9 relative) plus fp32 accumulation
+    assert np.abs(got - ref).max() <= 2.0 ** -8 * np.abs(ref).max()
+    assert U.errors(got, ref)["rel_fro"] < 3e-3
+
+
+def test_project_stage_bf16():
+    from oracle import trimul_oracle as orc
+    cfg = synth.CONFIGS[1]
+    z, M, p = synth.make_inputs(cfg, OUT, "cpu", N=136)
+    a, b = B.project(z.to(DEV), M.to(DEV), to_dev(p))
+    torch.cuda.synchronize()
+    q = U.params64(p)
+    zp = orc.layer_norm(U.np64(z), q["ln_in_gamma"], q["ln_in_beta"], 1e-5)
+    ra = orc.gated_projection(zp, U.np64(M), q["w_a"], q["b_a"], q["w_a_gate"], q["b_a_gate"])
+    rb = orc.gated_projection(zp, U.np64(M), q["w_b"], q["b_b"], q["w_b_gate"], q["b_b_gate"])
+    for got, ref in ((a, ra), (b, rb)):
+        e = U.errors(np.transpose(U.np64(got), (1, 2, 0)), ref)
+        assert e["rel_fro"] < 1e-2 and e["max_over_rms"] < 5e-2
+
+
+# ---------------------------------------------------------------- BASELINE configs 2-4 (sub-grid oracle)
+def run_subgrid(cfg, direction, n_idx, seed):
+    N = cfg.N
+    z = synth.make_z(cfg.seed, N, cfg.c_z, cfg.dtype, DEV)
+    m = synth.make_token_mask(cfg.mask_kind, N, cfg.seed)
+    M = synth.pair_mask(m, cfg.dtype, DEV)
+    p = to_dev(synth.make_params(cfg.seed * 2 + direction, cfg.c_z, cfg.c_hidden, cfg.dtype))
+    out = B.trimul(z, M, p, direction)
+    torch.cuda.synchronize()
+    masked = np.where(m.numpy() == 0)[0]
+    extra = masked[:4] if len(masked) else ()
+    I = U.sample_indices(N, n_idx, seed, tile=256, extra=extra)
+    J = U.sample_indices(N, n_idx, seed + 1, tile=256, extra=extra)
+    ref = U.oracle_subgrid(z, M, p, direction, I, J)
+    It, Jt = torch.as_tensor(I, device=DEV), torch.as_tensor(J, device=DEV)
+    got = U.np64(out[It][:, Jt])
+    e = U.assert_parity(got, ref, cfg.dtype, f"cfg{cfg.index} N={N} dir={direction} (sub-grid {n_idx}^2)")
+    # masked pairs are exactly zero with the output mask on
+    if len(masked):
+        assert torch.all(out[int(masked[0])] == 0) and torch.all(out[:, int(masked[0])] == 0)
+    return e
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_config2_bf16_n2048_chains(direction):
+    run_subgrid(synth.CONFIGS[2], direction, 48, 11)
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_config3_bf16_n4096_headline(direction):
+    run_subgrid(synth.CONFIGS[3], direction, 64, 12)
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_config4_bf16_n8192_single_call(direction):
+    free, _ = torch.cuda.mem_get_info()
+    if free < 100 * 2 ** 30:
+        pytest.skip("needs ~85 GiB of free HBM")
+    run_subgrid(synth.CONFIGS[4], direction, 48, 13)
+    torch.cuda.empty_cache()
