@@ -1,8 +1,389 @@
-// placeholder until the tcgen05 K1 lands
+// K1 -- input LayerNorm + the four gated projections + pair mask (
+// a, b are "projections of the pair representation ... with element-wise
+// gating"; north_star / AF3 Alg. 12 lines 1-3):
+//
+//   z'  = LN(z; gamma_in, beta_in, eps)                     per pair, over the 128 channels
+//   a   = M * sigmoid(W_ga z' + b_ga) * (W_a z' + b_a)      b likewise
+//
+// z is [R = N*N][128] channel-last bf16; a and b are written channel-major [128][R] bf16, which
+// is the layout K2's TMA boxes want for both directions.
+//
+// The GEMM is oriented so that the OUTPUT CHANNEL is the MMA M dimension (TMEM lane) and the
+// PAIR is the MMA N dimension (TMEM column):   D[ch][pair] = W[ch][k] * z'[pair][k]^T.
+// A thread of the epilogue then owns one channel and a run of consecutive pairs -- exactly a
+// contiguous run of the channel-major output -- and the projection and its gate for the same
+// (channel, pair) sit in the same thread (two accumulators, same lane, same column).
+//
+// Persistent kernel, one CTA per SM, 16 warps, tile = 128 pairs:
+//   warp 0       TMA producer : weights once (4 x 32 KB, resident), then z tiles into a 2-deep ring
+//   warp 1       MMA issuer   : per tile two "units" (a, b), each = projection + gate MMA
+//                               (M=128 ch, N=128 pairs, K=128) into one 256-column TMEM slot
+//   warp 2       TMEM allocator (512 columns = 2 slots; the epilogue of unit a overlaps the
+//                               MMAs of unit b and vice versa)
+//   warps 4-7    LayerNorm    : thread = pair; z row (bf16, 128-byte-swizzled TMA tile) ->
+//                               registers -> two-pass mean/variance in fp32 -> z' written back in
+//                               place as the K-major B operand; also stages the pair mask
+//   warps 8-15   epilogue     : tcgen05.ld both accumulators -> bias, sigmoid, gate, mask in
+//                               fp32 -> bf16 -> swizzled smem -> TMA store [128 ch][64 pairs]
+#include <cuda_bf16.h>
+
 #include "common.h"
+#include "ptx.cuh"
+
 namespace foldcp {
-int launch_k1_project_bf16(const void*, const void*, const foldcp_trimul_params*, int, void*, void*,
-                           cudaStream_t) {
-  return FOLDCP_ERR_UNSUPPORTED;
+namespace {
+
+constexpr int kC = kChannels;                   // 128
+constexpr int kTilePairs = 128;
+constexpr int kThreads = 512;
+constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box, 128 rows x 64 bf16
+constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 bf16 operand (two k-halves)
+constexpr int kZStages = 2;
+constexpr int kMaskSlots = 3;
+
+constexpr int kOffW = 0;                                  // 4 weight matrices
+constexpr int kOffZ = kOffW + 4 * kMatBytes;              // z ring
+constexpr int kOffOut = kOffZ + kZStages * kMatBytes;     // 2 staging buffers [128 ch][64 pairs]
+constexpr int kOffGamma = kOffOut + 2 * kHalfBox;
+constexpr int kOffBeta = kOffGamma + kC * 4;
+constexpr int kOffMask = kOffBeta + kC * 4;
+constexpr int kOffBar = kOffMask + kMaskSlots * kTilePairs * 4;
+constexpr int kSmemBytes = kOffBar + 128;
+static_assert(kSmemBytes <= 232448, "K1 shared memory exceeds 227 KB");
+
+struct K1Params {
+  const __nv_bfloat16* mask;   // [R] or nullptr
+  const float* gamma;
+  const float* beta;
+  const float* bias[4];        // b_a, b_ga, b_b, b_gb (each may be nullptr)
+  float eps;
+  long long R;                 // number of pairs
+  int num_tiles;
+};
+
+template <bool kTanhSigmoid>
+__global__ void __launch_bounds__(kThreads, 1)
+k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
+                  const __grid_constant__ CUtensorMap tmap_w0,
+                  const __grid_constant__ CUtensorMap tmap_w1,
+                  const __grid_constant__ CUtensorMap tmap_w2,
+                  const __grid_constant__ CUtensorMap tmap_w3,
+                  const __grid_constant__ CUtensorMap tmap_a,
+                  const __grid_constant__ CUtensorMap tmap_b, const K1Params prm) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t smem = ptx::smem_u32(smem_raw);
+  if ((smem & 1023u) != 0) __trap();   // 128-byte swizzle needs 1024-byte aligned tiles
+
+  const uint32_t bar = smem + kOffBar;
+  const uint32_t wfull = bar;
+  auto zfull = [&](int s) { return bar + 8u * (1 + s); };
+  auto zempty = [&](int s) { return bar + 8u * (3 + s); };
+  auto zready = [&](int s) { return bar + 8u * (5 + s); };
+  auto tfull = [&](int u) { return bar + 8u * (7 + u); };
+  auto tempty = [&](int u) { return bar + 8u * (9 + u); };
+  const uint32_t tmem_slot = bar + 8u * 11;
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmap_z);
+    ptx::prefetch_tmap(&tmap_a);
+    ptx::prefetch_tmap(&tmap_b);
+  }
+  if (warp == 1 && lane == 0) {
+    ptx::mbar_init(wfull, 1);
+    for (int s = 0; s < kZStages; ++s) {
+      ptx::mbar_init(zfull(s), 1);
+      ptx::mbar_init(zempty(s), 1);
+      ptx::mbar_init(zready(s), 128);
+    }
+    for (int u = 0; u < 2; ++u) {
+      ptx::mbar_init(tfull(u), 1);
+      ptx::mbar_init(tempty(u), 8);
+    }
+    ptx::fence_mbar_init();
+  }
+  if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
+  if (warp == 3) {
+    float* g = reinterpret_cast<float*>(smem_raw + kOffGamma);
+    float* b = reinterpret_cast<float*>(smem_raw + kOffBeta);
+    for (int c = lane; c < kC; c += 32) {
+      g[c] = prm.gamma[c];
+      b[c] = prm.beta[c];
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int first = blockIdx.x;
+  const int stride = gridDim.x;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (ptx::elect_one()) {
+      ptx::mbar_arrive_expect_tx(wfull, 4 * kMatBytes);
+      const CUtensorMap* wm[4] = {&tmap_w0, &tmap_w1, &tmap_w2, &tmap_w3};
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        ptx::tma_load_2d(smem + kOffW + m * kMatBytes, wm[m], wfull, 0, 0);
+        ptx::tma_load_2d(smem + kOffW + m * kMatBytes + kHalfBox, wm[m], wfull, 64, 0);
+      }
+      int it = 0;
+      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+        const int s = it & 1;
+        ptx::mbar_wait(zempty(s), ((it >> 1) & 1) ^ 1u);
+        ptx::mbar_arrive_expect_tx(zfull(s), kMatBytes);
+        const uint32_t dst = smem + kOffZ + s * kMatBytes;
+        const int row0 = t * kTilePairs;          // < 2^31: R <= 2^30 (N <= 32768)
+        ptx::tma_load_2d(dst, &tmap_z, zfull(s), 0, row0);
+        ptx::tma_load_2d(dst + kHalfBox, &tmap_z, zfull(s), 64, row0);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (ptx::elect_one()) {
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(128, kTilePairs, 0, 0);
+      ptx::mbar_wait(wfull, 0);
+      int it = 0;
+      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+        const int s = it & 1;
+        ptx::mbar_wait(zready(s), (it >> 1) & 1);
+        ptx::tc_fence_after();
+        const uint32_t zb = smem + kOffZ + s * kMatBytes;
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          ptx::mbar_wait(tempty(u), (it & 1) ^ 1u);
+          ptx::tc_fence_after();
+#pragma unroll
+          for (int m2 = 0; m2 < 2; ++m2) {
+            const uint32_t wa = smem + kOffW + (2 * u + m2) * kMatBytes;
+            const uint32_t d_tmem = tmem_base + u * 256 + m2 * 128;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const uint32_t off = (k >> 2) * kHalfBox + (k & 3) * 32;
+              const uint64_t da = ptx::make_smem_desc_sw128(wa + off, 16, 1024);
+              const uint64_t db = ptx::make_smem_desc_sw128(zb + off, 16, 1024);
+              ptx::umma_bf16<1>(d_tmem, da, db, idesc, k != 0 ? 1u : 0u);
+            }
+          }
+          ptx::umma_commit<1>(tfull(u));
+        }
+        ptx::umma_commit<1>(zempty(s));   // z' stage reusable once all four MMAs retired
+      }
+    }
+  } else if (warp >= 4 && warp < 8) {
+    // ===================== LayerNorm (thread = pair) =====================
+    const int r = threadIdx.x - 128;
+    const uint32_t sw = static_cast<uint32_t>(r & 7);
+    const uint32_t gaddr = smem + kOffGamma, baddr = smem + kOffBeta;
+    int it = 0;
+    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      const int s = it & 1;
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
+      float mval = 1.0f;
+      if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
+      ptx::mbar_wait(zfull(s), (it >> 1) & 1);
+      const uint32_t row = smem + kOffZ + s * kMatBytes + r * 128;
+      uint32_t x[16][4];
+#pragma unroll
+      for (int c = 0; c < 16; ++c)
+        ptx::lds128(row + (c >> 3) * kHalfBox + (((c & 7) ^ sw) << 4), x[c]);
+      float sum = 0.f;
+#pragma unroll
+      for (int c = 0; c < 16; ++c)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) sum += ptx::bf16_lo(x[c][e]) + ptx::bf16_hi(x[c][e]);
+      const float mu = sum * (1.0f / kC);
+      float var = 0.f;
+#pragma unroll
+      for (int c = 0; c < 16; ++c)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float d0 = ptx::bf16_lo(x[c][e]) - mu, d1 = ptx::bf16_hi(x[c][e]) - mu;
+          var = fmaf(d0, d0, var);
+          var = fmaf(d1, d1, var);
+        }
+      const float rstd = rsqrtf(var * (1.0f / kC) + prm.eps);
+      const float nmr = -mu * rstd;
+#pragma unroll
+      for (int c = 0; c < 16; ++c) {
+        float g[8], b[8];
+        ptx::lds128f(gaddr + c * 32, *reinterpret_cast<float(*)[4]>(&g[0]));
+        ptx::lds128f(gaddr + c * 32 + 16, *reinterpret_cast<float(*)[4]>(&g[4]));
+        ptx::lds128f(baddr + c * 32, *reinterpret_cast<float(*)[4]>(&b[0]));
+        ptx::lds128f(baddr + c * 32 + 16, *reinterpret_cast<float(*)[4]>(&b[4]));
+        uint32_t y[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float n0 = fmaf(ptx::bf16_lo(x[c][e]), rstd, nmr);
+          const float n1 = fmaf(ptx::bf16_hi(x[c][e]), rstd, nmr);
+          y[e] = ptx::pack_bf16x2(fmaf(n0, g[2 * e], b[2 * e]), fmaf(n1, g[2 * e + 1], b[2 * e + 1]));
+        }
+        ptx::sts128(row + (c >> 3) * kHalfBox + (((c & 7) ^ sw) << 4), y[0], y[1], y[2], y[3]);
+      }
+      reinterpret_cast<float*>(smem_raw + kOffMask)[(it % kMaskSlots) * kTilePairs + r] = mval;
+      ptx::fence_proxy_async_smem();
+      ptx::mbar_arrive(zready(s));
+    }
+  } else if (warp >= 8) {
+    // ===================== epilogue =====================
+    // warp -> TMEM lane quadrant q (hardware rule: warp % 4) and column half h (64 pairs)
+    const int q = warp & 3;
+    const int h = (warp - 8) >> 2;
+    const int ch = q * 32 + lane;                       // output channel = TMEM lane
+    const uint32_t stage_buf = smem + kOffOut + h * kHalfBox;
+    const uint32_t row_addr = stage_buf + ch * 128;
+    const uint32_t sw = static_cast<uint32_t>(ch & 7);
+    const bool store_thread = (q == 0 && lane == 0);
+    const uint32_t bar_id = 1 + h;
+    constexpr float kLog2e = 1.4426950408889634f;
+    float bias_p[2], bias_g[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      bias_p[u] = prm.bias[2 * u] ? prm.bias[2 * u][ch] : 0.f;
+      const float bg = prm.bias[2 * u + 1] ? prm.bias[2 * u + 1][ch] : 0.f;
+      bias_g[u] = kTanhSigmoid ? 0.5f * bg : -kLog2e * bg;
+    }
+    int it = 0;
+    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      const uint32_t mask_addr =
+          smem + kOffMask + ((it % kMaskSlots) * kTilePairs + h * 64) * 4;
+      const int p0 = t * kTilePairs + h * 64;
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        ptx::mbar_wait(tfull(u), it & 1);
+        ptx::tc_fence_after();
+        const uint32_t taddr =
+            tmem_base + (static_cast<uint32_t>(q * 32) << 16) + u * 256 + h * 64;
+#pragma unroll
+        for (int chunk = 0; chunk < 2; ++chunk) {
+          uint32_t vp[32], vg[32];
+          ptx::tmem_ld_32x32(taddr + chunk * 32, vp);
+          ptx::tmem_ld_32x32(taddr + 128 + chunk * 32, vg);
+          ptx::tmem_ld_wait();
+          uint32_t packed[16];
+#pragma unroll
+          for (int j4 = 0; j4 < 8; ++j4) {
+            float m[4];
+            ptx::lds128f(mask_addr + (chunk * 32 + j4 * 4) * 4, m);
+            float v[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int j = j4 * 4 + e;
+              const float pj = __uint_as_float(vp[j]) + bias_p[u];
+              float sg;
+              if constexpr (kTanhSigmoid) {
+                sg = fmaf(ptx::tanh_approx(fmaf(__uint_as_float(vg[j]), 0.5f, bias_g[u])), 0.5f,
+                          0.5f);
+              } else {
+                sg = ptx::sigmoid_from_scaled(fmaf(__uint_as_float(vg[j]), -kLog2e, bias_g[u]));
+              }
+              v[e] = (pj * m[e]) * sg;
+            }
+            packed[j4 * 2] = ptx::pack_bf16x2(v[0], v[1]);
+            packed[j4 * 2 + 1] = ptx::pack_bf16x2(v[2], v[3]);
+          }
+          if (chunk == 1) {
+            // accumulators and mask slot fully consumed: hand the TMEM slot back to the issuer
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(tempty(u));
+          }
+          if (chunk == 0) {
+            // the previous unit's TMA store must have finished reading the staging buffer
+            if (store_thread) ptx::tma_store_wait_read<0>();
+            ptx::named_bar_sync(bar_id, 128);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const uint32_t cchunk = static_cast<uint32_t>(chunk * 4 + i);
+            ptx::sts128(row_addr + ((cchunk ^ sw) << 4), packed[4 * i], packed[4 * i + 1],
+                        packed[4 * i + 2], packed[4 * i + 3]);
+          }
+        }
+        ptx::fence_proxy_async_smem();
+        ptx::named_bar_sync(bar_id, 128);
+        if (store_thread) {
+          ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, stage_buf, p0, 0);
+          ptx::tma_store_commit();
+        }
+      }
+    }
+    if (store_thread) ptx::tma_store_wait<0>();
+  }
+
+  // ===================== teardown =====================
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
 }
+
+bool k1_tanh_sigmoid() {
+  static const bool v = [] {
+    const char* e = getenv("FOLDCP_K1_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
+    return !(e && e[0] == 'e');
+  }();
+  return v;
+}
+
+}  // namespace
+
+int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
+                           void* a, void* b, cudaStream_t stream) {
+  DeviceInfo dev;
+  if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
+  const uint64_t R = static_cast<uint64_t>(N) * N;
+  CUtensorMap tz, tw[4], ta, tb;
+  int st;
+  {
+    const uint64_t dims[2] = {kC, R};
+    const uint64_t strides[1] = {kC * 2};
+    const uint32_t box[2] = {64, 128};
+    if ((st = encode_tensor_map(&tz, z, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
+  }
+  {
+    const uint64_t dims[2] = {kC, kC};
+    const uint64_t strides[1] = {kC * 2};
+    const uint32_t box[2] = {64, 128};
+    const void* w[4] = {p->w_a, p->w_a_gate, p->w_b, p->w_b_gate};
+    for (int m = 0; m < 4; ++m)
+      if ((st = encode_tensor_map(&tw[m], w[m], 2, 2, dims, strides, box, true)) != FOLDCP_OK)
+        return st;
+  }
+  {
+    const uint64_t dims[2] = {R, kC};
+    const uint64_t strides[1] = {R * 2};
+    const uint32_t box[2] = {64, 128};
+    if ((st = encode_tensor_map(&ta, a, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
+    if ((st = encode_tensor_map(&tb, b, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
+  }
+  K1Params prm;
+  prm.mask = static_cast<const __nv_bfloat16*>(mask);
+  prm.gamma = p->ln_in_gamma;
+  prm.beta = p->ln_in_beta;
+  prm.bias[0] = p->b_a;
+  prm.bias[1] = p->b_a_gate;
+  prm.bias[2] = p->b_b;
+  prm.bias[3] = p->b_b_gate;
+  prm.eps = p->ln_eps;
+  prm.R = static_cast<long long>(R);
+  prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
+  const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
+  const bool tanh_sig = k1_tanh_sigmoid();
+  auto kern = tanh_sig ? k1_project_kernel<true> : k1_project_kernel<false>;
+  static bool attr_set[2] = {false, false};
+  if (!attr_set[tanh_sig]) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) !=
+        cudaSuccess)
+      return FOLDCP_ERR_CUDA;
+    attr_set[tanh_sig] = true;
+  }
+  kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, tw[0], tw[1], tw[2], tw[3], ta, tb, prm);
+  return check_launch();
+}
+
 }  // namespace foldcp
