@@ -9,7 +9,7 @@
 
 // default implementation of the three bf16 stages: bit0 K1, bit1 K2, bit2 K3 on tcgen05
 #ifndef FOLDCP_DEFAULT_TC_STAGES
-#define FOLDCP_DEFAULT_TC_STAGES 3
+#define FOLDCP_DEFAULT_TC_STAGES 7
 #endif
 
 namespace foldcp {

@@ -20,7 +20,7 @@
 //                               (M=128 ch, N=128 pairs, K=128) into one 256-column TMEM slot
 //   warp 2       TMEM allocator (512 columns = 2 slots; the epilogue of unit a overlaps the
 //                               MMAs of unit b and vice versa)
-//   warps 4-7    LayerNorm    : thread = pair; z row (bf16, 128-byte-swizzled TMA tile) ->
+//   warps 4-7    LayerNorm    : ln_rows.cuh -- z rows (bf16, 128-byte-swizzled TMA tile) ->
 //                               registers -> two-pass mean/variance in fp32 -> z' written back in
 //                               place as the K-major B operand; also stages the pair mask
 //   warps 8-15   epilogue     : tcgen05.ld both accumulators -> bias, sigmoid, gate, mask in
@@ -28,6 +28,7 @@
 #include <cuda_bf16.h>
 
 #include "common.h"
+#include "ln_rows.cuh"
 #include "ptx.cuh"
 
 namespace foldcp {
@@ -122,6 +123,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   const int first = blockIdx.x;
   const int stride = gridDim.x;
 
+
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
@@ -178,7 +180,6 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp >= 4 && warp < 8) {
     // ===================== LayerNorm (thread = pair) =====================
     const int r = threadIdx.x - 128;
-    const uint32_t sw = static_cast<uint32_t>(r & 7);
     const uint32_t gaddr = smem + kOffGamma, baddr = smem + kOffBeta;
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
@@ -187,44 +188,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       float mval = 1.0f;
       if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
       ptx::mbar_wait(zfull(s), (it >> 1) & 1);
-      const uint32_t row = smem + kOffZ + s * kMatBytes + r * 128;
-      uint32_t x[16][4];
-#pragma unroll
-      for (int c = 0; c < 16; ++c)
-        ptx::lds128(row + (c >> 3) * kHalfBox + (((c & 7) ^ sw) << 4), x[c]);
-      float sum = 0.f;
-#pragma unroll
-      for (int c = 0; c < 16; ++c)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) sum += ptx::bf16_lo(x[c][e]) + ptx::bf16_hi(x[c][e]);
-      const float mu = sum * (1.0f / kC);
-      float var = 0.f;
-#pragma unroll
-      for (int c = 0; c < 16; ++c)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const float d0 = ptx::bf16_lo(x[c][e]) - mu, d1 = ptx::bf16_hi(x[c][e]) - mu;
-          var = fmaf(d0, d0, var);
-          var = fmaf(d1, d1, var);
-        }
-      const float rstd = rsqrtf(var * (1.0f / kC) + prm.eps);
-      const float nmr = -mu * rstd;
-#pragma unroll
-      for (int c = 0; c < 16; ++c) {
-        float g[8], b[8];
-        ptx::lds128f(gaddr + c * 32, *reinterpret_cast<float(*)[4]>(&g[0]));
-        ptx::lds128f(gaddr + c * 32 + 16, *reinterpret_cast<float(*)[4]>(&g[4]));
-        ptx::lds128f(baddr + c * 32, *reinterpret_cast<float(*)[4]>(&b[0]));
-        ptx::lds128f(baddr + c * 32 + 16, *reinterpret_cast<float(*)[4]>(&b[4]));
-        uint32_t y[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const float n0 = fmaf(ptx::bf16_lo(x[c][e]), rstd, nmr);
-          const float n1 = fmaf(ptx::bf16_hi(x[c][e]), rstd, nmr);
-          y[e] = ptx::pack_bf16x2(fmaf(n0, g[2 * e], b[2 * e]), fmaf(n1, g[2 * e + 1], b[2 * e + 1]));
-        }
-        ptx::sts128(row + (c >> 3) * kHalfBox + (((c & 7) ^ sw) << 4), y[0], y[1], y[2], y[3]);
-      }
+      layernorm_rows_inplace(smem + kOffZ + s * kMatBytes, kHalfBox, r, gaddr, baddr, prm.eps);
       reinterpret_cast<float*>(smem_raw + kOffMask)[(it % kMaskSlots) * kTilePairs + r] = mval;
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));

@@ -1,8 +1,404 @@
-// placeholder until the tcgen05 K3 lands
+// K3 -- output gate + output LayerNorm + output projection + mask (
+// north_star subsystem (3); AF3 Alg. 12 line 4):
+//
+//   g   = sigmoid(W_g LN(z; gamma_in, beta_in) + b_g)          recomputed from z, never stored
+//   out = [M *] g * (W_o LN(o; gamma_out, beta_out) + b_o)     written bf16, channel-last
+//
+// o is channel-major [128][R] bf16 (K2's output), z and out are [R][128] channel-last bf16.
+// Recomputing g here instead of materialising it in K1 keeps the workspace at a + b + o
+// (N = 8192 fits) and keeps g in fp32 (a bf16 round trip of g costs accuracy -- SURVEY 8(c)).
+//
+// GEMM orientation: the PAIR is the MMA M dimension (TMEM lane), the OUTPUT CHANNEL the N
+// dimension (TMEM column), so an epilogue thread owns a contiguous run of one pair's output row:
+//   D_g[pair][ch] = z'[pair][k]      * W_g[ch][k]^T     A K-major  (z tile as TMA delivers it)
+//   D_o[pair][ch] = LN(o)[k][pair]^T * W_o[ch][k]^T     A MN-major (o tile is [k][pair], pairs
+//                                                       contiguous: the transposition K2's
+//                                                       channel-major output needs is done by the
+//                                                       tensor core's operand fetch, not by us)
+//
+// Persistent kernel, one CTA per SM, 20 warps, tile = 128 pairs:
+//   warp 0       TMA producer : W_g, W_o once (resident), then (z tile, o tile) into a 2-deep ring
+//   warp 1       MMA issuer   : two MMAs (M=128 pairs, N=128 ch, K=128) into a 256-column TMEM
+//                               slot; two slots, so the epilogue overlaps the next tile's MMAs
+//   warp 2       TMEM allocator;  warp 3 stages the LayerNorm gammas / betas in smem
+//   warps 4-7    LayerNorm(z) : ln_rows.cuh (rows in registers, two-pass statistics, in place)
+//   warps 8-11   LayerNorm(o) : thread = 2 pairs x 64 channels of the [k][pair] tile, shifted
+//                               one-pass statistics combined across the half-warps, in place
+//   warps 12-19  epilogue     : tcgen05.ld -> bias, sigmoid gate, mask in fp32 -> bf16 -> swizzled
+//                               smem -> TMA store [128 pairs][64 ch]
+#include <cuda_bf16.h>
+
 #include "common.h"
+#include "ln_rows.cuh"
+#include "ptx.cuh"
+
 namespace foldcp {
-int launch_k3_finalize_bf16(const void*, const void*, const void*, const foldcp_trimul_params*, int,
-                            void*, cudaStream_t) {
-  return FOLDCP_ERR_UNSUPPORTED;
+namespace {
+
+constexpr int kC = kChannels;
+constexpr int kTilePairs = 128;
+constexpr int kThreads = 640;
+constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box (128 rows x 128 bytes)
+constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB
+constexpr int kStages = 2;
+constexpr int kStageBytes = 2 * kMatBytes;      // z tile + o tile
+
+constexpr int kOffW = 0;                                   // W_g, W_o
+constexpr int kOffStage = kOffW + 2 * kMatBytes;           // ring: [z | o] per stage
+constexpr int kOffOut = kOffStage + kStages * kStageBytes; // 2 staging buffers [128 pairs][64 ch]
+constexpr int kOffVec = kOffOut + 2 * kHalfBox;            // gamma_in, beta_in, gamma_out, beta_out
+constexpr int kOffBar = kOffVec + 4 * kC * 4;
+constexpr int kSmemBytes = kOffBar + 128;
+static_assert(kSmemBytes <= 232448, "K3 shared memory exceeds 227 KB");
+
+struct K3Params {
+  const __nv_bfloat16* mask;   // [R] or nullptr (also nullptr when mask_output == 0)
+  const float* g_in;
+  const float* b_in;
+  const float* g_out;
+  const float* b_out;
+  const float* bias_g;         // may be nullptr
+  const float* bias_o;         // may be nullptr
+  float eps;
+  long long R;
+  int num_tiles;
+};
+
+template <bool kTanhSigmoid>
+__global__ void __launch_bounds__(kThreads, 1)
+k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
+                   const __grid_constant__ CUtensorMap tmap_o,
+                   const __grid_constant__ CUtensorMap tmap_wg,
+                   const __grid_constant__ CUtensorMap tmap_wo,
+                   const __grid_constant__ CUtensorMap tmap_out, const K3Params prm) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t smem = ptx::smem_u32(smem_raw);
+  if ((smem & 1023u) != 0) __trap();
+
+  const uint32_t bar = smem + kOffBar;
+  const uint32_t wfull = bar;
+  auto full = [&](int s) { return bar + 8u * (1 + s); };
+  auto sempty = [&](int s) { return bar + 8u * (3 + s); };
+  auto zready = [&](int s) { return bar + 8u * (5 + s); };
+  auto oready = [&](int s) { return bar + 8u * (7 + s); };
+  auto tfull = [&](int u) { return bar + 8u * (9 + u); };
+  auto tempty = [&](int u) { return bar + 8u * (11 + u); };
+  const uint32_t tmem_slot = bar + 8u * 13;
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmap_z);
+    ptx::prefetch_tmap(&tmap_o);
+    ptx::prefetch_tmap(&tmap_out);
+  }
+  if (warp == 1 && lane == 0) {
+    ptx::mbar_init(wfull, 1);
+    for (int s = 0; s < kStages; ++s) {
+      ptx::mbar_init(full(s), 1);
+      ptx::mbar_init(sempty(s), 1);
+      ptx::mbar_init(zready(s), 128);
+      ptx::mbar_init(oready(s), 128);
+    }
+    for (int u = 0; u < 2; ++u) {
+      ptx::mbar_init(tfull(u), 1);
+      ptx::mbar_init(tempty(u), 8);
+    }
+    ptx::fence_mbar_init();
+  }
+  if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
+  if (warp == 3) {
+    float* v = reinterpret_cast<float*>(smem_raw + kOffVec);
+    for (int c = lane; c < kC; c += 32) {
+      v[c] = prm.g_in[c];
+      v[kC + c] = prm.b_in[c];
+      v[2 * kC + c] = prm.g_out[c];
+      v[3 * kC + c] = prm.b_out[c];
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int first = blockIdx.x;
+  const int stride = gridDim.x;
+
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (ptx::elect_one()) {
+      ptx::mbar_arrive_expect_tx(wfull, 2 * kMatBytes);
+      ptx::tma_load_2d(smem + kOffW, &tmap_wg, wfull, 0, 0);
+      ptx::tma_load_2d(smem + kOffW + kHalfBox, &tmap_wg, wfull, 64, 0);
+      ptx::tma_load_2d(smem + kOffW + kMatBytes, &tmap_wo, wfull, 0, 0);
+      ptx::tma_load_2d(smem + kOffW + kMatBytes + kHalfBox, &tmap_wo, wfull, 64, 0);
+      int it = 0;
+      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+        const int s = it & 1;
+        ptx::mbar_wait(sempty(s), ((it >> 1) & 1) ^ 1u);
+        ptx::mbar_arrive_expect_tx(full(s), kStageBytes);
+        const uint32_t zdst = smem + kOffStage + s * kStageBytes;
+        const uint32_t odst = zdst + kMatBytes;
+        const int p0 = t * kTilePairs;
+        ptx::tma_load_2d(zdst, &tmap_z, full(s), 0, p0);             // [128 pairs][ch 0..63]
+        ptx::tma_load_2d(zdst + kHalfBox, &tmap_z, full(s), 64, p0); // [128 pairs][ch 64..127]
+        ptx::tma_load_2d(odst, &tmap_o, full(s), p0, 0);             // [128 ch][pairs 0..63]
+        ptx::tma_load_2d(odst + kHalfBox, &tmap_o, full(s), p0 + 64, 0);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (ptx::elect_one()) {
+      constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, kC, 0, 0);
+      constexpr uint32_t idesc_o = ptx::make_idesc_bf16(128, kC, 1, 0);   // A = LN(o) MN-major
+      ptx::mbar_wait(wfull, 0);
+      int it = 0;
+      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+        const int s = it & 1;
+        const int slot = it & 1;
+        const uint32_t zb = smem + kOffStage + s * kStageBytes;
+        const uint32_t ob = zb + kMatBytes;
+        ptx::mbar_wait(tempty(slot), ((it >> 1) & 1) ^ 1u);
+        ptx::mbar_wait(zready(s), (it >> 1) & 1);
+        ptx::tc_fence_after();
+        const uint32_t d_g = tmem_base + slot * 256;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const uint32_t off = (k >> 2) * kHalfBox + (k & 3) * 32;
+          const uint64_t da = ptx::make_smem_desc_sw128(zb + off, 16, 1024);
+          const uint64_t db = ptx::make_smem_desc_sw128(smem + kOffW + off, 16, 1024);
+          ptx::umma_bf16<1>(d_g, da, db, idesc_g, k != 0 ? 1u : 0u);
+        }
+        ptx::mbar_wait(oready(s), (it >> 1) & 1);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          // A MN-major: 64-pair groups kHalfBox apart (LBO), 8-channel atoms 1024 B apart (SBO),
+          // one UMMA_K = 16 channels = 2048 B
+          const uint64_t da = ptx::make_smem_desc_sw128(ob + k * 2048, kHalfBox, 1024);
+          const uint32_t off = (k >> 2) * kHalfBox + (k & 3) * 32;
+          const uint64_t db = ptx::make_smem_desc_sw128(smem + kOffW + kMatBytes + off, 16, 1024);
+          ptx::umma_bf16<1>(d_g + 128, da, db, idesc_o, k != 0 ? 1u : 0u);
+        }
+        ptx::umma_commit<1>(tfull(slot));
+        ptx::umma_commit<1>(sempty(s));
+      }
+    }
+  } else if (warp >= 4 && warp < 8) {
+    // ===================== LayerNorm(z) (thread = pair) =====================
+    const int r = threadIdx.x - 128;
+    const uint32_t gaddr = smem + kOffVec, baddr = gaddr + kC * 4;
+    int it = 0;
+    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      const int s = it & 1;
+      ptx::mbar_wait(full(s), (it >> 1) & 1);
+      layernorm_rows_inplace(smem + kOffStage + s * kStageBytes, kHalfBox, r, gaddr, baddr, prm.eps);
+      ptx::fence_proxy_async_smem();
+      ptx::mbar_arrive(zready(s));
+    }
+  } else if (warp >= 8 && warp < 12) {
+    // ===================== LayerNorm(o) on the [channel][pair] tile =====================
+    // warp w4 owns pairs w4*32 .. +31; lane = (half-warp chalf = 64 channels, 16 pair-pairs).
+    // One ld.shared.b32 = 2 adjacent pairs of one channel; a half-warp reads 64 contiguous bytes
+    // of a row, the other half-warp a row whose swizzle phase differs by 4 -> conflict-free.
+    const int w4 = warp - 8;
+    const int chalf = lane >> 4;
+    const int pp = lane & 15;
+    const uint32_t box = static_cast<uint32_t>(w4 >> 1);
+    const uint32_t c16 = static_cast<uint32_t>((w4 & 1) * 4 + (pp >> 2));   // 16-byte chunk in row
+    const uint32_t within = static_cast<uint32_t>((pp & 3) * 4);
+    const uint32_t gaddr = smem + kOffVec + 2 * kC * 4, baddr = gaddr + kC * 4;
+    const int kflip = chalf * 4;
+    int it = 0;
+    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      const int s = it & 1;
+      ptx::mbar_wait(full(s), (it >> 1) & 1);
+      const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes + box * kHalfBox;
+      auto addr_of = [&](int k) {
+        return tile + static_cast<uint32_t>(k) * 128u + ((c16 ^ static_cast<uint32_t>(k & 7)) << 4) +
+               within;
+      };
+      // shift = channel 0's value of each pair (robust one-pass variance)
+      const uint32_t v0 = ptx::lds32(addr_of(0));
+      const float sh0 = ptx::bf16_lo(v0), sh1 = ptx::bf16_hi(v0);
+      float s0 = 0.f, s1 = 0.f, q0 = 0.f, q1 = 0.f;
+#pragma unroll 16
+      for (int i = 0; i < 64; ++i) {
+        const int k = chalf * 64 + (i ^ kflip);
+        const uint32_t v = ptx::lds32(addr_of(k));
+        const float d0 = ptx::bf16_lo(v) - sh0, d1 = ptx::bf16_hi(v) - sh1;
+        s0 += d0;
+        s1 += d1;
+        q0 = fmaf(d0, d0, q0);
+        q1 = fmaf(d1, d1, q1);
+      }
+      s0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+      s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+      q0 += __shfl_xor_sync(0xffffffffu, q0, 16);
+      q1 += __shfl_xor_sync(0xffffffffu, q1, 16);
+      const float m0 = s0 * (1.0f / kC), m1 = s1 * (1.0f / kC);
+      const float var0 = fmaxf(q0 * (1.0f / kC) - m0 * m0, 0.f);
+      const float var1 = fmaxf(q1 * (1.0f / kC) - m1 * m1, 0.f);
+      const float r0 = rsqrtf(var0 + prm.eps), r1 = rsqrtf(var1 + prm.eps);
+      const float n0 = -(sh0 + m0) * r0, n1 = -(sh1 + m1) * r1;
+#pragma unroll 16
+      for (int i = 0; i < 64; ++i) {
+        const int k = chalf * 64 + (i ^ kflip);
+        const uint32_t a = addr_of(k);
+        const uint32_t v = ptx::lds32(a);
+        const float g = ptx::lds32f(gaddr + k * 4), b = ptx::lds32f(baddr + k * 4);
+        const float y0 = fmaf(fmaf(ptx::bf16_lo(v), r0, n0), g, b);
+        const float y1 = fmaf(fmaf(ptx::bf16_hi(v), r1, n1), g, b);
+        ptx::sts32(a, ptx::pack_bf16x2(y0, y1));
+      }
+      ptx::fence_proxy_async_smem();
+      ptx::mbar_arrive(oready(s));
+    }
+  } else if (warp >= 12) {
+    // ===================== epilogue (thread = pair, 64 output channels) =====================
+    const int q = warp & 3;                       // TMEM lane quadrant (hardware: warp % 4)
+    const int h = (warp - 12) >> 2;               // channel half
+    const int r = q * 32 + lane;                  // pair within the tile
+    const uint32_t stage_buf = smem + kOffOut + h * kHalfBox;
+    const uint32_t row_addr = stage_buf + r * 128;
+    const uint32_t sw = static_cast<uint32_t>(r & 7);
+    const bool store_thread = (q == 0 && lane == 0);
+    const uint32_t bar_id = 1 + h;
+    constexpr float kLog2e = 1.4426950408889634f;
+    const float4* bg4 = reinterpret_cast<const float4*>(prm.bias_g) + h * 16;
+    const float4* bo4 = reinterpret_cast<const float4*>(prm.bias_o) + h * 16;
+    int it = 0;
+    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      const int slot = it & 1;
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
+      float mval = 1.0f;
+      if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
+      ptx::mbar_wait(tfull(slot), (it >> 1) & 1);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + h * 64;
+#pragma unroll
+      for (int chunk = 0; chunk < 4; ++chunk) {
+        uint32_t vg[16], vo[16];
+        ptx::tmem_ld_32x16(taddr + chunk * 16, vg);
+        ptx::tmem_ld_32x16(taddr + 128 + chunk * 16, vo);
+        ptx::tmem_ld_wait();
+        if (chunk == 3) {
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(tempty(slot));
+        }
+        uint32_t packed[8];
+#pragma unroll
+        for (int j4 = 0; j4 < 4; ++j4) {
+          float4 bg = make_float4(0.f, 0.f, 0.f, 0.f), bo = bg;
+          if (prm.bias_g) bg = __ldg(bg4 + chunk * 4 + j4);
+          if (prm.bias_o) bo = __ldg(bo4 + chunk * 4 + j4);
+          const float bgv[4] = {bg.x, bg.y, bg.z, bg.w}, bov[4] = {bo.x, bo.y, bo.z, bo.w};
+          float v[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int j = j4 * 4 + e;
+            const float x = __uint_as_float(vg[j]) + bgv[e];
+            float sg;
+            if constexpr (kTanhSigmoid) {
+              sg = fmaf(ptx::tanh_approx(0.5f * x), 0.5f, 0.5f);
+            } else {
+              sg = ptx::sigmoid_from_scaled(-kLog2e * x);
+            }
+            v[e] = ((__uint_as_float(vo[j]) + bov[e]) * mval) * sg;
+          }
+          packed[j4 * 2] = ptx::pack_bf16x2(v[0], v[1]);
+          packed[j4 * 2 + 1] = ptx::pack_bf16x2(v[2], v[3]);
+        }
+        if (chunk == 0) {
+          if (store_thread) ptx::tma_store_wait_read<0>();
+          ptx::named_bar_sync(bar_id, 128);
+        }
+        ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2) ^ sw) << 4), packed[0], packed[1],
+                    packed[2], packed[3]);
+        ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2 + 1) ^ sw) << 4), packed[4],
+                    packed[5], packed[6], packed[7]);
+      }
+      ptx::fence_proxy_async_smem();
+      ptx::named_bar_sync(bar_id, 128);
+      if (store_thread) {
+        ptx::tma_store_2d(&tmap_out, stage_buf, h * 64, t * kTilePairs);
+        ptx::tma_store_commit();
+      }
+    }
+    if (store_thread) ptx::tma_store_wait<0>();
+  }
+
+  // ===================== teardown =====================
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
 }
+
+bool k3_tanh_sigmoid() {
+  static const bool v = [] {
+    const char* e = getenv("FOLDCP_K3_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
+    return !(e && e[0] == 'e');
+  }();
+  return v;
+}
+
+}  // namespace
+
+int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
+                            const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream) {
+  DeviceInfo dev;
+  if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
+  const uint64_t R = static_cast<uint64_t>(N) * N;
+  CUtensorMap tz, to, twg, two, tout;
+  int st;
+  const uint32_t box[2] = {64, 128};
+  {
+    const uint64_t dims[2] = {kC, R};
+    const uint64_t strides[1] = {kC * 2};
+    if ((st = encode_tensor_map(&tz, z, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
+    if ((st = encode_tensor_map(&tout, out, 2, 2, dims, strides, box, true)) != FOLDCP_OK)
+      return st;
+  }
+  {
+    const uint64_t dims[2] = {R, kC};
+    const uint64_t strides[1] = {R * 2};
+    if ((st = encode_tensor_map(&to, o, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
+  }
+  {
+    const uint64_t dims[2] = {kC, kC};
+    const uint64_t strides[1] = {kC * 2};
+    if ((st = encode_tensor_map(&twg, p->w_g, 2, 2, dims, strides, box, true)) != FOLDCP_OK)
+      return st;
+    if ((st = encode_tensor_map(&two, p->w_o, 2, 2, dims, strides, box, true)) != FOLDCP_OK)
+      return st;
+  }
+  K3Params prm;
+  prm.mask = p->mask_output ? static_cast<const __nv_bfloat16*>(mask) : nullptr;
+  prm.g_in = p->ln_in_gamma;
+  prm.b_in = p->ln_in_beta;
+  prm.g_out = p->ln_out_gamma;
+  prm.b_out = p->ln_out_beta;
+  prm.bias_g = p->b_g;
+  prm.bias_o = p->b_o;
+  prm.eps = p->ln_eps;
+  prm.R = static_cast<long long>(R);
+  prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
+  const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
+  const bool tanh_sig = k3_tanh_sigmoid();
+  auto kern = tanh_sig ? k3_finalize_kernel<true> : k3_finalize_kernel<false>;
+  static bool attr_set[2] = {false, false};
+  if (!attr_set[tanh_sig]) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) !=
+        cudaSuccess)
+      return FOLDCP_ERR_CUDA;
+    attr_set[tanh_sig] = true;
+  }
+  kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, to, twg, two, tout, prm);
+  return check_launch();
+}
+
 }  // namespace foldcp
