@@ -11,6 +11,18 @@
 
 namespace foldcp {
 
+// The LayerNorm outputs z' and LN(o) only ever exist as on-chip MMA operand tiles.  They are bounded
+// (|LN(x)| <= sqrt(c-1) |gamma| + |beta|), so they are held in fp16 (11-bit significand) rather
+// than bf16 (8-bit).  tcgen05 kind::f16 wants A and B in the same format (a mixed f16 x bf16
+// descriptor is an illegal instruction on sm_100a), so each CTA converts its resident bf16 weights
+// to fp16 in shared memory once (exact for 2^-14 <= |w| <= 65504).  Two of the four bf16 rounding
+// points of the pipeline disappear at no cost
+// (error budget).  Set to 0 to fall back to bf16 operand tiles.
+#ifndef FOLDCP_NORM_FP16
+#define FOLDCP_NORM_FP16 1
+#endif
+constexpr bool kNormFp16 = FOLDCP_NORM_FP16 != 0;
+
 constexpr int kChannels = 128;  // c_z = c_hidden = 128 is the only supported channel count (A13)
 
 struct DeviceInfo {

@@ -120,6 +120,24 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
+  // weights: loaded once per CTA, resident for the whole kernel
+  if (warp == 0 && ptx::elect_one()) {
+    ptx::mbar_arrive_expect_tx(wfull, 4 * kMatBytes);
+    const CUtensorMap* wm[4] = {&tmap_w0, &tmap_w1, &tmap_w2, &tmap_w3};
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+      ptx::tma_load_2d(smem + kOffW + m * kMatBytes, wm[m], wfull, 0, 0);
+      ptx::tma_load_2d(smem + kOffW + m * kMatBytes + kHalfBox, wm[m], wfull, 64, 0);
+    }
+  }
+  if constexpr (kNormFp16) {
+    // kind::f16 needs A and B in the same 16-bit format: the bf16 weights become fp16 in place
+    ptx::mbar_wait(wfull, 0);
+    ptx::smem_bf16_to_f16_inplace(smem + kOffW, 4 * kMatBytes, threadIdx.x, kThreads);
+    ptx::fence_proxy_async_smem();
+    __syncthreads();
+  }
+
   const int first = blockIdx.x;
   const int stride = gridDim.x;
 
@@ -127,13 +145,6 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
-      ptx::mbar_arrive_expect_tx(wfull, 4 * kMatBytes);
-      const CUtensorMap* wm[4] = {&tmap_w0, &tmap_w1, &tmap_w2, &tmap_w3};
-#pragma unroll
-      for (int m = 0; m < 4; ++m) {
-        ptx::tma_load_2d(smem + kOffW + m * kMatBytes, wm[m], wfull, 0, 0);
-        ptx::tma_load_2d(smem + kOffW + m * kMatBytes + kHalfBox, wm[m], wfull, 64, 0);
-      }
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
         const int s = it & 1;
@@ -148,7 +159,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (ptx::elect_one()) {
-      constexpr uint32_t idesc = ptx::make_idesc_bf16(128, kTilePairs, 0, 0);
+      // A = weights, B = z', both K-major, both fp16 (or both bf16)
+      constexpr uint32_t kFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
+      constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, kTilePairs, kFmt, kFmt, 0, 0);
       ptx::mbar_wait(wfull, 0);
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
@@ -188,7 +201,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       float mval = 1.0f;
       if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
       ptx::mbar_wait(zfull(s), (it >> 1) & 1);
-      layernorm_rows_inplace(smem + kOffZ + s * kMatBytes, kHalfBox, r, gaddr, baddr, prm.eps);
+      layernorm_rows_inplace<kNormFp16>(smem + kOffZ + s * kMatBytes, kHalfBox, r, gaddr, baddr, prm.eps);
       reinterpret_cast<float*>(smem_raw + kOffMask)[(it % kMaskSlots) * kTilePairs + r] = mval;
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));

@@ -123,6 +123,22 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
+  // weights: loaded once per CTA, resident for the whole kernel
+  if (warp == 0 && ptx::elect_one()) {
+    ptx::mbar_arrive_expect_tx(wfull, 2 * kMatBytes);
+    ptx::tma_load_2d(smem + kOffW, &tmap_wg, wfull, 0, 0);
+    ptx::tma_load_2d(smem + kOffW + kHalfBox, &tmap_wg, wfull, 64, 0);
+    ptx::tma_load_2d(smem + kOffW + kMatBytes, &tmap_wo, wfull, 0, 0);
+    ptx::tma_load_2d(smem + kOffW + kMatBytes + kHalfBox, &tmap_wo, wfull, 64, 0);
+  }
+  if constexpr (kNormFp16) {
+    // kind::f16 needs A and B in the same 16-bit format: the bf16 weights become fp16 in place
+    ptx::mbar_wait(wfull, 0);
+    ptx::smem_bf16_to_f16_inplace(smem + kOffW, 2 * kMatBytes, threadIdx.x, kThreads);
+    ptx::fence_proxy_async_smem();
+    __syncthreads();
+  }
+
   const int first = blockIdx.x;
   const int stride = gridDim.x;
 
@@ -130,11 +146,6 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
-      ptx::mbar_arrive_expect_tx(wfull, 2 * kMatBytes);
-      ptx::tma_load_2d(smem + kOffW, &tmap_wg, wfull, 0, 0);
-      ptx::tma_load_2d(smem + kOffW + kHalfBox, &tmap_wg, wfull, 64, 0);
-      ptx::tma_load_2d(smem + kOffW + kMatBytes, &tmap_wo, wfull, 0, 0);
-      ptx::tma_load_2d(smem + kOffW + kMatBytes + kHalfBox, &tmap_wo, wfull, 64, 0);
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
         const int s = it & 1;
@@ -152,8 +163,10 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (ptx::elect_one()) {
-      constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, kC, 0, 0);
-      constexpr uint32_t idesc_o = ptx::make_idesc_bf16(128, kC, 1, 0);   // A = LN(o) MN-major
+      constexpr uint32_t kNormFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
+      constexpr uint32_t idesc_g = ptx::make_idesc_f16kind(128, kC, kNormFmt, kNormFmt, 0, 0);
+      // A = LN(o), MN-major
+      constexpr uint32_t idesc_o = ptx::make_idesc_f16kind(128, kC, kNormFmt, kNormFmt, 1, 0);
       ptx::mbar_wait(wfull, 0);
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
@@ -195,7 +208,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      layernorm_rows_inplace(smem + kOffStage + s * kStageBytes, kHalfBox, r, gaddr, baddr, prm.eps);
+      layernorm_rows_inplace<kNormFp16>(smem + kOffStage + s * kStageBytes, kHalfBox, r, gaddr, baddr, prm.eps);
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
@@ -252,7 +265,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         const float g = ptx::lds32f(gaddr + k * 4), b = ptx::lds32f(baddr + k * 4);
         const float y0 = fmaf(fmaf(ptx::bf16_lo(v), r0, n0), g, b);
         const float y1 = fmaf(fmaf(ptx::bf16_hi(v), r1, n1), g, b);
-        ptx::sts32(a, ptx::pack_bf16x2(y0, y1));
+        ptx::sts32(a, ptx::pack_norm<kNormFp16>(y0, y1));
       }
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(oready(s));

@@ -1,7 +1,7 @@
 // Input LayerNorm of one [128 pairs][128 channels] bf16 tile held in shared memory exactly as TMA
 // delivers it: two boxes (channels 0..63 | 64..127) of 128 rows x 128 bytes with the 128-byte
 // swizzle (16-byte chunk index ^= row & 7).  The normalised, affine-transformed tile is written
-// back in place, which is the canonical K-major SWIZZLE_128B operand layout tcgen05.mma reads.
+// back in place (as fp16 when kF16, else bf16), which is the canonical K-major SWIZZLE_128B operand layout tcgen05.mma reads.
 //
 // 128 threads, two passes of 64 rows; two adjacent lanes share a row (one 64-channel box each)
 // and combine their statistics with one shuffle.  Statistics are two-pass (mean, then centred
@@ -16,6 +16,7 @@ namespace foldcp {
 // tile  : shared address of box 0 (box 1 is box_stride bytes further)
 // tid   : 0..127 within the LayerNorm warp group
 // gaddr / baddr : shared addresses of gamma[128] / beta[128] (fp32)
+template <bool kF16>
 __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t box_stride, int tid,
                                                        uint32_t gaddr, uint32_t baddr, float eps) {
   const uint32_t half = static_cast<uint32_t>(tid & 1);
@@ -64,7 +65,7 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
       for (int e = 0; e < 4; ++e) {
         const float n0 = fmaf(ptx::bf16_lo(x[c][e]), rstd, nmr);
         const float n1 = fmaf(ptx::bf16_hi(x[c][e]), rstd, nmr);
-        y[e] = ptx::pack_bf16x2(fmaf(n0, g[2 * e], b[2 * e]), fmaf(n1, g[2 * e + 1], b[2 * e + 1]));
+        y[e] = ptx::pack_norm<kF16>(fmaf(n0, g[2 * e], b[2 * e]), fmaf(n1, g[2 * e + 1], b[2 * e + 1]));
       }
       ptx::sts128(row + ((cl ^ sw) << 4), y[0], y[1], y[2], y[3]);
     }

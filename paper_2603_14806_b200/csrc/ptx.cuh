@@ -271,20 +271,55 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr, uin
   return d;
 }
 
-// Instruction descriptor for kind::f16 with bf16 A/B and fp32 D.
-//   [4,6) D format (1 = f32) | [7,10) A format (1 = bf16) | [10,13) B format | 15 A major
+// Instruction descriptor for kind::f16 (fp32 D).
+//   [4,6) D format (1 = f32) | [7,10) A format (0 = f16, 1 = bf16) | [10,13) B format | 15 A major
 //   (0 = K, 1 = MN) | 16 B major | [17,23) N>>3 | [24,29) M>>4
-__host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, int a_mn_major,
-                                                       int b_mn_major) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | (static_cast<uint32_t>(a_mn_major) << 15) |
+constexpr uint32_t kFmtF16 = 0, kFmtBF16 = 1;
+__host__ __device__ constexpr uint32_t make_idesc_f16kind(int M, int N, uint32_t a_fmt,
+                                                          uint32_t b_fmt, int a_mn_major,
+                                                          int b_mn_major) {
+  return (1u << 4) | (a_fmt << 7) | (b_fmt << 10) | (static_cast<uint32_t>(a_mn_major) << 15) |
          (static_cast<uint32_t>(b_mn_major) << 16) | (static_cast<uint32_t>(N >> 3) << 17) |
          (static_cast<uint32_t>(M >> 4) << 24);
+}
+__host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, int a_mn_major,
+                                                       int b_mn_major) {
+  return make_idesc_f16kind(M, N, kFmtBF16, kFmtBF16, a_mn_major, b_mn_major);
 }
 
 // ---------------------------------------------------------------- small math helpers
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+// pack two fp32 into the 16-bit format of the normalised on-chip operand tiles
+template <bool kF16>
+__device__ __forceinline__ uint32_t pack_norm(float lo, float hi) {
+  if constexpr (kF16) return pack_f16x2(lo, hi);
+  return pack_bf16x2(lo, hi);
+}
+// In-place bf16 -> fp16 conversion of `bytes` of shared memory by `nthreads` threads (elementwise,
+// so any swizzled layout is preserved).  bf16 values are exact in fp16 unless |x| < 2^-14 (then
+// the absolute error is <= 2^-25) or |x| > 65504 (saturates).
+__device__ __forceinline__ void smem_bf16_to_f16_inplace(uint32_t addr, int bytes, int tid,
+                                                         int nthreads) {
+  for (int off = tid * 16; off < bytes; off += nthreads * 16) {
+    uint32_t v[4];
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
+                 : "r"(addr + off));
+#pragma unroll
+    for (int e = 0; e < 4; ++e)
+      v[e] = pack_f16x2(__uint_as_float(v[e] << 16), __uint_as_float(v[e] & 0xffff0000u));
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr + off), "r"(v[0]),
+                 "r"(v[1]), "r"(v[2]), "r"(v[3])
+                 : "memory");
+  }
 }
 __device__ __forceinline__ float tanh_approx(float x) {
   float y;
