@@ -194,15 +194,24 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // ===================== LayerNorm (thread = pair) =====================
     const int r = threadIdx.x - 128;
     const uint32_t gaddr = smem + kOffGamma, baddr = smem + kOffBeta;
+    // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
+    auto load_mask = [&](int t) -> unsigned short {
+      if (prm.mask == nullptr) return static_cast<unsigned short>(0x3f80);   // bf16 1.0
+      if (t >= prm.num_tiles) return static_cast<unsigned short>(0);
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
+      return p < prm.R ? __ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)
+                       : static_cast<unsigned short>(0);
+    };
+    unsigned short mnext = load_mask(first);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
-      const long long p = static_cast<long long>(t) * kTilePairs + r;
-      float mval = 1.0f;
-      if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
+      const unsigned short mraw = mnext;
+      mnext = load_mask(t + stride);
       ptx::mbar_wait(zfull(s), (it >> 1) & 1);
       layernorm_rows_inplace<kNormFp16>(smem + kOffZ + s * kMatBytes, kHalfBox, r, gaddr, baddr, prm.eps);
-      reinterpret_cast<float*>(smem_raw + kOffMask)[(it % kMaskSlots) * kTilePairs + r] = mval;
+      reinterpret_cast<float*>(smem_raw + kOffMask)[(it % kMaskSlots) * kTilePairs + r] =
+          __uint_as_float(static_cast<uint32_t>(mraw) << 16);
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
@@ -218,12 +227,19 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     const bool store_thread = (q == 0 && lane == 0);
     const uint32_t bar_id = 1 + h;
     constexpr float kLog2e = 1.4426950408889634f;
-    float bias_p[2], bias_g[2];
+    // packed fp32x2 constants: sigmoid(x) = 0.5 tanh(0.5 x) + 0.5  or  1 / (1 + 2^(-x log2 e))
+    constexpr float kGateScale = kTanhSigmoid ? 0.5f : -kLog2e;
+    const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
+    const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
+    (void)half2;
+    (void)one2;
+    ptx::f32x2 bias_p2[2], bias_g2[2];
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
-      bias_p[u] = prm.bias[2 * u] ? prm.bias[2 * u][ch] : 0.f;
-      const float bg = prm.bias[2 * u + 1] ? prm.bias[2 * u + 1][ch] : 0.f;
-      bias_g[u] = kTanhSigmoid ? 0.5f * bg : -kLog2e * bg;
+      const float bp = prm.bias[2 * u] ? prm.bias[2 * u][ch] : 0.f;
+      const float bg = kGateScale * (prm.bias[2 * u + 1] ? prm.bias[2 * u + 1][ch] : 0.f);
+      bias_p2[u] = ptx::pk2(bp, bp);
+      bias_g2[u] = ptx::pk2(bg, bg);
     }
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
@@ -236,35 +252,46 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::tc_fence_after();
         const uint32_t taddr =
             tmem_base + (static_cast<uint32_t>(q * 32) << 16) + u * 256 + h * 64;
+        // 64 columns per warp and unit, in four chunks of 16; the tcgen05.ld of chunk c+1 is in
+        // flight while chunk c is being computed (two register buffers)
+        uint32_t vp[2][16], vg[2][16];
+        ptx::tmem_ld_32x16(taddr, vp[0]);
+        ptx::tmem_ld_32x16(taddr + 128, vg[0]);
 #pragma unroll
-        for (int chunk = 0; chunk < 2; ++chunk) {
-          uint32_t vp[32], vg[32];
-          ptx::tmem_ld_32x32(taddr + chunk * 32, vp);
-          ptx::tmem_ld_32x32(taddr + 128 + chunk * 32, vg);
+        for (int chunk = 0; chunk < 4; ++chunk) {
+          const int cb = chunk & 1;
           ptx::tmem_ld_wait();
-          uint32_t packed[16];
-#pragma unroll
-          for (int j4 = 0; j4 < 8; ++j4) {
-            float m[4];
-            ptx::lds128f(mask_addr + (chunk * 32 + j4 * 4) * 4, m);
-            float v[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int j = j4 * 4 + e;
-              const float pj = __uint_as_float(vp[j]) + bias_p[u];
-              float sg;
-              if constexpr (kTanhSigmoid) {
-                sg = fmaf(ptx::tanh_approx(fmaf(__uint_as_float(vg[j]), 0.5f, bias_g[u])), 0.5f,
-                          0.5f);
-              } else {
-                sg = ptx::sigmoid_from_scaled(fmaf(__uint_as_float(vg[j]), -kLog2e, bias_g[u]));
-              }
-              v[e] = (pj * m[e]) * sg;
-            }
-            packed[j4 * 2] = ptx::pack_bf16x2(v[0], v[1]);
-            packed[j4 * 2 + 1] = ptx::pack_bf16x2(v[2], v[3]);
+          if (chunk < 3) {
+            ptx::tmem_ld_32x16(taddr + (chunk + 1) * 16, vp[cb ^ 1]);
+            ptx::tmem_ld_32x16(taddr + 128 + (chunk + 1) * 16, vg[cb ^ 1]);
           }
-          if (chunk == 1) {
+          uint32_t packed[8];
+#pragma unroll
+          for (int j4 = 0; j4 < 4; ++j4) {
+            ptx::f32x2 m2[2];
+            ptx::lds128x2(mask_addr + (chunk * 16 + j4 * 4) * 4, m2);
+#pragma unroll
+            for (int e2 = 0; e2 < 2; ++e2) {
+              const int j = j4 * 4 + e2 * 2;
+              const ptx::f32x2 pj = ptx::add2(ptx::pk2u(vp[cb][j], vp[cb][j + 1]), bias_p2[u]);
+              const ptx::f32x2 gx =
+                  ptx::fma2(ptx::pk2u(vg[cb][j], vg[cb][j + 1]), gscale2, bias_g2[u]);
+              float g0, g1;
+              ptx::upk2(gx, g0, g1);
+              ptx::f32x2 sg;
+              if constexpr (kTanhSigmoid) {
+                sg = ptx::fma2(ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), half2, half2);
+              } else {
+                float d0, d1;
+                ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
+                sg = ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1));
+              }
+              float v0, v1;
+              ptx::upk2(ptx::mul2(ptx::mul2(pj, m2[e2]), sg), v0, v1);
+              packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
+            }
+          }
+          if (chunk == 3) {
             // accumulators and mask slot fully consumed: hand the TMEM slot back to the issuer
             ptx::tc_fence_before();
             __syncwarp();
@@ -275,12 +302,10 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
             if (store_thread) ptx::tma_store_wait_read<0>();
             ptx::named_bar_sync(bar_id, 128);
           }
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const uint32_t cchunk = static_cast<uint32_t>(chunk * 4 + i);
-            ptx::sts128(row_addr + ((cchunk ^ sw) << 4), packed[4 * i], packed[4 * i + 1],
-                        packed[4 * i + 2], packed[4 * i + 3]);
-          }
+          ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2) ^ sw) << 4), packed[0],
+                      packed[1], packed[2], packed[3]);
+          ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2 + 1) ^ sw) << 4), packed[4],
+                      packed[5], packed[6], packed[7]);
         }
         ptx::fence_proxy_async_smem();
         ptx::named_bar_sync(bar_id, 128);

@@ -218,36 +218,50 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // One ld.shared.b32 = 2 adjacent pairs of one channel; a half-warp reads 64 contiguous bytes
     // of a row, the other half-warp a row whose swizzle phase differs by 4 -> conflict-free.
     const int w4 = warp - 8;
-    const int chalf = lane >> 4;
-    const int pp = lane & 15;
+    const uint32_t chalf = static_cast<uint32_t>(lane >> 4);
+    const uint32_t pp = static_cast<uint32_t>(lane & 15);
     const uint32_t box = static_cast<uint32_t>(w4 >> 1);
-    const uint32_t c16 = static_cast<uint32_t>((w4 & 1) * 4 + (pp >> 2));   // 16-byte chunk in row
-    const uint32_t within = static_cast<uint32_t>((pp & 3) * 4);
-    const uint32_t gaddr = smem + kOffVec + 2 * kC * 4, baddr = gaddr + kC * 4;
-    const int kflip = chalf * 4;
+    const uint32_t c16 = static_cast<uint32_t>((w4 & 1) * 4) + (pp >> 2);   // 16-byte chunk in row
+    const uint32_t within = (pp & 3u) * 4u;
+    const uint32_t kflip = chalf * 4u;
+    // Row k = chalf*64 + 8g + (jj ^ kflip), g, jj = 0..7.  Everything that depends on jj is folded
+    // into eight per-thread offsets; 8g becomes an immediate (1024 B per g in the tile, 32 B in
+    // gamma / beta).
+    uint32_t toff[8], voff[8];
+#pragma unroll
+    for (uint32_t jj = 0; jj < 8; ++jj) {
+      const uint32_t k7 = jj ^ kflip;
+      toff[jj] = box * kHalfBox + (chalf * 64u + k7) * 128u + ((c16 ^ k7) << 4) + within;
+      voff[jj] = smem + kOffVec + 2 * kC * 4 + (chalf * 64u + k7) * 4u;
+    }
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes + box * kHalfBox;
-      auto addr_of = [&](int k) {
-        return tile + static_cast<uint32_t>(k) * 128u + ((c16 ^ static_cast<uint32_t>(k & 7)) << 4) +
-               within;
-      };
+      const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes;
       // shift = channel 0's value of each pair (robust one-pass variance)
-      const uint32_t v0 = ptx::lds32(addr_of(0));
-      const float sh0 = ptx::bf16_lo(v0), sh1 = ptx::bf16_hi(v0);
-      float s0 = 0.f, s1 = 0.f, q0 = 0.f, q1 = 0.f;
-#pragma unroll 16
-      for (int i = 0; i < 64; ++i) {
-        const int k = chalf * 64 + (i ^ kflip);
-        const uint32_t v = ptx::lds32(addr_of(k));
-        const float d0 = ptx::bf16_lo(v) - sh0, d1 = ptx::bf16_hi(v) - sh1;
-        s0 += d0;
-        s1 += d1;
-        q0 = fmaf(d0, d0, q0);
-        q1 = fmaf(d1, d1, q1);
-      }
+      const ptx::f32x2 sh = ptx::bf16x2_to_f32x2(
+          ptx::lds32(tile + box * kHalfBox + (c16 << 4) + within));
+      float sh0, sh1;
+      ptx::upk2(sh, sh0, sh1);
+      const ptx::f32x2 nsh = ptx::pk2(-sh0, -sh1);
+      ptx::f32x2 sa = ptx::pk2(0.f, 0.f), sb = sa, qa = sa, qb = sa;
+#pragma unroll
+      for (uint32_t g = 0; g < 8; ++g)
+#pragma unroll
+        for (uint32_t jj = 0; jj < 8; jj += 2) {
+          const ptx::f32x2 d0 = ptx::add2(
+              ptx::bf16x2_to_f32x2(ptx::lds32(tile + toff[jj] + g * 1024u)), nsh);
+          const ptx::f32x2 d1 = ptx::add2(
+              ptx::bf16x2_to_f32x2(ptx::lds32(tile + toff[jj + 1] + g * 1024u)), nsh);
+          sa = ptx::add2(sa, d0);
+          sb = ptx::add2(sb, d1);
+          qa = ptx::fma2(d0, d0, qa);
+          qb = ptx::fma2(d1, d1, qb);
+        }
+      float s0, s1, q0, q1;
+      ptx::upk2(ptx::add2(sa, sb), s0, s1);
+      ptx::upk2(ptx::add2(qa, qb), q0, q1);
       s0 += __shfl_xor_sync(0xffffffffu, s0, 16);
       s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
       q0 += __shfl_xor_sync(0xffffffffu, q0, 16);
@@ -256,17 +270,19 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const float var0 = fmaxf(q0 * (1.0f / kC) - m0 * m0, 0.f);
       const float var1 = fmaxf(q1 * (1.0f / kC) - m1 * m1, 0.f);
       const float r0 = rsqrtf(var0 + prm.eps), r1 = rsqrtf(var1 + prm.eps);
-      const float n0 = -(sh0 + m0) * r0, n1 = -(sh1 + m1) * r1;
-#pragma unroll 16
-      for (int i = 0; i < 64; ++i) {
-        const int k = chalf * 64 + (i ^ kflip);
-        const uint32_t a = addr_of(k);
-        const uint32_t v = ptx::lds32(a);
-        const float g = ptx::lds32f(gaddr + k * 4), b = ptx::lds32f(baddr + k * 4);
-        const float y0 = fmaf(fmaf(ptx::bf16_lo(v), r0, n0), g, b);
-        const float y1 = fmaf(fmaf(ptx::bf16_hi(v), r1, n1), g, b);
-        ptx::sts32(a, ptx::pack_norm<kNormFp16>(y0, y1));
-      }
+      const ptx::f32x2 rr = ptx::pk2(r0, r1);
+      const ptx::f32x2 nn = ptx::pk2(-(sh0 + m0) * r0, -(sh1 + m1) * r1);
+#pragma unroll
+      for (uint32_t g = 0; g < 8; ++g)
+#pragma unroll
+        for (uint32_t jj = 0; jj < 8; ++jj) {
+          const uint32_t a = tile + toff[jj] + g * 1024u;
+          const float gm = ptx::lds32f(voff[jj] + g * 32u);
+          const float bt = ptx::lds32f(voff[jj] + g * 32u + kC * 4);
+          const ptx::f32x2 y = ptx::fma2(ptx::fma2(ptx::bf16x2_to_f32x2(ptx::lds32(a)), rr, nn),
+                                         ptx::pk2(gm, gm), ptx::pk2(bt, bt));
+          ptx::sts32(a, ptx::pack_norm2<kNormFp16>(y));
+        }
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(oready(s));
     }
@@ -281,6 +297,11 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     const bool store_thread = (q == 0 && lane == 0);
     const uint32_t bar_id = 1 + h;
     constexpr float kLog2e = 1.4426950408889634f;
+    constexpr float kGateScale = kTanhSigmoid ? 0.5f : -kLog2e;
+    const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
+    const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
+    (void)half2;
+    (void)one2;
     const float4* bg4 = reinterpret_cast<const float4*>(prm.bias_g) + h * 16;
     const float4* bo4 = reinterpret_cast<const float4*>(prm.bias_o) + h * 16;
     int it = 0;
@@ -289,6 +310,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const long long p = static_cast<long long>(t) * kTilePairs + r;
       float mval = 1.0f;
       if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
+      const ptx::f32x2 mval2 = ptx::pk2(mval, mval);
       ptx::mbar_wait(tfull(slot), (it >> 1) & 1);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + h * 64;
@@ -309,22 +331,28 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           float4 bg = make_float4(0.f, 0.f, 0.f, 0.f), bo = bg;
           if (prm.bias_g) bg = __ldg(bg4 + chunk * 4 + j4);
           if (prm.bias_o) bo = __ldg(bo4 + chunk * 4 + j4);
-          const float bgv[4] = {bg.x, bg.y, bg.z, bg.w}, bov[4] = {bo.x, bo.y, bo.z, bo.w};
-          float v[4];
+          const ptx::f32x2 bg2[2] = {ptx::pk2(bg.x, bg.y), ptx::pk2(bg.z, bg.w)};
+          const ptx::f32x2 bo2[2] = {ptx::pk2(bo.x, bo.y), ptx::pk2(bo.z, bo.w)};
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int j = j4 * 4 + e;
-            const float x = __uint_as_float(vg[j]) + bgv[e];
-            float sg;
+          for (int e2 = 0; e2 < 2; ++e2) {
+            const int j = j4 * 4 + e2 * 2;
+            // gate pre-activation scaled for the sigmoid form in use
+            const ptx::f32x2 gx = ptx::mul2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bg2[e2]), gscale2);
+            float g0, g1;
+            ptx::upk2(gx, g0, g1);
+            ptx::f32x2 sg;
             if constexpr (kTanhSigmoid) {
-              sg = fmaf(ptx::tanh_approx(0.5f * x), 0.5f, 0.5f);
+              sg = ptx::fma2(ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), half2, half2);
             } else {
-              sg = ptx::sigmoid_from_scaled(-kLog2e * x);
+              float d0, d1;
+              ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
+              sg = ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1));
             }
-            v[e] = ((__uint_as_float(vo[j]) + bov[e]) * mval) * sg;
+            const ptx::f32x2 y = ptx::mul2(ptx::add2(ptx::pk2u(vo[j], vo[j + 1]), bo2[e2]), mval2);
+            float v0, v1;
+            ptx::upk2(ptx::mul2(y, sg), v0, v1);
+            packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
           }
-          packed[j4 * 2] = ptx::pack_bf16x2(v[0], v[1]);
-          packed[j4 * 2 + 1] = ptx::pack_bf16x2(v[2], v[3]);
         }
         if (chunk == 0) {
           if (store_thread) ptx::tma_store_wait_read<0>();

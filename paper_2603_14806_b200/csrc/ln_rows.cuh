@@ -1,12 +1,15 @@
 // Input LayerNorm of one [128 pairs][128 channels] bf16 tile held in shared memory exactly as TMA
 // delivers it: two boxes (channels 0..63 | 64..127) of 128 rows x 128 bytes with the 128-byte
 // swizzle (16-byte chunk index ^= row & 7).  The normalised, affine-transformed tile is written
-// back in place (as fp16 when kF16, else bf16), which is the canonical K-major SWIZZLE_128B operand layout tcgen05.mma reads.
+// back in place (as fp16 when kF16, else bf16), which is the canonical K-major SWIZZLE_128B
+// operand layout tcgen05.mma reads.
 //
-// 128 threads, two passes of 64 rows; two adjacent lanes share a row (one 64-channel box each)
-// and combine their statistics with one shuffle.  Statistics are two-pass (mean, then centred
-// sum of squares) in fp32 on the register-resident row, so they are exact for bf16 inputs up to
-// fp32 summation error.  Used by K1 (z' feeds the four projections) and K3 (z' feeds the gate).
+// 128 threads, two passes of 2 x 32 rows; four adjacent lanes share a row (32 channels each, held
+// unpacked in registers) and combine their statistics with two shuffles.  Statistics are
+// two-pass (mean, then centred sum of squares) in fp32, so they are exact for bf16 inputs up to
+// fp32 summation error.  All arithmetic is packed fp32x2 (FADD2 / FFMA2): the kernels that call
+// this are issue-bound, not FLOP-bound.  Used by K1 (z' feeds the four projections) and K3
+// (z' feeds the output gate).
 #pragma once
 
 #include "ptx.cuh"
@@ -19,55 +22,95 @@ namespace foldcp {
 template <bool kF16>
 __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t box_stride, int tid,
                                                        uint32_t gaddr, uint32_t baddr, float eps) {
-  const uint32_t half = static_cast<uint32_t>(tid & 1);
-  // chunk visiting order differs between the two lanes of a row (xor 5) so that a quarter-warp's
-  // eight 16-byte loads fall in eight different bank groups and the gamma/beta broadcasts of the
-  // two halves do not collide either
-  const uint32_t cx = half * 5u;
+  const uint32_t j = static_cast<uint32_t>(tid & 3);        // quarter of the row: channels 32j..
+  const uint32_t box = j >> 1;
+  const uint32_t cbase = (j & 1u) * 4u;                      // first 16-byte chunk inside the box
+  // Lane j visits its four chunks in the order t ^ j: a quarter-warp (2 rows x 4 lanes) then hits
+  // eight distinct bank groups with its data and four distinct ones with gamma / beta.
+  // Each thread works on two rows (r, r + 32) at once: the two dependency chains (loads, sums,
+  // shuffles, rsqrt) interleave, which matters because one LayerNorm warp per scheduler is
+  // latency-bound, not throughput-bound.
 #pragma unroll 1
   for (int pass = 0; pass < 2; ++pass) {
-    const uint32_t r = static_cast<uint32_t>(pass * 64 + (tid >> 1));
-    const uint32_t sw = r & 7u;
-    const uint32_t row = tile + half * box_stride + r * 128u;
-    uint32_t x[8][4];
+    const uint32_t r0 = static_cast<uint32_t>(pass * 64 + (tid >> 2));
+    const uint32_t sw = r0 & 7u;                              // (r0 + 32) & 7 is the same
+    const uint32_t row0 = tile + box * box_stride + r0 * 128u;
+    ptx::f32x2 x[2][4][4];
 #pragma unroll
-    for (uint32_t c = 0; c < 8; ++c) ptx::lds128(row + (((c ^ cx) ^ sw) << 4), x[c]);
-    float sum = 0.f;
+    for (uint32_t q = 0; q < 2; ++q)
 #pragma unroll
-    for (int c = 0; c < 8; ++c)
+      for (uint32_t t = 0; t < 4; ++t) {
+        uint32_t w[4];
+        ptx::lds128(row0 + q * 4096u + (((cbase + (t ^ j)) ^ sw) << 4), w);
 #pragma unroll
-      for (int e = 0; e < 4; ++e) sum += ptx::bf16_lo(x[c][e]) + ptx::bf16_hi(x[c][e]);
-    sum += __shfl_xor_sync(0xffffffffu, sum, 1);
-    const float mu = sum * (1.0f / 128.0f);
-    float var = 0.f;
-#pragma unroll
-    for (int c = 0; c < 8; ++c)
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const float d0 = ptx::bf16_lo(x[c][e]) - mu, d1 = ptx::bf16_hi(x[c][e]) - mu;
-        var = fmaf(d0, d0, var);
-        var = fmaf(d1, d1, var);
+        for (int e = 0; e < 4; ++e) x[q][t][e] = ptx::bf16x2_to_f32x2(w[e]);
       }
-    var += __shfl_xor_sync(0xffffffffu, var, 1);
-    const float rstd = rsqrtf(var * (1.0f / 128.0f) + eps);
-    const float nmr = -mu * rstd;
+    float mu[2], rstd[2];
+    float sum[2];
 #pragma unroll
-    for (uint32_t c = 0; c < 8; ++c) {
-      const uint32_t cl = c ^ cx;                         // logical chunk = 8 channels
-      const uint32_t voff = (half * 64u + cl * 8u) * 4u;  // byte offset of its gamma / beta
-      float g[8], b[8];
-      ptx::lds128f(gaddr + voff, *reinterpret_cast<float(*)[4]>(&g[0]));
-      ptx::lds128f(gaddr + voff + 16, *reinterpret_cast<float(*)[4]>(&g[4]));
-      ptx::lds128f(baddr + voff, *reinterpret_cast<float(*)[4]>(&b[0]));
-      ptx::lds128f(baddr + voff + 16, *reinterpret_cast<float(*)[4]>(&b[4]));
-      uint32_t y[4];
+    for (int q = 0; q < 2; ++q) {
+      ptx::f32x2 s2 = ptx::add2(x[q][0][0], x[q][0][1]), s3 = ptx::add2(x[q][0][2], x[q][0][3]);
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const float n0 = fmaf(ptx::bf16_lo(x[c][e]), rstd, nmr);
-        const float n1 = fmaf(ptx::bf16_hi(x[c][e]), rstd, nmr);
-        y[e] = ptx::pack_norm<kF16>(fmaf(n0, g[2 * e], b[2 * e]), fmaf(n1, g[2 * e + 1], b[2 * e + 1]));
+      for (int t = 1; t < 4; ++t) {
+        s2 = ptx::add2(s2, ptx::add2(x[q][t][0], x[q][t][1]));
+        s3 = ptx::add2(s3, ptx::add2(x[q][t][2], x[q][t][3]));
       }
-      ptx::sts128(row + ((cl ^ sw) << 4), y[0], y[1], y[2], y[3]);
+      float slo, shi;
+      ptx::upk2(ptx::add2(s2, s3), slo, shi);
+      sum[q] = slo + shi;
+    }
+#pragma unroll
+    for (int q = 0; q < 2; ++q) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], 1);
+#pragma unroll
+    for (int q = 0; q < 2; ++q) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], 2);
+    float var[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      mu[q] = sum[q] * (1.0f / 128.0f);
+      const ptx::f32x2 nmu = ptx::pk2(-mu[q], -mu[q]);
+      ptx::f32x2 v2 = ptx::pk2(0.f, 0.f), v3 = v2;
+#pragma unroll
+      for (int t = 0; t < 4; ++t)
+#pragma unroll
+        for (int e = 0; e < 4; e += 2) {
+          const ptx::f32x2 d0 = ptx::add2(x[q][t][e], nmu), d1 = ptx::add2(x[q][t][e + 1], nmu);
+          v2 = ptx::fma2(d0, d0, v2);
+          v3 = ptx::fma2(d1, d1, v3);
+        }
+      float slo, shi;
+      ptx::upk2(ptx::add2(v2, v3), slo, shi);
+      var[q] = slo + shi;
+    }
+#pragma unroll
+    for (int q = 0; q < 2; ++q) var[q] += __shfl_xor_sync(0xffffffffu, var[q], 1);
+#pragma unroll
+    for (int q = 0; q < 2; ++q) var[q] += __shfl_xor_sync(0xffffffffu, var[q], 2);
+    ptx::f32x2 rs2[2], nmr2[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      rstd[q] = rsqrtf(var[q] * (1.0f / 128.0f) + eps);
+      rs2[q] = ptx::pk2(rstd[q], rstd[q]);
+      const float nmr = -mu[q] * rstd[q];
+      nmr2[q] = ptx::pk2(nmr, nmr);
+    }
+#pragma unroll
+    for (uint32_t t = 0; t < 4; ++t) {
+      const uint32_t tt = t ^ j;
+      const uint32_t voff = (32u * j + 8u * tt) * 4u;       // byte offset of this chunk's gamma/beta
+      ptx::f32x2 g[4], b[4];
+      ptx::lds128x2(gaddr + voff, *reinterpret_cast<ptx::f32x2(*)[2]>(&g[0]));
+      ptx::lds128x2(gaddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&g[2]));
+      ptx::lds128x2(baddr + voff, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[0]));
+      ptx::lds128x2(baddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[2]));
+#pragma unroll
+      for (uint32_t q = 0; q < 2; ++q) {
+        uint32_t y[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          y[e] = ptx::pack_norm2<kF16>(
+              ptx::fma2(ptx::fma2(x[q][t][e], rs2[q], nmr2[q]), g[e], b[e]));
+        ptx::sts128(row0 + q * 4096u + (((cbase + tt) ^ sw) << 4), y[0], y[1], y[2], y[3]);
+      }
     }
   }
 }
