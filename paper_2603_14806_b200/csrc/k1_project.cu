@@ -14,17 +14,25 @@
 // contiguous run of the channel-major output -- and the projection and its gate for the same
 // (channel, pair) sit in the same thread (two accumulators, same lane, same column).
 //
+// With the weights as the A operand they can live in TENSOR MEMORY for the whole kernel
+// (tcgen05.mma with A from TMEM): 4 matrices x 64 columns = half of TMEM, no shared memory and
+// no shared-memory operand traffic for them.  The LayerNorm affine is folded into them once per
+// CTA:  W z' + b = (W diag(gamma)) n + (W beta + b),  n = (z - mean) * rstd,  so the LayerNorm
+// warps only normalise.  W diag(gamma) is rounded to fp16 (2^-12 relative; n is fp16 too -- see
+// common.h kNormFp16), the folded bias stays fp32 in registers.
+//
 // Persistent kernel, one CTA per SM, 16 warps, tile = 128 pairs:
-//   warp 0       TMA producer : weights once (4 x 32 KB, resident), then z tiles into a 2-deep ring
-//   warp 1       MMA issuer   : per tile two "units" (a, b), each = projection + gate MMA
-//                               (M=128 ch, N=128 pairs, K=128) into one 256-column TMEM slot
-//   warp 2       TMEM allocator (512 columns = 2 slots; the epilogue of unit a overlaps the
-//                               MMAs of unit b and vice versa)
-//   warps 4-7    LayerNorm    : ln_rows.cuh -- z rows (bf16, 128-byte-swizzled TMA tile) ->
-//                               registers -> two-pass mean/variance in fp32 -> z' written back in
-//                               place as the K-major B operand; also stages the pair mask
+//   warp 0       TMA producer : z tiles into a kZStages-deep ring
+//   warp 1       MMA issuer   : per tile four "units" (pair half hh, tensor u in {a, b}); a unit =
+//                               projection + gate MMA (M=128 ch, N=64 pairs, K=128) into one
+//                               128-column TMEM slot; two slots, so the epilogue of one unit
+//                               overlaps the MMAs of the next
+//   warp 2       TMEM allocator (512 columns: 256 weights + 2 x 128 accumulators)
+//   warps 4-7    LayerNorm    : ln_rows.cuh -- z rows -> registers -> two-pass mean/variance in
+//                               fp32 -> n written back in place as the K-major B operand; also
+//                               stages the pair mask and an "all ones" flag per tile
 //   warps 8-15   epilogue     : tcgen05.ld both accumulators -> bias, sigmoid, gate, mask in
-//                               fp32 -> bf16 -> swizzled smem -> TMA store [128 ch][64 pairs]
+//                               packed fp32 -> bf16 -> swizzled smem -> TMA store [128 ch][64 pairs]
 #include <cuda_bf16.h>
 
 #include "common.h"
@@ -38,25 +46,28 @@ constexpr int kC = kChannels;                   // 128
 constexpr int kTilePairs = 128;
 constexpr int kThreads = 512;
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box, 128 rows x 64 bf16
-constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 bf16 operand (two k-halves)
-constexpr int kZStages = 2;
-constexpr int kMaskSlots = 3;
+constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 16-bit tile (two k-halves)
+constexpr int kZStages = 4;
+constexpr int kMaskSlots = 8;                   // >= kZStages + 2 (see the epilogue), power of 2
+constexpr int kOutBufs = 4;                     // staging buffers [128 ch][64 pairs], one per unit
 
-constexpr int kOffW = 0;                                  // 4 weight matrices
-constexpr int kOffZ = kOffW + 4 * kMatBytes;              // z ring
-constexpr int kOffOut = kOffZ + kZStages * kMatBytes;     // 2 staging buffers [128 ch][64 pairs]
-constexpr int kOffGamma = kOffOut + 2 * kHalfBox;
-constexpr int kOffBeta = kOffGamma + kC * 4;
-constexpr int kOffMask = kOffBeta + kC * 4;
-constexpr int kOffBar = kOffMask + kMaskSlots * kTilePairs * 4;
-constexpr int kSmemBytes = kOffBar + 128;
+constexpr int kOffZ = 0;                                   // z ring
+constexpr int kOffOut = kOffZ + kZStages * kMatBytes;      // staging buffers
+constexpr int kOffMask = kOffOut + kOutBufs * kHalfBox;    // fp32 pair mask per tile slot
+constexpr int kOffFlag = kOffMask + kMaskSlots * kTilePairs * 4;   // 4 "all ones" words per slot
+constexpr int kOffBar = kOffFlag + kMaskSlots * 16;
+constexpr int kSmemBytes = kOffBar + 256;
 static_assert(kSmemBytes <= 232448, "K1 shared memory exceeds 227 KB");
+
+constexpr int kTmemW = 0;        // columns 0..255: four weight matrices, 64 columns each
+constexpr int kTmemAcc = 256;    // columns 256..511: two slots of (projection 64 | gate 64)
 
 struct K1Params {
   const __nv_bfloat16* mask;   // [R] or nullptr
+  const __nv_bfloat16* w[4];   // W_a, W_ga, W_b, W_gb: [128][128] row-major
+  const float* bias[4];        // b_a, b_ga, b_b, b_gb (each may be nullptr)
   const float* gamma;
   const float* beta;
-  const float* bias[4];        // b_a, b_ga, b_b, b_gb (each may be nullptr)
   float eps;
   long long R;                 // number of pairs
   int num_tiles;
@@ -65,10 +76,6 @@ struct K1Params {
 template <bool kTanhSigmoid>
 __global__ void __launch_bounds__(kThreads, 1)
 k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
-                  const __grid_constant__ CUtensorMap tmap_w0,
-                  const __grid_constant__ CUtensorMap tmap_w1,
-                  const __grid_constant__ CUtensorMap tmap_w2,
-                  const __grid_constant__ CUtensorMap tmap_w3,
                   const __grid_constant__ CUtensorMap tmap_a,
                   const __grid_constant__ CUtensorMap tmap_b, const K1Params prm) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -76,13 +83,13 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   if ((smem & 1023u) != 0) __trap();   // 128-byte swizzle needs 1024-byte aligned tiles
 
   const uint32_t bar = smem + kOffBar;
-  const uint32_t wfull = bar;
-  auto zfull = [&](int s) { return bar + 8u * (1 + s); };
-  auto zempty = [&](int s) { return bar + 8u * (3 + s); };
-  auto zready = [&](int s) { return bar + 8u * (5 + s); };
-  auto tfull = [&](int u) { return bar + 8u * (7 + u); };
-  auto tempty = [&](int u) { return bar + 8u * (9 + u); };
-  const uint32_t tmem_slot = bar + 8u * 11;
+  auto zfull = [&](int s) { return bar + 8u * s; };
+  auto zempty = [&](int s) { return bar + 8u * (kZStages + s); };
+  auto zready = [&](int s) { return bar + 8u * (2 * kZStages + s); };
+  auto tfull = [&](int u) { return bar + 8u * (3 * kZStages + u); };
+  auto tempty = [&](int u) { return bar + 8u * (3 * kZStages + 2 + u); };
+  const uint32_t tmem_slot = bar + 8u * (3 * kZStages + 4);
+  const uint32_t wready = bar + 8u * (3 * kZStages + 5);   // weights are in TMEM
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -93,7 +100,6 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::prefetch_tmap(&tmap_b);
   }
   if (warp == 1 && lane == 0) {
-    ptx::mbar_init(wfull, 1);
     for (int s = 0; s < kZStages; ++s) {
       ptx::mbar_init(zfull(s), 1);
       ptx::mbar_init(zempty(s), 1);
@@ -103,52 +109,26 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_init(tfull(u), 1);
       ptx::mbar_init(tempty(u), 8);
     }
+    ptx::mbar_init(wready, 8);
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
-  if (warp == 3) {
-    float* g = reinterpret_cast<float*>(smem_raw + kOffGamma);
-    float* b = reinterpret_cast<float*>(smem_raw + kOffBeta);
-    for (int c = lane; c < kC; c += 32) {
-      g[c] = prm.gamma[c];
-      b[c] = prm.beta[c];
-    }
-  }
   ptx::tc_fence_before();
   __syncthreads();
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-  // weights: loaded once per CTA, resident for the whole kernel
-  if (warp == 0 && ptx::elect_one()) {
-    ptx::mbar_arrive_expect_tx(wfull, 4 * kMatBytes);
-    const CUtensorMap* wm[4] = {&tmap_w0, &tmap_w1, &tmap_w2, &tmap_w3};
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-      ptx::tma_load_2d(smem + kOffW + m * kMatBytes, wm[m], wfull, 0, 0);
-      ptx::tma_load_2d(smem + kOffW + m * kMatBytes + kHalfBox, wm[m], wfull, 64, 0);
-    }
-  }
-  if constexpr (kNormFp16) {
-    // kind::f16 needs A and B in the same 16-bit format: the bf16 weights become fp16 in place
-    ptx::mbar_wait(wfull, 0);
-    ptx::smem_bf16_to_f16_inplace(smem + kOffW, 4 * kMatBytes, threadIdx.x, kThreads);
-    ptx::fence_proxy_async_smem();
-    __syncthreads();
-  }
-
   const int first = blockIdx.x;
   const int stride = gridDim.x;
-
 
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
-        const int s = it & 1;
-        ptx::mbar_wait(zempty(s), ((it >> 1) & 1) ^ 1u);
+        const int s = it % kZStages;
+        ptx::mbar_wait(zempty(s), ((it / kZStages) & 1) ^ 1u);
         ptx::mbar_arrive_expect_tx(zfull(s), kMatBytes);
         const uint32_t dst = smem + kOffZ + s * kMatBytes;
         const int row0 = t * kTilePairs;          // < 2^31: R <= 2^30 (N <= 32768)
@@ -159,41 +139,44 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (ptx::elect_one()) {
-      // A = weights, B = z', both K-major, both fp16 (or both bf16)
+      // A = folded weights in TMEM, B = n (K-major, 64 pairs), both fp16 (or both bf16)
       constexpr uint32_t kFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
-      constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, kTilePairs, kFmt, kFmt, 0, 0);
-      ptx::mbar_wait(wfull, 0);
+      constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, 64, kFmt, kFmt, 0, 0);
+      ptx::mbar_wait(wready, 0);
+      ptx::tc_fence_after();
       int it = 0;
+      uint32_t n = 0;   // unit counter
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
-        const int s = it & 1;
-        ptx::mbar_wait(zready(s), (it >> 1) & 1);
+        const int s = it % kZStages;
+        ptx::mbar_wait(zready(s), (it / kZStages) & 1);
         ptx::tc_fence_after();
         const uint32_t zb = smem + kOffZ + s * kMatBytes;
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          ptx::mbar_wait(tempty(u), (it & 1) ^ 1u);
+        for (int idx = 0; idx < 4; ++idx, ++n) {
+          const int hh = idx >> 1, u = idx & 1;
+          const uint32_t slot = n & 1u;
+          ptx::mbar_wait(tempty(slot), ((n >> 1) & 1u) ^ 1u);
           ptx::tc_fence_after();
 #pragma unroll
           for (int m2 = 0; m2 < 2; ++m2) {
-            const uint32_t wa = smem + kOffW + (2 * u + m2) * kMatBytes;
-            const uint32_t d_tmem = tmem_base + u * 256 + m2 * 128;
+            const uint32_t a_tmem = tmem_base + kTmemW + (2 * u + m2) * 64;
+            const uint32_t d_tmem = tmem_base + kTmemAcc + slot * 128 + m2 * 64;
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-              const uint32_t off = (k >> 2) * kHalfBox + (k & 3) * 32;
-              const uint64_t da = ptx::make_smem_desc_sw128(wa + off, 16, 1024);
+              // rows hh*64.. of the tile: 64 rows x 128 B = 8 KB into each k-half box
+              const uint32_t off = hh * 8192 + (k >> 2) * kHalfBox + (k & 3) * 32;
               const uint64_t db = ptx::make_smem_desc_sw128(zb + off, 16, 1024);
-              ptx::umma_bf16<1>(d_tmem, da, db, idesc, k != 0 ? 1u : 0u);
+              ptx::umma_f16_ts(d_tmem, a_tmem + k * 8, db, idesc, k != 0 ? 1u : 0u);
             }
           }
-          ptx::umma_commit<1>(tfull(u));
+          ptx::umma_commit<1>(tfull(slot));
         }
-        ptx::umma_commit<1>(zempty(s));   // z' stage reusable once all four MMAs retired
+        ptx::umma_commit<1>(zempty(s));   // stage reusable once all eight MMAs retired
       }
     }
   } else if (warp >= 4 && warp < 8) {
-    // ===================== LayerNorm (thread = pair) =====================
+    // ===================== LayerNorm =====================
     const int r = threadIdx.x - 128;
-    const uint32_t gaddr = smem + kOffGamma, baddr = smem + kOffBeta;
     // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
     auto load_mask = [&](int t) -> unsigned short {
       if (prm.mask == nullptr) return static_cast<unsigned short>(0x3f80);   // bf16 1.0
@@ -205,113 +188,175 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     unsigned short mnext = load_mask(first);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
-      const int s = it & 1;
+      const int s = it % kZStages;
       const unsigned short mraw = mnext;
       mnext = load_mask(t + stride);
-      ptx::mbar_wait(zfull(s), (it >> 1) & 1);
-      layernorm_rows_inplace<kNormFp16>(smem + kOffZ + s * kMatBytes, kHalfBox, r, gaddr, baddr, prm.eps);
-      reinterpret_cast<float*>(smem_raw + kOffMask)[(it % kMaskSlots) * kTilePairs + r] =
+      ptx::mbar_wait(zfull(s), (it / kZStages) & 1);
+      layernorm_rows_inplace<kNormFp16, false>(smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0,
+                                               prm.eps);
+      const int ms = it & (kMaskSlots - 1);
+      reinterpret_cast<float*>(smem_raw + kOffMask)[ms * kTilePairs + r] =
           __uint_as_float(static_cast<uint32_t>(mraw) << 16);
+      const bool ones = __all_sync(0xffffffffu, mraw == 0x3f80);
+      if (lane == 0)
+        reinterpret_cast<uint32_t*>(smem_raw + kOffFlag)[ms * 4 + (warp - 4)] = ones ? 1u : 0u;
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
   } else if (warp >= 8) {
     // ===================== epilogue =====================
-    // warp -> TMEM lane quadrant q (hardware rule: warp % 4) and column half h (64 pairs)
+    // warp -> TMEM lane quadrant q (hardware rule: warp % 4) and column half h (32 of a unit's 64)
     const int q = warp & 3;
     const int h = (warp - 8) >> 2;
     const int ch = q * 32 + lane;                       // output channel = TMEM lane
-    const uint32_t stage_buf = smem + kOffOut + h * kHalfBox;
-    const uint32_t row_addr = stage_buf + ch * 128;
-    const uint32_t sw = static_cast<uint32_t>(ch & 7);
-    const bool store_thread = (q == 0 && lane == 0);
-    const uint32_t bar_id = 1 + h;
+    const uint32_t lane_base = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
     constexpr float kLog2e = 1.4426950408889634f;
-    // packed fp32x2 constants: sigmoid(x) = 0.5 tanh(0.5 x) + 0.5  or  1 / (1 + 2^(-x log2 e))
+    // sigmoid(x) = 0.5 tanh(0.5 x) + 0.5   or   1 / (1 + 2^(-x log2 e))
     constexpr float kGateScale = kTanhSigmoid ? 0.5f : -kLog2e;
+
+    // ---- once per CTA: fold the LayerNorm affine into the weights, park them in TMEM ----
+    // every thread computes its channel's four folded biases  W beta + b ; warps 8-11 store
+    // W_a, W_ga and warps 12-15 store W_b, W_gb as  W diag(gamma)  (row ch -> TMEM lane ch)
+    float fb[4];
+#pragma unroll 1
+    for (int m = 0; m < 4; ++m) {
+      const uint4* wrow = reinterpret_cast<const uint4*>(prm.w[m] + static_cast<size_t>(ch) * kC);
+      const bool mine = (m >> 1) == h;
+      float acc = 0.f;
+#pragma unroll 1
+      for (int half = 0; half < 2; ++half) {
+        uint32_t packed[32];
+#pragma unroll
+        for (int kc = 0; kc < 8; ++kc) {
+          const int k0 = half * 64 + kc * 8;
+          const uint4 wv = __ldg(wrow + half * 8 + kc);
+          const float4 g0 = __ldg(reinterpret_cast<const float4*>(prm.gamma + k0));
+          const float4 g1 = __ldg(reinterpret_cast<const float4*>(prm.gamma + k0 + 4));
+          const float4 b0 = __ldg(reinterpret_cast<const float4*>(prm.beta + k0));
+          const float4 b1 = __ldg(reinterpret_cast<const float4*>(prm.beta + k0 + 4));
+          const uint32_t ww[4] = {wv.x, wv.y, wv.z, wv.w};
+          const float gg[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+          const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float lo = ptx::bf16_lo(ww[e]), hi = ptx::bf16_hi(ww[e]);
+            acc = fmaf(lo, bb[2 * e], acc);
+            acc = fmaf(hi, bb[2 * e + 1], acc);
+            packed[kc * 4 + e] = ptx::pack_norm<kNormFp16>(lo * gg[2 * e], hi * gg[2 * e + 1]);
+          }
+        }
+        if (mine) ptx::tmem_st_32x32(lane_base + kTmemW + m * 64 + half * 32, packed);
+      }
+      fb[m] = acc + (prm.bias[m] ? prm.bias[m][ch] : 0.f);
+    }
+    ptx::tmem_st_wait();
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(wready);
+
+    ptx::f32x2 bias_p2[2], bias_g2[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      bias_p2[u] = ptx::pk2(fb[2 * u], fb[2 * u]);
+      bias_g2[u] = ptx::pk2(kGateScale * fb[2 * u + 1], kGateScale * fb[2 * u + 1]);
+    }
     const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
     const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
     (void)half2;
     (void)one2;
-    ptx::f32x2 bias_p2[2], bias_g2[2];
+
+    const uint32_t sw = static_cast<uint32_t>(ch & 7);
+    const bool store_thread = (warp == 8 && lane == 0);
+
+    // one 16-column chunk: bias, sigmoid gate, (mask), bf16 pack
+    auto compute_chunk = [&](const uint32_t (&vp)[16], const uint32_t (&vg)[16], int u,
+                             uint32_t maddr, bool masked, uint32_t (&packed)[8]) {
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      const float bp = prm.bias[2 * u] ? prm.bias[2 * u][ch] : 0.f;
-      const float bg = kGateScale * (prm.bias[2 * u + 1] ? prm.bias[2 * u + 1][ch] : 0.f);
-      bias_p2[u] = ptx::pk2(bp, bp);
-      bias_g2[u] = ptx::pk2(bg, bg);
-    }
+      for (int j4 = 0; j4 < 4; ++j4) {
+        ptx::f32x2 m2[2];
+        if (masked) ptx::lds128x2(maddr + j4 * 16, m2);
+#pragma unroll
+        for (int e2 = 0; e2 < 2; ++e2) {
+          const int j = j4 * 4 + e2 * 2;
+          ptx::f32x2 pj = ptx::add2(ptx::pk2u(vp[j], vp[j + 1]), bias_p2[u]);
+          const ptx::f32x2 gx = ptx::fma2(ptx::pk2u(vg[j], vg[j + 1]), gscale2, bias_g2[u]);
+          float g0, g1;
+          ptx::upk2(gx, g0, g1);
+          ptx::f32x2 sg;
+          if constexpr (kTanhSigmoid) {
+            sg = ptx::fma2(ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), half2, half2);
+          } else {
+            float d0, d1;
+            ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
+            sg = ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1));
+          }
+          if (masked) pj = ptx::mul2(pj, m2[e2]);
+          float v0, v1;
+          ptx::upk2(ptx::mul2(pj, sg), v0, v1);
+          packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
+        }
+      }
+    };
+
     int it = 0;
+    uint32_t n = 0;   // unit counter (same sequence as the MMA issuer's)
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
-      const uint32_t mask_addr =
-          smem + kOffMask + ((it % kMaskSlots) * kTilePairs + h * 64) * 4;
-      const int p0 = t * kTilePairs + h * 64;
+      const int ms = it & (kMaskSlots - 1);
+      bool masked = true;
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        ptx::mbar_wait(tfull(u), it & 1);
+      for (int idx = 0; idx < 4; ++idx, ++n) {
+        const int hh = idx >> 1, u = idx & 1;
+        const uint32_t slot = n & 1u;
+        const uint32_t buf = smem + kOffOut + (n & (kOutBufs - 1)) * kHalfBox;
+        ptx::mbar_wait(tfull(slot), (n >> 1) & 1u);
         ptx::tc_fence_after();
-        const uint32_t taddr =
-            tmem_base + (static_cast<uint32_t>(q * 32) << 16) + u * 256 + h * 64;
-        // 64 columns per warp and unit, in four chunks of 16; the tcgen05.ld of chunk c+1 is in
-        // flight while chunk c is being computed (two register buffers)
+        if (idx == 0) {
+          // written by the LayerNorm warps before zready, hence visible after this tile's tfull
+          uint32_t f[4];
+          ptx::lds128(smem + kOffFlag + ms * 16, f);
+          masked = (f[0] & f[1] & f[2] & f[3]) == 0u;   // warp-uniform
+        }
+        const uint32_t taddr = lane_base + kTmemAcc + slot * 128 + h * 32;
+        const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + hh * 64 + h * 32) * 4;
+        const uint32_t row_addr = buf + ch * 128;
+        // 32 columns per warp and unit in two chunks of 16; the tcgen05.ld of the second chunk is
+        // in flight while the first is being computed
         uint32_t vp[2][16], vg[2][16];
         ptx::tmem_ld_32x16(taddr, vp[0]);
-        ptx::tmem_ld_32x16(taddr + 128, vg[0]);
+        ptx::tmem_ld_32x16(taddr + 64, vg[0]);
 #pragma unroll
-        for (int chunk = 0; chunk < 4; ++chunk) {
-          const int cb = chunk & 1;
+        for (int c = 0; c < 2; ++c) {
           ptx::tmem_ld_wait();
-          if (chunk < 3) {
-            ptx::tmem_ld_32x16(taddr + (chunk + 1) * 16, vp[cb ^ 1]);
-            ptx::tmem_ld_32x16(taddr + 128 + (chunk + 1) * 16, vg[cb ^ 1]);
+          if (c == 0) {
+            ptx::tmem_ld_32x16(taddr + 16, vp[1]);
+            ptx::tmem_ld_32x16(taddr + 64 + 16, vg[1]);
           }
           uint32_t packed[8];
-#pragma unroll
-          for (int j4 = 0; j4 < 4; ++j4) {
-            ptx::f32x2 m2[2];
-            ptx::lds128x2(mask_addr + (chunk * 16 + j4 * 4) * 4, m2);
-#pragma unroll
-            for (int e2 = 0; e2 < 2; ++e2) {
-              const int j = j4 * 4 + e2 * 2;
-              const ptx::f32x2 pj = ptx::add2(ptx::pk2u(vp[cb][j], vp[cb][j + 1]), bias_p2[u]);
-              const ptx::f32x2 gx =
-                  ptx::fma2(ptx::pk2u(vg[cb][j], vg[cb][j + 1]), gscale2, bias_g2[u]);
-              float g0, g1;
-              ptx::upk2(gx, g0, g1);
-              ptx::f32x2 sg;
-              if constexpr (kTanhSigmoid) {
-                sg = ptx::fma2(ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), half2, half2);
-              } else {
-                float d0, d1;
-                ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
-                sg = ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1));
-              }
-              float v0, v1;
-              ptx::upk2(ptx::mul2(ptx::mul2(pj, m2[e2]), sg), v0, v1);
-              packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
-            }
+          if (masked) {
+            compute_chunk(vp[c], vg[c], u, maddr + c * 64, true, packed);
+          } else {
+            compute_chunk(vp[c], vg[c], u, maddr + c * 64, false, packed);
           }
-          if (chunk == 3) {
+          if (c == 1) {
             // accumulators and mask slot fully consumed: hand the TMEM slot back to the issuer
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(tempty(u));
+            if (lane == 0) ptx::mbar_arrive(tempty(slot));
           }
-          if (chunk == 0) {
-            // the previous unit's TMA store must have finished reading the staging buffer
-            if (store_thread) ptx::tma_store_wait_read<0>();
-            ptx::named_bar_sync(bar_id, 128);
-          }
-          ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2) ^ sw) << 4), packed[0],
-                      packed[1], packed[2], packed[3]);
-          ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2 + 1) ^ sw) << 4), packed[4],
-                      packed[5], packed[6], packed[7]);
+          // staging buffer n % 4 is free: the store thread waited for store n-4 (see below)
+          const uint32_t c16 = static_cast<uint32_t>(h * 4 + c * 2);
+          ptx::sts128(row_addr + ((c16 ^ sw) << 4), packed[0], packed[1], packed[2], packed[3]);
+          ptx::sts128(row_addr + (((c16 + 1) ^ sw) << 4), packed[4], packed[5], packed[6],
+                      packed[7]);
         }
         ptx::fence_proxy_async_smem();
-        ptx::named_bar_sync(bar_id, 128);
+        ptx::named_bar_sync(1, 256);
         if (store_thread) {
-          ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, stage_buf, p0, 0);
+          ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + hh * 64, 0);
           ptx::tma_store_commit();
+          // at most this store and the previous one may still be reading shared memory when the
+          // store thread reaches the next barrier => buffer (n+2) % 4 is free for unit n+2
+          ptx::tma_store_wait_read<2>();
         }
       }
     }
@@ -339,22 +384,13 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   const uint64_t R = static_cast<uint64_t>(N) * N;
-  CUtensorMap tz, tw[4], ta, tb;
+  CUtensorMap tz, ta, tb;
   int st;
   {
     const uint64_t dims[2] = {kC, R};
     const uint64_t strides[1] = {kC * 2};
     const uint32_t box[2] = {64, 128};
     if ((st = encode_tensor_map(&tz, z, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
-  }
-  {
-    const uint64_t dims[2] = {kC, kC};
-    const uint64_t strides[1] = {kC * 2};
-    const uint32_t box[2] = {64, 128};
-    const void* w[4] = {p->w_a, p->w_a_gate, p->w_b, p->w_b_gate};
-    for (int m = 0; m < 4; ++m)
-      if ((st = encode_tensor_map(&tw[m], w[m], 2, 2, dims, strides, box, true)) != FOLDCP_OK)
-        return st;
   }
   {
     const uint64_t dims[2] = {R, kC};
@@ -365,12 +401,16 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   }
   K1Params prm;
   prm.mask = static_cast<const __nv_bfloat16*>(mask);
-  prm.gamma = p->ln_in_gamma;
-  prm.beta = p->ln_in_beta;
+  prm.w[0] = static_cast<const __nv_bfloat16*>(p->w_a);
+  prm.w[1] = static_cast<const __nv_bfloat16*>(p->w_a_gate);
+  prm.w[2] = static_cast<const __nv_bfloat16*>(p->w_b);
+  prm.w[3] = static_cast<const __nv_bfloat16*>(p->w_b_gate);
   prm.bias[0] = p->b_a;
   prm.bias[1] = p->b_a_gate;
   prm.bias[2] = p->b_b;
   prm.bias[3] = p->b_b_gate;
+  prm.gamma = p->ln_in_gamma;
+  prm.beta = p->ln_in_beta;
   prm.eps = p->ln_eps;
   prm.R = static_cast<long long>(R);
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
@@ -384,7 +424,7 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
       return FOLDCP_ERR_CUDA;
     attr_set[tanh_sig] = true;
   }
-  kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, tw[0], tw[1], tw[2], tw[3], ta, tb, prm);
+  kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, ta, tb, prm);
   return check_launch();
 }
 

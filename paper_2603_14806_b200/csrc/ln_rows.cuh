@@ -19,7 +19,9 @@ namespace foldcp {
 // tile  : shared address of box 0 (box 1 is box_stride bytes further)
 // tid   : 0..127 within the LayerNorm warp group
 // gaddr / baddr : shared addresses of gamma[128] / beta[128] (fp32)
-template <bool kF16>
+// kAffine = false: plain normalisation (x - mean) * rstd; gamma / beta are then folded into the
+// weights and biases of the GEMM that consumes the tile (gaddr / baddr unused).
+template <bool kF16, bool kAffine = true>
 __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t box_stride, int tid,
                                                        uint32_t gaddr, uint32_t baddr, float eps) {
   const uint32_t j = static_cast<uint32_t>(tid & 3);        // quarter of the row: channels 32j..
@@ -98,17 +100,21 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
       const uint32_t tt = t ^ j;
       const uint32_t voff = (32u * j + 8u * tt) * 4u;       // byte offset of this chunk's gamma/beta
       ptx::f32x2 g[4], b[4];
-      ptx::lds128x2(gaddr + voff, *reinterpret_cast<ptx::f32x2(*)[2]>(&g[0]));
-      ptx::lds128x2(gaddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&g[2]));
-      ptx::lds128x2(baddr + voff, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[0]));
-      ptx::lds128x2(baddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[2]));
+      if constexpr (kAffine) {
+        ptx::lds128x2(gaddr + voff, *reinterpret_cast<ptx::f32x2(*)[2]>(&g[0]));
+        ptx::lds128x2(gaddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&g[2]));
+        ptx::lds128x2(baddr + voff, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[0]));
+        ptx::lds128x2(baddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[2]));
+      }
 #pragma unroll
       for (uint32_t q = 0; q < 2; ++q) {
         uint32_t y[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e)
-          y[e] = ptx::pack_norm2<kF16>(
-              ptx::fma2(ptx::fma2(x[q][t][e], rs2[q], nmr2[q]), g[e], b[e]));
+        for (int e = 0; e < 4; ++e) {
+          ptx::f32x2 n = ptx::fma2(x[q][t][e], rs2[q], nmr2[q]);
+          if constexpr (kAffine) n = ptx::fma2(n, g[e], b[e]);
+          y[e] = ptx::pack_norm2<kF16>(n);
+        }
         ptx::sts128(row0 + q * 4096u + (((cbase + tt) ^ sw) << 4), y[0], y[1], y[2], y[3]);
       }
     }
