@@ -31,8 +31,10 @@
 //   warps 4-7    LayerNorm    : ln_rows.cuh -- z rows -> registers -> two-pass mean/variance in
 //                               fp32 -> n written back in place as the K-major B operand; also
 //                               stages the pair mask and an "all ones" flag per tile
-//   warps 8-15   epilogue     : tcgen05.ld both accumulators -> bias, sigmoid, gate, mask in
-//                               packed fp32 -> bf16 -> swizzled smem -> TMA store [128 ch][64 pairs]
+//   warps 8-15   epilogue     : two independent teams of four warps (team 0 = tensor a / TMEM slot
+//                               0, team 1 = b / slot 1): tcgen05.ld both accumulators -> bias,
+//                               sigmoid, gate, mask in packed fp32 -> bf16 -> swizzled smem ->
+//                               TMA store [128 ch][64 pairs]
 #include <cuda_bf16.h>
 
 #include "common.h"
@@ -107,7 +109,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     }
     for (int u = 0; u < 2; ++u) {
       ptx::mbar_init(tfull(u), 1);
-      ptx::mbar_init(tempty(u), 8);
+      ptx::mbar_init(tempty(u), 4);
     }
     ptx::mbar_init(wready, 8);
     ptx::fence_mbar_init();
@@ -254,23 +256,19 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     __syncwarp();
     if (lane == 0) ptx::mbar_arrive(wready);
 
-    ptx::f32x2 bias_p2[2], bias_g2[2];
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      bias_p2[u] = ptx::pk2(fb[2 * u], fb[2 * u]);
-      bias_g2[u] = ptx::pk2(kGateScale * fb[2 * u + 1], kGateScale * fb[2 * u + 1]);
-    }
+    // this thread's team handles tensor h only (a: matrices 0, 1; b: matrices 2, 3)
+    const float fbp = h ? fb[2] : fb[0], fbg = kGateScale * (h ? fb[3] : fb[1]);
+    const ptx::f32x2 bias_p2 = ptx::pk2(fbp, fbp), bias_g2 = ptx::pk2(fbg, fbg);
     const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
     const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
     (void)half2;
     (void)one2;
 
     const uint32_t sw = static_cast<uint32_t>(ch & 7);
-    const bool store_thread = (warp == 8 && lane == 0);
+    const bool store_thread = (q == 0 && lane == 0);   // one per team
 
     // one 16-column chunk: bias, sigmoid gate, (mask), bf16 pack
-    auto compute_chunk = [&](const uint32_t (&vp)[16], const uint32_t (&vg)[16], int u,
-                             uint32_t maddr, bool masked, uint32_t (&packed)[8]) {
+    auto compute_chunk = [&](const uint32_t (&vp)[16], const uint32_t (&vg)[16], uint32_t maddr, bool masked, uint32_t (&packed)[8]) {
 #pragma unroll
       for (int j4 = 0; j4 < 4; ++j4) {
         ptx::f32x2 m2[2];
@@ -278,8 +276,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
 #pragma unroll
         for (int e2 = 0; e2 < 2; ++e2) {
           const int j = j4 * 4 + e2 * 2;
-          ptx::f32x2 pj = ptx::add2(ptx::pk2u(vp[j], vp[j + 1]), bias_p2[u]);
-          const ptx::f32x2 gx = ptx::fma2(ptx::pk2u(vg[j], vg[j + 1]), gscale2, bias_g2[u]);
+          ptx::f32x2 pj = ptx::add2(ptx::pk2u(vp[j], vp[j + 1]), bias_p2);
+          const ptx::f32x2 gx = ptx::fma2(ptx::pk2u(vg[j], vg[j + 1]), gscale2, bias_g2);
           float g0, g1;
           ptx::upk2(gx, g0, g1);
           ptx::f32x2 sg;
@@ -298,65 +296,73 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       }
     };
 
+    // Team h (four warps, one per lane quadrant) owns TMEM slot h and therefore tensor u = h
+    // (a for team 0, b for team 1): per tile it handles the two pair halves hh = 0, 1.  The two
+    // teams run independently (own barrier, own store thread, own staging buffers), so the fixed
+    // latencies of one team's unit (mbarrier wake-up, tcgen05.ld, fence, barrier) overlap the
+    // other team's arithmetic.
+    const int u = h;
+    const uint32_t slot = static_cast<uint32_t>(h);
+    const uint32_t bar_id = 1 + h;
     int it = 0;
-    uint32_t n = 0;   // unit counter (same sequence as the MMA issuer's)
+    uint32_t c = 0;   // this team's unit counter
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int ms = it & (kMaskSlots - 1);
       bool masked = true;
 #pragma unroll
-      for (int idx = 0; idx < 4; ++idx, ++n) {
-        const int hh = idx >> 1, u = idx & 1;
-        const uint32_t slot = n & 1u;
-        const uint32_t buf = smem + kOffOut + (n & (kOutBufs - 1)) * kHalfBox;
-        ptx::mbar_wait(tfull(slot), (n >> 1) & 1u);
+      for (int hh = 0; hh < 2; ++hh, ++c) {
+        const uint32_t buf = smem + kOffOut + (2 * h + (c & 1u)) * kHalfBox;
+        ptx::mbar_wait(tfull(slot), c & 1u);
         ptx::tc_fence_after();
-        if (idx == 0) {
+        if (hh == 0) {
           // written by the LayerNorm warps before zready, hence visible after this tile's tfull
           uint32_t f[4];
           ptx::lds128(smem + kOffFlag + ms * 16, f);
           masked = (f[0] & f[1] & f[2] & f[3]) == 0u;   // warp-uniform
         }
-        const uint32_t taddr = lane_base + kTmemAcc + slot * 128 + h * 32;
-        const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + hh * 64 + h * 32) * 4;
+        const uint32_t taddr = lane_base + kTmemAcc + slot * 128;
+        const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + hh * 64) * 4;
         const uint32_t row_addr = buf + ch * 128;
-        // 32 columns per warp and unit in two chunks of 16; the tcgen05.ld of the second chunk is
-        // in flight while the first is being computed
+        // 64 columns in four chunks of 16; the tcgen05.ld of chunk k+1 is in flight while chunk
+        // k is being computed (two register buffers)
         uint32_t vp[2][16], vg[2][16];
         ptx::tmem_ld_32x16(taddr, vp[0]);
         ptx::tmem_ld_32x16(taddr + 64, vg[0]);
 #pragma unroll
-        for (int c = 0; c < 2; ++c) {
+        for (int k = 0; k < 4; ++k) {
+          const int cb = k & 1;
           ptx::tmem_ld_wait();
-          if (c == 0) {
-            ptx::tmem_ld_32x16(taddr + 16, vp[1]);
-            ptx::tmem_ld_32x16(taddr + 64 + 16, vg[1]);
+          if (k < 3) {
+            ptx::tmem_ld_32x16(taddr + (k + 1) * 16, vp[cb ^ 1]);
+            ptx::tmem_ld_32x16(taddr + 64 + (k + 1) * 16, vg[cb ^ 1]);
           }
           uint32_t packed[8];
           if (masked) {
-            compute_chunk(vp[c], vg[c], u, maddr + c * 64, true, packed);
+            compute_chunk(vp[cb], vg[cb], maddr + k * 64, true, packed);
           } else {
-            compute_chunk(vp[c], vg[c], u, maddr + c * 64, false, packed);
+            compute_chunk(vp[cb], vg[cb], maddr + k * 64, false, packed);
           }
-          if (c == 1) {
+          if (k == 3) {
             // accumulators and mask slot fully consumed: hand the TMEM slot back to the issuer
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(tempty(slot));
           }
-          // staging buffer n % 4 is free: the store thread waited for store n-4 (see below)
-          const uint32_t c16 = static_cast<uint32_t>(h * 4 + c * 2);
+          if (k == 0) {
+            // this buffer was last read by the team's store two units ago
+            if (store_thread) ptx::tma_store_wait_read<1>();
+            ptx::named_bar_sync(bar_id, 128);
+          }
+          const uint32_t c16 = static_cast<uint32_t>(k * 2);
           ptx::sts128(row_addr + ((c16 ^ sw) << 4), packed[0], packed[1], packed[2], packed[3]);
           ptx::sts128(row_addr + (((c16 + 1) ^ sw) << 4), packed[4], packed[5], packed[6],
                       packed[7]);
         }
         ptx::fence_proxy_async_smem();
-        ptx::named_bar_sync(1, 256);
+        ptx::named_bar_sync(bar_id, 128);
         if (store_thread) {
           ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + hh * 64, 0);
           ptx::tma_store_commit();
-          // at most this store and the previous one may still be reading shared memory when the
-          // store thread reaches the next barrier => buffer (n+2) % 4 is free for unit n+2
-          ptx::tma_store_wait_read<2>();
         }
       }
     }
