@@ -37,7 +37,7 @@ namespace {
 
 constexpr int kC = kChannels;
 constexpr int kTilePairs = 128;
-constexpr int kThreads = 640;
+constexpr int kThreads = 768;
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box (128 rows x 128 bytes)
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB
 constexpr int kStages = 2;
@@ -46,8 +46,8 @@ constexpr int kStageBytes = 2 * kMatBytes;      // z tile + o tile
 constexpr int kOffW = 0;                                   // W_g, W_o
 constexpr int kOffStage = kOffW + 2 * kMatBytes;           // ring: [z | o] per stage
 constexpr int kOffOut = kOffStage + kStages * kStageBytes; // 2 staging buffers [128 pairs][64 ch]
-constexpr int kOffVec = kOffOut + 2 * kHalfBox;            // gamma_in, beta_in, gamma_out, beta_out
-constexpr int kOffBar = kOffVec + 4 * kC * 4;
+constexpr int kOffVec = kOffOut + 2 * kHalfBox;            // folded biases t_g[128], t_o[128] (fp32)
+constexpr int kOffBar = kOffVec + 2 * kC * 4;
 constexpr int kSmemBytes = kOffBar + 128;
 static_assert(kSmemBytes <= 232448, "K3 shared memory exceeds 227 KB");
 
@@ -57,6 +57,8 @@ struct K3Params {
   const float* b_in;
   const float* g_out;
   const float* b_out;
+  const __nv_bfloat16* w_g;    // [128][128] row-major (also read through tmap_wg)
+  const __nv_bfloat16* w_o;
   const float* bias_g;         // may be nullptr
   const float* bias_o;         // may be nullptr
   float eps;
@@ -99,7 +101,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_init(full(s), 1);
       ptx::mbar_init(sempty(s), 1);
       ptx::mbar_init(zready(s), 128);
-      ptx::mbar_init(oready(s), 128);
+      ptx::mbar_init(oready(s), 256);
     }
     for (int u = 0; u < 2; ++u) {
       ptx::mbar_init(tfull(u), 1);
@@ -108,14 +110,30 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
-  if (warp == 3) {
-    float* v = reinterpret_cast<float*>(smem_raw + kOffVec);
-    for (int c = lane; c < kC; c += 32) {
-      v[c] = prm.g_in[c];
-      v[kC + c] = prm.b_in[c];
-      v[2 * kC + c] = prm.g_out[c];
-      v[3 * kC + c] = prm.b_out[c];
+  if (warp >= 4 && warp < 12) {
+    // Fold the LayerNorm shifts into the biases:  W LN(x) + b = (W diag(gamma)) n + (W beta + b)
+    // with n = (x - mean) * rstd.  Thread -> (matrix, output channel); fp32, from the bf16 weights.
+    const int id = threadIdx.x - 128;
+    const int m = id >> 7, ch = id & 127;
+    const uint4* wrow = reinterpret_cast<const uint4*>((m ? prm.w_o : prm.w_g) + ch * kC);
+    const float* beta = m ? prm.b_out : prm.b_in;
+    const float* bias = m ? prm.bias_o : prm.bias_g;
+    float acc = 0.f;
+#pragma unroll 4
+    for (int kc = 0; kc < 16; ++kc) {
+      const uint4 wv = __ldg(wrow + kc);
+      const float4 b0 = __ldg(reinterpret_cast<const float4*>(beta + kc * 8));
+      const float4 b1 = __ldg(reinterpret_cast<const float4*>(beta + kc * 8 + 4));
+      acc = fmaf(ptx::bf16_lo(wv.x), b0.x, acc);
+      acc = fmaf(ptx::bf16_hi(wv.x), b0.y, acc);
+      acc = fmaf(ptx::bf16_lo(wv.y), b0.z, acc);
+      acc = fmaf(ptx::bf16_hi(wv.y), b0.w, acc);
+      acc = fmaf(ptx::bf16_lo(wv.z), b1.x, acc);
+      acc = fmaf(ptx::bf16_hi(wv.z), b1.y, acc);
+      acc = fmaf(ptx::bf16_lo(wv.w), b1.z, acc);
+      acc = fmaf(ptx::bf16_hi(wv.w), b1.w, acc);
     }
+    reinterpret_cast<float*>(smem_raw + kOffVec)[id] = acc + (bias ? bias[ch] : 0.f);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -131,10 +149,26 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::tma_load_2d(smem + kOffW + kMatBytes, &tmap_wo, wfull, 0, 0);
     ptx::tma_load_2d(smem + kOffW + kMatBytes + kHalfBox, &tmap_wo, wfull, 64, 0);
   }
-  if constexpr (kNormFp16) {
-    // kind::f16 needs A and B in the same 16-bit format: the bf16 weights become fp16 in place
+  {
+    // The resident weights become  W diag(gamma)  in the operand format of the normalised tiles
+    // (fp16 unless FOLDCP_NORM_FP16=0), in place: elementwise apart from the gamma index, which
+    // follows from the position under the 128-byte swizzle.
     ptx::mbar_wait(wfull, 0);
-    ptx::smem_bf16_to_f16_inplace(smem + kOffW, 2 * kMatBytes, threadIdx.x, kThreads);
+    for (int off = threadIdx.x * 16; off < 2 * kMatBytes; off += kThreads * 16) {
+      const int m = off / kMatBytes, rem = off % kMatBytes;
+      const int box = rem / kHalfBox, row = (rem % kHalfBox) / 128, pc = (rem % 128) / 16;
+      const int k0 = box * 64 + ((pc ^ (row & 7)) * 8);
+      const float* gam = (m ? prm.g_out : prm.g_in) + k0;
+      const float4 g0 = __ldg(reinterpret_cast<const float4*>(gam));
+      const float4 g1 = __ldg(reinterpret_cast<const float4*>(gam + 4));
+      uint32_t v[4];
+      ptx::lds128(smem + kOffW + off, v);
+      v[0] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[0]) * g0.x, ptx::bf16_hi(v[0]) * g0.y);
+      v[1] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[1]) * g0.z, ptx::bf16_hi(v[1]) * g0.w);
+      v[2] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[2]) * g1.x, ptx::bf16_hi(v[2]) * g1.y);
+      v[3] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[3]) * g1.z, ptx::bf16_hi(v[3]) * g1.w);
+      ptx::sts128(smem + kOffW + off, v[0], v[1], v[2], v[3]);
+    }
     ptx::fence_proxy_async_smem();
     __syncthreads();
   }
@@ -203,93 +237,91 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp >= 4 && warp < 8) {
     // ===================== LayerNorm(z) (thread = pair) =====================
     const int r = threadIdx.x - 128;
-    const uint32_t gaddr = smem + kOffVec, baddr = gaddr + kC * 4;
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      layernorm_rows_inplace<kNormFp16>(smem + kOffStage + s * kStageBytes, kHalfBox, r, gaddr, baddr, prm.eps);
+      layernorm_rows_inplace<kNormFp16, false, 1>(smem + kOffStage + s * kStageBytes, kHalfBox, r, 0,
+                                                  0, prm.eps);
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
-  } else if (warp >= 8 && warp < 12) {
+  } else if (warp >= 8 && warp < 16) {
     // ===================== LayerNorm(o) on the [channel][pair] tile =====================
-    // warp w4 owns pairs w4*32 .. +31; lane = (half-warp chalf = 64 channels, 16 pair-pairs).
-    // One ld.shared.b32 = 2 adjacent pairs of one channel; a half-warp reads 64 contiguous bytes
-    // of a row, the other half-warp a row whose swizzle phase differs by 4 -> conflict-free.
-    const int w4 = warp - 8;
-    const uint32_t chalf = static_cast<uint32_t>(lane >> 4);
-    const uint32_t pp = static_cast<uint32_t>(lane & 15);
-    const uint32_t box = static_cast<uint32_t>(w4 >> 1);
-    const uint32_t c16 = static_cast<uint32_t>((w4 & 1) * 4) + (pp >> 2);   // 16-byte chunk in row
-    const uint32_t within = (pp & 3u) * 4u;
-    const uint32_t kflip = chalf * 4u;
-    // Row k = chalf*64 + 8g + (jj ^ kflip), g, jj = 0..7.  Everything that depends on jj is folded
-    // into eight per-thread offsets; 8g becomes an immediate (1024 B per g in the tile, 32 B in
-    // gamma / beta).
-    uint32_t toff[8], voff[8];
+    // Warp w8 owns 16 pairs; lane = (channel quarter cq = 32 channels, pair-pair pl).  One
+    // ld.shared.b32 = 2 adjacent pairs of one channel, and the thread's 32 words stay in registers
+    // (one pass over shared memory, exact two-pass statistics).  The four quarters visit their
+    // rows in the order i ^ 2cq, which puts their 32-byte segments under four different swizzle
+    // phases: conflict-free.  Statistics combine across the quarters with two shuffles.
+    const int w8 = warp - 8;
+    const uint32_t cq = static_cast<uint32_t>(lane >> 3);
+    const uint32_t pl = static_cast<uint32_t>(lane & 7);
+    const uint32_t box = static_cast<uint32_t>(w8 >> 2);
+    const uint32_t c16 = static_cast<uint32_t>((w8 & 3) * 2) + (pl >> 2);   // 16-byte chunk in row
+    const uint32_t within = (pl & 3u) * 4u;
+    // row k = 32 cq + 8 g + (jj ^ 2cq), g = 0..3, jj = 0..7: everything that depends on jj is
+    // folded into eight per-thread offsets, 8 g becomes an immediate (1024 B per g)
+    uint32_t toff[8];
 #pragma unroll
     for (uint32_t jj = 0; jj < 8; ++jj) {
-      const uint32_t k7 = jj ^ kflip;
-      toff[jj] = box * kHalfBox + (chalf * 64u + k7) * 128u + ((c16 ^ k7) << 4) + within;
-      voff[jj] = smem + kOffVec + 2 * kC * 4 + (chalf * 64u + k7) * 4u;
+      const uint32_t k7 = jj ^ (2u * cq);
+      toff[jj] = box * kHalfBox + (cq * 32u + k7) * 128u + ((c16 ^ k7) << 4) + within;
     }
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
       const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes;
-      // shift = channel 0's value of each pair (robust one-pass variance)
-      const ptx::f32x2 sh = ptx::bf16x2_to_f32x2(
-          ptx::lds32(tile + box * kHalfBox + (c16 << 4) + within));
-      float sh0, sh1;
-      ptx::upk2(sh, sh0, sh1);
-      const ptx::f32x2 nsh = ptx::pk2(-sh0, -sh1);
-      ptx::f32x2 sa = ptx::pk2(0.f, 0.f), sb = sa, qa = sa, qb = sa;
+      uint32_t w[32];
 #pragma unroll
-      for (uint32_t g = 0; g < 8; ++g)
+      for (uint32_t g = 0; g < 4; ++g)
 #pragma unroll
-        for (uint32_t jj = 0; jj < 8; jj += 2) {
-          const ptx::f32x2 d0 = ptx::add2(
-              ptx::bf16x2_to_f32x2(ptx::lds32(tile + toff[jj] + g * 1024u)), nsh);
-          const ptx::f32x2 d1 = ptx::add2(
-              ptx::bf16x2_to_f32x2(ptx::lds32(tile + toff[jj + 1] + g * 1024u)), nsh);
-          sa = ptx::add2(sa, d0);
-          sb = ptx::add2(sb, d1);
-          qa = ptx::fma2(d0, d0, qa);
-          qb = ptx::fma2(d1, d1, qb);
-        }
-      float s0, s1, q0, q1;
+        for (uint32_t jj = 0; jj < 8; ++jj) w[g * 8 + jj] = ptx::lds32(tile + toff[jj] + g * 1024u);
+      ptx::f32x2 sa = ptx::bf16x2_to_f32x2(w[0]), sb = ptx::bf16x2_to_f32x2(w[1]);
+#pragma unroll
+      for (int i = 2; i < 32; i += 2) {
+        sa = ptx::add2(sa, ptx::bf16x2_to_f32x2(w[i]));
+        sb = ptx::add2(sb, ptx::bf16x2_to_f32x2(w[i + 1]));
+      }
+      float s0, s1;
       ptx::upk2(ptx::add2(sa, sb), s0, s1);
-      ptx::upk2(ptx::add2(qa, qb), q0, q1);
+      s0 += __shfl_xor_sync(0xffffffffu, s0, 8);
+      s1 += __shfl_xor_sync(0xffffffffu, s1, 8);
       s0 += __shfl_xor_sync(0xffffffffu, s0, 16);
       s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+      const float m0 = s0 * (1.0f / kC), m1 = s1 * (1.0f / kC);
+      const ptx::f32x2 nm = ptx::pk2(-m0, -m1);
+      ptx::f32x2 qa = ptx::pk2(0.f, 0.f), qb = qa;
+#pragma unroll
+      for (int i = 0; i < 32; i += 2) {
+        const ptx::f32x2 d0 = ptx::add2(ptx::bf16x2_to_f32x2(w[i]), nm);
+        const ptx::f32x2 d1 = ptx::add2(ptx::bf16x2_to_f32x2(w[i + 1]), nm);
+        qa = ptx::fma2(d0, d0, qa);
+        qb = ptx::fma2(d1, d1, qb);
+      }
+      float q0, q1;
+      ptx::upk2(ptx::add2(qa, qb), q0, q1);
+      q0 += __shfl_xor_sync(0xffffffffu, q0, 8);
+      q1 += __shfl_xor_sync(0xffffffffu, q1, 8);
       q0 += __shfl_xor_sync(0xffffffffu, q0, 16);
       q1 += __shfl_xor_sync(0xffffffffu, q1, 16);
-      const float m0 = s0 * (1.0f / kC), m1 = s1 * (1.0f / kC);
-      const float var0 = fmaxf(q0 * (1.0f / kC) - m0 * m0, 0.f);
-      const float var1 = fmaxf(q1 * (1.0f / kC) - m1 * m1, 0.f);
-      const float r0 = rsqrtf(var0 + prm.eps), r1 = rsqrtf(var1 + prm.eps);
+      const float r0 = rsqrtf(q0 * (1.0f / kC) + prm.eps), r1 = rsqrtf(q1 * (1.0f / kC) + prm.eps);
       const ptx::f32x2 rr = ptx::pk2(r0, r1);
-      const ptx::f32x2 nn = ptx::pk2(-(sh0 + m0) * r0, -(sh1 + m1) * r1);
+      const ptx::f32x2 nn = ptx::pk2(-m0 * r0, -m1 * r1);
 #pragma unroll
-      for (uint32_t g = 0; g < 8; ++g)
+      for (uint32_t g = 0; g < 4; ++g)
 #pragma unroll
-        for (uint32_t jj = 0; jj < 8; ++jj) {
-          const uint32_t a = tile + toff[jj] + g * 1024u;
-          const float gm = ptx::lds32f(voff[jj] + g * 32u);
-          const float bt = ptx::lds32f(voff[jj] + g * 32u + kC * 4);
-          const ptx::f32x2 y = ptx::fma2(ptx::fma2(ptx::bf16x2_to_f32x2(ptx::lds32(a)), rr, nn),
-                                         ptx::pk2(gm, gm), ptx::pk2(bt, bt));
-          ptx::sts32(a, ptx::pack_norm2<kNormFp16>(y));
-        }
+        for (uint32_t jj = 0; jj < 8; ++jj)
+          ptx::sts32(tile + toff[jj] + g * 1024u,
+                     ptx::pack_norm2<kNormFp16>(
+                         ptx::fma2(ptx::bf16x2_to_f32x2(w[g * 8 + jj]), rr, nn)));
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(oready(s));
     }
-  } else if (warp >= 12) {
+  } else if (warp >= 16) {
     // ===================== epilogue (thread = pair, 64 output channels) =====================
     const int q = warp & 3;                       // TMEM lane quadrant (hardware: warp % 4)
-    const int h = (warp - 12) >> 2;               // channel half
+    const int h = (warp - 16) >> 2;               // channel half
     const int r = q * 32 + lane;                  // pair within the tile
     const uint32_t stage_buf = smem + kOffOut + h * kHalfBox;
     const uint32_t row_addr = stage_buf + r * 128;
@@ -302,8 +334,8 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
     (void)half2;
     (void)one2;
-    const float4* bg4 = reinterpret_cast<const float4*>(prm.bias_g) + h * 16;
-    const float4* bo4 = reinterpret_cast<const float4*>(prm.bias_o) + h * 16;
+    // folded biases (fp32) of this thread's 64 channels
+    const uint32_t tg_addr = smem + kOffVec + h * 64 * 4, to_addr = tg_addr + kC * 4;
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int slot = it & 1;
@@ -328,11 +360,9 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         uint32_t packed[8];
 #pragma unroll
         for (int j4 = 0; j4 < 4; ++j4) {
-          float4 bg = make_float4(0.f, 0.f, 0.f, 0.f), bo = bg;
-          if (prm.bias_g) bg = __ldg(bg4 + chunk * 4 + j4);
-          if (prm.bias_o) bo = __ldg(bo4 + chunk * 4 + j4);
-          const ptx::f32x2 bg2[2] = {ptx::pk2(bg.x, bg.y), ptx::pk2(bg.z, bg.w)};
-          const ptx::f32x2 bo2[2] = {ptx::pk2(bo.x, bo.y), ptx::pk2(bo.z, bo.w)};
+          ptx::f32x2 bg2[2], bo2[2];
+          ptx::lds128x2(tg_addr + (chunk * 16 + j4 * 4) * 4, bg2);
+          ptx::lds128x2(to_addr + (chunk * 16 + j4 * 4) * 4, bo2);
 #pragma unroll
           for (int e2 = 0; e2 < 2; ++e2) {
             const int j = j4 * 4 + e2 * 2;
@@ -423,6 +453,8 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   prm.b_in = p->ln_in_beta;
   prm.g_out = p->ln_out_gamma;
   prm.b_out = p->ln_out_beta;
+  prm.w_g = static_cast<const __nv_bfloat16*>(p->w_g);
+  prm.w_o = static_cast<const __nv_bfloat16*>(p->w_o);
   prm.bias_g = p->b_g;
   prm.bias_o = p->b_o;
   prm.eps = p->ln_eps;

@@ -21,7 +21,8 @@ namespace foldcp {
 // gaddr / baddr : shared addresses of gamma[128] / beta[128] (fp32)
 // kAffine = false: plain normalisation (x - mean) * rstd; gamma / beta are then folded into the
 // weights and biases of the GEMM that consumes the tile (gaddr / baddr unused).
-template <bool kF16, bool kAffine = true>
+// kRows = rows per thread in flight (2 = more latency hiding, ~100 registers; 1 = ~60 registers).
+template <bool kF16, bool kAffine = true, int kRows = 2>
 __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t box_stride, int tid,
                                                        uint32_t gaddr, uint32_t baddr, float eps) {
   const uint32_t j = static_cast<uint32_t>(tid & 3);        // quarter of the row: channels 32j..
@@ -33,13 +34,13 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
   // shuffles, rsqrt) interleave, which matters because one LayerNorm warp per scheduler is
   // latency-bound, not throughput-bound.
 #pragma unroll 1
-  for (int pass = 0; pass < 2; ++pass) {
-    const uint32_t r0 = static_cast<uint32_t>(pass * 64 + (tid >> 2));
+  for (int pass = 0; pass < 4 / kRows; ++pass) {
+    const uint32_t r0 = static_cast<uint32_t>(pass * 32 * kRows + (tid >> 2));
     const uint32_t sw = r0 & 7u;                              // (r0 + 32) & 7 is the same
     const uint32_t row0 = tile + box * box_stride + r0 * 128u;
-    ptx::f32x2 x[2][4][4];
+    ptx::f32x2 x[kRows][4][4];
 #pragma unroll
-    for (uint32_t q = 0; q < 2; ++q)
+    for (uint32_t q = 0; q < kRows; ++q)
 #pragma unroll
       for (uint32_t t = 0; t < 4; ++t) {
         uint32_t w[4];
@@ -47,10 +48,10 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
 #pragma unroll
         for (int e = 0; e < 4; ++e) x[q][t][e] = ptx::bf16x2_to_f32x2(w[e]);
       }
-    float mu[2], rstd[2];
-    float sum[2];
+    float mu[kRows], rstd[kRows];
+    float sum[kRows];
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < kRows; ++q) {
       ptx::f32x2 s2 = ptx::add2(x[q][0][0], x[q][0][1]), s3 = ptx::add2(x[q][0][2], x[q][0][3]);
 #pragma unroll
       for (int t = 1; t < 4; ++t) {
@@ -62,12 +63,12 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
       sum[q] = slo + shi;
     }
 #pragma unroll
-    for (int q = 0; q < 2; ++q) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], 1);
+    for (int q = 0; q < kRows; ++q) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], 1);
 #pragma unroll
-    for (int q = 0; q < 2; ++q) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], 2);
-    float var[2];
+    for (int q = 0; q < kRows; ++q) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], 2);
+    float var[kRows];
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < kRows; ++q) {
       mu[q] = sum[q] * (1.0f / 128.0f);
       const ptx::f32x2 nmu = ptx::pk2(-mu[q], -mu[q]);
       ptx::f32x2 v2 = ptx::pk2(0.f, 0.f), v3 = v2;
@@ -84,12 +85,12 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
       var[q] = slo + shi;
     }
 #pragma unroll
-    for (int q = 0; q < 2; ++q) var[q] += __shfl_xor_sync(0xffffffffu, var[q], 1);
+    for (int q = 0; q < kRows; ++q) var[q] += __shfl_xor_sync(0xffffffffu, var[q], 1);
 #pragma unroll
-    for (int q = 0; q < 2; ++q) var[q] += __shfl_xor_sync(0xffffffffu, var[q], 2);
-    ptx::f32x2 rs2[2], nmr2[2];
+    for (int q = 0; q < kRows; ++q) var[q] += __shfl_xor_sync(0xffffffffu, var[q], 2);
+    ptx::f32x2 rs2[kRows], nmr2[kRows];
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < kRows; ++q) {
       rstd[q] = rsqrtf(var[q] * (1.0f / 128.0f) + eps);
       rs2[q] = ptx::pk2(rstd[q], rstd[q]);
       const float nmr = -mu[q] * rstd[q];
@@ -107,7 +108,7 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
         ptx::lds128x2(baddr + voff + 16, *reinterpret_cast<ptx::f32x2(*)[2]>(&b[2]));
       }
 #pragma unroll
-      for (uint32_t q = 0; q < 2; ++q) {
+      for (uint32_t q = 0; q < kRows; ++q) {
         uint32_t y[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
