@@ -48,7 +48,29 @@ struct K2Params {
   int tiles_n;
   int num_tiles;   // channels * tiles_m * tiles_n
   int num_kb;      // ceil(N / 64)
+  int l2_hints;    // 1: evict_last loads / evict_first stores
+  int panel_n;     // tile rasterisation: n-tiles per column panel (>= 1)
 };
+
+// Tile rasterisation inside one channel: column panels of `panel_n` n-tiles, m fastest-varying
+// between panels' rows.  The ~74 tile pairs in flight then share a few A row-blocks and one narrow
+// B panel, and consecutive waves re-use that B panel from L2 instead of streaming all of B_c.
+__device__ __forceinline__ void decode_tile(const K2Params& prm, int r, int* tm, int* tn) {
+  const int w = prm.panel_n;
+  const int full = prm.tiles_n / w;
+  const int in_full = full * prm.tiles_m * w;
+  if (r < in_full) {
+    const int p = r / (prm.tiles_m * w);
+    const int q = r - p * prm.tiles_m * w;
+    *tm = q / w;
+    *tn = p * w + (q - (q / w) * w);
+  } else {
+    const int q = r - in_full;
+    const int wl = prm.tiles_n - full * w;
+    *tm = q / wl;
+    *tn = full * w + (q - (q / wl) * wl);
+  }
+}
 
 template <int kCtaGroup, bool kIncoming>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -110,13 +132,17 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
+      // a_c / b_c are re-read by every tile of channel c: keep them in L2, stream o past them
+      const uint64_t pol_ld = prm.l2_hints ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
       int stage = 0;
       uint32_t phase = 0;
       for (int t = group_id; t < prm.num_tiles; t += num_groups) {
         const int ch = t / tiles_per_ch;
         const int r = t - ch * tiles_per_ch;
-        const int m0 = (r / prm.tiles_n) * C::kTileM + static_cast<int>(cta_rank) * 128;
-        const int n0 = (r % prm.tiles_n) * kTileN + static_cast<int>(cta_rank) * (kTileN / kCtaGroup);
+        int tm, tn;
+        decode_tile(prm, r, &tm, &tn);
+        const int m0 = tm * C::kTileM + static_cast<int>(cta_rank) * 128;
+        const int n0 = tn * kTileN + static_cast<int>(cta_rank) * (kTileN / kCtaGroup);
         for (int kb = 0; kb < prm.num_kb; ++kb) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
           const uint32_t sa = stage_base + stage * C::kStageBytes;
@@ -135,9 +161,9 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
             const int c0 = kIncoming ? mn : k0;   // innermost tensor coordinate (column)
             const int c1 = kIncoming ? k0 : mn;   // row
             if constexpr (kCtaGroup == 2) {
-              ptx::tma_load_3d_2sm(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch);
+              ptx::tma_load_3d_2sm_hint(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch, pol_ld);
             } else {
-              ptx::tma_load_3d(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch);
+              ptx::tma_load_3d_hint(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch, pol_ld);
             }
           }
 #pragma unroll
@@ -146,9 +172,9 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
             const int c0 = kIncoming ? mn : k0;
             const int c1 = kIncoming ? k0 : mn;
             if constexpr (kCtaGroup == 2) {
-              ptx::tma_load_3d_2sm(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch);
+              ptx::tma_load_3d_2sm_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld);
             } else {
-              ptx::tma_load_3d(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch);
+              ptx::tma_load_3d_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld);
             }
           }
           if (++stage == C::kStages) {
@@ -203,13 +229,16 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const int q = warp - 4;                 // TMEM lane quadrant this warp may read
     const int row = q * 32 + lane;          // row of the CTA's 128-row tile
     const bool store_thread = (warp == 4 && lane == 0);
+    const uint64_t pol_st = prm.l2_hints ? ptx::kL2EvictFirst : ptx::kL2EvictNormal;
     int it = 0;
     int chunk_ctr = 0;
     for (int t = group_id; t < prm.num_tiles; t += num_groups, ++it) {
       const int ch = t / tiles_per_ch;
       const int r = t - ch * tiles_per_ch;
-      const int m0 = (r / prm.tiles_n) * C::kTileM + static_cast<int>(cta_rank) * 128;
-      const int n0 = (r % prm.tiles_n) * kTileN;
+      int tm, tn;
+      decode_tile(prm, r, &tm, &tn);
+      const int m0 = tm * C::kTileM + static_cast<int>(cta_rank) * 128;
+      const int n0 = tn * kTileN;
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
       ptx::mbar_wait(tfull_bar(as), aphase);
@@ -254,7 +283,7 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
         ptx::fence_proxy_async_smem();
         ptx::named_bar_sync(1, 128);
         if (store_thread) {
-          ptx::tma_store_3d(&tmap_o, buf, n0 + j * 64, m0, ch);
+          ptx::tma_store_3d_hint(&tmap_o, buf, n0 + j * 64, m0, ch, pol_st);
           ptx::tma_store_commit();
         }
       }
@@ -333,6 +362,17 @@ int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int di
   prm.tiles_n = (N + kTileN - 1) / kTileN;
   prm.num_tiles = kChannels * prm.tiles_m * prm.tiles_n;
   prm.num_kb = (N + kBlockK - 1) / kBlockK;
+  static const int l2_hints = [] {
+    const char* e = getenv("FOLDCP_K2_L2_HINTS");
+    return (e && e[0] == '1') ? 1 : 0;   // measured: hints raise DRAM traffic (55 vs 34 GB)
+  }();
+  prm.l2_hints = l2_hints;
+  static const int panel = [] {
+    const char* e = getenv("FOLDCP_K2_PANEL");
+    return e ? atoi(e) : 0;   // 0 = plain row-major order (measured: panels of 8 / 4 / 2 n-tiles
+                              // do not lower DRAM traffic or time at N = 4096)
+  }();
+  prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : prm.tiles_n;
   const bool inc = direction == FOLDCP_INCOMING;
   if (cta_group == 2) {
     return inc ? launch_variant<2, true>(ta, tb, to, prm, dev.sm_count, stream)
