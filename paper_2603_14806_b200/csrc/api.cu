@@ -58,7 +58,7 @@ static EncodeTiledFn get_encode_fn() {
 
 int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int rank,
                       const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
-                      bool swizzle128) {
+                      int swizzle) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return FOLDCP_ERR_CUDA;
   cuuint64_t d[5], s[4];
@@ -74,7 +74,9 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
   const CUresult r =
       fn(map, dt, static_cast<cuuint32_t>(rank), const_cast<void*>(base), d, s, b, e,
          CU_TENSOR_MAP_INTERLEAVE_NONE,
-         swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+         swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+         : swizzle != 0 ? CU_TENSOR_MAP_SWIZZLE_128B
+                        : CU_TENSOR_MAP_SWIZZLE_NONE,
          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? FOLDCP_OK : FOLDCP_ERR_CUDA;
 }

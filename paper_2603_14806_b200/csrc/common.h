@@ -36,11 +36,12 @@ bool get_device_info(DeviceInfo* info);
 
 // Encode a tiled tensor map over a row-major tensor whose innermost dimension is dims[0].
 //   elem_bytes: 2 (bf16) or 4 (f32); rank 2..4; strides_bytes[i] = byte stride of dims[i+1]
-//   swizzle128: CU_TENSOR_MAP_SWIZZLE_128B (inner box must be 128 bytes) or none
+//   swizzle: 0 = none, 64 = SWIZZLE_64B (inner box 64 bytes), anything else (1 / true / 128) =
+//            SWIZZLE_128B (inner box 128 bytes)
 // Returns FOLDCP_OK or FOLDCP_ERR_CUDA.
 int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int rank,
                       const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
-                      bool swizzle128);
+                      int swizzle);
 
 // ----- stage launchers (device pointers; return foldcp_status_t) -----
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,

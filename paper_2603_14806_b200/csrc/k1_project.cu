@@ -62,7 +62,7 @@ constexpr int kSmemBytes = kOffBar + 256;
 static_assert(kSmemBytes <= 232448, "K1 shared memory exceeds 227 KB");
 
 constexpr int kTmemW = 0;        // columns 0..255: four weight matrices, 64 columns each
-constexpr int kTmemAcc = 256;    // columns 256..511: two slots of (projection 64 | gate 64)
+constexpr int kTmemAcc = 256;    // columns 256..511: four slots of (projection 32 | gate 32)
 
 struct K1Params {
   const __nv_bfloat16* mask;   // [R] or nullptr
@@ -89,9 +89,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   auto zempty = [&](int s) { return bar + 8u * (kZStages + s); };
   auto zready = [&](int s) { return bar + 8u * (2 * kZStages + s); };
   auto tfull = [&](int u) { return bar + 8u * (3 * kZStages + u); };
-  auto tempty = [&](int u) { return bar + 8u * (3 * kZStages + 2 + u); };
-  const uint32_t tmem_slot = bar + 8u * (3 * kZStages + 4);
-  const uint32_t wready = bar + 8u * (3 * kZStages + 5);   // weights are in TMEM
+  auto tempty = [&](int u) { return bar + 8u * (3 * kZStages + 4 + u); };
+  const uint32_t tmem_slot = bar + 8u * (3 * kZStages + 8);
+  const uint32_t wready = bar + 8u * (3 * kZStages + 9);   // weights are in TMEM
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -107,7 +107,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_init(zempty(s), 1);
       ptx::mbar_init(zready(s), 128);
     }
-    for (int u = 0; u < 2; ++u) {
+    for (int u = 0; u < 4; ++u) {
       ptx::mbar_init(tfull(u), 1);
       ptx::mbar_init(tempty(u), 4);
     }
@@ -143,37 +143,41 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     if (ptx::elect_one()) {
       // A = folded weights in TMEM, B = n (K-major, 64 pairs), both fp16 (or both bf16)
       constexpr uint32_t kFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
-      constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, 64, kFmt, kFmt, 0, 0);
+      constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, 32, kFmt, kFmt, 0, 0);
       ptx::mbar_wait(wready, 0);
       ptx::tc_fence_after();
       int it = 0;
-      uint32_t n = 0;   // unit counter
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
         const int s = it % kZStages;
         ptx::mbar_wait(zready(s), (it / kZStages) & 1);
         ptx::tc_fence_after();
         const uint32_t zb = smem + kOffZ + s * kMatBytes;
 #pragma unroll
-        for (int idx = 0; idx < 4; ++idx, ++n) {
-          const int hh = idx >> 1, u = idx & 1;
-          const uint32_t slot = n & 1u;
-          ptx::mbar_wait(tempty(slot), ((n >> 1) & 1u) ^ 1u);
-          ptx::tc_fence_after();
+        for (int pq = 0; pq < 4; ++pq) {
 #pragma unroll
-          for (int m2 = 0; m2 < 2; ++m2) {
-            const uint32_t a_tmem = tmem_base + kTmemW + (2 * u + m2) * 64;
-            const uint32_t d_tmem = tmem_base + kTmemAcc + slot * 128 + m2 * 64;
+          for (int u = 0; u < 2; ++u) {
+            // slot 2u + (pq & 1): each tensor's team alternates between its two slots, so this
+            // unit's MMAs overlap the team's epilogue of the previous unit
+            const uint32_t slot = static_cast<uint32_t>(2 * u + (pq & 1));
+            const uint32_t use = static_cast<uint32_t>(it * 2 + (pq >> 1));   // per-slot use count
+            ptx::mbar_wait(tempty(slot), (use & 1u) ^ 1u);
+            ptx::tc_fence_after();
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              // rows hh*64.. of the tile: 64 rows x 128 B = 8 KB into each k-half box
-              const uint32_t off = hh * 8192 + (k >> 2) * kHalfBox + (k & 3) * 32;
-              const uint64_t db = ptx::make_smem_desc_sw128(zb + off, 16, 1024);
-              ptx::umma_f16_ts(d_tmem, a_tmem + k * 8, db, idesc, k != 0 ? 1u : 0u);
+            for (int m2 = 0; m2 < 2; ++m2) {
+              const uint32_t a_tmem = tmem_base + kTmemW + (2 * u + m2) * 64;
+              const uint32_t d_tmem = tmem_base + kTmemAcc + slot * 64 + m2 * 32;
+#pragma unroll
+              for (int k = 0; k < 8; ++k) {
+                // rows pq*32.. of the tile: 32 rows x 128 B = 4 KB into each k-half box
+                const uint32_t off = pq * 4096 + (k >> 2) * kHalfBox + (k & 3) * 32;
+                const uint64_t db = ptx::make_smem_desc_sw128(zb + off, 16, 1024);
+                ptx::umma_f16_ts(d_tmem, a_tmem + k * 8, db, idesc, k != 0 ? 1u : 0u);
+              }
             }
+            ptx::umma_commit<1>(tfull(slot));
           }
-          ptx::umma_commit<1>(tfull(slot));
         }
-        ptx::umma_commit<1>(zempty(s));   // stage reusable once all eight MMAs retired
+        ptx::umma_commit<1>(zempty(s));   // stage reusable once all MMAs of the tile retired
       }
     }
   } else if (warp >= 4 && warp < 8) {
@@ -296,75 +300,80 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       }
     };
 
-    // Team h (four warps, one per lane quadrant) owns TMEM slot h and therefore tensor u = h
-    // (a for team 0, b for team 1): per tile it handles the two pair halves hh = 0, 1.  The two
-    // teams run independently (own barrier, own store thread, own staging buffers), so the fixed
-    // latencies of one team's unit (mbarrier wake-up, tcgen05.ld, fence, barrier) overlap the
-    // other team's arithmetic.
+    // Team h (four warps, one per lane quadrant) owns tensor u = h (a for team 0, b for team 1)
+    // and its two TMEM slots 2h, 2h+1.  A unit is 32 pairs; per tile the team handles the four
+    // pair quarters pq = 0..3, alternating between its slots so that the MMAs of unit pq+1 run
+    // while it reads and post-processes unit pq.  Two units fill one [128 ch][64 pairs] staging
+    // buffer (128-byte rows: narrower TMA stores are markedly slower), stored after the second.
+    // The two teams run independently (own barrier, store thread and staging buffers).
     const int u = h;
-    const uint32_t slot = static_cast<uint32_t>(h);
     const uint32_t bar_id = 1 + h;
     int it = 0;
-    uint32_t c = 0;   // this team's unit counter
+    uint32_t c = 0;   // this team's 64-pair group counter (staging buffer parity)
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int ms = it & (kMaskSlots - 1);
       bool masked = true;
 #pragma unroll
-      for (int hh = 0; hh < 2; ++hh, ++c) {
+      for (int pq = 0; pq < 4; ++pq) {
+        const uint32_t slot = static_cast<uint32_t>(2 * h + (pq & 1));
+        const uint32_t use = static_cast<uint32_t>(it * 2 + (pq >> 1));   // per-slot use count
+        if ((pq & 1) == 0 && pq != 0) ++c;
         const uint32_t buf = smem + kOffOut + (2 * h + (c & 1u)) * kHalfBox;
-        ptx::mbar_wait(tfull(slot), c & 1u);
+        ptx::mbar_wait(tfull(slot), use & 1u);
         ptx::tc_fence_after();
-        if (hh == 0) {
+        if (pq == 0) {
           // written by the LayerNorm warps before zready, hence visible after this tile's tfull
           uint32_t f[4];
           ptx::lds128(smem + kOffFlag + ms * 16, f);
           masked = (f[0] & f[1] & f[2] & f[3]) == 0u;   // warp-uniform
         }
-        const uint32_t taddr = lane_base + kTmemAcc + slot * 128;
-        const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + hh * 64) * 4;
+        const uint32_t taddr = lane_base + kTmemAcc + slot * 64;
+        const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + pq * 32) * 4;
         const uint32_t row_addr = buf + ch * 128;
-        // 64 columns in four chunks of 16; the tcgen05.ld of chunk k+1 is in flight while chunk
-        // k is being computed (two register buffers)
+        // 32 columns in two chunks of 16; the tcgen05.ld of the second chunk is in flight while
+        // the first is being computed
         uint32_t vp[2][16], vg[2][16];
         ptx::tmem_ld_32x16(taddr, vp[0]);
-        ptx::tmem_ld_32x16(taddr + 64, vg[0]);
+        ptx::tmem_ld_32x16(taddr + 32, vg[0]);
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const int cb = k & 1;
+        for (int k = 0; k < 2; ++k) {
           ptx::tmem_ld_wait();
-          if (k < 3) {
-            ptx::tmem_ld_32x16(taddr + (k + 1) * 16, vp[cb ^ 1]);
-            ptx::tmem_ld_32x16(taddr + 64 + (k + 1) * 16, vg[cb ^ 1]);
-          }
-          uint32_t packed[8];
-          if (masked) {
-            compute_chunk(vp[cb], vg[cb], maddr + k * 64, true, packed);
+          if (k == 0) {
+            ptx::tmem_ld_32x16(taddr + 16, vp[1]);
+            ptx::tmem_ld_32x16(taddr + 32 + 16, vg[1]);
           } else {
-            compute_chunk(vp[cb], vg[cb], maddr + k * 64, false, packed);
-          }
-          if (k == 3) {
-            // accumulators and mask slot fully consumed: hand the TMEM slot back to the issuer
+            // accumulators are in registers: hand the TMEM slot back to the issuer (the mask
+            // slot stays valid: kMaskSlots >= kZStages + 3)
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(tempty(slot));
           }
-          if (k == 0) {
-            // this buffer was last read by the team's store two units ago
+          uint32_t packed[8];
+          if (masked) {
+            compute_chunk(vp[k], vg[k], maddr + k * 64, true, packed);
+          } else {
+            compute_chunk(vp[k], vg[k], maddr + k * 64, false, packed);
+          }
+          if (pq % 2 == 0 && k == 0) {
+            // first write into this staging buffer: the team's store two groups ago has read it
             if (store_thread) ptx::tma_store_wait_read<1>();
             ptx::named_bar_sync(bar_id, 128);
           }
-          const uint32_t c16 = static_cast<uint32_t>(k * 2);
+          const uint32_t c16 = static_cast<uint32_t>((pq & 1) * 4 + k * 2);
           ptx::sts128(row_addr + ((c16 ^ sw) << 4), packed[0], packed[1], packed[2], packed[3]);
           ptx::sts128(row_addr + (((c16 + 1) ^ sw) << 4), packed[4], packed[5], packed[6],
                       packed[7]);
         }
-        ptx::fence_proxy_async_smem();
-        ptx::named_bar_sync(bar_id, 128);
-        if (store_thread) {
-          ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + hh * 64, 0);
-          ptx::tma_store_commit();
+        if (pq & 1) {
+          ptx::fence_proxy_async_smem();
+          ptx::named_bar_sync(bar_id, 128);
+          if (store_thread) {
+            ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + (pq >> 1) * 64, 0);
+            ptx::tma_store_commit();
+          }
         }
       }
+      ++c;
     }
     if (store_thread) ptx::tma_store_wait<0>();
   }
