@@ -24,6 +24,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 C = 128
+K2_DRAM_BYTES_PER_LAUNCH_N4096 = 18.83e9 + 4.28e9   # ncu, profiles/r1_k2_contract_ncu_full.txt
 
 
 def counted_flops(N: int) -> float:
@@ -40,6 +41,27 @@ def measured_peaks():
                     tf_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]), source="measured")
     # fallback stated in B200_PROFILING.md
     return dict(hbm_gbs=6650.0, tf_burst=1590.0, tf_sustained=1400.0, source="fallback")
+
+
+def max_over_ranks(ms: float, world: int, dist=None, device="cpu") -> float:
+    """Replicas only: every rank times its own replica; the job's time is the slowest rank's."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_tflops(flops_per_rank_step: float, ms_per_step: float, world: int) -> float:
+    """value = the FLOPs all ranks processed / the max-over-ranks time (weak scaling, no collective
+    on the data path)."""
+    return world * flops_per_rank_step / (ms_per_step * 1e-3) / 1e12
+
+
+def replica_seed(base_seed: int, rank: int) -> int:
+    """Each replica runs the same-shaped problem on its own seeded z."""
+    return base_seed + rank
 
 
 class ClockSampler:
@@ -186,7 +208,7 @@ def run_ours(args):
     N, K, W = args.n, args.steps, max(args.warmup, 3)
     cfg = synth.CONFIGS[3]
     # replicas: every rank runs the same-shaped problem on its own seeded inputs
-    z = synth.make_z(cfg.seed + rank, N, C, "bf16", dev)
+    z = synth.make_z(replica_seed(cfg.seed, rank), N, C, "bf16", dev)
     M = synth.pair_mask(synth.make_token_mask("ones", N, cfg.seed), "bf16", dev)
     ps = [{k: v.to(dev) for k, v in synth.make_params(cfg.seed * 2 + d, C, C, "bf16").items()}
           for d in (0, 1)]
@@ -215,14 +237,10 @@ def run_ours(args):
         step()
     e1.record()
     barrier()
-    ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dist, dev)
     ms_per_step = ms / K
     flops_step = 2 * counted_flops(N)
-    value = world * flops_step / (ms_per_step * 1e-3) / 1e12
+    value = whole_job_tflops(flops_step, ms_per_step, world)
 
     # ---- per-stage durations inside a timed region (stage entry points, same kernels, same stream)
     a = ws[: ws.numel() // 3].view(torch.bfloat16).view(C, N, N)
@@ -292,14 +310,10 @@ def run_e2e(ctx, steps):
         step()
     e1.record()
     torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / steps
-    if ctx["world"] > 1:
-        t = torch.tensor([ms], device=dev)
-        ctx["dist"].all_reduce(t, op=ctx["dist"].ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(e0.elapsed_time(e1) / steps, ctx["world"], ctx["dist"], dev)
     h2d = hz.numel() * hz.element_size() + hM.numel() * hM.element_size()
     d2h = 2 * ho[0].numel() * ho[0].element_size()
-    return {"value": ctx["world"] * ctx["flops_step"] / (ms * 1e-3) / 1e12, "unit": "TFLOP/s",
+    return {"value": whole_job_tflops(ctx["flops_step"], ms, ctx["world"]), "unit": "TFLOP/s",
             "ms_per_step": ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps}
 
 
@@ -341,7 +355,12 @@ def main():
         "algorithmic_flops_per_launch": 2.0 * C * N ** 3,
         "ms_per_launch": {"outgoing": sm["k2_out"], "incoming": sm["k2_in"]},
         "share_of_step": (sm["k2_out"] + sm["k2_in"]) / step_sum,
-        "traffic": None,
+        # dram__bytes_read.sum + dram__bytes_write.sum of one k2_contract launch at N=4096, from the
+        # ncu --set full capture summarised in profiles/ (18.8 GB read + 4.3 GB written; the
+        # algorithmic bytes are 8.6 GB read + 4.3 GB written)
+        "traffic": K2_DRAM_BYTES_PER_LAUNCH_N4096 if N == 4096 else None,
+        "traffic_source": "profiles/r1_k2_contract_ncu_full.txt",
+        "algorithmic_bytes_per_launch": 3.0 * C * N * N * 2,
         "other_kernels": {
             "k1_project": {"ms": sm["k1"], "bound": "hbm",
                            "achieved_GBs": 3 * N * N * C * 2 / (sm["k1"] * 1e-3) / 1e9,
