@@ -37,7 +37,16 @@ namespace {
 
 constexpr int kC = kChannels;
 constexpr int kTilePairs = 128;
-constexpr int kThreads = 768;
+// warp roles: 0 TMA, 1 MMA, 2 TMEM allocator, 3 idle, then LayerNorm(z), LayerNorm(o), epilogue
+#ifndef FOLDCP_K3_LNZ_WARPS
+#define FOLDCP_K3_LNZ_WARPS 4
+#endif
+constexpr int kLnzWarps = FOLDCP_K3_LNZ_WARPS;       // 4 or 8
+constexpr int kWarpLnz = 4;
+constexpr int kWarpLno = kWarpLnz + kLnzWarps;       // 8 warps
+constexpr int kWarpEpi = kWarpLno + 8;               // 8 warps; a multiple of 4 (TMEM lane quadrants)
+constexpr int kThreads = (kWarpEpi + 8) * 32;
+static_assert(kLnzWarps == 4 || kLnzWarps == 8, "LayerNorm(z) runs on 4 or 8 warps");
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box (128 rows x 128 bytes)
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB
 constexpr int kStages = 2;
@@ -100,7 +109,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     for (int s = 0; s < kStages; ++s) {
       ptx::mbar_init(full(s), 1);
       ptx::mbar_init(sempty(s), 1);
-      ptx::mbar_init(zready(s), 128);
+      ptx::mbar_init(zready(s), kLnzWarps * 32);
       ptx::mbar_init(oready(s), 256);
     }
     for (int u = 0; u < 2; ++u) {
@@ -110,7 +119,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
-  if (warp >= 4 && warp < 12) {
+  if (threadIdx.x >= 128 && threadIdx.x < 384) {
     // Fold the LayerNorm shifts into the biases:  W LN(x) + b = (W diag(gamma)) n + (W beta + b)
     // with n = (x - mean) * rstd.  Thread -> (matrix, output channel); fp32, from the bf16 weights.
     const int id = threadIdx.x - 128;
@@ -234,26 +243,26 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::umma_commit<1>(sempty(s));
       }
     }
-  } else if (warp >= 4 && warp < 8) {
-    // ===================== LayerNorm(z) (thread = pair) =====================
+  } else if (warp >= kWarpLnz && warp < kWarpLno) {
+    // ===================== LayerNorm(z) (4 lanes per pair row) =====================
     const int r = threadIdx.x - 128;
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      layernorm_rows_inplace<kNormFp16, false, 1>(smem + kOffStage + s * kStageBytes, kHalfBox, r, 0,
-                                                  0, prm.eps);
+      layernorm_rows_inplace<kNormFp16, false, 1, kLnzWarps * 32>(smem + kOffStage + s * kStageBytes, kHalfBox,
+                                                       r, 0, 0, prm.eps);
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
-  } else if (warp >= 8 && warp < 16) {
+  } else if (warp >= kWarpLno && warp < kWarpEpi) {
     // ===================== LayerNorm(o) on the [channel][pair] tile =====================
     // Warp w8 owns 16 pairs; lane = (channel quarter cq = 32 channels, pair-pair pl).  One
     // ld.shared.b32 = 2 adjacent pairs of one channel, and the thread's 32 words stay in registers
     // (one pass over shared memory, exact two-pass statistics).  The four quarters visit their
     // rows in the order i ^ 2cq, which puts their 32-byte segments under four different swizzle
     // phases: conflict-free.  Statistics combine across the quarters with two shuffles.
-    const int w8 = warp - 8;
+    const int w8 = warp - kWarpLno;
     const uint32_t cq = static_cast<uint32_t>(lane >> 3);
     const uint32_t pl = static_cast<uint32_t>(lane & 7);
     const uint32_t box = static_cast<uint32_t>(w8 >> 2);
@@ -318,10 +327,10 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(oready(s));
     }
-  } else if (warp >= 16) {
+  } else if (warp >= kWarpEpi) {
     // ===================== epilogue (thread = pair, 64 output channels) =====================
     const int q = warp & 3;                       // TMEM lane quadrant (hardware: warp % 4)
-    const int h = (warp - 16) >> 2;               // channel half
+    const int h = (warp - kWarpEpi) >> 2;               // channel half
     const int r = q * 32 + lane;                  // pair within the tile
     const uint32_t stage_buf = smem + kOffOut + h * kHalfBox;
     const uint32_t row_addr = stage_buf + r * 128;
@@ -336,15 +345,24 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     (void)one2;
     // folded biases (fp32) of this thread's 64 channels
     const uint32_t tg_addr = smem + kOffVec + h * 64 * 4, to_addr = tg_addr + kC * 4;
+    // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
+    auto load_mask = [&](int t) -> unsigned short {
+      if (prm.mask == nullptr) return static_cast<unsigned short>(0x3f80);   // bf16 1.0
+      if (t >= prm.num_tiles) return static_cast<unsigned short>(0);
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
+      return p < prm.R ? __ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)
+                       : static_cast<unsigned short>(0);
+    };
+    unsigned short mnext = load_mask(first);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int slot = it & 1;
-      const long long p = static_cast<long long>(t) * kTilePairs + r;
-      float mval = 1.0f;
-      if (prm.mask != nullptr) mval = p < prm.R ? __bfloat162float(prm.mask[p]) : 0.0f;
-      const ptx::f32x2 mval2 = ptx::pk2(mval, mval);
+      const unsigned short mraw = mnext;
+      mnext = load_mask(t + stride);
       ptx::mbar_wait(tfull(slot), (it >> 1) & 1);
       ptx::tc_fence_after();
+      const float mval = __uint_as_float(static_cast<uint32_t>(mraw) << 16);
+      const ptx::f32x2 mval2 = ptx::pk2(mval, mval);
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + h * 64;
 #pragma unroll
       for (int chunk = 0; chunk < 4; ++chunk) {

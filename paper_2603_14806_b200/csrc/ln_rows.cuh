@@ -22,7 +22,8 @@ namespace foldcp {
 // kAffine = false: plain normalisation (x - mean) * rstd; gamma / beta are then folded into the
 // weights and biases of the GEMM that consumes the tile (gaddr / baddr unused).
 // kRows = rows per thread in flight (2 = more latency hiding, ~100 registers; 1 = ~60 registers).
-template <bool kF16, bool kAffine = true, int kRows = 2>
+// kLnThreads = threads of the LayerNorm group (128 or 256; 256 only with kRows = 1).
+template <bool kF16, bool kAffine = true, int kRows = 2, int kLnThreads = 128>
 __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t box_stride, int tid,
                                                        uint32_t gaddr, uint32_t baddr, float eps) {
   const uint32_t j = static_cast<uint32_t>(tid & 3);        // quarter of the row: channels 32j..
@@ -33,9 +34,11 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
   // Each thread works on two rows (r, r + 32) at once: the two dependency chains (loads, sums,
   // shuffles, rsqrt) interleave, which matters because one LayerNorm warp per scheduler is
   // latency-bound, not throughput-bound.
+  static_assert(kLnThreads == 128 || (kLnThreads == 256 && kRows == 1), "unsupported LayerNorm shape");
+  constexpr int kRowsPerPass = (kLnThreads / 4) * kRows;
 #pragma unroll 1
-  for (int pass = 0; pass < 4 / kRows; ++pass) {
-    const uint32_t r0 = static_cast<uint32_t>(pass * 32 * kRows + (tid >> 2));
+  for (int pass = 0; pass < 128 / kRowsPerPass; ++pass) {
+    const uint32_t r0 = static_cast<uint32_t>(pass * kRowsPerPass + (tid >> 2));
     const uint32_t sw = r0 & 7u;                              // (r0 + 32) & 7 is the same
     const uint32_t row0 = tile + box * box_stride + r0 * 128u;
     ptx::f32x2 x[kRows][4][4];
