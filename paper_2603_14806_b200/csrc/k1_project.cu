@@ -23,18 +23,18 @@
 //
 // Persistent kernel, one CTA per SM, 16 warps, tile = 128 pairs:
 //   warp 0       TMA producer : z tiles into a kZStages-deep ring
-//   warp 1       MMA issuer   : per tile four "units" (pair half hh, tensor u in {a, b}); a unit =
-//                               projection + gate MMA (M=128 ch, N=64 pairs, K=128) into one
-//                               128-column TMEM slot; two slots, so the epilogue of one unit
-//                               overlaps the MMAs of the next
-//   warp 2       TMEM allocator (512 columns: 256 weights + 2 x 128 accumulators)
+//   warp 1       MMA issuer   : per tile eight "units" (pair quarter pq, tensor u in {a, b}); a unit
+//                               = projection + gate MMA (M=128 ch, N=32 pairs, K=128) into one
+//                               64-column TMEM slot; four slots, two per tensor, so the MMAs of
+//                               unit pq+1 overlap the epilogue of unit pq of the same tensor
+//   warp 2       TMEM allocator (512 columns: 256 weights + 4 x 64 accumulators)
 //   warps 4-7    LayerNorm    : ln_rows.cuh -- z rows -> registers -> two-pass mean/variance in
 //                               fp32 -> n written back in place as the K-major B operand; also
 //                               stages the pair mask and an "all ones" flag per tile
-//   warps 8-15   epilogue     : two independent teams of four warps (team 0 = tensor a / TMEM slot
-//                               0, team 1 = b / slot 1): tcgen05.ld both accumulators -> bias,
-//                               sigmoid, gate, mask in packed fp32 -> bf16 -> swizzled smem ->
-//                               TMA store [128 ch][64 pairs]
+//   warps 8-15   epilogue     : two independent teams of four warps (team 0 = tensor a, team 1 =
+//                               b): tcgen05.ld both accumulators -> bias, sigmoid, gate, mask in
+//                               packed fp32 -> bf16 -> swizzled smem -> TMA store [128 ch][64 pairs]
+//                               (also: once per CTA they fold and park the weights in TMEM)
 #include <cuda_bf16.h>
 
 #include "common.h"
@@ -50,8 +50,8 @@ constexpr int kThreads = 512;
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box, 128 rows x 64 bf16
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 16-bit tile (two k-halves)
 constexpr int kZStages = 4;
-constexpr int kMaskSlots = 8;                   // >= kZStages + 2 (see the epilogue), power of 2
-constexpr int kOutBufs = 4;                     // staging buffers [128 ch][64 pairs], one per unit
+constexpr int kMaskSlots = 8;                   // >= kZStages + 3 (see the epilogue), power of 2
+constexpr int kOutBufs = 4;                     // staging buffers [128 ch][64 pairs], two per team
 
 constexpr int kOffZ = 0;                                   // z ring
 constexpr int kOffOut = kOffZ + kZStages * kMatBytes;      // staging buffers
@@ -141,7 +141,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (ptx::elect_one()) {
-      // A = folded weights in TMEM, B = n (K-major, 64 pairs), both fp16 (or both bf16)
+      // A = folded weights in TMEM, B = n (K-major, 32 pairs), both fp16 (or both bf16)
       constexpr uint32_t kFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
       constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, 32, kFmt, kFmt, 0, 0);
       ptx::mbar_wait(wready, 0);

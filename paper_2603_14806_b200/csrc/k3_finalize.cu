@@ -16,16 +16,22 @@
 //                                                       channel-major output needs is done by the
 //                                                       tensor core's operand fetch, not by us)
 //
-// Persistent kernel, one CTA per SM, 20 warps, tile = 128 pairs:
+// Both LayerNorm affines are folded into the GEMMs once per CTA (W LN(x) + b =
+// (W diag(gamma)) n + (W beta + b), n = (x - mean) * rstd): gamma goes into the resident weights
+// while they are converted to the operand format of the normalised tiles (fp16, see common.h),
+// beta into per-channel fp32 biases in shared memory.  The LayerNorm warps only normalise.
+//
+// Persistent kernel, one CTA per SM, 24 warps, tile = 128 pairs:
 //   warp 0       TMA producer : W_g, W_o once (resident), then (z tile, o tile) into a 2-deep ring
 //   warp 1       MMA issuer   : two MMAs (M=128 pairs, N=128 ch, K=128) into a 256-column TMEM
 //                               slot; two slots, so the epilogue overlaps the next tile's MMAs
-//   warp 2       TMEM allocator;  warp 3 stages the LayerNorm gammas / betas in smem
+//   warp 2       TMEM allocator
 //   warps 4-7    LayerNorm(z) : ln_rows.cuh (rows in registers, two-pass statistics, in place)
-//   warps 8-11   LayerNorm(o) : thread = 2 pairs x 64 channels of the [k][pair] tile, shifted
-//                               one-pass statistics combined across the half-warps, in place
-//   warps 12-19  epilogue     : tcgen05.ld -> bias, sigmoid gate, mask in fp32 -> bf16 -> swizzled
-//                               smem -> TMA store [128 pairs][64 ch]
+//   warps 8-15   LayerNorm(o) : thread = 2 pairs x 32 channels of the [k][pair] tile, held in
+//                               registers, exact two-pass statistics combined across the four
+//                               channel quarters with shuffles, in place
+//   warps 16-23  epilogue     : tcgen05.ld -> bias, sigmoid gate, mask in packed fp32 -> bf16 ->
+//                               swizzled smem -> TMA store [128 pairs][64 ch]
 #include <cuda_bf16.h>
 
 #include "common.h"
