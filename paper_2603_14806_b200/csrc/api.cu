@@ -56,6 +56,19 @@ static EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
+// FOLDCP_TMAP_L2PROMO = 0 / 64 / 128 / 256 (default 256): L2 promotion size of every tensor map
+static CUtensorMapL2promotion l2_promotion() {
+  static const CUtensorMapL2promotion v = [] {
+    const char* e = getenv("FOLDCP_TMAP_L2PROMO");
+    const int n = e ? atoi(e) : 256;
+    return n == 0     ? CU_TENSOR_MAP_L2_PROMOTION_NONE
+           : n == 64  ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
+           : n == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                      : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
+  }();
+  return v;
+}
+
 int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int rank,
                       const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
                       int swizzle) {
@@ -77,7 +90,7 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
          swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
          : swizzle != 0 ? CU_TENSOR_MAP_SWIZZLE_128B
                         : CU_TENSOR_MAP_SWIZZLE_NONE,
-         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+         l2_promotion(), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? FOLDCP_OK : FOLDCP_ERR_CUDA;
 }
 

@@ -133,7 +133,7 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
       // a_c / b_c are re-read by every tile of channel c: keep them in L2, stream o past them
-      const uint64_t pol_ld = prm.l2_hints ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
+      const uint64_t pol_ld = prm.l2_hints == 1 ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
       int stage = 0;
       uint32_t phase = 0;
       for (int t = group_id; t < prm.num_tiles; t += num_groups) {
@@ -364,7 +364,7 @@ int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int di
   prm.num_kb = (N + kBlockK - 1) / kBlockK;
   static const int l2_hints = [] {
     const char* e = getenv("FOLDCP_K2_L2_HINTS");
-    return (e && e[0] == '1') ? 1 : 0;   // measured: hints raise DRAM traffic (55 vs 34 GB)
+    return e ? atoi(e) : 0;   // 1: loads evict_last + stores evict_first; 2: stores only
   }();
   prm.l2_hints = l2_hints;
   static const int panel = [] {
