@@ -29,7 +29,8 @@ gating, A8 `mask_output` flag.
 A library primitive (numpy matmul) serves as the dense-contraction step; there is no
 blocking, fusion or reordering beyond the definition.  Pins: tests/test_oracle_pins.py
 (brute-force index loops from oracle/brute_force.py on tiny shapes, closed forms S1-S4,
-invariants I1/I1'/I2/I3/I6/S8, N=1) -- every function below is pinned there.
+invariants I1/I1'/I2/I3/I6/S8, N=1; residual / batched forms against the brute force) --
+every function below is pinned there.
 """
 from __future__ import annotations
 
@@ -119,6 +120,25 @@ def trimul(z: np.ndarray, mask: Optional[np.ndarray], p: Dict[str, np.ndarray], 
     b = gated_projection(zp, mask, p["w_b"], p.get("b_b"), p["w_b_gate"], p.get("b_b_gate"))
     o = contraction(a, b, direction)
     return output_stage(o, zp, mask, p, eps, mask_output)
+
+
+def trimul_residual(z: np.ndarray, mask: Optional[np.ndarray], p: Dict[str, np.ndarray],
+                    direction: int, eps: float = 1e-5, mask_output: bool = True) -> np.ndarray:
+    """The paper's own form of the update, PAPER.md lines 121-128 (Eq. 2-3 are written
+    "z_nm += ..."): z + trimul(z).  SURVEY 8(f) NEXT-1; c_hidden need not equal c_z, the update
+    always has c_z channels."""
+    z = np.asarray(z, _F)
+    return z + trimul(z, mask, p, direction, eps=eps, mask_output=mask_output)
+
+
+def trimul_batched(z: np.ndarray, mask: Optional[np.ndarray], p: Dict[str, np.ndarray],
+                   direction: int, eps: float = 1e-5, mask_output: bool = True,
+                   residual: bool = False) -> np.ndarray:
+    """z[B, N, N, c_z] (z in R^{B x N x N x D}), pair mask [B, N, N] or None:
+    the batch elements are independent problems with shared parameters."""
+    f = trimul_residual if residual else trimul
+    return np.stack([f(z[b], None if mask is None else mask[b], p, direction, eps=eps,
+                       mask_output=mask_output) for b in range(z.shape[0])])
 
 
 def trimul_subgrid(z_a: np.ndarray, mask_a: Optional[np.ndarray],

@@ -66,6 +66,32 @@ def test_brute_force(N, c_z, c, direction, mask_output):
     assert relerr(got, ref) < 1e-12
 
 
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_residual_and_batched_forms_against_brute_force(direction):
+    """PAPER.md lines 121-128 write the update as `z_nm += ...`; line 130 carries a batch
+    dimension.  Pinned against the scalar loops: residual = z + brute-force update, element by
+    element; batched = the brute force applied to every batch element separately."""
+    rng = np.random.default_rng(31 + direction)
+    Bn, N, c_z, c = 2, 4, 8, 3
+    z = rng.standard_normal((Bn, N, N, c_z))
+    M = (rng.random((Bn, N, N)) > 0.3).astype(np.float64)
+    p = rand_params(rng, c_z, c)
+    upd = [np.array(brute_force.trimul_brute(z[b].tolist(), M[b].tolist(), tolist(p), direction))
+           for b in range(Bn)]
+    for b in range(Bn):
+        got = orc.trimul_residual(z[b], M[b], p, direction)
+        want = np.array([[[z[b, i, j, ch] + upd[b][i, j, ch] for ch in range(c_z)]
+                          for j in range(N)] for i in range(N)])
+        assert relerr(got, want) < 1e-12
+    got = orc.trimul_batched(z, M, p, direction)
+    assert got.shape == (Bn, N, N, c_z) and relerr(got, np.stack(upd)) < 1e-12
+    got = orc.trimul_batched(z, M, p, direction, residual=True)
+    assert relerr(got, z + np.stack(upd)) < 1e-12
+    # a zero update (W_o = 0, b_o = 0: closed form S4) leaves exactly z
+    q = dict(p); q["w_o"] = np.zeros_like(p["w_o"]); q["b_o"] = np.zeros_like(p["b_o"])
+    assert np.array_equal(orc.trimul_residual(z[0], M[0], q, direction), z[0])
+
+
 def test_brute_force_no_bias_no_mask_soft_mask():
     rng = np.random.default_rng(7)
     N, c_z, c = 4, 8, 4
