@@ -15,8 +15,8 @@
  *       o   = Eq. 2 (direction = FOLDCP_OUTGOING) or Eq. 3 (FOLDCP_INCOMING), per channel
  *       out = [M (.)] sigmoid(W_g z' + b_g) (.) (W_o LayerNorm(o; ln_out_*) + b_o)   [N,N,c_z]
  *
- *   `out` is the UPDATE only: the paper's "z_nm +=" residual add belongs to the caller
- *   (reading A1).
+ *   `out` is the UPDATE only by default (reading A1); params->add_residual = 1 gives
+ *   the paper's "z_nm +=" form, out = z + update, fused into the last kernel.
  *
  * Memory: every tensor pointer below is a DEVICE pointer owned by the caller and must stay valid
  * until the work enqueued on `stream` has finished.  The params struct itself is HOST memory and
@@ -58,6 +58,9 @@ typedef struct {
   int32_t dtype;        /* foldcp_dtype_t                                                          */
   float ln_eps;         /* LayerNorm epsilon (inside the sqrt); 1e-5 in every BASELINE config      */
   int32_t mask_output;  /* 1: out_ij *= M_ij (north_star's epilogue); 0: mask only a and b (AF3)   */
+  int32_t add_residual; /* 1: out = z + update, the paper's "z_nm +=" form;
+                         * 0: out = update only (reading A1)                             */
+  int32_t reserved0;    /* must be 0                                                               */
   const float* ln_in_gamma;  /* [c_z]      fp32 in both modes                                      */
   const float* ln_in_beta;   /* [c_z]                                                              */
   const void* w_a;           /* [c_hidden][c_z] row-major (= torch Linear.weight), dtype above     */
@@ -95,6 +98,16 @@ typedef struct {
  */
 int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
                   int c_z, int c_hidden, int direction, void* out, void* stream);
+
+/*
+ * Batched form (z in R^{B x N x N x D}): `batch` independent problems with
+ * shared parameters, z [batch][N][N][c_z], mask [batch][N][N] or NULL, out [batch][N][N][c_z].
+ * The same workspace (sized for ONE problem) is reused by the batch elements, which are enqueued
+ * back to back on `stream`.  Equivalent to `batch` foldcp_trimul calls, bit for bit.
+ */
+int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_params* params,
+                          int batch, int N, int c_z, int c_hidden, int direction, void* out,
+                          void* stream);
 
 /* Bytes of device scratch foldcp_trimul needs for this problem (a, b and o, channel-major);
  * 0 if the shape / dtype is unsupported.  Monotone in N. */

@@ -21,7 +21,7 @@ _LIB_NAME = "libfoldcp_trimul.so"
 _lib = None
 
 EXPORTS = (
-    "foldcp_trimul", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
+    "foldcp_trimul", "foldcp_trimul_batched", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
     "foldcp_trimul_contract", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
     "foldcp_status_string", "foldcp_version",
 )
@@ -37,6 +37,7 @@ class _Params(ctypes.Structure):
     _fields_ = [
         ("struct_size", ctypes.c_uint32), ("dtype", ctypes.c_int32),
         ("ln_eps", ctypes.c_float), ("mask_output", ctypes.c_int32),
+        ("add_residual", ctypes.c_int32), ("reserved0", ctypes.c_int32),
         ("ln_in_gamma", ctypes.c_void_p), ("ln_in_beta", ctypes.c_void_p),
         ("w_a", ctypes.c_void_p), ("w_a_gate", ctypes.c_void_p),
         ("w_b", ctypes.c_void_p), ("w_b_gate", ctypes.c_void_p),
@@ -67,6 +68,8 @@ def load() -> ctypes.CDLL:
     vp, ci = ctypes.c_void_p, ctypes.c_int
     lib.foldcp_trimul.restype = ci
     lib.foldcp_trimul.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_batched.restype = ci
+    lib.foldcp_trimul_batched.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, ci, ci, vp, vp]
     lib.foldcp_trimul_workspace_bytes.restype = ctypes.c_size_t
     lib.foldcp_trimul_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.foldcp_trimul_project.restype = ci
@@ -114,13 +117,16 @@ def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
 
 
 def make_params(p: Dict[str, Optional[torch.Tensor]], dtype: int, eps: float = 1e-5,
-                mask_output: bool = True, workspace: Optional[torch.Tensor] = None) -> _Params:
+                mask_output: bool = True, workspace: Optional[torch.Tensor] = None,
+                residual: bool = False) -> _Params:
     """Fill the C struct from a dict of device tensors (names of synth.make_params)."""
     s = _Params()
     s.struct_size = ctypes.sizeof(_Params)
     s.dtype = dtype
     s.ln_eps = eps
     s.mask_output = 1 if mask_output else 0
+    s.add_residual = 1 if residual else 0
+    s.reserved0 = 0
     for name in ("ln_in_gamma", "ln_in_beta", "w_a", "w_a_gate", "w_b", "w_b_gate", "b_a",
                  "b_a_gate", "b_b", "b_b_gate", "w_g", "b_g", "ln_out_gamma", "ln_out_beta",
                  "w_o", "b_o"):
@@ -141,29 +147,41 @@ def _stream() -> int:
 def trimul(z: torch.Tensor, mask: Optional[torch.Tensor], p: Dict[str, torch.Tensor],
            direction: int, out: Optional[torch.Tensor] = None,
            workspace: Optional[torch.Tensor] = None, eps: float = 1e-5,
-           mask_output: bool = True) -> torch.Tensor:
+           mask_output: bool = True, residual: bool = False) -> torch.Tensor:
     """One forward triangle multiplicative update on the current CUDA stream (asynchronous).
 
-    z [N, N, c_z] and mask [N, N] (or None) are CUDA tensors of the same dtype (fp32 / bf16).
+    z [N, N, c_z] and mask [N, N] (or None) are CUDA tensors of the same dtype (fp32 / bf16);
+    a leading batch dimension (z [B, N, N, c_z], mask [B, N, N]) goes through
+    foldcp_trimul_batched.  `residual=True` returns z + update (the paper's "z +=" form).
     `workspace` (uint8, >= workspace_bytes(N)) and `out` are allocated here if not given.
     """
     lib = load()
     if not z.is_cuda:
         raise ValueError("z must be a CUDA tensor (no CPU fallback)")
-    assert z.dim() == 3 and z.shape[0] == z.shape[1] and z.is_contiguous()
-    N, c_z = z.shape[0], z.shape[2]
+    batch = None
+    if z.dim() == 4:
+        batch = z.shape[0]
+        assert z.shape[1] == z.shape[2] and z.is_contiguous()
+        N, c_z = z.shape[1], z.shape[3]
+    else:
+        assert z.dim() == 3 and z.shape[0] == z.shape[1] and z.is_contiguous()
+        N, c_z = z.shape[0], z.shape[2]
     c_hidden = p["w_a"].shape[0]
     dt = dtype_code(z)
     if mask is not None:
-        assert mask.dtype == z.dtype and mask.is_contiguous() and mask.shape == (N, N)
+        assert mask.dtype == z.dtype and mask.is_contiguous() and mask.shape == z.shape[:-1]
     if workspace is None:
         workspace = torch.empty(max(workspace_bytes(N, c_z, c_hidden, dt), 1), dtype=torch.uint8,
                                 device=z.device)
     if out is None:
         out = torch.empty_like(z)
-    s = make_params(p, dt, eps, mask_output, workspace)
-    st = lib.foldcp_trimul(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
-                           int(direction), out.data_ptr(), _stream())
+    s = make_params(p, dt, eps, mask_output, workspace, residual)
+    if batch is None:
+        st = lib.foldcp_trimul(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
+                               int(direction), out.data_ptr(), _stream())
+    else:
+        st = lib.foldcp_trimul_batched(z.data_ptr(), _ptr(mask), ctypes.byref(s), batch, N, c_z,
+                                       c_hidden, int(direction), out.data_ptr(), _stream())
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul")
     return out

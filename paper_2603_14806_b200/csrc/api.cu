@@ -120,6 +120,9 @@ int check_params(const foldcp_trimul_params* p) {
   if (p->struct_size != sizeof(foldcp_trimul_params)) return FOLDCP_ERR_INVALID_ARG;
   if (p->dtype != FOLDCP_F32 && p->dtype != FOLDCP_BF16) return FOLDCP_ERR_INVALID_ARG;
   if (!(p->ln_eps >= 0.0f)) return FOLDCP_ERR_INVALID_ARG;
+  if (p->reserved0 != 0 || (p->add_residual != 0 && p->add_residual != 1) ||
+      (p->mask_output != 0 && p->mask_output != 1))
+    return FOLDCP_ERR_INVALID_ARG;
   const void* required[] = {p->ln_in_gamma, p->ln_in_beta, p->w_a, p->w_a_gate, p->w_b,
                             p->w_b_gate, p->w_g, p->ln_out_gamma, p->ln_out_beta, p->w_o};
   for (const void* q : required)
@@ -241,6 +244,30 @@ int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* p
       FOLDCP_OK)
     return st;
   return foldcp_trimul_finalize(o, z, mask, params, N, c_z, c_hidden, out, stream);
+}
+
+int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_params* params,
+                          int batch, int N, int c_z, int c_hidden, int direction, void* out,
+                          void* stream) {
+  if (batch <= 0) return FOLDCP_ERR_INVALID_ARG;
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (!z || !out) return FOLDCP_ERR_INVALID_ARG;
+  const size_t eb = elem_bytes(params->dtype);
+  const size_t tensor_bytes = static_cast<size_t>(N) * N * kChannels * eb;
+  const size_t mask_bytes = static_cast<size_t>(N) * N * eb;
+  // every batch element must itself satisfy the 16-byte alignment rule
+  if (batch > 1 && ((tensor_bytes | mask_bytes) & 15u) != 0) return FOLDCP_ERR_ALIGNMENT;
+  if (overlaps(out, tensor_bytes * batch, z, tensor_bytes * batch)) return FOLDCP_ERR_ALIAS;
+  for (int b = 0; b < batch; ++b) {
+    const uint8_t* zb = static_cast<const uint8_t*>(z) + b * tensor_bytes;
+    const uint8_t* mb = mask ? static_cast<const uint8_t*>(mask) + b * mask_bytes : nullptr;
+    uint8_t* ob = static_cast<uint8_t*>(out) + b * tensor_bytes;
+    if ((st = foldcp_trimul(zb, mb, params, N, c_z, c_hidden, direction, ob, stream)) != FOLDCP_OK)
+      return st;
+  }
+  return FOLDCP_OK;
 }
 
 int foldcp_trimul_launches_per_call(int dtype) {

@@ -68,6 +68,7 @@ static_assert(kSmemBytes <= 232448, "K3 shared memory exceeds 227 KB");
 
 struct K3Params {
   const __nv_bfloat16* mask;   // [R] or nullptr (also nullptr when mask_output == 0)
+  const __nv_bfloat16* z_res;  // z [R][128] when out = z + update (add_residual), else nullptr
   const float* g_in;
   const float* b_in;
   const float* g_out;
@@ -370,8 +371,17 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const float mval = __uint_as_float(static_cast<uint32_t>(mraw) << 16);
       const ptx::f32x2 mval2 = ptx::pk2(mval, mval);
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + h * 64;
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
 #pragma unroll
       for (int chunk = 0; chunk < 4; ++chunk) {
+        // residual: this pair's 16 raw z channels (the tile was just read by TMA: an L2 hit)
+        uint4 zr0 = make_uint4(0u, 0u, 0u, 0u), zr1 = zr0;
+        if (prm.z_res != nullptr && p < prm.R) {
+          const uint4* zp = reinterpret_cast<const uint4*>(prm.z_res + p * kC + h * 64 + chunk * 16);
+          zr0 = __ldg(zp);
+          zr1 = __ldg(zp + 1);
+        }
+        const uint32_t zr[8] = {zr0.x, zr0.y, zr0.z, zr0.w, zr1.x, zr1.y, zr1.z, zr1.w};
         uint32_t vg[16], vo[16];
         ptx::tmem_ld_32x16(taddr + chunk * 16, vg);
         ptx::tmem_ld_32x16(taddr + 128 + chunk * 16, vo);
@@ -404,7 +414,8 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
             }
             const ptx::f32x2 y = ptx::mul2(ptx::add2(ptx::pk2u(vo[j], vo[j + 1]), bo2[e2]), mval2);
             float v0, v1;
-            ptx::upk2(ptx::mul2(y, sg), v0, v1);
+            // + z (exactly 0 when there is no residual: bf16 zero bits)
+            ptx::upk2(ptx::fma2(y, sg, ptx::bf16x2_to_f32x2(zr[j4 * 2 + e2])), v0, v1);
             packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
           }
         }
@@ -473,6 +484,7 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   }
   K3Params prm;
   prm.mask = p->mask_output ? static_cast<const __nv_bfloat16*>(mask) : nullptr;
+  prm.z_res = p->add_residual ? static_cast<const __nv_bfloat16*>(z) : nullptr;
   prm.g_in = p->ln_in_gamma;
   prm.b_in = p->ln_in_beta;
   prm.g_out = p->ln_out_gamma;

@@ -178,15 +178,21 @@ simt_finalize_kernel(const T* __restrict__ o, const T* __restrict__ z, const T* 
                      const float* __restrict__ b_g, const float* __restrict__ b_o,
                      const float* __restrict__ g_in, const float* __restrict__ be_in,
                      const float* __restrict__ g_out, const float* __restrict__ be_out, float eps,
-                     int mask_output, long long npairs, T* __restrict__ out) {
+                     int mask_output, int add_residual, long long npairs, T* __restrict__ out) {
   __shared__ float zs[kPairsPerBlock][C];
   __shared__ float os[kPairsPerBlock][C];
   __shared__ float ms[kPairsPerBlock];
   const long long p0 = static_cast<long long>(blockIdx.x) * kPairsPerBlock;
   const int np = static_cast<int>(min(static_cast<long long>(kPairsPerBlock), npairs - p0));
   const int tid = threadIdx.x;
-  for (int p = 0; p < np; ++p) {
+  float zres[kPairsPerBlock];
+#pragma unroll
+  for (int p = 0; p < kPairsPerBlock; ++p) zres[p] = 0.f;
+#pragma unroll
+  for (int p = 0; p < kPairsPerBlock; ++p) {
+    if (p >= np) break;
     zs[p][tid] = ldf(z + (p0 + p) * C + tid);
+    if (add_residual) zres[p] = zs[p][tid];
     os[p][tid] = ldf(o + static_cast<long long>(tid) * npairs + p0 + p);
   }
   if (tid < np) ms[tid] = (mask && mask_output) ? ldf(mask + p0 + tid) : 1.0f;
@@ -208,9 +214,11 @@ simt_finalize_kernel(const T* __restrict__ o, const T* __restrict__ z, const T* 
     }
   }
   const float bg = b_g ? b_g[tid] : 0.f, bo = b_o ? b_o[tid] : 0.f;
-  for (int p = 0; p < np; ++p) {
+#pragma unroll
+  for (int p = 0; p < kPairsPerBlock; ++p) {
+    if (p >= np) break;
     const float v = ms[p] * sigmoidf_acc(accg[p] + bg) * (acco[p] + bo);
-    stf(out + (p0 + p) * C + tid, v);
+    stf(out + (p0 + p) * C + tid, zres[p] + v);
   }
 }
 
@@ -252,7 +260,7 @@ int finalize_t(const void* o, const void* z, const void* mask, const foldcp_trim
       static_cast<const T*>(o), static_cast<const T*>(z), static_cast<const T*>(mask),
       static_cast<const T*>(p->w_g), static_cast<const T*>(p->w_o), p->b_g, p->b_o,
       p->ln_in_gamma, p->ln_in_beta, p->ln_out_gamma, p->ln_out_beta, p->ln_eps, p->mask_output,
-      npairs, static_cast<T*>(out));
+      p->add_residual, npairs, static_cast<T*>(out));
   return check_launch();
 }
 

@@ -57,7 +57,9 @@ def _params(lib, dtype=B.BF16, ws=0x10000, ws_bytes=1 << 40):
     s.ln_eps = 1e-5
     s.mask_output = 1
     fake = 0x1000    # never dereferenced: all of these calls must fail on the host first
-    for i, (name, _) in enumerate(B._Params._fields_[4:20]):
+    ptrs = [n for n, t in B._Params._fields_ if t is ctypes.c_void_p and n != "workspace"]
+    assert len(ptrs) == 16
+    for i, name in enumerate(ptrs):
         setattr(s, name, fake + 0x100 * i)
     s.workspace = ws
     s.workspace_bytes = ws_bytes
@@ -88,6 +90,14 @@ def test_host_side_rejections(lib):
     assert _call(lib, bad) == INVALID
     bad = _params(lib); bad.dtype = 7
     assert _call(lib, bad) == INVALID
+    bad = _params(lib); bad.add_residual = 2
+    assert _call(lib, bad) == INVALID
+    bad = _params(lib); bad.reserved0 = 1
+    assert _call(lib, bad) == INVALID
+    bad = _params(lib); bad.mask_output = 5
+    assert _call(lib, bad) == INVALID
+    assert lib.foldcp_trimul_batched(0x100000, None, ctypes.byref(_params(lib)), 0, 64, 128, 128, 0,
+                                     0x900000, None) == INVALID
     for name in ("ln_in_gamma", "w_a", "w_b_gate", "w_g", "ln_out_beta", "w_o"):
         bad = _params(lib); setattr(bad, name, None)
         assert _call(lib, bad) == INVALID, name

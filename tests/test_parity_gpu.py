@@ -116,6 +116,53 @@ def test_bf16_n1024_full_tensor(direction):
     assert e["rel_fro"] < 5e-3
 
 
+# ---------------------------------------------------------------- NEXT-1: residual-fused and batched forms
+@pytest.mark.parametrize("cfg_i,N", [(0, 67), (1, 264)])
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_residual_fused(cfg_i, N, direction):
+    """out = z + update (PAPER.md lines 121-128 write the update as `z_nm +=`), fused into K3."""
+    from oracle import trimul_oracle as orc
+    cfg = synth.CONFIGS[cfg_i]
+    z, M, p = synth.make_inputs(cfg, direction, "cpu", N=N)
+    M = synth.pair_mask(synth.make_token_mask("tail", N, cfg.seed), cfg.dtype)
+    ref_u = U.oracle_full(z, M, p, direction)
+    ref = orc.trimul_residual(U.np64(z), U.np64(M), U.params64(p), direction)
+    out = B.trimul(z.to(DEV), M.to(DEV), to_dev(p), direction, residual=True)
+    torch.cuda.synchronize()
+    got = U.np64(out)
+    assert np.all(np.isfinite(got))
+    # the error budget is the update's (north_star tolerance on the update) plus the rounding of
+    # the sum to the output dtype (half an ulp of |z + update|)
+    ulp = 2.0 ** -8 if cfg.dtype == "bf16" else 2.0 ** -23
+    rms_u = np.sqrt(np.mean(ref_u ** 2))
+    tol = U.TOL[cfg.dtype]["max_over_rms"] * rms_u + 0.5 * ulp * np.abs(ref).max()
+    assert np.abs(got - ref).max() <= tol
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= U.TOL[cfg.dtype]["rel_fro"]
+
+
+@pytest.mark.parametrize("residual", [False, True])
+def test_batched_equals_single_calls_bitwise(residual):
+    cfg = synth.CONFIGS[1]
+    N, Bn = 136, 3
+    zs, Ms = [], []
+    for b in range(Bn):
+        z, _, p = synth.make_inputs(cfg, OUT, "cpu", N=N)
+        g = torch.Generator().manual_seed(100 + b)
+        zs.append((z.float() + 0.25 * torch.randn(z.shape, generator=g)).to(z.dtype))
+        Ms.append(synth.pair_mask(synth.make_token_mask("scatter", N, cfg.seed + b), cfg.dtype))
+    zb, Mb, pd = torch.stack(zs).to(DEV), torch.stack(Ms).to(DEV), to_dev(p)
+    out_b = B.trimul(zb, Mb, pd, INC, residual=residual)
+    singles = [B.trimul(zb[b].contiguous(), Mb[b].contiguous(), pd, INC, residual=residual)
+               for b in range(Bn)]
+    torch.cuda.synchronize()
+    assert out_b.shape == zb.shape
+    for b in range(Bn):
+        assert torch.equal(out_b[b], singles[b])
+    e = U.errors(U.np64(out_b[1]) - (U.np64(zb[1]) if residual else 0.0),
+                 U.oracle_full(zs[1], Ms[1], p, INC))
+    assert e["rel_fro"] < 1e-2 + (2e-2 if residual else 0.0)
+
+
 # ---------------------------------------------------------------- BASELINE configs 2-4 (sub-grid oracle)
 def run_subgrid(cfg, direction, n_idx, seed):
     N = cfg.N
