@@ -21,20 +21,21 @@
 // warps only normalise.  W diag(gamma) is rounded to fp16 (2^-12 relative; n is fp16 too -- see
 // common.h kNormFp16), the folded bias stays fp32 in registers.
 //
-// Persistent kernel, one CTA per SM, 16 warps, tile = 128 pairs:
+// Persistent kernel, one CTA per SM, 28 warps (FOLDCP_K1_TEAMS = 4; 16 warps with 2), tile = 128 pairs:
 //   warp 0       TMA producer : z tiles into a kZStages-deep ring
 //   warp 1       MMA issuer   : per tile eight "units" (pair quarter pq, tensor u in {a, b}); a unit
 //                               = projection + gate MMA (M=128 ch, N=32 pairs, K=128) into one
-//                               64-column TMEM slot; four slots, two per tensor, so the MMAs of
-//                               unit pq+1 overlap the epilogue of unit pq of the same tensor
+//                               64-column TMEM slot; four slots, two per tensor
 //   warp 2       TMEM allocator (512 columns: 256 weights + 4 x 64 accumulators)
-//   warps 4-7    LayerNorm    : ln_rows.cuh -- z rows -> registers -> two-pass mean/variance in
+//   LayerNorm    8 warps      : ln_rows.cuh -- z rows -> registers -> two-pass mean/variance in
 //                               fp32 -> n written back in place as the K-major B operand; also
-//                               stages the pair mask and an "all ones" flag per tile
-//   warps 8-15   epilogue     : two independent teams of four warps (team 0 = tensor a, team 1 =
-//                               b): tcgen05.ld both accumulators -> bias, sigmoid, gate, mask in
-//                               packed fp32 -> bf16 -> swizzled smem -> TMA store [128 ch][64 pairs]
-//                               (also: once per CTA they fold and park the weights in TMEM)
+//                               stage the pair mask and an "all ones" flag per tile
+//   epilogue     16 warps     : four teams of four warps (tensor x pair-quarter parity = one TMEM
+//                               slot each): tcgen05.ld both accumulators -> bias, sigmoid, gate,
+//                               mask in packed fp32 -> bf16 -> swizzled smem -> TMA store
+//                               [128 ch][64 pairs] per tensor (also: once per CTA they fold and
+//                               park the weights in TMEM).  Four sigmoid-issuing warps per
+//                               scheduler keep the MUFU pipe busier than two (measured -7 %).
 #include <cuda_bf16.h>
 
 #include "common.h"
@@ -46,7 +47,17 @@ namespace {
 
 constexpr int kC = kChannels;                   // 128
 constexpr int kTilePairs = 128;
-constexpr int kThreads = 512;
+// warp roles: 0 TMA, 1 MMA, 2 TMEM allocator, 3 idle, then LayerNorm warps, then epilogue teams
+#ifndef FOLDCP_K1_TEAMS
+#define FOLDCP_K1_TEAMS 4
+#endif
+constexpr int kTeams = FOLDCP_K1_TEAMS;         // epilogue teams of 4 warps: 2 or 4
+constexpr int kPar = kTeams / 2;                // teams per output tensor (pair-quarter parities)
+constexpr int kLnWarps = kTeams == 2 ? 4 : 8;   // 4 teams leave 72 registers/thread: one row in flight
+constexpr int kWarpLn = 4;
+constexpr int kWarpEpi = kWarpLn + kLnWarps;    // a multiple of 4 (TMEM lane quadrants)
+constexpr int kThreads = (kWarpEpi + 4 * kTeams) * 32;
+static_assert(kTeams == 2 || kTeams == 4, "two or four epilogue teams");
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box, 128 rows x 64 bf16
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 16-bit tile (two k-halves)
 constexpr int kZStages = 4;
@@ -105,13 +116,13 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     for (int s = 0; s < kZStages; ++s) {
       ptx::mbar_init(zfull(s), 1);
       ptx::mbar_init(zempty(s), 1);
-      ptx::mbar_init(zready(s), 128);
+      ptx::mbar_init(zready(s), kLnWarps * 32);
     }
     for (int u = 0; u < 4; ++u) {
       ptx::mbar_init(tfull(u), 1);
       ptx::mbar_init(tempty(u), 4);
     }
-    ptx::mbar_init(wready, 8);
+    ptx::mbar_init(wready, 4 * kTeams);
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
@@ -180,12 +191,12 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::umma_commit<1>(zempty(s));   // stage reusable once all MMAs of the tile retired
       }
     }
-  } else if (warp >= 4 && warp < 8) {
+  } else if (warp >= kWarpLn && warp < kWarpEpi) {
     // ===================== LayerNorm =====================
     const int r = threadIdx.x - 128;
     // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
     auto load_mask = [&](int t) -> unsigned short {
-      if (prm.mask == nullptr) return static_cast<unsigned short>(0x3f80);   // bf16 1.0
+      if (prm.mask == nullptr || r >= kTilePairs) return static_cast<unsigned short>(0x3f80);
       if (t >= prm.num_tiles) return static_cast<unsigned short>(0);
       const long long p = static_cast<long long>(t) * kTilePairs + r;
       return p < prm.R ? __ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)
@@ -198,22 +209,27 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const unsigned short mraw = mnext;
       mnext = load_mask(t + stride);
       ptx::mbar_wait(zfull(s), (it / kZStages) & 1);
-      layernorm_rows_inplace<kNormFp16, false>(smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0,
-                                               prm.eps);
+      layernorm_rows_inplace<kNormFp16, false, kLnWarps == 4 ? 2 : 1, kLnWarps * 32>(
+          smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0, prm.eps);
       const int ms = it & (kMaskSlots - 1);
-      reinterpret_cast<float*>(smem_raw + kOffMask)[ms * kTilePairs + r] =
-          __uint_as_float(static_cast<uint32_t>(mraw) << 16);
-      const bool ones = __all_sync(0xffffffffu, mraw == 0x3f80);
-      if (lane == 0)
-        reinterpret_cast<uint32_t*>(smem_raw + kOffFlag)[ms * 4 + (warp - 4)] = ones ? 1u : 0u;
+      if (r < kTilePairs) {   // warp-uniform: the first four LayerNorm warps stage mask and flag
+        reinterpret_cast<float*>(smem_raw + kOffMask)[ms * kTilePairs + r] =
+            __uint_as_float(static_cast<uint32_t>(mraw) << 16);
+        const bool ones = __all_sync(0xffffffffu, mraw == 0x3f80);
+        if (lane == 0)
+          reinterpret_cast<uint32_t*>(smem_raw + kOffFlag)[ms * 4 + (warp - kWarpLn)] =
+              ones ? 1u : 0u;
+      }
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
-  } else if (warp >= 8) {
+  } else if (warp >= kWarpEpi) {
     // ===================== epilogue =====================
-    // warp -> TMEM lane quadrant q (hardware rule: warp % 4) and column half h (32 of a unit's 64)
+    // warp -> TMEM lane quadrant q (hardware rule: warp % 4) and team = (tensor h, parity par)
     const int q = warp & 3;
-    const int h = (warp - 8) >> 2;
+    const int team = (warp - kWarpEpi) >> 2;
+    const int h = team & 1;          // output tensor: 0 = a, 1 = b
+    const int par = team >> 1;       // which pair quarters (pq % kPar == par) this team handles
     const int ch = q * 32 + lane;                       // output channel = TMEM lane
     const uint32_t lane_base = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
     constexpr float kLog2e = 1.4426950408889634f;
@@ -227,7 +243,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
 #pragma unroll 1
     for (int m = 0; m < 4; ++m) {
       const uint4* wrow = reinterpret_cast<const uint4*>(prm.w[m] + static_cast<size_t>(ch) * kC);
-      const bool mine = (m >> 1) == h;
+      const bool mine = par == 0 && (m >> 1) == h;
       float acc = 0.f;
 #pragma unroll 1
       for (int half = 0; half < 2; ++half) {
@@ -269,7 +285,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     (void)one2;
 
     const uint32_t sw = static_cast<uint32_t>(ch & 7);
-    const bool store_thread = (q == 0 && lane == 0);   // one per team
+    const bool store_thread = (par == 0 && q == 0 && lane == 0);   // one per output tensor
 
     // one 16-column chunk: bias, sigmoid gate, (mask), bf16 pack
     auto compute_chunk = [&](const uint32_t (&vp)[16], const uint32_t (&vg)[16], uint32_t maddr, bool masked, uint32_t (&packed)[8]) {
@@ -300,28 +316,31 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       }
     };
 
-    // Team h (four warps, one per lane quadrant) owns tensor u = h (a for team 0, b for team 1)
-    // and its two TMEM slots 2h, 2h+1.  A unit is 32 pairs; per tile the team handles the four
-    // pair quarters pq = 0..3, alternating between its slots so that the MMAs of unit pq+1 run
-    // while it reads and post-processes unit pq.  Two units fill one [128 ch][64 pairs] staging
-    // buffer (128-byte rows: narrower TMA stores are markedly slower), stored after the second.
-    // The two teams run independently (own barrier, store thread and staging buffers).
+    // A team is four warps, one per TMEM lane quadrant.  kTeams = 2: team h owns tensor h (a / b)
+    // and both of its TMEM slots, so the MMAs of unit pq+1 run while it post-processes unit pq.
+    // kTeams = 4: two teams per tensor, one per slot (pair quarters of one parity each); more
+    // warps per scheduler keep the MUFU pipe (the sigmoids) busier.  A unit is 32 pairs; two units
+    // fill one [128 ch][64 pairs] staging buffer (128-byte rows: narrower TMA stores are markedly
+    // slower), stored once both halves are in.  Tensors a and b are handled independently (own
+    // barrier, store thread and staging buffers).
     const int u = h;
     const uint32_t bar_id = 1 + h;
+    constexpr uint32_t kBarThreads = 128 * kPar;
+    constexpr bool kPrefetch = kTeams == 2;     // enough registers for a second tcgen05.ld buffer
     int it = 0;
-    uint32_t c = 0;   // this team's 64-pair group counter (staging buffer parity)
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int ms = it & (kMaskSlots - 1);
       bool masked = true;
 #pragma unroll
-      for (int pq = 0; pq < 4; ++pq) {
+      for (int i = 0; i < 4 / kPar; ++i) {
+        const int pq = par + kPar * i;
+        const int g = pq >> 1;                                            // 64-pair group
         const uint32_t slot = static_cast<uint32_t>(2 * h + (pq & 1));
-        const uint32_t use = static_cast<uint32_t>(it * 2 + (pq >> 1));   // per-slot use count
-        if ((pq & 1) == 0 && pq != 0) ++c;
-        const uint32_t buf = smem + kOffOut + (2 * h + (c & 1u)) * kHalfBox;
+        const uint32_t use = static_cast<uint32_t>(it * 2 + g);          // per-slot use count
+        const uint32_t buf = smem + kOffOut + (2 * h + (use & 1u)) * kHalfBox;
         ptx::mbar_wait(tfull(slot), use & 1u);
         ptx::tc_fence_after();
-        if (pq == 0) {
+        if (i == 0) {
           // written by the LayerNorm warps before zready, hence visible after this tile's tfull
           uint32_t f[4];
           ptx::lds128(smem + kOffFlag + ms * 16, f);
@@ -330,17 +349,20 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         const uint32_t taddr = lane_base + kTmemAcc + slot * 64;
         const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + pq * 32) * 4;
         const uint32_t row_addr = buf + ch * 128;
-        // 32 columns in two chunks of 16; the tcgen05.ld of the second chunk is in flight while
-        // the first is being computed
-        uint32_t vp[2][16], vg[2][16];
+        // 32 columns in two chunks of 16
+        uint32_t vp[kPrefetch ? 2 : 1][16], vg[kPrefetch ? 2 : 1][16];
         ptx::tmem_ld_32x16(taddr, vp[0]);
         ptx::tmem_ld_32x16(taddr + 32, vg[0]);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
+          const int cb = kPrefetch ? k : 0;
           ptx::tmem_ld_wait();
           if (k == 0) {
-            ptx::tmem_ld_32x16(taddr + 16, vp[1]);
-            ptx::tmem_ld_32x16(taddr + 32 + 16, vg[1]);
+            if constexpr (kPrefetch) {
+              // the tcgen05.ld of the second chunk is in flight while the first is computed
+              ptx::tmem_ld_32x16(taddr + 16, vp[1]);
+              ptx::tmem_ld_32x16(taddr + 32 + 16, vg[1]);
+            }
           } else {
             // accumulators are in registers: hand the TMEM slot back to the issuer (the mask
             // slot stays valid: kMaskSlots >= kZStages + 3)
@@ -350,30 +372,36 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
           }
           uint32_t packed[8];
           if (masked) {
-            compute_chunk(vp[k], vg[k], maddr + k * 64, true, packed);
+            compute_chunk(vp[cb], vg[cb], maddr + k * 64, true, packed);
           } else {
-            compute_chunk(vp[k], vg[k], maddr + k * 64, false, packed);
+            compute_chunk(vp[cb], vg[cb], maddr + k * 64, false, packed);
           }
-          if (pq % 2 == 0 && k == 0) {
-            // first write into this staging buffer: the team's store two groups ago has read it
-            if (store_thread) ptx::tma_store_wait_read<1>();
-            ptx::named_bar_sync(bar_id, 128);
+          if constexpr (!kPrefetch) {
+            if (k == 0) {
+              ptx::tmem_ld_32x16(taddr + 16, vp[0]);
+              ptx::tmem_ld_32x16(taddr + 32 + 16, vg[0]);
+            }
           }
+          // the staging buffer is free: its previous store was waited for before the barrier
+          // that closed the previous group (below)
           const uint32_t c16 = static_cast<uint32_t>((pq & 1) * 4 + k * 2);
           ptx::sts128(row_addr + ((c16 ^ sw) << 4), packed[0], packed[1], packed[2], packed[3]);
           ptx::sts128(row_addr + (((c16 + 1) ^ sw) << 4), packed[4], packed[5], packed[6],
                       packed[7]);
         }
-        if (pq & 1) {
+        if (kPar == 2 || (pq & 1)) {
+          // group complete (for kPar = 2 the other team of this tensor fills the other half)
           ptx::fence_proxy_async_smem();
-          ptx::named_bar_sync(bar_id, 128);
+          // the store of the previous group (other buffer) must have finished reading shared
+          // memory before anyone passes this barrier and starts refilling that buffer
+          if (store_thread) ptx::tma_store_wait_read<0>();
+          ptx::named_bar_sync(bar_id, kBarThreads);
           if (store_thread) {
-            ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + (pq >> 1) * 64, 0);
+            ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + g * 64, 0);
             ptx::tma_store_commit();
           }
         }
       }
-      ++c;
     }
     if (store_thread) ptx::tma_store_wait<0>();
   }
