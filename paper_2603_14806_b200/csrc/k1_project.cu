@@ -239,6 +239,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // ---- once per CTA: fold the LayerNorm affine into the weights, park them in TMEM ----
     // every thread computes its channel's four folded biases  W beta + b ; warps 8-11 store
     // W_a, W_ga and warps 12-15 store W_b, W_gb as  W diag(gamma)  (row ch -> TMEM lane ch)
+    // tanh form: a = M sigma(g) p = M (tanh(g/2) + 1) (p/2) -- the two factors 1/2 go into the
+    // folded weights and biases (exact: a power of two), saving a multiply per element
+    constexpr float kWScale = kTanhSigmoid ? 0.5f : 1.0f;
     float fb[4];
 #pragma unroll 1
     for (int m = 0; m < 4; ++m) {
@@ -264,7 +267,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
             const float lo = ptx::bf16_lo(ww[e]), hi = ptx::bf16_hi(ww[e]);
             acc = fmaf(lo, bb[2 * e], acc);
             acc = fmaf(hi, bb[2 * e + 1], acc);
-            packed[kc * 4 + e] = ptx::pack_norm<kNormFp16>(lo * gg[2 * e], hi * gg[2 * e + 1]);
+            packed[kc * 4 + e] =
+                ptx::pack_norm<kNormFp16>(kWScale * lo * gg[2 * e], kWScale * hi * gg[2 * e + 1]);
           }
         }
         if (mine) ptx::tmem_st_32x32(lane_base + kTmemW + m * 64 + half * 32, packed);
@@ -277,11 +281,12 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     if (lane == 0) ptx::mbar_arrive(wready);
 
     // this thread's team handles tensor h only (a: matrices 0, 1; b: matrices 2, 3)
-    const float fbp = h ? fb[2] : fb[0], fbg = kGateScale * (h ? fb[3] : fb[1]);
+    const float fbp = kWScale * (h ? fb[2] : fb[0]);
+    const float fbg = (kTanhSigmoid ? 0.5f : kGateScale) * (h ? fb[3] : fb[1]);
     const ptx::f32x2 bias_p2 = ptx::pk2(fbp, fbp), bias_g2 = ptx::pk2(fbg, fbg);
     const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
-    const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
-    (void)half2;
+    const ptx::f32x2 one2 = ptx::pk2(1.0f, 1.0f);
+    (void)gscale2;
     (void)one2;
 
     const uint32_t sw = static_cast<uint32_t>(ch & 7);
@@ -297,20 +302,20 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         for (int e2 = 0; e2 < 2; ++e2) {
           const int j = j4 * 4 + e2 * 2;
           ptx::f32x2 pj = ptx::add2(ptx::pk2u(vp[j], vp[j + 1]), bias_p2);
-          const ptx::f32x2 gx = ptx::fma2(ptx::pk2u(vg[j], vg[j + 1]), gscale2, bias_g2);
-          float g0, g1;
-          ptx::upk2(gx, g0, g1);
-          ptx::f32x2 sg;
-          if constexpr (kTanhSigmoid) {
-            sg = ptx::fma2(ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), half2, half2);
-          } else {
-            float d0, d1;
-            ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
-            sg = ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1));
-          }
-          if (masked) pj = ptx::mul2(pj, m2[e2]);
           float v0, v1;
-          ptx::upk2(ptx::mul2(pj, sg), v0, v1);
+          if constexpr (kTanhSigmoid) {
+            // pj = p/2, gx = g/2 (scales folded into the weights): a = M (tanh(gx) + 1) pj
+            float g0, g1;
+            ptx::upk2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bias_g2), g0, g1);
+            if (masked) pj = ptx::mul2(pj, m2[e2]);
+            ptx::upk2(ptx::fma2(pj, ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), pj), v0, v1);
+          } else {
+            float g0, g1, d0, d1;
+            ptx::upk2(ptx::fma2(ptx::pk2u(vg[j], vg[j + 1]), gscale2, bias_g2), g0, g1);
+            ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
+            if (masked) pj = ptx::mul2(pj, m2[e2]);
+            ptx::upk2(ptx::mul2(pj, ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1))), v0, v1);
+          }
           packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
         }
       }

@@ -149,7 +149,10 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       acc = fmaf(ptx::bf16_lo(wv.w), b1.z, acc);
       acc = fmaf(ptx::bf16_hi(wv.w), b1.w, acc);
     }
-    reinterpret_cast<float*>(smem_raw + kOffVec)[id] = acc + (bias ? bias[ch] : 0.f);
+    // tanh form: out = M sigma(g) y = M (tanh(g/2) + 1) (y/2): both factors 1/2 are folded into
+    // the weights and these biases (exact: a power of two)
+    reinterpret_cast<float*>(smem_raw + kOffVec)[id] =
+        (kTanhSigmoid ? 0.5f : 1.0f) * (acc + (bias ? bias[ch] : 0.f));
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -177,12 +180,13 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const float* gam = (m ? prm.g_out : prm.g_in) + k0;
       const float4 g0 = __ldg(reinterpret_cast<const float4*>(gam));
       const float4 g1 = __ldg(reinterpret_cast<const float4*>(gam + 4));
+      constexpr float ws = kTanhSigmoid ? 0.5f : 1.0f;
       uint32_t v[4];
       ptx::lds128(smem + kOffW + off, v);
-      v[0] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[0]) * g0.x, ptx::bf16_hi(v[0]) * g0.y);
-      v[1] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[1]) * g0.z, ptx::bf16_hi(v[1]) * g0.w);
-      v[2] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[2]) * g1.x, ptx::bf16_hi(v[2]) * g1.y);
-      v[3] = ptx::pack_norm<kNormFp16>(ptx::bf16_lo(v[3]) * g1.z, ptx::bf16_hi(v[3]) * g1.w);
+      v[0] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[0]) * g0.x, ws * ptx::bf16_hi(v[0]) * g0.y);
+      v[1] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[1]) * g0.z, ws * ptx::bf16_hi(v[1]) * g0.w);
+      v[2] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[2]) * g1.x, ws * ptx::bf16_hi(v[2]) * g1.y);
+      v[3] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[3]) * g1.z, ws * ptx::bf16_hi(v[3]) * g1.w);
       ptx::sts128(smem + kOffW + off, v[0], v[1], v[2], v[3]);
     }
     ptx::fence_proxy_async_smem();
@@ -347,8 +351,8 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     constexpr float kLog2e = 1.4426950408889634f;
     constexpr float kGateScale = kTanhSigmoid ? 0.5f : -kLog2e;
     const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
-    const ptx::f32x2 half2 = ptx::pk2(0.5f, 0.5f), one2 = ptx::pk2(1.0f, 1.0f);
-    (void)half2;
+    const ptx::f32x2 one2 = ptx::pk2(1.0f, 1.0f);
+    (void)gscale2;
     (void)one2;
     // folded biases (fp32) of this thread's 64 channels
     const uint32_t tg_addr = smem + kOffVec + h * 64 * 4, to_addr = tg_addr + kC * 4;
@@ -400,22 +404,20 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
 #pragma unroll
           for (int e2 = 0; e2 < 2; ++e2) {
             const int j = j4 * 4 + e2 * 2;
-            // gate pre-activation scaled for the sigmoid form in use
-            const ptx::f32x2 gx = ptx::mul2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bg2[e2]), gscale2);
-            float g0, g1;
-            ptx::upk2(gx, g0, g1);
-            ptx::f32x2 sg;
+            const ptx::f32x2 zres = ptx::bf16x2_to_f32x2(zr[j4 * 2 + e2]);   // 0 without residual
+            const ptx::f32x2 y = ptx::mul2(ptx::add2(ptx::pk2u(vo[j], vo[j + 1]), bo2[e2]), mval2);
+            float g0, g1, v0, v1;
             if constexpr (kTanhSigmoid) {
-              sg = ptx::fma2(ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)), half2, half2);
+              // y and the gate pre-activation arrive halved: out = (tanh(g/2) + 1) (y/2) [+ z]
+              ptx::upk2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bg2[e2]), g0, g1);
+              ptx::upk2(ptx::fma2(y, ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)),
+                                  ptx::add2(y, zres)), v0, v1);
             } else {
               float d0, d1;
+              ptx::upk2(ptx::mul2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bg2[e2]), gscale2), g0, g1);
               ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
-              sg = ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1));
+              ptx::upk2(ptx::fma2(y, ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1)), zres), v0, v1);
             }
-            const ptx::f32x2 y = ptx::mul2(ptx::add2(ptx::pk2u(vo[j], vo[j + 1]), bo2[e2]), mval2);
-            float v0, v1;
-            // + z (exactly 0 when there is no residual: bf16 zero bits)
-            ptx::upk2(ptx::fma2(y, sg, ptx::bf16x2_to_f32x2(zr[j4 * 2 + e2])), v0, v1);
             packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
           }
         }
