@@ -71,6 +71,7 @@ constexpr int kOffFlag = kOffMask + kMaskSlots * kTilePairs * 4;   // 4 "all one
 constexpr int kOffBar = kOffFlag + kMaskSlots * 16;
 constexpr int kSmemBytes = kOffBar + 256;
 static_assert(kSmemBytes <= 232448, "K1 shared memory exceeds 227 KB");
+static_assert((3 * kZStages + 18) * 8 <= 256, "barrier region too small");
 
 constexpr int kTmemW = 0;        // columns 0..255: four weight matrices, 64 columns each
 constexpr int kTmemAcc = 256;    // columns 256..511: four slots of (projection 32 | gate 32)
@@ -103,6 +104,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   auto tempty = [&](int u) { return bar + 8u * (3 * kZStages + 4 + u); };
   const uint32_t tmem_slot = bar + 8u * (3 * kZStages + 8);
   const uint32_t wready = bar + 8u * (3 * kZStages + 9);   // weights are in TMEM
+  auto ofull = [&](int b) { return bar + 8u * (3 * kZStages + 10 + b); };    // staging buffer b
+  auto oempty = [&](int b) { return bar + 8u * (3 * kZStages + 14 + b); };   // (tensor, group)
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -123,6 +126,10 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_init(tempty(u), 4);
     }
     ptx::mbar_init(wready, 4 * kTeams);
+    for (int b = 0; b < kOutBufs; ++b) {
+      ptx::mbar_init(ofull(b), 4 * kPar);   // one arrival per warp that fills the buffer
+      ptx::mbar_init(oempty(b), 1);
+    }
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
@@ -190,6 +197,33 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         }
         ptx::umma_commit<1>(zempty(s));   // stage reusable once all MMAs of the tile retired
       }
+    }
+  } else if (warp == 3) {
+    // ===================== TMA store issuer =====================
+    // The epilogue warps only arrive on ofull(b) when their part of staging buffer b is written
+    // and carry on; this thread issues the store and hands the buffer back (oempty) once the
+    // previous store has finished reading shared memory.  No block-wide barrier in the epilogue.
+    if (ptx::elect_one()) {
+      int it = 0, prev = -1;
+      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            const int b = 2 * u + g;
+            ptx::mbar_wait(ofull(b), it & 1);
+            ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, smem + kOffOut + b * kHalfBox,
+                              t * kTilePairs + g * 64, 0);
+            ptx::tma_store_commit();
+            if (prev >= 0) {
+              ptx::tma_store_wait_read<1>();
+              ptx::mbar_arrive(oempty(prev));
+            }
+            prev = b;
+          }
+        }
+      }
+      ptx::tma_store_wait<0>();
     }
   } else if (warp >= kWarpLn && warp < kWarpEpi) {
     // ===================== LayerNorm =====================
@@ -290,7 +324,6 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     (void)one2;
 
     const uint32_t sw = static_cast<uint32_t>(ch & 7);
-    const bool store_thread = (par == 0 && q == 0 && lane == 0);   // one per output tensor
 
     // one 16-column chunk: bias, sigmoid gate, (mask), bf16 pack
     auto compute_chunk = [&](const uint32_t (&vp)[16], const uint32_t (&vg)[16], uint32_t maddr, bool masked, uint32_t (&packed)[8]) {
@@ -328,9 +361,6 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // fill one [128 ch][64 pairs] staging buffer (128-byte rows: narrower TMA stores are markedly
     // slower), stored once both halves are in.  Tensors a and b are handled independently (own
     // barrier, store thread and staging buffers).
-    const int u = h;
-    const uint32_t bar_id = 1 + h;
-    constexpr uint32_t kBarThreads = 128 * kPar;
     constexpr bool kPrefetch = kTeams == 2;     // enough registers for a second tcgen05.ld buffer
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
@@ -342,7 +372,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         const int g = pq >> 1;                                            // 64-pair group
         const uint32_t slot = static_cast<uint32_t>(2 * h + (pq & 1));
         const uint32_t use = static_cast<uint32_t>(it * 2 + g);          // per-slot use count
-        const uint32_t buf = smem + kOffOut + (2 * h + (use & 1u)) * kHalfBox;
+        const int b = 2 * h + g;                                          // staging buffer
         ptx::mbar_wait(tfull(slot), use & 1u);
         ptx::tc_fence_after();
         if (i == 0) {
@@ -353,11 +383,13 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         }
         const uint32_t taddr = lane_base + kTmemAcc + slot * 64;
         const uint32_t maddr = smem + kOffMask + (ms * kTilePairs + pq * 32) * 4;
-        const uint32_t row_addr = buf + ch * 128;
+        const uint32_t row_addr = smem + kOffOut + b * kHalfBox + ch * 128;
         // 32 columns in two chunks of 16
         uint32_t vp[kPrefetch ? 2 : 1][16], vg[kPrefetch ? 2 : 1][16];
         ptx::tmem_ld_32x16(taddr, vp[0]);
         ptx::tmem_ld_32x16(taddr + 32, vg[0]);
+        // first write of this team into buffer b for this tile: last tile's store has read it
+        if (kPar == 2 || (pq & 1) == 0) ptx::mbar_wait(oempty(b), (it & 1) ^ 1u);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           const int cb = kPrefetch ? k : 0;
@@ -387,28 +419,19 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
               ptx::tmem_ld_32x16(taddr + 32 + 16, vg[0]);
             }
           }
-          // the staging buffer is free: its previous store was waited for before the barrier
-          // that closed the previous group (below)
           const uint32_t c16 = static_cast<uint32_t>((pq & 1) * 4 + k * 2);
           ptx::sts128(row_addr + ((c16 ^ sw) << 4), packed[0], packed[1], packed[2], packed[3]);
           ptx::sts128(row_addr + (((c16 + 1) ^ sw) << 4), packed[4], packed[5], packed[6],
                       packed[7]);
         }
         if (kPar == 2 || (pq & 1)) {
-          // group complete (for kPar = 2 the other team of this tensor fills the other half)
+          // this warp's share of the 64-pair group is in shared memory: tell the store issuer
           ptx::fence_proxy_async_smem();
-          // the store of the previous group (other buffer) must have finished reading shared
-          // memory before anyone passes this barrier and starts refilling that buffer
-          if (store_thread) ptx::tma_store_wait_read<0>();
-          ptx::named_bar_sync(bar_id, kBarThreads);
-          if (store_thread) {
-            ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, buf, t * kTilePairs + g * 64, 0);
-            ptx::tma_store_commit();
-          }
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(ofull(b));
         }
       }
     }
-    if (store_thread) ptx::tma_store_wait<0>();
   }
 
   // ===================== teardown =====================
