@@ -37,6 +37,26 @@ bool get_device_info(DeviceInfo* info) {
   return true;
 }
 
+// ----------------------------------------------------------------------------- launch attributes
+int ensure_dynamic_smem(const void* kernel, int bytes) {
+  constexpr int kMaxDev = 64, kMaxKernels = 32;
+  static const void* seen[kMaxDev][kMaxKernels] = {};
+  static std::mutex mu;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) return FOLDCP_ERR_CUDA;
+  std::lock_guard<std::mutex> lock(mu);
+  int free_slot = -1;
+  for (int i = 0; i < kMaxKernels; ++i) {
+    if (seen[dev][i] == kernel) return FOLDCP_OK;
+    if (seen[dev][i] == nullptr && free_slot < 0) free_slot = i;
+  }
+  if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) !=
+      cudaSuccess)
+    return FOLDCP_ERR_CUDA;
+  if (free_slot >= 0) seen[dev][free_slot] = kernel;
+  return FOLDCP_OK;
+}
+
 // ----------------------------------------------------------------------------- tensor maps
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,

@@ -59,6 +59,10 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
                             const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
 
+// Opt a kernel in to `bytes` of dynamic shared memory, once per (kernel, device); thread-safe.
+// Returns FOLDCP_OK or FOLDCP_ERR_CUDA.
+int ensure_dynamic_smem(const void* kernel, int bytes);
+
 inline int check_launch() {
   return cudaPeekAtLastError() == cudaSuccess ? FOLDCP_OK : FOLDCP_ERR_CUDA;
 }

@@ -308,13 +308,8 @@ int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorM
                    const K2Params& prm, int sm_count, cudaStream_t stream) {
   using C = Cfg<kCtaGroup>;
   auto kern = k2_contract_kernel<kCtaGroup, kIncoming>;
-  static bool attr_set = false;   // per template instance
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes) !=
-        cudaSuccess)
-      return FOLDCP_ERR_CUDA;
-    attr_set = true;
-  }
+  if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), C::kSmemBytes) != FOLDCP_OK)
+    return FOLDCP_ERR_CUDA;
   int groups = sm_count / kCtaGroup;
   if (groups > prm.num_tiles) groups = prm.num_tiles;
   cudaLaunchConfig_t cfg = {};

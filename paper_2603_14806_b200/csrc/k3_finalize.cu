@@ -501,13 +501,8 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k3_tanh_sigmoid();
   auto kern = tanh_sig ? k3_finalize_kernel<true> : k3_finalize_kernel<false>;
-  static bool attr_set[2] = {false, false};
-  if (!attr_set[tanh_sig]) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) !=
-        cudaSuccess)
-      return FOLDCP_ERR_CUDA;
-    attr_set[tanh_sig] = true;
-  }
+  if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), kSmemBytes) != FOLDCP_OK)
+    return FOLDCP_ERR_CUDA;
   kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, to, twg, two, tout, prm);
   return check_launch();
 }
