@@ -96,6 +96,30 @@ def contraction(a: np.ndarray, b: np.ndarray, direction: int) -> np.ndarray:
     return np.transpose(O, (1, 2, 0))
 
 
+def contraction_backward(d_o: np.ndarray, a: np.ndarray, b: np.ndarray, direction: int):
+    """Gradients of Eq. 2-3 with respect to a and b, given d_o = dL/do
+    (all [N, N, c]); the paper hand-writes every backward with the same algorithm as the forward
+    (lines 92-96), SURVEY 8(f) NEXT-2.  Differentiating the definition term by term:
+
+    outgoing  o[i,j] = sum_k a[i,k] b[j,k]:  d_a[i,k] = sum_j d_o[i,j] b[j,k]     (dO  B)
+                                             d_b[j,k] = sum_i d_o[i,j] a[i,k]     (dO^T A)
+    incoming  o[i,j] = sum_k a[k,i] b[k,j]:  d_a[k,i] = sum_j b[k,j] d_o[i,j]     (B  dO^T)
+                                             d_b[k,j] = sum_i a[k,i] d_o[i,j]     (A  dO)
+    per channel.  Returns (d_a, d_b), each [N, N, c].
+    """
+    G = np.transpose(np.asarray(d_o, _F), (2, 0, 1))
+    A = np.transpose(np.asarray(a, _F), (2, 0, 1))
+    B = np.transpose(np.asarray(b, _F), (2, 0, 1))
+    T = lambda x: np.transpose(x, (0, 2, 1))
+    if direction == OUTGOING:
+        dA, dB = G @ B, T(G) @ A
+    elif direction == INCOMING:
+        dA, dB = B @ T(G), A @ G
+    else:
+        raise ValueError("direction must be 0 (outgoing) or 1 (incoming)")
+    return np.transpose(dA, (1, 2, 0)), np.transpose(dB, (1, 2, 0))
+
+
 def output_stage(o: np.ndarray, zp: np.ndarray, mask: Optional[np.ndarray],
                  p: Dict[str, np.ndarray], eps: float, mask_output: bool) -> np.ndarray:
     """out = [M *] sigmoid(W_g z' + b_g) * (W_o LayerNorm(o) + b_o)   (north_star)."""

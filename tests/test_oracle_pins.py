@@ -92,6 +92,35 @@ def test_residual_and_batched_forms_against_brute_force(direction):
     assert np.array_equal(orc.trimul_residual(z[0], M[0], q, direction), z[0])
 
 
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_contraction_backward_against_loops_and_directional_derivative(direction):
+    """d_a, d_b of Eq. 2-3: (i) literal index loops of the differentiated definition; (ii) the
+    forward contraction is bilinear, so <d_o, o(a + u, b) - o(a, b)> = <d_a, u> exactly (and the
+    same for b) -- a wrong index or a transposed operand breaks it."""
+    rng = np.random.default_rng(77 + direction)
+    N, c = 5, 3
+    a, b, g = (rng.standard_normal((N, N, c)) for _ in range(3))
+    da, db = orc.contraction_backward(g, a, b, direction)
+    ra, rb = np.zeros_like(a), np.zeros_like(b)
+    for ch in range(c):
+        for i in range(N):
+            for j in range(N):
+                for k in range(N):
+                    if direction == OUT:      # o[i,j] += a[i,k] b[j,k]
+                        ra[i, k, ch] += g[i, j, ch] * b[j, k, ch]
+                        rb[j, k, ch] += g[i, j, ch] * a[i, k, ch]
+                    else:                     # o[i,j] += a[k,i] b[k,j]
+                        ra[k, i, ch] += g[i, j, ch] * b[k, j, ch]
+                        rb[k, j, ch] += g[i, j, ch] * a[k, i, ch]
+    assert relerr(da, ra) < 1e-12 and relerr(db, rb) < 1e-12
+    u, v = rng.standard_normal(a.shape), rng.standard_normal(b.shape)
+    o0 = orc.contraction(a, b, direction)
+    lhs_a = np.sum(g * (orc.contraction(a + u, b, direction) - o0))
+    lhs_b = np.sum(g * (orc.contraction(a, b + v, direction) - o0))
+    assert abs(lhs_a - np.sum(da * u)) < 1e-10 * max(1.0, abs(lhs_a))
+    assert abs(lhs_b - np.sum(db * v)) < 1e-10 * max(1.0, abs(lhs_b))
+
+
 def test_brute_force_no_bias_no_mask_soft_mask():
     rng = np.random.default_rng(7)
     N, c_z, c = 4, 8, 4
