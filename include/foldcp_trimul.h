@@ -126,6 +126,17 @@ int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_p
                           int N, int c_z, int c_hidden, void* a, void* b, void* stream);
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
                            int direction, void* o, void* stream);
+/*
+ * Backward of step a4 (the O(N^3) part of training; the paper hand-writes
+ * every backward with the forward's algorithm).  Given d_o = dL/do:
+ *     outgoing  d_a[i][k] = sum_j d_o[i][j] b[j][k]     d_b[j][k] = sum_i d_o[i][j] a[i][k]
+ *     incoming  d_a[k][i] = sum_j b[k][j] d_o[i][j]     d_b[k][j] = sum_i a[k][i] d_o[i][j]
+ * per channel.  All five tensors are [c_hidden][N][N] channel-major device pointers of `dtype`;
+ * d_a / d_b must not overlap the inputs or each other.  Two launches of the contraction kernel.
+ */
+int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* b, int N,
+                                    int c_hidden, int dtype, int direction, void* d_a, void* d_b,
+                                    void* stream);
 int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
                            const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
                            void* out, void* stream);

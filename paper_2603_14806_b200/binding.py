@@ -22,7 +22,7 @@ _lib = None
 
 EXPORTS = (
     "foldcp_trimul", "foldcp_trimul_batched", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
-    "foldcp_trimul_contract", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
+    "foldcp_trimul_contract", "foldcp_trimul_contract_backward", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
     "foldcp_status_string", "foldcp_version",
 )
 
@@ -74,6 +74,8 @@ def load() -> ctypes.CDLL:
     lib.foldcp_trimul_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.foldcp_trimul_project.restype = ci
     lib.foldcp_trimul_project.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp, vp]
+    lib.foldcp_trimul_contract_backward.restype = ci
+    lib.foldcp_trimul_contract_backward.argtypes = [vp, vp, vp, ci, ci, ci, ci, vp, vp, vp]
     lib.foldcp_trimul_contract.restype = ci
     lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp]
     lib.foldcp_trimul_finalize.restype = ci
@@ -214,6 +216,19 @@ def contract(a: torch.Tensor, b: torch.Tensor, direction: int,
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_contract")
     return o
+
+
+def contract_backward(d_o: torch.Tensor, a: torch.Tensor, b: torch.Tensor, direction: int):
+    """Backward of stage a4: returns (d_a, d_b), each [c, N, N] channel-major."""
+    lib = load()
+    c, N = a.shape[0], a.shape[1]
+    d_a, d_b = torch.empty_like(a), torch.empty_like(b)
+    st = lib.foldcp_trimul_contract_backward(d_o.data_ptr(), a.data_ptr(), b.data_ptr(), N, c,
+                                             dtype_code(a), int(direction), d_a.data_ptr(),
+                                             d_b.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_contract_backward")
+    return d_a, d_b
 
 
 def finalize(o, z, mask, p, eps: float = 1e-5, mask_output: bool = True,

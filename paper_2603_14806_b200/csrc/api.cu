@@ -220,6 +220,27 @@ int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, in
   return launch_simt_contract(a, b, o, N, dtype, direction, s);
 }
 
+int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* b, int N,
+                                    int c_hidden, int dtype, int direction, void* d_a, void* d_b,
+                                    void* stream) {
+  int st = check_shape(N, kChannels, c_hidden, dtype);
+  if (st != FOLDCP_OK) return st;
+  if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
+  if (!d_o || !a || !b || !d_a || !d_b) return FOLDCP_ERR_INVALID_ARG;
+  if (!aligned16(d_o) || !aligned16(a) || !aligned16(b) || !aligned16(d_a) || !aligned16(d_b))
+    return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(dtype);
+  const void* ins[3] = {d_o, a, b};
+  for (const void* in : ins)
+    if (overlaps(d_a, bytes, in, bytes) || overlaps(d_b, bytes, in, bytes)) return FOLDCP_ERR_ALIAS;
+  if (overlaps(d_a, bytes, d_b, bytes)) return FOLDCP_ERR_ALIAS;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
+    return launch_k2_contract_backward_bf16(d_o, a, b, d_a, d_b, N, direction, s);
+  return launch_simt_contract_backward(d_o, a, b, d_a, d_b, N, dtype, direction, s);
+}
+
 int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
                            const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
                            void* out, void* stream) {

@@ -47,10 +47,15 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
                             cudaStream_t stream);
 
+int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void* b, void* d_a,
+                                     void* d_b, int N, int direction, cudaStream_t stream);
+
 int launch_simt_project(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
                         void* a, void* b, cudaStream_t stream);
 int launch_simt_contract(const void* a, const void* b, void* o, int N, int dtype, int direction,
                          cudaStream_t stream);
+int launch_simt_contract_backward(const void* d_o, const void* a, const void* b, void* d_a,
+                                  void* d_b, int N, int dtype, int direction, cudaStream_t stream);
 int launch_simt_finalize(const void* o, const void* z, const void* mask,
                          const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
 

@@ -72,7 +72,7 @@ __device__ __forceinline__ void decode_tile(const K2Params& prm, int r, int* tm,
   }
 }
 
-template <int kCtaGroup, bool kIncoming>
+template <int kCtaGroup, bool kAMn, bool kBMn>
 __global__ void __launch_bounds__(kThreads, 1)
 k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
                    const __grid_constant__ CUtensorMap tmap_b,
@@ -158,8 +158,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
 #pragma unroll
           for (int bx = 0; bx < 2; ++bx) {
             const int mn = m0 + 64 * bx;
-            const int c0 = kIncoming ? mn : k0;   // innermost tensor coordinate (column)
-            const int c1 = kIncoming ? k0 : mn;   // row
+            const int c0 = kAMn ? mn : k0;   // innermost tensor coordinate (column)
+            const int c1 = kAMn ? k0 : mn;   // row
             if constexpr (kCtaGroup == 2) {
               ptx::tma_load_3d_2sm_hint(sa + bx * kBoxBytes, &tmap_a, bar, c0, c1, ch, pol_ld);
             } else {
@@ -169,8 +169,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
 #pragma unroll
           for (int bx = 0; bx < C::kBBoxes; ++bx) {
             const int mn = n0 + 64 * bx;
-            const int c0 = kIncoming ? mn : k0;
-            const int c1 = kIncoming ? k0 : mn;
+            const int c0 = kBMn ? mn : k0;
+            const int c1 = kBMn ? k0 : mn;
             if constexpr (kCtaGroup == 2) {
               ptx::tma_load_3d_2sm_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld);
             } else {
@@ -187,14 +187,13 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA only) =====================
     if (is_leader && ptx::elect_one()) {
-      constexpr uint32_t idesc =
-          ptx::make_idesc_bf16(C::kTileM, kTileN, kIncoming ? 1 : 0, kIncoming ? 1 : 0);
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(C::kTileM, kTileN, kAMn ? 1 : 0, kBMn ? 1 : 0);
       // K-major : rows of 128 B, 8-row atoms 1024 B apart (SBO); one UMMA_K = 32 B along the row
       // MN-major: 64-element MN groups kBoxBytes apart (LBO), 8-k atoms 1024 B apart (SBO);
       //           one UMMA_K = two 8-k atoms = 2048 B
-      constexpr uint32_t lbo = kIncoming ? kBoxBytes : 16;
+      constexpr uint32_t lbo_a = kAMn ? kBoxBytes : 16, lbo_b = kBMn ? kBoxBytes : 16;
       constexpr uint32_t sbo = 1024;
-      constexpr uint32_t kstep = kIncoming ? 2048 : 32;
+      constexpr uint32_t kstep_a = kAMn ? 2048 : 32, kstep_b = kBMn ? 2048 : 32;
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
@@ -211,8 +210,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
           const uint32_t sb = sa + C::kABytes;
 #pragma unroll
           for (int k = 0; k < kBlockK / kUmmaK; ++k) {
-            const uint64_t da = ptx::make_smem_desc_sw128(sa + k * kstep, lbo, sbo);
-            const uint64_t db = ptx::make_smem_desc_sw128(sb + k * kstep, lbo, sbo);
+            const uint64_t da = ptx::make_smem_desc_sw128(sa + k * kstep_a, lbo_a, sbo);
+            const uint64_t db = ptx::make_smem_desc_sw128(sb + k * kstep_b, lbo_b, sbo);
             ptx::umma_bf16<kCtaGroup>(d_tmem, da, db, idesc, (kb | k) != 0 ? 1u : 0u);
           }
           ptx::umma_commit<kCtaGroup>(empty_bar(stage));   // smem slot free once these MMAs retire
@@ -303,11 +302,11 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   }
 }
 
-template <int kCtaGroup, bool kIncoming>
+template <int kCtaGroup, bool kAMn, bool kBMn>
 int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& to,
                    const K2Params& prm, int sm_count, cudaStream_t stream) {
   using C = Cfg<kCtaGroup>;
-  auto kern = k2_contract_kernel<kCtaGroup, kIncoming>;
+  auto kern = k2_contract_kernel<kCtaGroup, kAMn, kBMn>;
   if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), C::kSmemBytes) != FOLDCP_OK)
     return FOLDCP_ERR_CUDA;
   int groups = sm_count / kCtaGroup;
@@ -332,8 +331,13 @@ int g_k2_cta_group = 2;   // FOLDCP_K2_CTA_GROUP=1 selects the single-CTA varian
 
 }  // namespace
 
-int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            cudaStream_t stream) {
+// D_c = op(X_c) op(Y_c)^T per channel for the four operand layouts:
+//   x_mn = 0: X_c is [m][k] (k contiguous, K-major)    x_mn = 1: X_c is [k][m] (m contiguous)
+//   y_mn = 0: Y_c is [n][k]                            y_mn = 1: Y_c is [k][n]
+// i.e. d[c][m][n] = sum_k X(m, k) Y(n, k).  The forward contraction uses (0,0) / (1,1); its
+// gradients also need the mixed (0,1) form.
+int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn,
+                        cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   static const int cta_group = [] {
@@ -347,9 +351,9 @@ int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int di
   const uint32_t box_st[3] = {64, 128, 1};
   CUtensorMap ta, tb, to;
   int st;
-  if ((st = encode_tensor_map(&ta, a, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
-  if ((st = encode_tensor_map(&tb, b, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
-  if ((st = encode_tensor_map(&to, o, 2, 3, dims, strides, box_st, true)) != FOLDCP_OK) return st;
+  if ((st = encode_tensor_map(&ta, x, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
+  if ((st = encode_tensor_map(&tb, y, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
+  if ((st = encode_tensor_map(&to, d, 2, 3, dims, strides, box_st, true)) != FOLDCP_OK) return st;
   K2Params prm;
   prm.N = N;
   const int tile_m = 128 * cta_group;
@@ -368,13 +372,39 @@ int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int di
                               // do not lower DRAM traffic or time at N = 4096)
   }();
   prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : prm.tiles_n;
-  const bool inc = direction == FOLDCP_INCOMING;
+  const int sms = dev.sm_count;
   if (cta_group == 2) {
-    return inc ? launch_variant<2, true>(ta, tb, to, prm, dev.sm_count, stream)
-               : launch_variant<2, false>(ta, tb, to, prm, dev.sm_count, stream);
+    if (x_mn) return y_mn ? launch_variant<2, true, true>(ta, tb, to, prm, sms, stream)
+                          : launch_variant<2, true, false>(ta, tb, to, prm, sms, stream);
+    return y_mn ? launch_variant<2, false, true>(ta, tb, to, prm, sms, stream)
+                : launch_variant<2, false, false>(ta, tb, to, prm, sms, stream);
   }
-  return inc ? launch_variant<1, true>(ta, tb, to, prm, dev.sm_count, stream)
-             : launch_variant<1, false>(ta, tb, to, prm, dev.sm_count, stream);
+  if (x_mn) return y_mn ? launch_variant<1, true, true>(ta, tb, to, prm, sms, stream)
+                        : launch_variant<1, true, false>(ta, tb, to, prm, sms, stream);
+  return y_mn ? launch_variant<1, false, true>(ta, tb, to, prm, sms, stream)
+              : launch_variant<1, false, false>(ta, tb, to, prm, sms, stream);
+}
+
+int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
+                            cudaStream_t stream) {
+  const bool inc = direction == FOLDCP_INCOMING;
+  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, stream);
+}
+
+// Gradients of the contraction (oracle/trimul_oracle.py contraction_backward):
+//   outgoing: d_a = dO B       -> X = dO (K-major), Y = B (MN-major)
+//             d_b = dO^T A     -> X = dO (MN-major), Y = A (MN-major)
+//   incoming: d_a = B dO^T     -> X = B (K-major),  Y = dO (K-major)
+//             d_b = A dO       -> X = A (K-major),  Y = dO (MN-major)
+int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void* b, void* d_a,
+                                     void* d_b, int N, int direction, cudaStream_t stream) {
+  int st;
+  if (direction == FOLDCP_OUTGOING) {
+    if ((st = launch_k2_gemm_bf16(d_o, b, d_a, N, false, true, stream)) != FOLDCP_OK) return st;
+    return launch_k2_gemm_bf16(d_o, a, d_b, N, true, true, stream);
+  }
+  if ((st = launch_k2_gemm_bf16(b, d_o, d_a, N, false, false, stream)) != FOLDCP_OK) return st;
+  return launch_k2_gemm_bf16(a, d_o, d_b, N, false, true, stream);
 }
 
 }  // namespace foldcp

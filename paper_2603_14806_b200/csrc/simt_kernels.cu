@@ -114,7 +114,7 @@ simt_project_kernel(const T* __restrict__ z, const T* __restrict__ mask, const T
 // stage 2: per-channel contraction, 64 x 64 output tile per block, 16 x 16 threads, 4 x 4 each
 //   outgoing: o[i][j] = sum_k A[i][k] B[j][k]      incoming: o[i][j] = sum_k A[k][i] B[k][j]
 // ---------------------------------------------------------------------------------------------
-template <typename T, bool kIncoming>
+template <typename T, bool kXMn, bool kYMn>
 __global__ void __launch_bounds__(256)
 simt_contract_kernel(const T* __restrict__ a, const T* __restrict__ b, T* __restrict__ o, int N) {
   constexpr int TS = 64, KS = 16;
@@ -128,19 +128,27 @@ simt_contract_kernel(const T* __restrict__ a, const T* __restrict__ b, T* __rest
   float acc[4][4] = {};
   for (int k0 = 0; k0 < N; k0 += KS) {
     for (int e = threadIdx.x; e < TS * KS; e += 256) {
-      int mn, kk;
-      if (kIncoming) { mn = e % TS; kk = e / TS; } else { kk = e % KS; mn = e / KS; }
-      const int k = k0 + kk;
-      const int gi = i0 + mn, gj = j0 + mn;
-      float av = 0.f, bv = 0.f;
-      if (k < N) {
-        if (gi < N) av = ldf(kIncoming ? A + static_cast<long long>(k) * N + gi
-                                       : A + static_cast<long long>(gi) * N + k);
-        if (gj < N) bv = ldf(kIncoming ? B + static_cast<long long>(k) * N + gj
-                                       : B + static_cast<long long>(gj) * N + k);
+      // each operand is read along its contiguous index: [k][mn] when MN-major, [mn][k] otherwise
+      {
+        int mn, kk;
+        if (kXMn) { mn = e % TS; kk = e / TS; } else { kk = e % KS; mn = e / KS; }
+        const int k = k0 + kk, gi = i0 + mn;
+        float av = 0.f;
+        if (k < N && gi < N)
+          av = ldf(kXMn ? A + static_cast<long long>(k) * N + gi
+                        : A + static_cast<long long>(gi) * N + k);
+        As[kk][mn] = av;
       }
-      As[kk][mn] = av;
-      Bs[kk][mn] = bv;
+      {
+        int mn, kk;
+        if (kYMn) { mn = e % TS; kk = e / TS; } else { kk = e % KS; mn = e / KS; }
+        const int k = k0 + kk, gj = j0 + mn;
+        float bv = 0.f;
+        if (k < N && gj < N)
+          bv = ldf(kYMn ? B + static_cast<long long>(k) * N + gj
+                        : B + static_cast<long long>(gj) * N + k);
+        Bs[kk][mn] = bv;
+      }
     }
     __syncthreads();
 #pragma unroll
@@ -235,20 +243,38 @@ int project_t(const void* z, const void* mask, const foldcp_trimul_params* p, in
   return check_launch();
 }
 
+// d[c][m][n] = sum_k X(m, k) Y(n, k); x_mn / y_mn: the operand is stored [k][m] / [k][n]
 template <typename T>
-int contract_t(const void* a, const void* b, void* o, int N, int direction, cudaStream_t s) {
+int gemm_t(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn, cudaStream_t s) {
   const unsigned t = (N + 63) / 64;
   dim3 grid(t, t, C);
-  if (direction == FOLDCP_INCOMING) {
-    simt_contract_kernel<T, true><<<grid, 256, 0, s>>>(static_cast<const T*>(a),
-                                                      static_cast<const T*>(b),
-                                                      static_cast<T*>(o), N);
-  } else {
-    simt_contract_kernel<T, false><<<grid, 256, 0, s>>>(static_cast<const T*>(a),
-                                                       static_cast<const T*>(b),
-                                                       static_cast<T*>(o), N);
-  }
+  const T* X = static_cast<const T*>(x);
+  const T* Y = static_cast<const T*>(y);
+  T* D = static_cast<T*>(d);
+  if (x_mn && y_mn) simt_contract_kernel<T, true, true><<<grid, 256, 0, s>>>(X, Y, D, N);
+  else if (x_mn) simt_contract_kernel<T, true, false><<<grid, 256, 0, s>>>(X, Y, D, N);
+  else if (y_mn) simt_contract_kernel<T, false, true><<<grid, 256, 0, s>>>(X, Y, D, N);
+  else simt_contract_kernel<T, false, false><<<grid, 256, 0, s>>>(X, Y, D, N);
   return check_launch();
+}
+
+template <typename T>
+int contract_t(const void* a, const void* b, void* o, int N, int direction, cudaStream_t s) {
+  const bool inc = direction == FOLDCP_INCOMING;
+  return gemm_t<T>(a, b, o, N, inc, inc, s);
+}
+
+// same operand assignments as launch_k2_contract_backward_bf16 (k2_contract.cu)
+template <typename T>
+int contract_backward_t(const void* d_o, const void* a, const void* b, void* d_a, void* d_b, int N,
+                        int direction, cudaStream_t s) {
+  int st;
+  if (direction == FOLDCP_OUTGOING) {
+    if ((st = gemm_t<T>(d_o, b, d_a, N, false, true, s)) != FOLDCP_OK) return st;
+    return gemm_t<T>(d_o, a, d_b, N, true, true, s);
+  }
+  if ((st = gemm_t<T>(b, d_o, d_a, N, false, false, s)) != FOLDCP_OK) return st;
+  return gemm_t<T>(a, d_o, d_b, N, false, true, s);
 }
 
 template <typename T>
@@ -275,6 +301,11 @@ int launch_simt_contract(const void* a, const void* b, void* o, int N, int dtype
                          cudaStream_t s) {
   return dtype == FOLDCP_F32 ? contract_t<float>(a, b, o, N, direction, s)
                              : contract_t<__nv_bfloat16>(a, b, o, N, direction, s);
+}
+int launch_simt_contract_backward(const void* d_o, const void* a, const void* b, void* d_a,
+                                  void* d_b, int N, int dtype, int direction, cudaStream_t s) {
+  return dtype == FOLDCP_F32 ? contract_backward_t<float>(d_o, a, b, d_a, d_b, N, direction, s)
+                             : contract_backward_t<__nv_bfloat16>(d_o, a, b, d_a, d_b, N, direction, s);
 }
 int launch_simt_finalize(const void* o, const void* z, const void* mask,
                          const foldcp_trimul_params* p, int N, void* out, cudaStream_t s) {

@@ -163,6 +163,27 @@ def test_batched_equals_single_calls_bitwise(residual):
     assert e["rel_fro"] < 1e-2 + (2e-2 if residual else 0.0)
 
 
+# ---------------------------------------------------------------- NEXT-2 (part): contraction backward
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("N,dtype", [(64, torch.bfloat16), (328, torch.bfloat16), (520, torch.bfloat16),
+                                     (67, torch.float32)])
+def test_contract_backward_stage(direction, N, dtype):
+    from oracle import trimul_oracle as orc
+    g = torch.Generator().manual_seed(3 * N + direction)
+    a, b, d_o = (torch.randn(128, N, N, generator=g).to(dtype) for _ in range(3))
+    d_a, d_b = B.contract_backward(d_o.to(DEV), a.to(DEV), b.to(DEV), direction)
+    torch.cuda.synchronize()
+    t = lambda x: np.transpose(U.np64(x), (1, 2, 0))
+    ra, rb = orc.contraction_backward(t(d_o), t(a), t(b), direction)
+    for got, ref in ((t(d_a), ra), (t(d_b), rb)):
+        if dtype == torch.bfloat16:
+            # only the final bf16 rounding (2^-9 relative) plus fp32 accumulation
+            assert np.abs(got - ref).max() <= 2.0 ** -8 * np.abs(ref).max()
+            assert U.errors(got, ref)["rel_fro"] < 3e-3
+        else:
+            assert U.errors(got, ref)["rel_fro"] < 1e-5
+
+
 # ---------------------------------------------------------------- BASELINE configs 2-4 (sub-grid oracle)
 def run_subgrid(cfg, direction, n_idx, seed):
     N = cfg.N
