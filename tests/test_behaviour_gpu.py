@@ -154,3 +154,67 @@ def test_error_codes_leave_out_untouched():
     assert ei.value.status == 5
     torch.cuda.synchronize()
     assert torch.all(out == 7.0)
+
+
+# ---------------------------------------------------------------- degenerate cases the method has
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_degenerate_layernorm_rows_match_oracle(direction):
+    """Constant rows (variance 0: LN -> beta, finite thanks to eps -- reading A20), all-zero
+    rows, rows with a large common offset (the two-pass statistics must not cancel) and rows of
+    large magnitude, mixed into ordinary data."""
+    N = 136
+    cfg = synth.CONFIGS[1]
+    z, _, p = synth.make_inputs(cfg, direction, "cpu", N=N)
+    M = synth.pair_mask(synth.make_token_mask("scatter", N, cfg.seed), cfg.dtype)
+    zf = z.float()
+    zf[3, :, :] = 0.75                       # constant over channels and over a whole row of pairs
+    zf[:, 5, :] = 0.0                        # zero column of pairs
+    zf[10:14] += 48.0                        # common offset >> spread (bf16 keeps ~2 digits of it)
+    zf[20:24] *= 200.0                       # large magnitude
+    z = zf.to(torch.bfloat16)
+    ref = U.oracle_full(z, M, p, direction)
+    out = B.trimul(z.to(DEV), M.to(DEV), {k: v.to(DEV) for k, v in p.items()}, direction)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out).all()
+    U.assert_parity(U.np64(out), ref, "bf16", "degenerate LayerNorm rows")
+
+
+def test_S4_zero_output_projection_gives_exact_zero_and_residual_returns_z():
+    """Closed form S4 on the GPU: W_o = 0, b_o = 0 => update == 0 exactly; with the residual
+    fused the result is z bit for bit (isolates the epilogue's gate / residual arithmetic)."""
+    z, M, p = inputs(264, INC)
+    p = dict(p)
+    p["w_o"] = torch.zeros_like(p["w_o"])
+    p["b_o"] = torch.zeros_like(p["b_o"])
+    upd = B.trimul(z, M, p, INC)
+    res = B.trimul(z, M, p, INC, residual=True)
+    torch.cuda.synchronize()
+    assert torch.count_nonzero(upd) == 0
+    assert torch.equal(res, z)
+
+
+def test_S3_zero_output_gamma_isolates_the_gate():
+    """Closed form S3: gamma_out = 0 => out_ij = M_ij g_ij (W_o beta_out + b_o), independent of
+    the contraction; checked against a direct fp64 evaluation of that expression."""
+    from oracle import trimul_oracle as orc
+    N = 136
+    cfg = synth.CONFIGS[1]
+    z, _, p = synth.make_inputs(cfg, OUT, "cpu", N=N)
+    M = synth.pair_mask(synth.make_token_mask("tail", N, cfg.seed), cfg.dtype)
+    p = dict(p)
+    p["ln_out_gamma"] = torch.zeros_like(p["ln_out_gamma"])
+    out = B.trimul(z.to(DEV), M.to(DEV), {k: v.to(DEV) for k, v in p.items()}, OUT)
+    torch.cuda.synchronize()
+    q = U.params64(p)
+    zp = orc.layer_norm(U.np64(z), q["ln_in_gamma"], q["ln_in_beta"], 1e-5)
+    g = orc.sigmoid(zp @ q["w_g"].T + q["b_g"])
+    ref = U.np64(M)[..., None] * g * (q["w_o"] @ q["ln_out_beta"] + q["b_o"])
+    e = U.errors(U.np64(out), ref)
+    assert e["rel_fro"] < 3e-3 and e["max_over_rms"] < 2e-2
+
+
+def test_fully_masked_input_gives_exact_zero():
+    z, M, p = inputs(136)
+    out = B.trimul(z, torch.zeros_like(M), p, OUT)
+    torch.cuda.synchronize()
+    assert torch.count_nonzero(out) == 0 and torch.isfinite(out).all()
