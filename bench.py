@@ -284,37 +284,62 @@ def run_ours(args):
 
 def run_e2e(ctx, steps):
     """Same metric end to end: every step copies z and the mask from pinned host memory, runs both
-    directions through the public binding and reads both results back to pinned host memory."""
+    directions through the public binding and reads both results back to pinned host memory.
+    The three legs run on their own streams with double-buffered device tensors, so step i+1's
+    upload and step i-1's download overlap step i's kernels (PCIe is full duplex); every step
+    still moves its own 4.3 GB in and 8.6 GB out inside the timed region."""
     torch, B = ctx["torch"], ctx["B"]
-    z, M, ps, ws, outs, dev = ctx["z"], ctx["M"], ctx["ps"], ctx["ws"], ctx["outs"], ctx["dev"]
+    z, M, ps, ws, dev = ctx["z"], ctx["M"], ctx["ps"], ctx["ws"], ctx["dev"]
     hz = torch.empty(z.shape, dtype=z.dtype, pin_memory=True)
     hM = torch.empty(M.shape, dtype=M.dtype, pin_memory=True)
     hz.copy_(z)
     hM.copy_(M)
     ho = [torch.empty(z.shape, dtype=z.dtype, pin_memory=True) for _ in range(2)]
-    dz, dM = torch.empty_like(z), torch.empty_like(M)
+    dz = [torch.empty_like(z) for _ in range(2)]
+    dM = [torch.empty_like(M) for _ in range(2)]
+    douts = [[torch.empty_like(z), torch.empty_like(z)] for _ in range(2)]
+    s_in, s_cmp, s_out = (torch.cuda.Stream(device=dev) for _ in range(3))
+    ev_in = [torch.cuda.Event() for _ in range(2)]
+    ev_cmp = [torch.cuda.Event() for _ in range(2)]
+    ev_out = [torch.cuda.Event() for _ in range(2)]
 
-    def step():
-        dz.copy_(hz, non_blocking=True)
-        dM.copy_(hM, non_blocking=True)
-        B.trimul(dz, dM, ps[0], B.OUTGOING, out=outs[0], workspace=ws)
-        ho[0].copy_(outs[0], non_blocking=True)
-        B.trimul(dz, dM, ps[1], B.INCOMING, out=outs[1], workspace=ws)
-        ho[1].copy_(outs[1], non_blocking=True)
+    def step(i):
+        b = i & 1
+        with torch.cuda.stream(s_in):
+            s_in.wait_event(ev_cmp[b])            # dz[b] was read by step i-2's kernels
+            dz[b].copy_(hz, non_blocking=True)
+            dM[b].copy_(hM, non_blocking=True)
+            ev_in[b].record(s_in)
+        with torch.cuda.stream(s_cmp):
+            s_cmp.wait_event(ev_in[b])
+            s_cmp.wait_event(ev_out[b])           # douts[b] was downloaded by step i-2
+            B.trimul(dz[b], dM[b], ps[0], B.OUTGOING, out=douts[b][0], workspace=ws)
+            B.trimul(dz[b], dM[b], ps[1], B.INCOMING, out=douts[b][1], workspace=ws)
+            ev_cmp[b].record(s_cmp)
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(ev_cmp[b])
+            ho[0].copy_(douts[b][0], non_blocking=True)
+            ho[1].copy_(douts[b][1], non_blocking=True)
+            ev_out[b].record(s_out)
 
-    step()
+    torch.cuda.synchronize()
+    for i in range(2):
+        step(i)                                   # warm-up, also arms every event once
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(steps):
-        step()
-    e1.record()
+    e0.record(s_in)
+    for i in range(steps):
+        step(i)
+    s_out.wait_stream(s_cmp)
+    s_out.wait_stream(s_in)
+    e1.record(s_out)
     torch.cuda.synchronize()
     ms = max_over_ranks(e0.elapsed_time(e1) / steps, ctx["world"], ctx["dist"], dev)
     h2d = hz.numel() * hz.element_size() + hM.numel() * hM.element_size()
     d2h = 2 * ho[0].numel() * ho[0].element_size()
     return {"value": whole_job_tflops(ctx["flops_step"], ms, ctx["world"]), "unit": "TFLOP/s",
-            "ms_per_step": ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps}
+            "ms_per_step": ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps,
+            "overlap": "upload / kernels / download on three streams, double-buffered"}
 
 
 def main():
@@ -334,7 +359,7 @@ def main():
 
     ctx = run_ours(args)
     N, K, world = ctx["N"], ctx["K"], ctx["world"]
-    e2e = None if args.no_e2e else run_e2e(ctx, max(1, min(K, 3)))
+    e2e = None if args.no_e2e else run_e2e(ctx, max(4, min(K, 6)))
     if ctx["rank"] != 0:
         if world > 1:
             ctx["dist"].barrier()
