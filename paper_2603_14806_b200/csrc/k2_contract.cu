@@ -16,6 +16,8 @@
 //                                with the next tile's main loop through the second accumulator
 // kCtaGroup = 2 pairs two SMs on one 256 x 256 tile (cta_group::2): each CTA stages its own 128
 // rows of A and 128 of the 256 B rows, halving per-SM shared-memory operand traffic.
+#include <atomic>
+
 #include "common.h"
 #include "ptx.cuh"
 
@@ -50,6 +52,7 @@ struct K2Params {
   int num_kb;      // ceil(N / 64)
   int l2_hints;    // 1: evict_last loads / evict_first stores
   int panel_n;     // tile rasterisation: n-tiles per column panel (>= 1)
+  unsigned int* sched;   // [0] next tile index, [1] number of CTA groups that have drained
 };
 
 // Tile rasterisation inside one channel: column panels of `panel_n` n-tiles, m fastest-varying
@@ -90,12 +93,16 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + s); };
   auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 2 + s); };
   const uint32_t tmem_slot = bar_base + 8u * (2 * C::kStages + 4);
+  // dynamic tile scheduler: a 2-deep ring of tile indices per CTA, written by the leader's
+  // producer thread into both CTAs of the pair
+  auto tsfull_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 6 + s); };
+  auto tsempty_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 8 + s); };   // leader's
+  auto tile_slot = [&](int s) { return bar_base + 8u * (2 * C::kStages + 10) + 4u * s; };
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   const uint32_t cta_rank = (kCtaGroup == 2) ? ptx::cluster_ctarank() : 0u;
   const bool is_leader = cta_rank == 0;
-  const int group_id = blockIdx.x / kCtaGroup;
   const int num_groups = gridDim.x / kCtaGroup;
 
   if (warp == 0 && lane == 0) {
@@ -109,6 +116,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       ptx::mbar_init(empty_bar(s), 1);
     }
     for (int s = 0; s < 2; ++s) {
+      ptx::mbar_init(tsfull_bar(s), 1);
+      ptx::mbar_init(tsempty_bar(s), 5 * kCtaGroup);   // every consumer of both CTAs, see below
       ptx::mbar_init(tfull_bar(s), 1);
       ptx::mbar_init(tempty_bar(s), 4 * kCtaGroup);   // one arrival per epilogue warp per CTA
     }
@@ -129,6 +138,45 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
 
   const int tiles_per_ch = prm.tiles_m * prm.tiles_n;
 
+  // ---- dynamic, in-order tile scheduler ---------------------------------------------------
+  // Tiles are handed out in index order from one global counter, like the hardware block
+  // scheduler would, but to persistent CTA pairs.  With a static assignment (pair g takes tiles
+  // g, g + G, ...) nothing keeps the pairs in step: small speed differences between SMs add up
+  // over the ~440 tiles of a pair, the tiles in flight spread over many channels / row blocks,
+  // and the sharing of A_c / B_c blocks through L2 collapses (measured at N = 4096: 41-58 GB of
+  // DRAM reads per launch on some B200s against 8.6 GB of operands; 9 GB with one tile per CTA
+  // pair under the hardware scheduler).  In-order dispatch keeps the window of tiles in flight
+  // compact.  Every tile is computed the same way whichever pair gets it: results stay bitwise
+  // reproducible.
+  // The leader's producer thread draws the index and writes it into a 2-deep ring in both CTAs;
+  // every other consumer (peer producer, MMA issuer, epilogue warps) waits on its local "full"
+  // barrier, reads it and releases the entry on the leader's "empty" barrier.  -1 = no more tiles.
+  auto consume_tile = [&](int i) -> int {
+    const int s = i & 1;
+    ptx::mbar_wait_cluster(tsfull_bar(s), (i >> 1) & 1);
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(tile_slot(s)) : "memory");
+    if constexpr (kCtaGroup == 2) {
+      ptx::mbar_arrive_cluster(ptx::mapa(tsempty_bar(s), 0));
+    } else {
+      ptx::mbar_arrive(tsempty_bar(s));
+    }
+    return static_cast<int>(v);
+  };
+  auto produce_tile = [&](int i) -> int {
+    const int s = i & 1;
+    ptx::mbar_wait_cluster(tsempty_bar(s), ((i >> 1) & 1) ^ 1u);
+    const unsigned int drawn = atomicAdd(prm.sched, 1u);
+    const int tile = drawn < static_cast<unsigned int>(prm.num_tiles) ? static_cast<int>(drawn) : -1;
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(tile_slot(s)), "r"(tile) : "memory");
+    ptx::mbar_arrive_release_cluster_local(tsfull_bar(s));
+    if constexpr (kCtaGroup == 2) {
+      ptx::st_shared_cluster_u32(ptx::mapa(tile_slot(s), 1), static_cast<uint32_t>(tile));
+      ptx::mbar_arrive_cluster(ptx::mapa(tsfull_bar(s), 1));
+    }
+    return tile;
+  };
+
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
@@ -136,7 +184,9 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const uint64_t pol_ld = prm.l2_hints == 1 ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
       int stage = 0;
       uint32_t phase = 0;
-      for (int t = group_id; t < prm.num_tiles; t += num_groups) {
+      for (int it = 0;; ++it) {
+        const int t = is_leader ? produce_tile(it) : consume_tile(it);
+        if (t < 0) break;
         const int ch = t / tiles_per_ch;
         const int r = t - ch * tiles_per_ch;
         int tm, tn;
@@ -183,6 +233,15 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
           }
         }
       }
+      if (is_leader) {
+        // the last pair to run dry re-arms the scheduler words for a later launch
+        const unsigned int drained = atomicAdd(prm.sched + 1, 1u);
+        if (drained == static_cast<unsigned int>(num_groups) - 1u) {
+          prm.sched[0] = 0u;
+          prm.sched[1] = 0u;
+          __threadfence();
+        }
+      }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA only) =====================
@@ -196,8 +255,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       constexpr uint32_t kstep_a = kAMn ? 2048 : 32, kstep_b = kBMn ? 2048 : 32;
       int stage = 0;
       uint32_t phase = 0;
-      int it = 0;
-      for (int t = group_id; t < prm.num_tiles; t += num_groups, ++it) {
+      for (int it = 0;; ++it) {
+        if (consume_tile(it) < 0) break;
         const int as = it & 1;
         const uint32_t aphase = (it >> 1) & 1;
         ptx::mbar_wait_cluster(tempty_bar(as), aphase ^ 1u);
@@ -229,9 +288,12 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const int row = q * 32 + lane;          // row of the CTA's 128-row tile
     const bool store_thread = (warp == 4 && lane == 0);
     const uint64_t pol_st = prm.l2_hints ? ptx::kL2EvictFirst : ptx::kL2EvictNormal;
-    int it = 0;
     int chunk_ctr = 0;
-    for (int t = group_id; t < prm.num_tiles; t += num_groups, ++it) {
+    for (int it = 0;; ++it) {
+      int t = 0;
+      if (lane == 0) t = consume_tile(it);
+      t = __shfl_sync(0xffffffffu, t, 0);
+      if (t < 0) break;
       const int ch = t / tiles_per_ch;
       const int r = t - ch * tiles_per_ch;
       int tm, tn;
@@ -327,7 +389,19 @@ int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorM
   return FOLDCP_OK;
 }
 
-int g_k2_cta_group = 2;   // FOLDCP_K2_CTA_GROUP=1 selects the single-CTA variant (debug / A-B test)
+int g_k2_cta_group = 2;
+
+// scheduler words {next tile, drained groups}; one pair per launch in flight, handed out round
+// robin (a launch leaves its pair zeroed again, see the producer's drain code)
+constexpr int kSchedSlots = 256;
+__device__ unsigned int g_k2_sched[kSchedSlots][2];
+
+unsigned int* next_sched_slot() {
+  static std::atomic<unsigned int> ticket{0};
+  unsigned int* base = nullptr;
+  if (cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_k2_sched) != cudaSuccess) return nullptr;
+  return base + 2 * (ticket.fetch_add(1) % kSchedSlots);
+}   // FOLDCP_K2_CTA_GROUP=1 selects the single-CTA variant (debug / A-B test)
 
 }  // namespace
 
@@ -368,10 +442,16 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
   prm.l2_hints = l2_hints;
   static const int panel = [] {
     const char* e = getenv("FOLDCP_K2_PANEL");
-    return e ? atoi(e) : 0;   // 0 = plain row-major order (measured: panels of 8 / 4 / 2 n-tiles
-                              // do not lower DRAM traffic or time at N = 4096)
+    return e ? atoi(e) : 0;
   }();
-  prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : prm.tiles_n;
+  // Default rasterisation (measured with the in-order scheduler): plain row-major while one row
+  // of tiles spans at most 16 n-tiles (N <= 4096: 9 GB of DRAM reads for 8.6 GB of operands);
+  // beyond that, column panels of 8 n-tiles, so that the ~74 tiles in flight keep sharing one
+  // narrow B panel (N = 8192: 104 GB instead of 554 GB, 105 instead of 132 ms).
+  const int auto_panel = prm.tiles_n <= 16 ? prm.tiles_n : 8;
+  prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : auto_panel;
+  prm.sched = next_sched_slot();
+  if (prm.sched == nullptr) return FOLDCP_ERR_CUDA;
   const int sms = dev.sm_count;
   if (cta_group == 2) {
     if (x_mn) return y_mn ? launch_variant<2, true, true>(ta, tb, to, prm, sms, stream)
