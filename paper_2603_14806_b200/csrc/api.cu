@@ -5,7 +5,10 @@
 #include <cstring>
 #include <mutex>
 
+#include <atomic>
+
 #include "common.h"
+#include "tile_sched.cuh"
 
 // default implementation of the three bf16 stages: bit0 K1, bit1 K2, bit2 K3 on tcgen05
 #ifndef FOLDCP_DEFAULT_TC_STAGES
@@ -35,6 +38,22 @@ bool get_device_info(DeviceInfo* info) {
   }
   *info = cache[dev];
   return true;
+}
+
+// ----------------------------------------------------------------------------- tile scheduler
+// scheduler words {next tile, drained CTAs}; one pair per launch in flight, handed out round robin
+// (a launch leaves its pair zeroed again, see TileRing::drain)
+namespace {
+constexpr int kSchedSlots = 1024;
+__device__ unsigned int g_sched_words[kSchedSlots][2];
+}  // namespace
+
+unsigned int* next_sched_slot() {
+  static std::atomic<unsigned int> ticket{0};
+  unsigned int* base = nullptr;
+  if (cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_sched_words) != cudaSuccess)
+    return nullptr;
+  return base + 2 * (ticket.fetch_add(1) % kSchedSlots);
 }
 
 // ----------------------------------------------------------------------------- launch attributes

@@ -16,10 +16,9 @@
 //                                with the next tile's main loop through the second accumulator
 // kCtaGroup = 2 pairs two SMs on one 256 x 256 tile (cta_group::2): each CTA stages its own 128
 // rows of A and 128 of the 256 B rows, halving per-SM shared-memory operand traffic.
-#include <atomic>
-
 #include "common.h"
 #include "ptx.cuh"
+#include "tile_sched.cuh"
 
 namespace foldcp {
 namespace {
@@ -390,18 +389,6 @@ int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorM
 }
 
 int g_k2_cta_group = 2;
-
-// scheduler words {next tile, drained groups}; one pair per launch in flight, handed out round
-// robin (a launch leaves its pair zeroed again, see the producer's drain code)
-constexpr int kSchedSlots = 256;
-__device__ unsigned int g_k2_sched[kSchedSlots][2];
-
-unsigned int* next_sched_slot() {
-  static std::atomic<unsigned int> ticket{0};
-  unsigned int* base = nullptr;
-  if (cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_k2_sched) != cudaSuccess) return nullptr;
-  return base + 2 * (ticket.fetch_add(1) % kSchedSlots);
-}   // FOLDCP_K2_CTA_GROUP=1 selects the single-CTA variant (debug / A-B test)
 
 }  // namespace
 
