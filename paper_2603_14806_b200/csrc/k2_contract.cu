@@ -92,11 +92,12 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + s); };
   auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 2 + s); };
   const uint32_t tmem_slot = bar_base + 8u * (2 * C::kStages + 4);
-  // dynamic tile scheduler: a 2-deep ring of tile indices per CTA, written by the leader's
+  // dynamic tile scheduler: a 4-deep ring of tile indices per CTA, written by the leader's
   // producer thread into both CTAs of the pair
+  constexpr int kRing = 4;
   auto tsfull_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 6 + s); };
-  auto tsempty_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 8 + s); };   // leader's
-  auto tile_slot = [&](int s) { return bar_base + 8u * (2 * C::kStages + 10) + 4u * s; };
+  auto tsempty_bar = [&](int s) { return bar_base + 8u * (2 * C::kStages + 6 + kRing + s); };  // leader's
+  auto tile_slot = [&](int s) { return bar_base + 8u * (2 * C::kStages + 6 + 2 * kRing) + 4u * s; };
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -114,9 +115,11 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       ptx::mbar_init(full_bar(s), 1);
       ptx::mbar_init(empty_bar(s), 1);
     }
-    for (int s = 0; s < 2; ++s) {
+    for (int s = 0; s < kRing; ++s) {
       ptx::mbar_init(tsfull_bar(s), 1);
       ptx::mbar_init(tsempty_bar(s), 5 * kCtaGroup);   // every consumer of both CTAs, see below
+    }
+    for (int s = 0; s < 2; ++s) {
       ptx::mbar_init(tfull_bar(s), 1);
       ptx::mbar_init(tempty_bar(s), 4 * kCtaGroup);   // one arrival per epilogue warp per CTA
     }
@@ -147,12 +150,12 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   // pair under the hardware scheduler).  In-order dispatch keeps the window of tiles in flight
   // compact.  Every tile is computed the same way whichever pair gets it: results stay bitwise
   // reproducible.
-  // The leader's producer thread draws the index and writes it into a 2-deep ring in both CTAs;
+  // The leader's producer thread draws the index and writes it into a 4-deep ring in both CTAs;
   // every other consumer (peer producer, MMA issuer, epilogue warps) waits on its local "full"
   // barrier, reads it and releases the entry on the leader's "empty" barrier.  -1 = no more tiles.
   auto consume_tile = [&](int i) -> int {
-    const int s = i & 1;
-    ptx::mbar_wait_cluster(tsfull_bar(s), (i >> 1) & 1);
+    const int s = i % kRing;
+    ptx::mbar_wait_cluster(tsfull_bar(s), (i / kRing) & 1);
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(tile_slot(s)) : "memory");
     if constexpr (kCtaGroup == 2) {
@@ -163,8 +166,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
     return static_cast<int>(v);
   };
   auto produce_tile = [&](int i) -> int {
-    const int s = i & 1;
-    ptx::mbar_wait_cluster(tsempty_bar(s), ((i >> 1) & 1) ^ 1u);
+    const int s = i % kRing;
+    ptx::mbar_wait_cluster(tsempty_bar(s), ((i / kRing) & 1) ^ 1u);
     const unsigned int drawn = atomicAdd(prm.sched, 1u);
     const int tile = drawn < static_cast<unsigned int>(prm.num_tiles) ? static_cast<int>(drawn) : -1;
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(tile_slot(s)), "r"(tile) : "memory");
@@ -183,9 +186,12 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const uint64_t pol_ld = prm.l2_hints == 1 ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
       int stage = 0;
       uint32_t phase = 0;
+      // the leader draws one tile ahead, so the atomic's round trip never stalls the load pipeline
+      int tnext = is_leader ? produce_tile(0) : consume_tile(0);
       for (int it = 0;; ++it) {
-        const int t = is_leader ? produce_tile(it) : consume_tile(it);
+        const int t = tnext;
         if (t < 0) break;
+        tnext = is_leader ? produce_tile(it + 1) : consume_tile(it + 1);
         const int ch = t / tiles_per_ch;
         const int r = t - ch * tiles_per_ch;
         int tm, tn;
