@@ -24,7 +24,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 C = 128
-K2_DRAM_BYTES_PER_LAUNCH_N4096 = 16.92e9 + 4.28e9   # ncu, profiles/r1_k2_contract_ncu_full.txt
+K2_DRAM_BYTES_PER_LAUNCH_N4096 = 9.06e9 + 4.28e9   # ncu, profiles/r1_k2_contract_ncu_full.txt
 
 
 def counted_flops(N: int) -> float:
@@ -381,9 +381,8 @@ def main():
         "ms_per_launch": {"outgoing": sm["k2_out"], "incoming": sm["k2_in"]},
         "share_of_step": (sm["k2_out"] + sm["k2_in"]) / step_sum,
         # dram__bytes_read.sum + dram__bytes_write.sum of one k2_contract launch at N=4096, from the
-        # ncu --set full capture summarised in profiles/ (16.9 GB read + 4.3 GB written; the
-        # algorithmic bytes are 8.6 GB read + 4.3 GB written; other boxes of the pool showed up to
-        # 45 GB read for the same launch -- DESIGN.md section 6)
+        # ncu --set full capture summarised in profiles/ (9.06 GB read + 4.28 GB written; the
+        # algorithmic bytes are 8.59 GB read + 4.29 GB written)
         "traffic": K2_DRAM_BYTES_PER_LAUNCH_N4096 if N == 4096 else None,
         "traffic_source": "profiles/r1_k2_contract_ncu_full.txt",
         "algorithmic_bytes_per_launch": 3.0 * C * N * N * 2,
