@@ -349,7 +349,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=4096, help="tokens (default: BASELINE configs[3])")
-    ap.add_argument("--ref-rows", type=int, default=24, help="sub-grid size of the oracle sample")
+    ap.add_argument("--ref-rows", type=int, default=128,
+                    help="sub-grid size of the oracle sample (128: ~12 s of CPU work per step)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
