@@ -41,6 +41,7 @@
 #include "common.h"
 #include "ln_rows.cuh"
 #include "ptx.cuh"
+#include "tile_sched.cuh"
 
 namespace foldcp {
 namespace {
@@ -69,7 +70,9 @@ constexpr int kOffOut = kOffZ + kZStages * kMatBytes;      // staging buffers
 constexpr int kOffMask = kOffOut + kOutBufs * kHalfBox;    // fp32 pair mask per tile slot
 constexpr int kOffFlag = kOffMask + kMaskSlots * kTilePairs * 4;   // 4 "all ones" words per slot
 constexpr int kOffBar = kOffFlag + kMaskSlots * 16;
-constexpr int kSmemBytes = kOffBar + 256;
+constexpr int kRingDepth = 8;
+constexpr int kOffRing = kOffBar + 256;
+constexpr int kSmemBytes = kOffRing + TileRing<kRingDepth>::kBytes;
 static_assert(kSmemBytes <= 232448, "K1 shared memory exceeds 227 KB");
 static_assert((3 * kZStages + 18) * 8 <= 256, "barrier region too small");
 
@@ -85,6 +88,7 @@ struct K1Params {
   float eps;
   long long R;                 // number of pairs
   int num_tiles;
+  unsigned int* sched;
 };
 
 template <bool kTanhSigmoid>
@@ -106,6 +110,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   const uint32_t wready = bar + 8u * (3 * kZStages + 9);   // weights are in TMEM
   auto ofull = [&](int b) { return bar + 8u * (3 * kZStages + 10 + b); };    // staging buffer b
   auto oempty = [&](int b) { return bar + 8u * (3 * kZStages + 14 + b); };   // (tensor, group)
+  const TileRing<kRingDepth> ring{smem + kOffRing};
+  constexpr uint32_t kRingConsumers = 1 + 1 + kLnWarps + 4 * kTeams;   // MMA, store, LN, epilogue
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -126,6 +132,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_init(tempty(u), 4);
     }
     ptx::mbar_init(wready, 4 * kTeams);
+    ring.init(kRingConsumers);
     for (int b = 0; b < kOutBufs; ++b) {
       ptx::mbar_init(ofull(b), 4 * kPar);   // one arrival per warp that fills the buffer
       ptx::mbar_init(oempty(b), 1);
@@ -139,14 +146,14 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-  const int first = blockIdx.x;
-  const int stride = gridDim.x;
 
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
       int it = 0;
-      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      for (;; ++it) {
+        const int t = ring.produce(it, prm.sched, prm.num_tiles);
+        if (t < 0) break;
         const int s = it % kZStages;
         ptx::mbar_wait(zempty(s), ((it / kZStages) & 1) ^ 1u);
         ptx::mbar_arrive_expect_tx(zfull(s), kMatBytes);
@@ -155,6 +162,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::tma_load_2d(dst, &tmap_z, zfull(s), 0, row0);
         ptx::tma_load_2d(dst + kHalfBox, &tmap_z, zfull(s), 64, row0);
       }
+      ring.drain(prm.sched, gridDim.x);
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
@@ -165,7 +173,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_wait(wready, 0);
       ptx::tc_fence_after();
       int it = 0;
-      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      for (;; ++it) {
+        if (ring.consume(it) < 0) break;
         const int s = it % kZStages;
         ptx::mbar_wait(zready(s), (it / kZStages) & 1);
         ptx::tc_fence_after();
@@ -205,7 +214,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // previous store has finished reading shared memory.  No block-wide barrier in the epilogue.
     if (ptx::elect_one()) {
       int it = 0, prev = -1;
-      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      for (;; ++it) {
+        const int t = ring.consume(it);
+        if (t < 0) break;
 #pragma unroll
         for (int g = 0; g < 2; ++g) {
 #pragma unroll
@@ -231,17 +242,21 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
     auto load_mask = [&](int t) -> unsigned short {
       if (prm.mask == nullptr || r >= kTilePairs) return static_cast<unsigned short>(0x3f80);
-      if (t >= prm.num_tiles) return static_cast<unsigned short>(0);
+      if (t < 0) return static_cast<unsigned short>(0);
       const long long p = static_cast<long long>(t) * kTilePairs + r;
       return p < prm.R ? __ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)
                        : static_cast<unsigned short>(0);
     };
-    unsigned short mnext = load_mask(first);
+    int tnext = ring.consume_warp(0, lane);
+    unsigned short mnext = load_mask(tnext);
     int it = 0;
-    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+    for (;; ++it) {
+      const int t = tnext;
+      if (t < 0) break;
       const int s = it % kZStages;
       const unsigned short mraw = mnext;
-      mnext = load_mask(t + stride);
+      tnext = ring.consume_warp(it + 1, lane);
+      mnext = load_mask(tnext);
       ptx::mbar_wait(zfull(s), (it / kZStages) & 1);
       layernorm_rows_inplace<kNormFp16, false, kLnWarps == 4 ? 2 : 1, kLnWarps * 32>(
           smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0, prm.eps);
@@ -363,7 +378,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // barrier, store thread and staging buffers).
     constexpr bool kPrefetch = kTeams == 2;     // enough registers for a second tcgen05.ld buffer
     int it = 0;
-    for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+    for (;; ++it) {
+      if (ring.consume_warp(it, lane) < 0) break;
       const int ms = it & (kMaskSlots - 1);
       bool masked = true;
 #pragma unroll
@@ -485,6 +501,8 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   prm.eps = p->ln_eps;
   prm.R = static_cast<long long>(R);
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
+  prm.sched = next_sched_slot();
+  if (prm.sched == nullptr) return FOLDCP_ERR_CUDA;
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k1_tanh_sigmoid();
   auto kern = tanh_sig ? k1_project_kernel<true> : k1_project_kernel<false>;

@@ -1,4 +1,4 @@
-// Dynamic, in-order tile scheduling for the persistent contraction kernel (K2).
+// Dynamic, in-order tile scheduling for the persistent kernels (K2 and K1).
 //
 // With a static assignment (CTA pair g takes tiles g, g + G, g + 2G, ...) nothing keeps the pairs
 // in step: small speed differences between SMs accumulate over the ~440 tiles of a pair, the set
@@ -10,13 +10,63 @@
 //
 // The scheduler words live in a pool in global memory ({next tile, drained CTA groups} per
 // launch); the last group to run dry re-arms its pair for a later launch (k2_contract.cu).
-// K1 / K3 keep the static assignment: their tiles share nothing, and the same scheduler measured
-// no gain there.
+// K1's tiles share nothing, but its a / b stores are 128-byte rows 32 MB apart: adjacent tiles fill
+// the same DRAM pages only if they are written at about the same time, and the in-order scheduler
+// (TileRing below) made K1 13-15 % faster.  K3 keeps the static assignment: the same scheduler
+// measured no gain there (its stores are contiguous 32 KB blocks).
 #pragma once
+
+#include "ptx.cuh"
 
 namespace foldcp {
 
 // host side (api.cu): a pair of zeroed scheduler words for one launch; nullptr on CUDA error
 unsigned int* next_sched_slot();
+
+// Single-CTA flavour: one thread draws tile indices and publishes them in a ring in shared memory;
+// every other role waits on the entry's "full" mbarrier, reads it and releases it on "empty".
+template <int kDepth>
+struct TileRing {
+  uint32_t base;   // shared address: kDepth full barriers, kDepth empty barriers, kDepth slots
+  static constexpr int kBytes = kDepth * 20;
+  __device__ __forceinline__ uint32_t full(int s) const { return base + 8u * s; }
+  __device__ __forceinline__ uint32_t empty(int s) const { return base + 8u * (kDepth + s); }
+  __device__ __forceinline__ uint32_t slot(int s) const { return base + 16u * kDepth + 4u * s; }
+  __device__ __forceinline__ void init(uint32_t consumers) const {
+    for (int s = 0; s < kDepth; ++s) {
+      ptx::mbar_init(full(s), 1);
+      ptx::mbar_init(empty(s), consumers);
+    }
+  }
+  __device__ __forceinline__ int produce(int i, unsigned int* sched, int num_tiles) const {
+    const int s = i % kDepth;
+    ptx::mbar_wait(empty(s), ((i / kDepth) & 1) ^ 1u);
+    const unsigned int drawn = atomicAdd(sched, 1u);
+    const int tile = drawn < static_cast<unsigned int>(num_tiles) ? static_cast<int>(drawn) : -1;
+    ptx::sts32(slot(s), static_cast<uint32_t>(tile));
+    ptx::mbar_arrive(full(s));
+    return tile;
+  }
+  __device__ __forceinline__ void drain(unsigned int* sched, unsigned int num_ctas) const {
+    const unsigned int drained = atomicAdd(sched + 1, 1u);
+    if (drained == num_ctas - 1u) {
+      sched[0] = 0u;
+      sched[1] = 0u;
+      __threadfence();
+    }
+  }
+  __device__ __forceinline__ int consume(int i) const {
+    const int s = i % kDepth;
+    ptx::mbar_wait(full(s), (i / kDepth) & 1);
+    const int tile = static_cast<int>(ptx::lds32(slot(s)));
+    ptx::mbar_arrive(empty(s));
+    return tile;
+  }
+  __device__ __forceinline__ int consume_warp(int i, int lane) const {
+    int tile = 0;
+    if (lane == 0) tile = consume(i);
+    return __shfl_sync(0xffffffffu, tile, 0);
+  }
+};
 
 }  // namespace foldcp
