@@ -218,3 +218,21 @@ def test_fully_masked_input_gives_exact_zero():
     out = B.trimul(z, torch.zeros_like(M), p, OUT)
     torch.cuda.synchronize()
     assert torch.count_nonzero(out) == 0 and torch.isfinite(out).all()
+
+
+def test_scheduler_slots_are_rearmed_after_wrap_around():
+    """K1 and K2 draw their tiles from a pool of 1024 scheduler-word pairs handed out round robin;
+    every launch must leave its pair zeroed for the launch that re-uses it.  More launches than
+    slots, results bitwise identical throughout."""
+    z, M, p = inputs(136)
+    ref = B.trimul(z, M, p, OUT)
+    torch.cuda.synchronize()
+    ws = torch.empty(B.workspace_bytes(136), dtype=torch.uint8, device=DEV)
+    out = torch.empty_like(z)
+    for i in range(700):                      # 2 scheduler-using launches per call -> 1400 draws
+        B.trimul(z, M, p, OUT, out=out, workspace=ws)
+        if i % 100 == 99:
+            torch.cuda.synchronize()
+            assert torch.equal(out, ref), f"call {i}"
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
