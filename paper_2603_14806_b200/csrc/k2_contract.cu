@@ -16,6 +16,10 @@
 //                                with the next tile's main loop through the second accumulator
 // kCtaGroup = 2 pairs two SMs on one 256 x 256 tile (cta_group::2): each CTA stages its own 128
 // rows of A and 128 of the 256 B rows, halving per-SM shared-memory operand traffic.
+// The two operand majors are independent template parameters (kAMn, kBMn): the forward uses
+// (K, K) and (MN, MN), the gradients of the contraction also the mixed (K, MN) form.
+// Tiles are not assigned statically: the leader's producer thread draws them in index order from
+// a global counter (tile_sched.cuh) and publishes them to the other roles through a small ring.
 #include "common.h"
 #include "ptx.cuh"
 #include "tile_sched.cuh"
