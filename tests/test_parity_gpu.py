@@ -224,3 +224,45 @@ def test_config4_bf16_n8192_single_call(direction):
         pytest.skip("needs ~85 GiB of free HBM")
     run_subgrid(synth.CONFIGS[4], direction, 48, 13)
     torch.cuda.empty_cache()
+
+
+# ---------------------------------------------------------------- randomised sweep (full oracle)
+def test_randomised_sweep_against_oracle():
+    """Seeded sweep over sizes (multiples of 8 up to 320: partial tiles in every kernel), both
+    directions, mask kinds (incl. a general non-symmetric pair mask and NULL), missing biases,
+    output mask on / off, residual on / off, and input scale / offset."""
+    import random
+    from oracle import trimul_oracle as orc
+    rnd = random.Random(20260314)
+    cfg = synth.CONFIGS[1]
+    for trial in range(12):
+        N = 8 * rnd.randint(1, 40)
+        d = rnd.randint(0, 1)
+        mo, res = rnd.random() < 0.7, rnd.random() < 0.4
+        mk = rnd.choice(["ones", "tail", "scatter", "none", "rand"])
+        z, _, p = synth.make_inputs(cfg, d, "cpu", N=N)
+        g = torch.Generator().manual_seed(trial)
+        z = (z.float() * (0.2 + 3 * torch.rand(1, generator=g)) + torch.randn(1, generator=g)).to(torch.bfloat16)
+        if mk == "none":
+            M = None
+        elif mk == "rand":
+            M = (torch.rand(N, N, generator=g) > 0.3).to(torch.bfloat16)
+        else:
+            M = synth.pair_mask(synth.make_token_mask(mk, N, trial), "bf16")
+        if rnd.random() < 0.3:
+            p = dict(p)
+            p[rnd.choice(["b_a", "b_g", "b_o", "b_b_gate"])] = None
+        upd = orc.trimul(U.np64(z), None if M is None else U.np64(M), U.params64(p), d, mask_output=mo)
+        ref = upd + (U.np64(z) if res else 0.0)
+        out = B.trimul(z.to(DEV), None if M is None else M.to(DEV),
+                       {k: (None if v is None else v.to(DEV)) for k, v in p.items()}, d,
+                       mask_output=mo, residual=res)
+        torch.cuda.synchronize()
+        got = U.np64(out)
+        what = f"trial {trial}: N={N} dir={d} mask={mk} mask_output={mo} residual={res}"
+        assert np.all(np.isfinite(got)), what
+        # north_star tolerance on the update; the residual form adds the rounding of z + update
+        tol = U.TOL["bf16"]["max_over_rms"] * np.sqrt(np.mean(upd ** 2)) + \
+            (2.0 ** -9 * np.abs(ref).max() if res else 0.0)
+        assert np.abs(got - ref).max() <= tol, what
+        assert np.linalg.norm(got - ref) <= U.TOL["bf16"]["rel_fro"] * np.linalg.norm(ref), what
