@@ -145,6 +145,8 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
 int foldcp_trimul_launches_per_call(int dtype);
 
 const char* foldcp_status_string(int status);
+/* major * 100 + minor * 10; 110 added params->add_residual, foldcp_trimul_batched and
+ * foldcp_trimul_contract_backward (the params struct grew: struct_size guards mismatches). */
 int foldcp_version(void);
 
 #ifdef __cplusplus

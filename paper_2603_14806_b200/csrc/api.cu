@@ -349,6 +349,6 @@ const char* foldcp_status_string(int status) {
   }
 }
 
-int foldcp_version(void) { return 100; }
+int foldcp_version(void) { return 110; }   // 1.1: add_residual, batched, contract_backward
 
 }  // extern "C"
