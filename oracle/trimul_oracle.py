@@ -29,8 +29,8 @@ gating, A8 `mask_output` flag.
 A library primitive (numpy matmul) serves as the dense-contraction step; there is no
 blocking, fusion or reordering beyond the definition.  Pins: tests/test_oracle_pins.py
 (brute-force index loops from oracle/brute_force.py on tiny shapes, closed forms S1-S4,
-invariants I1/I1'/I2/I3/I6/S8, N=1; residual / batched forms against the brute force) --
-every function below is pinned there.
+invariants I1/I1'/I2/I3/I6/S8, N=1; residual / batched / row-block forms against the brute
+force) -- every function below is pinned there.
 """
 from __future__ import annotations
 
@@ -189,6 +189,42 @@ def trimul_subgrid(z_a: np.ndarray, mask_a: Optional[np.ndarray],
     o = np.transpose(A @ np.transpose(B, (0, 2, 1)), (1, 2, 0))   # [|I|, |J|, c]
     zp_ij = layer_norm(z_ij, p["ln_in_gamma"], p["ln_in_beta"], eps)
     return output_stage(o, zp_ij, mask_ij, p, eps, mask_output)
+
+
+def projections(z: np.ndarray, mask: Optional[np.ndarray], p: Dict[str, np.ndarray],
+                eps: float = 1e-5):
+    """(a, b) = the two gated, masked projections of LayerNorm(z) (north_star),
+    for z of any leading shape [..., c_z] and a mask of that leading shape: every pair is
+    independent, so a caller may evaluate a tensor too large for host memory slice by slice."""
+    zp = layer_norm(z, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    a = gated_projection(zp, mask, p["w_a"], p.get("b_a"), p["w_a_gate"], p.get("b_a_gate"))
+    b = gated_projection(zp, mask, p["w_b"], p.get("b_b"), p["w_b_gate"], p.get("b_b_gate"))
+    return a, b
+
+
+def trimul_rowblock(a: np.ndarray, b: np.ndarray, z_rows: np.ndarray,
+                    mask_rows: Optional[np.ndarray], p: Dict[str, np.ndarray], direction: int,
+                    i0: int, i1: int, eps: float = 1e-5, mask_output: bool = True) -> np.ndarray:
+    """Exact out[i0:i1, :, :] of the full op with bounded memory (whole-tensor parity at N = 4096,
+    where out alone is 17 GB in fp64).  `a`, `b` [N, N, c] are the projections of the WHOLE z
+    (from `projections`); z_rows = z[i0:i1], mask_rows = M[i0:i1] feed the output gate / mask.
+
+    PAPER.md Eq. 2-3 (lines 121-128) restricted to output rows i0..i1-1, nothing else changed:
+      outgoing: o[i, j] = sum_k a[i, k] b[j, k]   needs a's ROWS    i0:i1 and all of b
+      incoming: o[i, j] = sum_k a[k, i] b[k, j]   needs a's COLUMNS i0:i1 and all of b
+    followed by the same output stage as `trimul`."""
+    B = np.transpose(np.asarray(b, _F), (2, 0, 1))                       # [c, row, col]
+    if direction == OUTGOING:
+        A = np.transpose(np.asarray(a[i0:i1], _F), (2, 0, 1))            # [c, i, k]
+        O = A @ np.transpose(B, (0, 2, 1))                               # sum_k a[i,k] b[j,k]
+    elif direction == INCOMING:
+        A = np.transpose(np.asarray(a[:, i0:i1], _F), (2, 1, 0))         # [c, i, k] = a[k, i]
+        O = A @ B                                                        # sum_k a[k,i] b[k,j]
+    else:
+        raise ValueError("direction must be 0 (outgoing) or 1 (incoming)")
+    o = np.transpose(O, (1, 2, 0))                                       # [i1 - i0, N, c]
+    zp = layer_norm(z_rows, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    return output_stage(o, zp, mask_rows, p, eps, mask_output)
 
 
 def flops(N: int, c_z: int, c_hidden: int) -> float:

@@ -432,6 +432,51 @@ def test_subgrid_matches_full(direction, mask_output):
     assert relerr(got, full[I][:, J]) < 1e-12
 
 
+# ----------------------------------------------------------------------------------------
+# row-block form (bounded memory, used for whole-tensor parity at N = 4096): pinned against the
+# scalar loops and against the whole-tensor oracle, both directions, general pair mask, ragged
+# blocks, projections evaluated slice by slice
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("mask_output", [True, False])
+def test_rowblock_against_brute_force_and_full(direction, mask_output):
+    rng = np.random.default_rng(77 + direction)
+    N, c_z, c = 7, 8, 5
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)       # general, non-symmetric pair mask
+    p = rand_params(rng, c_z, c)
+    # projections of the whole z, evaluated in row slices of unequal height
+    a = np.empty((N, N, c))
+    b = np.empty((N, N, c))
+    for r0, r1 in ((0, 2), (2, 3), (3, 7)):
+        a[r0:r1], b[r0:r1] = orc.projections(z[r0:r1], M[r0:r1], p)
+    blocks = [(0, 3), (3, 4), (4, 7)]                         # ragged row blocks
+    got = np.concatenate([orc.trimul_rowblock(a, b, z[i0:i1], M[i0:i1], p, direction, i0, i1,
+                                              mask_output=mask_output) for i0, i1 in blocks])
+    brute = np.array(brute_force.trimul_brute(z.tolist(), M.tolist(), tolist(p), direction,
+                                              mask_output=mask_output))
+    assert got.shape == (N, N, c_z)
+    assert relerr(got, brute) < 1e-12
+    assert relerr(got, orc.trimul(z, M, p, direction, mask_output=mask_output)) < 1e-13
+    # a transposed operand or a swapped direction must not pass: the two directions differ
+    other = np.concatenate([orc.trimul_rowblock(a, b, z[i0:i1], M[i0:i1], p, 1 - direction, i0, i1,
+                                                mask_output=mask_output) for i0, i1 in blocks])
+    assert relerr(other, brute) > 1e-2
+
+
+def test_rowblock_null_mask_and_single_row():
+    rng = np.random.default_rng(5)
+    N, c_z, c = 5, 4, 6
+    z = rng.standard_normal((N, N, c_z))
+    p = rand_params(rng, c_z, c, bias=False)
+    a, b = orc.projections(z, None, p)
+    for direction in (OUT, INC):
+        full = orc.trimul(z, None, p, direction)
+        for i in range(N):
+            row = orc.trimul_rowblock(a, b, z[i:i + 1], None, p, direction, i, i + 1)
+            assert relerr(row[0], full[i]) < 1e-13
+
+
 def test_flop_count_matches_baseline_md():
     # 17.592 + 2.749 + 0.550 = 20.891 TFLOP at N=4096, c=c_z=128
     assert abs(orc.flops(4096, 128, 128) / 1e12 - 20.891) < 1e-3
