@@ -62,7 +62,10 @@ def layer_norm(x: np.ndarray, gamma: np.ndarray, beta: np.ndarray, eps: float) -
 
 def _linear(x: np.ndarray, w: np.ndarray, b: Optional[np.ndarray]) -> np.ndarray:
     """torch.nn.Linear convention: y = x W^T + b, W is [out_features, in_features]."""
-    y = x @ np.asarray(w, _F).T
+    x = np.asarray(x, _F)
+    # leading dimensions flattened so that the product is ONE dense matmul (same definition,
+    # same value per element; a 3-D @ 2-D numpy matmul would issue one small gemm per leading row)
+    y = (x.reshape(-1, x.shape[-1]) @ np.asarray(w, _F).T).reshape(x.shape[:-1] + (np.shape(w)[0],))
     if b is not None:
         y = y + np.asarray(b, _F)
     return y

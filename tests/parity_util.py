@@ -71,8 +71,123 @@ def errors(got, ref):
 def assert_parity(got, ref, dtype, what=""):
     e = errors(got, ref)
     tol = TOL[dtype]
+    e["outputs"] = int(np.asarray(ref).size)
+    record_parity(what, e, dtype)      # recorded before asserting: a failing run leaves its numbers
     assert np.all(np.isfinite(np.asarray(got, np.float64))), f"{what}: non-finite output"
     assert e["rel_fro"] <= tol["rel_fro"], f"{what}: rel Frobenius {e['rel_fro']:.3e} > {tol['rel_fro']}"
     assert e["max_over_rms"] <= tol["max_over_rms"], \
         f"{what}: max abs / rms {e['max_over_rms']:.3e} > {tol['max_over_rms']}"
     return e
+
+
+# ------------------------------------------------------------------------------------------------
+# measured-error records: every parity test prints what it measured and appends it to a JSON-lines
+# file (gpurun_out/ is the only folder that comes back from the GPU box); tests/parity_report.py
+# turns those lines into the tracked profiles/parity_r*.json
+# ------------------------------------------------------------------------------------------------
+import json
+import os
+import time
+
+_ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def record_parity(what, e, dtype, **fields):
+    tol = TOL[dtype]
+    rec = dict(what=what, dtype=dtype, rel_fro=e["rel_fro"], max_over_rms=e["max_over_rms"],
+               rms=e.get("rms"), tol_rel_fro=tol["rel_fro"], tol_max_over_rms=tol["max_over_rms"],
+               margin_rel_fro=1.0 - e["rel_fro"] / tol["rel_fro"],
+               margin_max_over_rms=1.0 - e["max_over_rms"] / tol["max_over_rms"],
+               when=time.strftime("%Y-%m-%dT%H:%M:%SZ", time.gmtime()))
+    for k in ("outputs", "argmax", "max_abs"):
+        if k in e:
+            rec[k] = e[k]
+    rec.update(fields)
+    print(f"[parity] {what}: rel_fro={e['rel_fro']:.3e} (tol {tol['rel_fro']:.0e}) "
+          f"max/rms={e['max_over_rms']:.3e} (tol {tol['max_over_rms']:.0e})", flush=True)
+    path = os.environ.get("FOLDCP_PARITY_LOG", os.path.join(_ROOT, "gpurun_out", "parity_records.jsonl"))
+    try:
+        os.makedirs(os.path.dirname(path), exist_ok=True)
+        with open(path, "a") as f:
+            f.write(json.dumps(rec) + "\n")
+    except OSError:
+        pass
+    return rec
+
+
+# ------------------------------------------------------------------------------------------------
+# whole-tensor oracle walk (N = 4096: out alone is 17 GB in fp64): the projections a, b of the
+# whole z are evaluated slice by slice (orc.projections), then orc.trimul_rowblock gives the exact
+# out[i0:i1] block by block and the error sums are accumulated.  The arithmetic is the oracle's;
+# this harness only slices, runs blocks on host threads and adds up squared errors.
+# ------------------------------------------------------------------------------------------------
+def _host_workers(bytes_per_worker):
+    import psutil
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    avail = psutil.virtual_memory().available
+    return max(1, min(cores, int(0.6 * avail // max(bytes_per_worker, 1))))
+
+
+def oracle_projections_whole(z, M, p, eps=1e-5, chunk_rows=16):
+    """(a, b) of the whole z as fp64 views [N, N, c] over channel-major storage (the layout in which
+    trimul_rowblock's per-channel matmuls read contiguous matrices).  z / M may live on the GPU."""
+    from concurrent.futures import ThreadPoolExecutor
+    from threadpoolctl import threadpool_limits
+    N, c_z = z.shape[0], z.shape[2]
+    q = params64(p)
+    c = q["w_a"].shape[0]
+    a_cm = np.empty((c, N, N), np.float64)
+    b_cm = np.empty((c, N, N), np.float64)
+
+    def work(r0):
+        r1 = min(N, r0 + chunk_rows)
+        zc = np64(z[r0:r1]).reshape(-1, c_z)
+        mc = None if M is None else np64(M[r0:r1]).reshape(-1)
+        a, b = orc.projections(zc, mc, q, eps)
+        a_cm[:, r0:r1, :] = a.reshape(r1 - r0, N, c).transpose(2, 0, 1)
+        b_cm[:, r0:r1, :] = b.reshape(r1 - r0, N, c).transpose(2, 0, 1)
+
+    workers = _host_workers(chunk_rows * N * c_z * 8 * 12)
+    with threadpool_limits(limits=1):
+        with ThreadPoolExecutor(workers) as ex:
+            list(ex.map(work, range(0, N, chunk_rows)))
+    return a_cm.transpose(1, 2, 0), b_cm.transpose(1, 2, 0)
+
+
+def whole_tensor_errors(out, z, M, p, direction, row_blocks=None, block_rows=32, mask_output=True,
+                        eps=1e-5, ab=None):
+    """Errors of `out` (device or host tensor [N, N, c_z]) against the oracle over the given row
+    blocks (default: every row, i.e. the WHOLE tensor).  Returns rel_fro, max_over_rms (rms over the
+    compared oracle outputs), the arg-max location and the number of outputs compared."""
+    from concurrent.futures import ThreadPoolExecutor
+    from threadpoolctl import threadpool_limits
+    N, c_z = z.shape[0], z.shape[2]
+    q = params64(p)
+    c = q["w_a"].shape[0]
+    a, b = ab if ab is not None else oracle_projections_whole(z, M, p, eps)
+    if row_blocks is None:
+        row_blocks = [(i0, min(N, i0 + block_rows)) for i0 in range(0, N, block_rows)]
+
+    def work(blk):
+        i0, i1 = blk
+        ref = orc.trimul_rowblock(a, b, np64(z[i0:i1]), None if M is None else np64(M[i0:i1]), q,
+                                  direction, i0, i1, eps=eps, mask_output=mask_output)
+        got = np64(out[i0:i1])
+        d = np.abs(got - ref)
+        k = int(np.argmax(d))
+        return (float((d * d).sum()), float((ref * ref).sum()), float(d.flat[k]),
+                tuple(int(v) for v in np.unravel_index(k, d.shape)), i0, ref.size,
+                bool(np.all(np.isfinite(got))))
+
+    workers = _host_workers(block_rows * N * max(c, c_z) * 8 * 12)
+    with threadpool_limits(limits=1):
+        with ThreadPoolExecutor(workers) as ex:
+            res = list(ex.map(work, row_blocks))
+    sd = sum(r[0] for r in res)
+    sr = sum(r[1] for r in res)
+    n = sum(r[5] for r in res)
+    worst = max(res, key=lambda r: r[2])
+    rms = (sr / n) ** 0.5
+    return dict(rel_fro=(sd / max(sr, 1e-300)) ** 0.5, max_over_rms=worst[2] / max(rms, 1e-300),
+                rms=rms, max_abs=worst[2], argmax=[worst[4] + worst[3][0], worst[3][1], worst[3][2]],
+                outputs=n, finite=all(r[6] for r in res), host_workers=workers)

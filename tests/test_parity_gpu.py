@@ -209,12 +209,12 @@ def run_subgrid(cfg, direction, n_idx, seed):
 
 @pytest.mark.parametrize("direction", [OUT, INC])
 def test_config2_bf16_n2048_chains(direction):
-    run_subgrid(synth.CONFIGS[2], direction, 48, 11)
+    run_subgrid(synth.CONFIGS[2], direction, 128, 11)
 
 
 @pytest.mark.parametrize("direction", [OUT, INC])
 def test_config3_bf16_n4096_headline(direction):
-    run_subgrid(synth.CONFIGS[3], direction, 64, 12)
+    run_subgrid(synth.CONFIGS[3], direction, 128, 12)
 
 
 @pytest.mark.parametrize("direction", [OUT, INC])
@@ -222,7 +222,7 @@ def test_config4_bf16_n8192_single_call(direction):
     free, _ = torch.cuda.mem_get_info()
     if free < 100 * 2 ** 30:
         pytest.skip("needs ~85 GiB of free HBM")
-    run_subgrid(synth.CONFIGS[4], direction, 48, 13)
+    run_subgrid(synth.CONFIGS[4], direction, 128, 13)
     torch.cuda.empty_cache()
 
 

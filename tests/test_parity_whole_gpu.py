@@ -1,0 +1,242 @@
+"""Whole-tensor parity at the headline size and the large-N GPU-vs-GPU invariants (SURVEY 8(c)
+"Full vs sub-grid").  The max-abs criterion (5e-2 * rms) grows with the number of
+outputs compared, so a sub-grid cannot stand in for the whole tensor:
+
+  * N = 4096, both directions: EVERY output against the fp64 oracle, walked in row blocks
+    (orc.projections + orc.trimul_rowblock), errors and arg-max recorded;
+  * N = 4096 / 8192: every output against the library's own fp32 exact mode (itself held to 1e-5
+    against the oracle), as far as HBM allows;
+  * N = 8192: the oracle over 1/8 of the rows, spread over every 256-row tile row;
+  * whole-tensor I1 (direction identity with the a/b swap), I2 (token permutation, and the chain
+    permutation of config 2) and I3 (garbage under the mask, bitwise) on the device.
+Slow tests are marked `slow` but stay collected.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import parity_util as U
+from paper_2603_14806_b200 import binding as B
+from paper_2603_14806_b200 import synth
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+DEV = "cuda"
+OUT, INC = B.OUTGOING, B.INCOMING
+DIRNAME = {OUT: "outgoing", INC: "incoming"}
+
+
+def to_dev(p):
+    return {k: v.to(DEV) for k, v in p.items()}
+
+
+def device_inputs(cfg, direction, mask_kind=None):
+    N = cfg.N
+    z = synth.make_z(cfg.seed, N, cfg.c_z, cfg.dtype, DEV)
+    m = synth.make_token_mask(mask_kind or cfg.mask_kind, N, cfg.seed)
+    M = synth.pair_mask(m, cfg.dtype, DEV)
+    p = to_dev(synth.make_params(cfg.seed * 2 + direction, cfg.c_z, cfg.c_hidden, cfg.dtype))
+    return z, m, M, p
+
+
+def device_errors(got, ref, chunk=256):
+    """rel-F and max-abs / rms between two device tensors [N, N, c] (fp64 accumulation, chunked)."""
+    sd = torch.zeros((), dtype=torch.float64, device=got.device)
+    sr = torch.zeros_like(sd)
+    mx = torch.zeros_like(sd)
+    for r0 in range(0, got.shape[0], chunk):
+        g = got[r0:r0 + chunk].double()
+        r = ref[r0:r0 + chunk].double()
+        d = (g - r).abs()
+        sd += (d * d).sum()
+        sr += (r * r).sum()
+        mx = torch.maximum(mx, d.max())
+    n = ref.numel()
+    rms = float((sr / n).sqrt())
+    return dict(rel_fro=float((sd / sr).sqrt()), max_over_rms=float(mx) / rms, rms=rms, outputs=n)
+
+
+# ---------------------------------------------------------------- N = 4096, whole tensor vs the oracle
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_n4096_whole_tensor_against_oracle(direction):
+    cfg = synth.CONFIGS[3]
+    z, m, M, p = device_inputs(cfg, direction)
+    out = B.trimul(z, M, p, direction)
+    torch.cuda.synchronize()
+    e = U.whole_tensor_errors(out, z, M, p, direction)
+    U.record_parity(f"cfg3 N=4096 {DIRNAME[direction]} WHOLE tensor vs fp64 oracle (row blocks)", e, "bf16",
+                    N=cfg.N, config=3, direction=DIRNAME[direction], reference="fp64 oracle", scope="whole tensor")
+    assert e["finite"] and e["outputs"] == cfg.N * cfg.N * cfg.c_z
+    assert e["rel_fro"] <= U.TOL["bf16"]["rel_fro"]
+    assert e["max_over_rms"] <= U.TOL["bf16"]["max_over_rms"]
+
+
+# ---------------------------------------------------------------- whole tensor vs the fp32 exact mode
+def fp32_mode_reference(z, M, p, direction):
+    """The library's FOLDCP_F32 mode on the same values (bf16 -> fp32 is exact)."""
+    p32 = {k: v.float() for k, v in p.items()}
+    return B.trimul(z.float(), None if M is None else M.float(), p32, direction)
+
+
+@pytest.mark.parametrize("cfg_i", [2, 3])
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_whole_tensor_against_fp32_mode(cfg_i, direction):
+    cfg = synth.CONFIGS[cfg_i]
+    z, m, M, p = device_inputs(cfg, direction)
+    out = B.trimul(z, M, p, direction)
+    ref = fp32_mode_reference(z, M, p, direction)
+    torch.cuda.synchronize()
+    e = device_errors(out, ref)
+    U.record_parity(f"cfg{cfg_i} N={cfg.N} {DIRNAME[direction]} WHOLE tensor vs fp32 exact mode", e, "bf16",
+                    N=cfg.N, config=cfg_i, direction=DIRNAME[direction], reference="library fp32 mode (<=1e-5 vs oracle)",
+                    scope="whole tensor")
+    assert e["rel_fro"] <= U.TOL["bf16"]["rel_fro"] and e["max_over_rms"] <= U.TOL["bf16"]["max_over_rms"]
+    # and the fp32 mode itself against the oracle on a 128 x 128 sub-grid of the same problem
+    I = U.sample_indices(cfg.N, 128, 21, tile=256)
+    J = U.sample_indices(cfg.N, 128, 22, tile=256)
+    sub = U.oracle_subgrid(z, M, p, direction, I, J)
+    It, Jt = torch.as_tensor(I, device=DEV), torch.as_tensor(J, device=DEV)
+    e32 = U.errors(U.np64(ref[It][:, Jt]), sub)
+    U.record_parity(f"cfg{cfg_i} N={cfg.N} {DIRNAME[direction]} fp32 mode vs oracle (sub-grid 128^2)", e32, "f32",
+                    N=cfg.N, config=cfg_i, direction=DIRNAME[direction], reference="fp64 oracle", scope="sub-grid 128x128")
+    assert e32["rel_fro"] <= 1e-5
+
+
+# ---------------------------------------------------------------- N = 8192: 1/8 of the rows vs the oracle
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_n8192_eighth_of_rows_against_oracle(direction):
+    """Config 4 (N = 8192, 5 % of tokens masked): 32 rows out of every 256-row tile row (1024 rows,
+    1/8 of the tensor = 1.07e9 outputs) against the fp64 oracle.  The oracle's a (needed rows /
+    columns only) and b are evaluated in fp64 column block by column block through trimul_subgrid."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 100 * 2 ** 30:
+        pytest.skip("needs ~85 GiB of free HBM")
+    import psutil
+    if psutil.virtual_memory().available < 60 * 2 ** 30:
+        pytest.skip("needs ~60 GB of host memory for the fp64 oracle blocks")
+    cfg = synth.CONFIGS[4]
+    N = cfg.N
+    z, m, M, p = device_inputs(cfg, direction)
+    out = B.trimul(z, M, p, direction)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(8192 + direction)
+    rows = np.sort(np.concatenate([t0 + rng.choice(256, size=32, replace=False) for t0 in range(0, N, 256)]))
+    e = subgrid_walk(out, z, M, p, direction, rows, N)
+    U.record_parity(f"cfg4 N=8192 {DIRNAME[direction]} 1/8 of the rows (32 per 256-row tile row) vs fp64 oracle", e,
+                    "bf16", N=N, config=4, direction=DIRNAME[direction], reference="fp64 oracle",
+                    scope="1024 of 8192 rows, all columns")
+    assert e["outputs"] == rows.size * N * cfg.c_z
+    assert e["rel_fro"] <= U.TOL["bf16"]["rel_fro"] and e["max_over_rms"] <= U.TOL["bf16"]["max_over_rms"]
+    del out, z, M
+    torch.cuda.empty_cache()
+
+
+def subgrid_walk(out, z, M, p, direction, rows, N, row_group=64, col_block=512):
+    """Exact out[rows, :] through orc.trimul_subgrid, (row group) x (column block) at a time, on host
+    threads; accumulates the same error sums as whole_tensor_errors."""
+    from concurrent.futures import ThreadPoolExecutor
+    from threadpoolctl import threadpool_limits
+    jobs = [(rows[g:g + row_group], np.arange(j0, min(N, j0 + col_block)))
+            for g in range(0, rows.size, row_group) for j0 in range(0, N, col_block)]
+
+    def work(job):
+        I, J = job
+        ref = U.oracle_subgrid(z, M, p, direction, I, J)
+        It, Jt = torch.as_tensor(I, device=out.device), torch.as_tensor(J, device=out.device)
+        got = U.np64(out[It][:, Jt])
+        d = np.abs(got - ref)
+        k = int(np.argmax(d))
+        loc = np.unravel_index(k, d.shape)
+        return (float((d * d).sum()), float((ref * ref).sum()), float(d.flat[k]),
+                [int(I[loc[0]]), int(J[loc[1]]), int(loc[2])], ref.size)
+
+    workers = U._host_workers((row_group + col_block) * N * 128 * 8 * 10)
+    with threadpool_limits(limits=1):
+        with ThreadPoolExecutor(workers) as ex:
+            res = list(ex.map(work, jobs))
+    sd, sr, n = sum(r[0] for r in res), sum(r[1] for r in res), sum(r[4] for r in res)
+    worst = max(res, key=lambda r: r[2])
+    rms = (sr / n) ** 0.5
+    return dict(rel_fro=(sd / sr) ** 0.5, max_over_rms=worst[2] / rms, rms=rms, max_abs=worst[2],
+                argmax=worst[3], outputs=n, host_workers=workers)
+
+
+# ---------------------------------------------------------------- large-N GPU-vs-GPU invariants (whole tensor)
+def swap_ab(p):
+    sw = dict(p)
+    for x, y in (("w_a", "w_b"), ("w_a_gate", "w_b_gate"), ("b_a", "b_b"), ("b_a_gate", "b_b_gate")):
+        sw[x], sw[y] = p[y], p[x]
+    return sw
+
+
+def test_n4096_I1_direction_identity_whole_tensor():
+    """incoming(z, M; theta) = T(outgoing(Tz, TM; theta with the a / b sets swapped)) -- reading A10."""
+    cfg = synth.CONFIGS[3]
+    z, m, M, p = device_inputs(cfg, INC, mask_kind="scatter")
+    inc = B.trimul(z, M, p, INC)
+    zt = z.transpose(0, 1).contiguous()
+    out_t = B.trimul(zt, M.t().contiguous(), swap_ab(p), OUT)
+    torch.cuda.synchronize()
+    del zt
+    e = device_errors(out_t.transpose(0, 1), inc)
+    U.record_parity("cfg3-shape N=4096 I1 (incoming vs transposed outgoing, a/b swapped), whole tensor, GPU vs GPU",
+                    e, "bf16", N=cfg.N, reference="GPU (other direction)", scope="whole tensor")
+    # two independent bf16 pipelines: within 2x the parity tolerance (SURVEY 8(c) last pin row)
+    assert e["rel_fro"] <= 2e-2 and e["max_over_rms"] <= 1e-1
+
+
+def test_n4096_I2_token_permutation_whole_tensor():
+    cfg = synth.CONFIGS[3]
+    z, m, M, p = device_inputs(cfg, OUT, mask_kind="scatter")
+    pi = torch.randperm(cfg.N, generator=torch.Generator().manual_seed(5)).to(DEV)
+    rhs = B.trimul(z, M, p, OUT)
+    zp = z[pi][:, pi].contiguous()
+    Mp = M[pi][:, pi].contiguous()
+    lhs = B.trimul(zp, Mp, p, OUT)
+    torch.cuda.synchronize()
+    del zp
+    rhs_p = rhs[pi][:, pi]
+    e = device_errors(lhs, rhs_p)
+    U.record_parity("cfg3-shape N=4096 I2 (token permutation equivariance), whole tensor, GPU vs GPU", e, "bf16",
+                    N=cfg.N, reference="GPU (permuted)", scope="whole tensor")
+    assert e["rel_fro"] <= 2e-2 and e["max_over_rms"] <= 1e-1
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_n4096_I3_masked_garbage_bitwise_whole_tensor(direction):
+    cfg = synth.CONFIGS[3]
+    z, m, M, p = device_inputs(cfg, direction, mask_kind="scatter")
+    o1 = B.trimul(z, M, p, direction)
+    dead_tok = torch.nonzero(m == 0).flatten().to(DEV)
+    g = torch.Generator(device=DEV).manual_seed(9)
+    z2 = z.clone()
+    z2[dead_tok] = (100.0 * torch.randn(dead_tok.numel(), cfg.N, cfg.c_z, generator=g, device=DEV)).to(z.dtype)
+    z2[:, dead_tok] = (100.0 * torch.randn(cfg.N, dead_tok.numel(), cfg.c_z, generator=g, device=DEV)).to(z.dtype)
+    o2 = B.trimul(z2, M, p, direction)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, o2)
+    assert torch.count_nonzero(o1[dead_tok]) == 0 and torch.count_nonzero(o1[:, dead_tok]) == 0
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_config2_chain_permutation_I2(direction):
+    """Config 2: four chains laid out contiguously, then padding.  Re-ordering the chains is a token
+    permutation that keeps the padding at the end: the update must follow the permutation."""
+    cfg = synth.CONFIGS[2]
+    z, m, M, p = device_inputs(cfg, direction)
+    lens = synth.chain_lengths(cfg.N, cfg.seed)
+    assert len(lens) == 4 and sum(lens) == int(m.sum()) == 1900
+    starts = np.concatenate([[0], np.cumsum(lens)])
+    order = [2, 0, 3, 1]
+    pi = np.concatenate([np.arange(starts[c], starts[c + 1]) for c in order] + [np.arange(sum(lens), cfg.N)])
+    pi = torch.as_tensor(pi, device=DEV)
+    assert torch.equal(M[pi][:, pi], M)                 # padding stays where it was
+    rhs = B.trimul(z, M, p, direction)
+    lhs = B.trimul(z[pi][:, pi].contiguous(), M, p, direction)
+    torch.cuda.synchronize()
+    e = device_errors(lhs, rhs[pi][:, pi])
+    U.record_parity(f"cfg2 N=2048 {DIRNAME[direction]} chain-permutation I2, whole tensor, GPU vs GPU", e, "bf16",
+                    N=cfg.N, config=2, direction=DIRNAME[direction], reference="GPU (chains re-ordered)",
+                    scope="whole tensor")
+    assert e["rel_fro"] <= 2e-2 and e["max_over_rms"] <= 1e-1
