@@ -243,9 +243,11 @@ def run_ours(args):
     value = whole_job_tflops(flops_step, ms_per_step, world)
 
     # ---- per-stage durations inside a timed region (stage entry points, same kernels, same stream)
-    a = ws[: ws.numel() // 3].view(torch.bfloat16).view(C, N, N)
-    b = ws[ws.numel() // 3: 2 * (ws.numel() // 3)].view(torch.bfloat16).view(C, N, N)
-    o = ws[2 * (ws.numel() // 3):].view(torch.bfloat16).view(C, N, N)
+    tb = C * N * N * 2
+    a = ws[:tb].view(torch.bfloat16).view(C, N, N)
+    b = ws[tb: 2 * tb].view(torch.bfloat16).view(C, N, N)
+    o = ws[2 * tb: 3 * tb].view(torch.bfloat16).view(C, N, N)
+    scratch = B.stage_scratch(dev)
     import ctypes
     lib = B.load()
     stream = torch.cuda.current_stream().cuda_stream
@@ -257,10 +259,10 @@ def run_ours(args):
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
             ev[0].record()
             st = lib.foldcp_trimul_project(z.data_ptr(), M.data_ptr(), ctypes.byref(prm), N, C, C,
-                                           a.data_ptr(), b.data_ptr(), stream)
+                                           a.data_ptr(), b.data_ptr(), scratch.data_ptr(), stream)
             ev[1].record()
             st |= lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, C, B.BF16, d,
-                                             o.data_ptr(), stream)
+                                             o.data_ptr(), scratch.data_ptr(), stream)
             ev[2].record()
             st |= lib.foldcp_trimul_finalize(o.data_ptr(), z.data_ptr(), M.data_ptr(),
                                              ctypes.byref(prm), N, C, C, outs[d].data_ptr(), stream)

@@ -21,9 +21,28 @@
  * Memory: every tensor pointer below is a DEVICE pointer owned by the caller and must stay valid
  * until the work enqueued on `stream` has finished.  The params struct itself is HOST memory and
  * is only read during the call.  The library never allocates, frees or synchronises inside
- * foldcp_trimul(): it enqueues kernels on `stream` and returns.  Same inputs give bitwise
- * identical outputs (no atomics, no split-K).  No exceptions cross this boundary; every failure
- * is a status code and, when detected on the host, leaves `out` untouched.
+ * foldcp_trimul(): it enqueues kernels (and one 256-byte memset node) on `stream` and returns.
+ *
+ * Determinism: same inputs give bitwise identical outputs.  The persistent kernels hand tiles to
+ * their CTAs through an atomic counter, but every tile is computed the same way whichever CTA gets
+ * it, there is no split-K and no floating-point atomic: the schedule varies, the result does not.
+ *
+ * Concurrency: the library keeps no device-side global state.  The tile counters of a call live
+ * in the last FOLDCP_SCHED_SCRATCH_BYTES of its workspace (or in the `scratch` argument of the
+ * stage entry points) and are zeroed on `stream` ahead of the kernels, so any number of calls may
+ * be in flight on any number of streams / host threads as long as calls that may overlap in time
+ * use different workspaces, scratch areas and outputs.  Calls may be captured into CUDA graphs;
+ * a graph replay must not overlap another use of the same workspace.
+ *
+ * Numeric preconditions of the bf16 mode (FOLDCP_BF16; the fp32 mode has none beyond finiteness):
+ *   - inputs finite; |z| below ~1e18 so that the fp32 LayerNorm variance does not overflow (the
+ *     fp64 oracle has no such limit; bf16 z in any realistic range is far inside);
+ *   - the LayerNorm outputs and the gamma-folded weights W diag(gamma) are held on chip as fp16
+ *     operand tiles (11-bit significand instead of bf16's 8): |gamma_k * W[r][k]| must be
+ *     <= 65504 (larger values saturate to +-65504) and values below 2^-14 in magnitude are stored
+ *     as fp16 subnormals (absolute error <= 2^-25).  tests/test_behaviour_gpu.py shows both edges.
+ * No exceptions cross this boundary; every failure is a status code and, when detected on the
+ * host, leaves `out` untouched.
  */
 #ifndef FOLDCP_TRIMUL_H_
 #define FOLDCP_TRIMUL_H_
@@ -41,8 +60,8 @@ typedef enum {
   FOLDCP_ERR_UNSUPPORTED = 2, /* c_z or c_hidden != 128; bf16 mode with N not a multiple of 8      */
   FOLDCP_ERR_ALIGNMENT = 3,   /* a tensor pointer is not 16-byte aligned                           */
   FOLDCP_ERR_WORKSPACE = 4,   /* workspace NULL or smaller than foldcp_trimul_workspace_bytes()    */
-  FOLDCP_ERR_ALIAS = 5,       /* out overlaps z or the workspace                                   */
-  FOLDCP_ERR_ARCH = 6,        /* current device is not compute capability 10.x (sm_100)           */
+  FOLDCP_ERR_ALIAS = 5,       /* an output overlaps an input, another output or the workspace     */
+  FOLDCP_ERR_ARCH = 6,        /* current device is not compute capability 10.0 (sm_100a cubin)    */
   FOLDCP_ERR_CUDA = 7         /* launch / tensor-map failure (cudaGetLastError is preserved)       */
 } foldcp_status_t;
 
@@ -109,8 +128,13 @@ int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_p
                           int batch, int N, int c_z, int c_hidden, int direction, void* out,
                           void* stream);
 
-/* Bytes of device scratch foldcp_trimul needs for this problem (a, b and o, channel-major);
- * 0 if the shape / dtype is unsupported.  Monotone in N. */
+/* Bytes of the tile-counter area: the tail of the workspace, and the size of the `scratch`
+ * argument of the stage entry points. */
+#define FOLDCP_SCHED_SCRATCH_BYTES 256
+
+/* Bytes of device scratch foldcp_trimul needs for this problem (a, b and o, channel-major, plus
+ * FOLDCP_SCHED_SCRATCH_BYTES of tile counters); 0 if the shape / dtype is unsupported.
+ * Monotone in N. */
 size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
 
 /* Stage-level entry points (same conventions; used by the tests, the benchmark's per-kernel
@@ -121,11 +145,18 @@ size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
  *   foldcp_trimul_contract: step a4 -- Eq. 2 / Eq. 3 per channel
  *        o     [c_hidden][N][N]  channel-major, dtype
  *   foldcp_trimul_finalize: step a3+a5 -- LayerNorm(o) + output projection + sigmoid gate + mask
+ *
+ *   scratch: FOLDCP_SCHED_SCRATCH_BYTES of caller-owned device memory, 16-byte aligned, contents
+ *        arbitrary (the call zeroes it on `stream`); must not be shared by calls that may overlap
+ *        in time.  Required in bf16 mode (FOLDCP_ERR_WORKSPACE if NULL), ignored in fp32 mode.
+ *   Outputs must not overlap inputs or each other (FOLDCP_ERR_ALIAS): the kernels are persistent
+ *   and store tiles while later tiles still read the operands.
  */
 int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_params* params,
-                          int N, int c_z, int c_hidden, void* a, void* b, void* stream);
+                          int N, int c_z, int c_hidden, void* a, void* b, void* scratch,
+                          void* stream);
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
-                           int direction, void* o, void* stream);
+                           int direction, void* o, void* scratch, void* stream);
 /*
  * Backward of step a4 (the O(N^3) part of training; the paper hand-writes
  * every backward with the forward's algorithm).  Given d_o = dL/do:
@@ -136,7 +167,7 @@ int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, in
  */
 int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* b, int N,
                                     int c_hidden, int dtype, int direction, void* d_a, void* d_b,
-                                    void* stream);
+                                    void* scratch, void* stream);
 int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
                            const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
                            void* out, void* stream);
@@ -146,7 +177,9 @@ int foldcp_trimul_launches_per_call(int dtype);
 
 const char* foldcp_status_string(int status);
 /* major * 100 + minor * 10; 110 added params->add_residual, foldcp_trimul_batched and
- * foldcp_trimul_contract_backward (the params struct grew: struct_size guards mismatches). */
+ * foldcp_trimul_contract_backward (the params struct grew: struct_size guards mismatches);
+ * 120 made the tile counters per call (workspace grew by FOLDCP_SCHED_SCRATCH_BYTES, the stage
+ * entry points take `scratch`). */
 int foldcp_version(void);
 
 #ifdef __cplusplus

@@ -230,6 +230,99 @@ def trimul_rowblock(a: np.ndarray, b: np.ndarray, z_rows: np.ndarray,
     return output_stage(o, zp, mask_rows, p, eps, mask_output)
 
 
+# ------------------------------------------------------------------------------------------------
+# Backward pass.  PAPER.md lines 92-96 (section 3.1): every Fold-CP module
+# hand-writes its forward AND backward with the same algorithm.  The functions below are the chain
+# rule applied to the definition above, one forward line at a time in reverse order; nothing is
+# fused or reordered.  Pins (tests/test_oracle_pins.py): central finite differences of `trimul` for
+# every input and parameter, the adjoint identity <d_out, J u> = <J^T d_out, u>, and a scalar-loop
+# Jacobian for the LayerNorm backward.
+# ------------------------------------------------------------------------------------------------
+def layer_norm_backward(d_y: np.ndarray, x: np.ndarray, gamma: np.ndarray, eps: float):
+    """Backward of y = (x - mean) / sqrt(var + eps) * gamma + beta over the last axis (biased var).
+    With xh = (x - mean) / sqrt(var + eps) and d_xh = d_y * gamma:
+        d_x     = (d_xh - mean(d_xh) - xh * mean(d_xh * xh)) / sqrt(var + eps)
+        d_gamma = sum over rows of d_y * xh        d_beta = sum over rows of d_y
+    Returns (d_x, d_gamma, d_beta)."""
+    x = np.asarray(x, _F)
+    d_y = np.asarray(d_y, _F)
+    mu = x.mean(axis=-1, keepdims=True)
+    var = ((x - mu) ** 2).mean(axis=-1, keepdims=True)
+    rstd = 1.0 / np.sqrt(var + eps)
+    xh = (x - mu) * rstd
+    d_xh = d_y * np.asarray(gamma, _F)
+    d_x = (d_xh - d_xh.mean(axis=-1, keepdims=True)
+           - xh * (d_xh * xh).mean(axis=-1, keepdims=True)) * rstd
+    lead = tuple(range(x.ndim - 1))
+    return d_x, (d_y * xh).sum(axis=lead), d_y.sum(axis=lead)
+
+
+def _linear_backward(d_y: np.ndarray, x: np.ndarray, w: np.ndarray):
+    """Backward of y = x W^T + b:  d_x = d_y W,  d_W = d_y^T x,  d_b = sum of d_y (rows flattened)."""
+    d2 = np.asarray(d_y, _F).reshape(-1, d_y.shape[-1])
+    x2 = np.asarray(x, _F).reshape(-1, x.shape[-1])
+    d_x = (d2 @ np.asarray(w, _F)).reshape(x.shape)
+    return d_x, d2.T @ x2, d2.sum(axis=0)
+
+
+def trimul_backward(d_out: np.ndarray, z: np.ndarray, mask: Optional[np.ndarray],
+                    p: Dict[str, np.ndarray], direction: int, eps: float = 1e-5,
+                    mask_output: bool = True, residual: bool = False):
+    """Gradients of L = <d_out, trimul(z)> (or of the residual form z + trimul(z)).
+
+    Returns (d_z [N, N, c_z], grads) where grads maps every parameter name of `p` (the six weight
+    matrices, the biases that are present, both LayerNorm gammas and betas) to its gradient.
+    The forward intermediates are recomputed here exactly as `trimul` computes them."""
+    z = np.asarray(z, _F)
+    d_out = np.asarray(d_out, _F)
+    Mf = None if mask is None else np.asarray(mask, _F)[..., None]
+    # ---- forward, keeping the intermediates
+    zp = layer_norm(z, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    pa, ga = _linear(zp, p["w_a"], p.get("b_a")), _linear(zp, p["w_a_gate"], p.get("b_a_gate"))
+    pb, gb = _linear(zp, p["w_b"], p.get("b_b")), _linear(zp, p["w_b_gate"], p.get("b_b_gate"))
+    sa, sb = sigmoid(ga), sigmoid(gb)
+    a, b = sa * pa, sb * pb
+    if Mf is not None:
+        a, b = Mf * a, Mf * b
+    g = sigmoid(_linear(zp, p["w_g"], p.get("b_g")))
+    o = contraction(a, b, direction)
+    on = layer_norm(o, p["ln_out_gamma"], p["ln_out_beta"], eps)
+    y = _linear(on, p["w_o"], p.get("b_o"))
+    # ---- out = [M] g y
+    d_gy = d_out if (Mf is None or not mask_output) else d_out * Mf
+    d_y = d_gy * g
+    d_gg = d_gy * y * g * (1.0 - g)                       # through g = sigmoid(gg)
+    grads: Dict[str, np.ndarray] = {}
+    d_on, grads["w_o"], db = _linear_backward(d_y, on, p["w_o"])
+    if p.get("b_o") is not None:
+        grads["b_o"] = db
+    d_o, grads["ln_out_gamma"], grads["ln_out_beta"] = layer_norm_backward(d_on, o, p["ln_out_gamma"], eps)
+    # ---- Eq. 2-3
+    d_a, d_b = contraction_backward(d_o, a, b, direction)
+    if Mf is not None:
+        d_a, d_b = d_a * Mf, d_b * Mf
+    # ---- a = M sigmoid(ga) pa, b likewise
+    d_zp, grads["w_g"], db = _linear_backward(d_gg, zp, p["w_g"])
+    if p.get("b_g") is not None:
+        grads["b_g"] = db
+    for d_t, s_t, p_t, wn, bn, gwn, gbn in ((d_a, sa, pa, "w_a", "b_a", "w_a_gate", "b_a_gate"),
+                                            (d_b, sb, pb, "w_b", "b_b", "w_b_gate", "b_b_gate")):
+        d_p = d_t * s_t
+        d_gate = d_t * p_t * s_t * (1.0 - s_t)
+        dx, grads[wn], db = _linear_backward(d_p, zp, p[wn])
+        if p.get(bn) is not None:
+            grads[bn] = db
+        d_zp = d_zp + dx
+        dx, grads[gwn], db = _linear_backward(d_gate, zp, p[gwn])
+        if p.get(gbn) is not None:
+            grads[gbn] = db
+        d_zp = d_zp + dx
+    d_z, grads["ln_in_gamma"], grads["ln_in_beta"] = layer_norm_backward(d_zp, z, p["ln_in_gamma"], eps)
+    if residual:
+        d_z = d_z + d_out
+    return d_z, grads
+
+
 def flops(N: int, c_z: int, c_hidden: int) -> float:
     """Counted FLOPs of one call: contraction 2 c N^3 + five
     projections 2 N^2 c_z (4c + c_z) + output projection 2 N^2 c c_z."""

@@ -73,11 +73,11 @@ def load() -> ctypes.CDLL:
     lib.foldcp_trimul_workspace_bytes.restype = ctypes.c_size_t
     lib.foldcp_trimul_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.foldcp_trimul_project.restype = ci
-    lib.foldcp_trimul_project.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp, vp]
+    lib.foldcp_trimul_project.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp, vp, vp]
     lib.foldcp_trimul_contract_backward.restype = ci
-    lib.foldcp_trimul_contract_backward.argtypes = [vp, vp, vp, ci, ci, ci, ci, vp, vp, vp]
+    lib.foldcp_trimul_contract_backward.argtypes = [vp, vp, vp, ci, ci, ci, ci, vp, vp, vp, vp]
     lib.foldcp_trimul_contract.restype = ci
-    lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp, vp]
     lib.foldcp_trimul_finalize.restype = ci
     lib.foldcp_trimul_finalize.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp]
     lib.foldcp_trimul_launches_per_call.restype = ci
@@ -118,6 +118,41 @@ def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
     return None if t is None else t.data_ptr()
 
 
+SCHED_SCRATCH_BYTES = 256      # FOLDCP_SCHED_SCRATCH_BYTES
+
+
+def stage_scratch(device) -> torch.Tensor:
+    """The `scratch` argument of the stage entry points: tile counters of one call (the library
+    zeroes it on the stream).  Allocated per call on the current stream: torch's caching allocator
+    only hands the block out again to work ordered after this call on the same stream."""
+    return torch.empty(SCHED_SCRATCH_BYTES, dtype=torch.uint8, device=device)
+
+
+_MATRICES = ("w_a", "w_a_gate", "w_b", "w_b_gate", "w_g", "w_o")
+
+
+def _check_tensors(z: torch.Tensor, p: Dict[str, Optional[torch.Tensor]], others=()) -> None:
+    """The C ABI sees raw pointers: dtype / device / contiguity mismatches would be silent garbage,
+    so they are rejected here.  The library launches on the CURRENT device and stream."""
+    if not z.is_cuda:
+        raise ValueError("tensors must be CUDA tensors (no CPU fallback)")
+    if z.device.index != torch.cuda.current_device():
+        raise ValueError(f"z is on {z.device} but the current CUDA device is "
+                         f"cuda:{torch.cuda.current_device()} (use torch.cuda.device(...))")
+    for name, t in list(p.items()) + [(f"arg{i}", t) for i, t in enumerate(others)]:
+        if t is None:
+            continue
+        if t.device != z.device:
+            raise ValueError(f"{name} is on {t.device}, z on {z.device}")
+        if not t.is_contiguous():
+            raise ValueError(f"{name} must be contiguous")
+        if name in _MATRICES:
+            if t.dtype != z.dtype:
+                raise TypeError(f"{name} has dtype {t.dtype}; weight matrices must match z ({z.dtype})")
+        elif name in p and t.dtype != torch.float32:
+            raise TypeError(f"{name} has dtype {t.dtype}; LayerNorm parameters and biases are float32")
+
+
 def make_params(p: Dict[str, Optional[torch.Tensor]], dtype: int, eps: float = 1e-5,
                 mask_output: bool = True, workspace: Optional[torch.Tensor] = None,
                 residual: bool = False) -> _Params:
@@ -132,10 +167,7 @@ def make_params(p: Dict[str, Optional[torch.Tensor]], dtype: int, eps: float = 1
     for name in ("ln_in_gamma", "ln_in_beta", "w_a", "w_a_gate", "w_b", "w_b_gate", "b_a",
                  "b_a_gate", "b_b", "b_b_gate", "w_g", "b_g", "ln_out_gamma", "ln_out_beta",
                  "w_o", "b_o"):
-        t = p.get(name)
-        if t is not None:
-            assert t.is_contiguous(), name
-        setattr(s, name, _ptr(t))
+        setattr(s, name, _ptr(p.get(name)))
     if workspace is not None:
         s.workspace = workspace.data_ptr()
         s.workspace_bytes = workspace.numel() * workspace.element_size()
@@ -158,8 +190,7 @@ def trimul(z: torch.Tensor, mask: Optional[torch.Tensor], p: Dict[str, torch.Ten
     `workspace` (uint8, >= workspace_bytes(N)) and `out` are allocated here if not given.
     """
     lib = load()
-    if not z.is_cuda:
-        raise ValueError("z must be a CUDA tensor (no CPU fallback)")
+    _check_tensors(z, p, (mask, out, workspace))
     batch = None
     if z.dim() == 4:
         batch = z.shape[0]
@@ -194,11 +225,13 @@ def project(z, mask, p, eps: float = 1e-5):
     lib = load()
     N, c_z = z.shape[0], z.shape[2]
     c_hidden = p["w_a"].shape[0]
+    _check_tensors(z, p, (mask,))
     a = torch.empty(c_hidden, N, N, dtype=z.dtype, device=z.device)
     b = torch.empty_like(a)
     s = make_params(p, dtype_code(z), eps)
     st = lib.foldcp_trimul_project(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
-                                   a.data_ptr(), b.data_ptr(), _stream())
+                                   a.data_ptr(), b.data_ptr(), stage_scratch(z.device).data_ptr(),
+                                   _stream())
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_project")
     return a, b
@@ -211,8 +244,10 @@ def contract(a: torch.Tensor, b: torch.Tensor, direction: int,
     c, N = a.shape[0], a.shape[1]
     if o is None:
         o = torch.empty_like(a)
+    _check_tensors(a, {}, (b, o))
     st = lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, c, dtype_code(a),
-                                    int(direction), o.data_ptr(), _stream())
+                                    int(direction), o.data_ptr(),
+                                    stage_scratch(a.device).data_ptr(), _stream())
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_contract")
     return o
@@ -225,7 +260,8 @@ def contract_backward(d_o: torch.Tensor, a: torch.Tensor, b: torch.Tensor, direc
     d_a, d_b = torch.empty_like(a), torch.empty_like(b)
     st = lib.foldcp_trimul_contract_backward(d_o.data_ptr(), a.data_ptr(), b.data_ptr(), N, c,
                                              dtype_code(a), int(direction), d_a.data_ptr(),
-                                             d_b.data_ptr(), _stream())
+                                             d_b.data_ptr(), stage_scratch(a.device).data_ptr(),
+                                             _stream())
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_contract_backward")
     return d_a, d_b
@@ -239,6 +275,7 @@ def finalize(o, z, mask, p, eps: float = 1e-5, mask_output: bool = True,
     c_hidden = o.shape[0]
     if out is None:
         out = torch.empty_like(z)
+    _check_tensors(z, p, (o, mask, out))
     s = make_params(p, dtype_code(z), eps, mask_output)
     st = lib.foldcp_trimul_finalize(o.data_ptr(), z.data_ptr(), _ptr(mask), ctypes.byref(s), N,
                                     c_z, c_hidden, out.data_ptr(), _stream())

@@ -1,6 +1,10 @@
 """Builds libfoldcp_trimul.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2603_14806_b200.build [--force]
+    python -m paper_2603_14806_b200.build [--force] [-v] [--debug-knobs]
+
+--debug-knobs builds a SEPARATE library, libfoldcp_trimul_dbg.so, with -DFOLDCP_DEBUG_KNOBS: the A/B
+environment knobs of DESIGN.md section 10 exist only there.  The product library reads no
+environment variable.
 """
 from __future__ import annotations
 
@@ -42,7 +46,16 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, debug_knobs: bool = False) -> str:
+    if debug_knobs:
+        out = LIB_PATH.replace(".so", "_dbg.so")
+        cmd = [_nvcc()] + NVCC_FLAGS + ["-DFOLDCP_DEBUG_KNOBS", "-I", INCLUDE, "-o", out]
+        cmd += [os.path.join(CSRC, s) for s in SOURCES]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed building libfoldcp_trimul_dbg.so")
+        return out
     if not force and not needs_build():
         return LIB_PATH
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE, "-o", LIB_PATH]
@@ -59,4 +72,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                debug_knobs="--debug-knobs" in sys.argv))

@@ -5,10 +5,7 @@
 #include <cstring>
 #include <mutex>
 
-#include <atomic>
-
 #include "common.h"
-#include "tile_sched.cuh"
 
 // default implementation of the three bf16 stages: bit0 K1, bit1 K2, bit2 K3 on tcgen05
 #ifndef FOLDCP_DEFAULT_TC_STAGES
@@ -41,19 +38,15 @@ bool get_device_info(DeviceInfo* info) {
 }
 
 // ----------------------------------------------------------------------------- tile scheduler
-// scheduler words {next tile, drained CTAs}; one pair per launch in flight, handed out round robin
-// (a launch leaves its pair zeroed again, see TileRing::drain)
-namespace {
-constexpr int kSchedSlots = 1024;
-__device__ unsigned int g_sched_words[kSchedSlots][2];
-}  // namespace
-
-unsigned int* next_sched_slot() {
-  static std::atomic<unsigned int> ticket{0};
-  unsigned int* base = nullptr;
-  if (cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_sched_words) != cudaSuccess)
-    return nullptr;
-  return base + 2 * (ticket.fetch_add(1) % kSchedSlots);
+// K1 and K2 draw their tiles in index order from an atomic counter (tile_sched.cuh).  The counter
+// is launch-private and stream-ordered: it lives in caller-owned device memory (the tail of the
+// workspace for foldcp_trimul, the `scratch` argument of the stage entry points) and is zeroed
+// with a memset node on the caller's stream ahead of the launches that use it.  No process-global
+// device state: any number of calls may be in flight on any number of streams (each with its own
+// workspace / scratch), and a captured graph carries its own memset.
+int arm_sched_words(void* scratch, cudaStream_t stream) {
+  return cudaMemsetAsync(scratch, 0, kSchedScratchBytes, stream) == cudaSuccess ? FOLDCP_OK
+                                                                               : FOLDCP_ERR_CUDA;
 }
 
 // ----------------------------------------------------------------------------- launch attributes
@@ -95,10 +88,10 @@ static EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-// FOLDCP_TMAP_L2PROMO = 0 / 64 / 128 / 256 (default 256): L2 promotion size of every tensor map
+// L2 promotion size of every tensor map: 256 B (debug knob FOLDCP_TMAP_L2PROMO = 0 / 64 / 128 / 256)
 static CUtensorMapL2promotion l2_promotion() {
   static const CUtensorMapL2promotion v = [] {
-    const char* e = getenv("FOLDCP_TMAP_L2PROMO");
+    const char* e = debug_env("FOLDCP_TMAP_L2PROMO");
     const int n = e ? atoi(e) : 256;
     return n == 0     ? CU_TENSOR_MAP_L2_PROMOTION_NONE
            : n == 64  ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
@@ -177,22 +170,18 @@ int check_params(const foldcp_trimul_params* p) {
 int check_arch() {
   DeviceInfo d;
   if (!get_device_info(&d)) return FOLDCP_ERR_CUDA;
-  return d.cc_major == 10 ? FOLDCP_OK : FOLDCP_ERR_ARCH;
+  return (d.cc_major == 10 && d.cc_minor == 0) ? FOLDCP_OK : FOLDCP_ERR_ARCH;   // sm_100a cubin only
 }
 
-bool force_simt() {
-  static const bool v = [] {
-    const char* e = getenv("FOLDCP_FORCE_SIMT");
-    return e && e[0] == '1';
-  }();
-  return v;
-}
-
-// which implementation runs a bf16 stage: bit0 = K1 tcgen05, bit1 = K2 tcgen05, bit2 = K3 tcgen05
+// Which implementation runs a bf16 stage: bit0 = K1, bit1 = K2, bit2 = K3 on tcgen05.  The shipped
+// library has ONE path per dtype (bf16 -> the tcgen05 kernels, fp32 -> the FFMA kernels); only a
+// -DFOLDCP_DEBUG_KNOBS build can re-route bf16 stages to the FFMA kernels for bring-up A/B runs
+// (FOLDCP_FORCE_SIMT=1, FOLDCP_TC_STAGES=<mask>).
 int bf16_stage_mask() {
   static const int v = [] {
-    if (force_simt()) return 0;
-    const char* e = getenv("FOLDCP_TC_STAGES");
+    const char* f = debug_env("FOLDCP_FORCE_SIMT");
+    if (f && f[0] == '1') return 0;
+    const char* e = debug_env("FOLDCP_TC_STAGES");
     return e ? atoi(e) : FOLDCP_DEFAULT_TC_STAGES;
   }();
   return v;
@@ -207,41 +196,82 @@ extern "C" {
 
 size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype) {
   if (check_shape(N, c_z, c_hidden, dtype) != FOLDCP_OK) return 0;
-  return 3 * static_cast<size_t>(kChannels) * N * N * elem_bytes(dtype);
+  return 3 * static_cast<size_t>(kChannels) * N * N * elem_bytes(dtype) + kSchedScratchBytes;
 }
 
+namespace {
+// scratch of a stage entry point: required in bf16 mode (checked on the host, before anything is
+// enqueued), then zeroed on the stream
+int check_scratch(const void* scratch, int dtype) {
+  if (dtype != FOLDCP_BF16) return FOLDCP_OK;
+  if (!scratch) return FOLDCP_ERR_WORKSPACE;
+  return aligned16(scratch) ? FOLDCP_OK : FOLDCP_ERR_ALIGNMENT;
+}
+int prepare_scratch(void* scratch, int dtype, cudaStream_t s) {
+  return dtype == FOLDCP_BF16 ? arm_sched_words(scratch, s) : FOLDCP_OK;
+}
+}  // namespace
+
+namespace {
+// the stage bodies: arguments already validated, scheduler words already zeroed on the stream
+int project_stage(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
+                  void* a, void* b, void* sched_area, cudaStream_t s) {
+  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 1))
+    return launch_k1_project_bf16(z, mask, params, N, a, b, sched_word(sched_area, 0), s);
+  return launch_simt_project(z, mask, params, N, a, b, s);
+}
+int contract_stage(const void* a, const void* b, int N, int dtype, int direction, void* o,
+                   void* sched_area, int word, cudaStream_t s) {
+  if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
+    return launch_k2_contract_bf16(a, b, o, N, direction, sched_word(sched_area, word), s);
+  return launch_simt_contract(a, b, o, N, dtype, direction, s);
+}
+int finalize_stage(const void* o, const void* z, const void* mask,
+                   const foldcp_trimul_params* params, int N, void* out, cudaStream_t s) {
+  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 4))
+    return launch_k3_finalize_bf16(o, z, mask, params, N, out, s);
+  return launch_simt_finalize(o, z, mask, params, N, out, s);
+}
+}  // namespace
+
 int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_params* params,
-                          int N, int c_z, int c_hidden, void* a, void* b, void* stream) {
+                          int N, int c_z, int c_hidden, void* a, void* b, void* scratch,
+                          void* stream) {
   int st = check_params(params);
   if (st != FOLDCP_OK) return st;
   if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
   if (!z || !a || !b) return FOLDCP_ERR_INVALID_ARG;
   if (!aligned16(z) || !aligned16(a) || !aligned16(b) || (mask && !aligned16(mask)))
     return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
+  if (overlaps(a, bytes, z, bytes) || overlaps(b, bytes, z, bytes) || overlaps(a, bytes, b, bytes))
+    return FOLDCP_ERR_ALIAS;
+  if ((st = check_scratch(scratch, params->dtype)) != FOLDCP_OK) return st;
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 1))
-    return launch_k1_project_bf16(z, mask, params, N, a, b, s);
-  return launch_simt_project(z, mask, params, N, a, b, s);
+  if ((st = prepare_scratch(scratch, params->dtype, s)) != FOLDCP_OK) return st;
+  return project_stage(z, mask, params, N, a, b, scratch, s);
 }
 
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
-                           int direction, void* o, void* stream) {
+                           int direction, void* o, void* scratch, void* stream) {
   int st = check_shape(N, kChannels, c_hidden, dtype);
   if (st != FOLDCP_OK) return st;
   if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
   if (!a || !b || !o) return FOLDCP_ERR_INVALID_ARG;
   if (!aligned16(a) || !aligned16(b) || !aligned16(o)) return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(dtype);
+  if (overlaps(o, bytes, a, bytes) || overlaps(o, bytes, b, bytes)) return FOLDCP_ERR_ALIAS;
+  if ((st = check_scratch(scratch, dtype)) != FOLDCP_OK) return st;
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
-    return launch_k2_contract_bf16(a, b, o, N, direction, s);
-  return launch_simt_contract(a, b, o, N, dtype, direction, s);
+  if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
+  return contract_stage(a, b, N, dtype, direction, o, scratch, 0, s);
 }
 
 int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* b, int N,
                                     int c_hidden, int dtype, int direction, void* d_a, void* d_b,
-                                    void* stream) {
+                                    void* scratch, void* stream) {
   int st = check_shape(N, kChannels, c_hidden, dtype);
   if (st != FOLDCP_OK) return st;
   if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
@@ -253,10 +283,13 @@ int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* 
   for (const void* in : ins)
     if (overlaps(d_a, bytes, in, bytes) || overlaps(d_b, bytes, in, bytes)) return FOLDCP_ERR_ALIAS;
   if (overlaps(d_a, bytes, d_b, bytes)) return FOLDCP_ERR_ALIAS;
+  if ((st = check_scratch(scratch, dtype)) != FOLDCP_OK) return st;
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
   if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
-    return launch_k2_contract_backward_bf16(d_o, a, b, d_a, d_b, N, direction, s);
+    return launch_k2_contract_backward_bf16(d_o, a, b, d_a, d_b, N, direction,
+                                            sched_word(scratch, 0), sched_word(scratch, 1), s);
   return launch_simt_contract_backward(d_o, a, b, d_a, d_b, N, dtype, direction, s);
 }
 
@@ -269,11 +302,10 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
   if (!o || !z || !out) return FOLDCP_ERR_INVALID_ARG;
   if (!aligned16(o) || !aligned16(z) || !aligned16(out) || (mask && !aligned16(mask)))
     return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
+  if (overlaps(out, bytes, z, bytes) || overlaps(out, bytes, o, bytes)) return FOLDCP_ERR_ALIAS;
   if ((st = check_arch()) != FOLDCP_OK) return st;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 4))
-    return launch_k3_finalize_bf16(o, z, mask, params, N, out, s);
-  return launch_simt_finalize(o, z, mask, params, N, out, s);
+  return finalize_stage(o, z, mask, params, N, out, static_cast<cudaStream_t>(stream));
 }
 
 int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
@@ -294,16 +326,18 @@ int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* p
     return FOLDCP_ERR_ALIAS;
   if ((st = check_arch()) != FOLDCP_OK) return st;
 
+  // workspace: a | b | o (channel-major) | tile counters of this call
   uint8_t* ws = static_cast<uint8_t*>(params->workspace);
   void* a = ws;
-  void* b = ws + need / 3;
-  void* o = ws + 2 * (need / 3);
-  if ((st = foldcp_trimul_project(z, mask, params, N, c_z, c_hidden, a, b, stream)) != FOLDCP_OK)
+  void* b = ws + tensor_bytes;
+  void* o = ws + 2 * tensor_bytes;
+  void* sched_area = ws + 3 * tensor_bytes;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (params->dtype == FOLDCP_BF16 && (st = arm_sched_words(sched_area, s)) != FOLDCP_OK) return st;
+  if ((st = project_stage(z, mask, params, N, a, b, sched_area, s)) != FOLDCP_OK) return st;
+  if ((st = contract_stage(a, b, N, params->dtype, direction, o, sched_area, 1, s)) != FOLDCP_OK)
     return st;
-  if ((st = foldcp_trimul_contract(a, b, N, c_hidden, params->dtype, direction, o, stream)) !=
-      FOLDCP_OK)
-    return st;
-  return foldcp_trimul_finalize(o, z, mask, params, N, c_z, c_hidden, out, stream);
+  return finalize_stage(o, z, mask, params, N, out, s);
 }
 
 int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_params* params,
@@ -342,13 +376,13 @@ const char* foldcp_status_string(int status) {
     case FOLDCP_ERR_UNSUPPORTED: return "unsupported shape";
     case FOLDCP_ERR_ALIGNMENT: return "misaligned pointer";
     case FOLDCP_ERR_WORKSPACE: return "workspace missing or too small";
-    case FOLDCP_ERR_ALIAS: return "out overlaps an input or the workspace";
-    case FOLDCP_ERR_ARCH: return "device is not sm_100";
+    case FOLDCP_ERR_ALIAS: return "an output overlaps an input, another output or the workspace";
+    case FOLDCP_ERR_ARCH: return "device is not sm_100 (compute capability 10.0)";
     case FOLDCP_ERR_CUDA: return "CUDA error";
     default: return "unknown status";
   }
 }
 
-int foldcp_version(void) { return 110; }   // 1.1: add_residual, batched, contract_backward
+int foldcp_version(void) { return 120; }   // 1.2: per-call tile counters (workspace tail / stage scratch)
 
 }  // extern "C"

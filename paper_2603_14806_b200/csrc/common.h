@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include "../../include/foldcp_trimul.h"
 
@@ -24,6 +25,27 @@ namespace foldcp {
 constexpr bool kNormFp16 = FOLDCP_NORM_FP16 != 0;
 
 constexpr int kChannels = 128;  // c_z = c_hidden = 128 is the only supported channel count (A13)
+
+// Tile-scheduler counters of one call: 256 bytes of caller-owned device memory (tail of the
+// workspace / `scratch` of the stage entry points), zeroed on the caller's stream by
+// arm_sched_words() ahead of the launches.  Word 0 serves K1 (or the first K2 launch of a stage
+// call), word 16 (byte 64) K2 (or the second launch of contract_backward).
+constexpr size_t kSchedScratchBytes = FOLDCP_SCHED_SCRATCH_BYTES;
+int arm_sched_words(void* scratch, cudaStream_t stream);
+inline unsigned int* sched_word(void* scratch, int which) {
+  return reinterpret_cast<unsigned int*>(static_cast<uint8_t*>(scratch) + 64 * which);
+}
+
+// A/B knobs read from the environment exist only in -DFOLDCP_DEBUG_KNOBS builds (bring-up and
+// measurement); the shipped library reads no environment variable and has one path per dtype.
+inline const char* debug_env(const char* name) {
+#ifdef FOLDCP_DEBUG_KNOBS
+  return getenv(name);
+#else
+  (void)name;
+  return nullptr;
+#endif
+}
 
 struct DeviceInfo {
   int sm_count;
@@ -44,11 +66,13 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
                       int swizzle);
 
 // ----- stage launchers (device pointers; return foldcp_status_t) -----
+// `sched`: zeroed tile-scheduler counter(s) of this launch (see kSchedScratchBytes)
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            cudaStream_t stream);
+                            unsigned int* sched, cudaStream_t stream);
 
 int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void* b, void* d_a,
-                                     void* d_b, int N, int direction, cudaStream_t stream);
+                                     void* d_b, int N, int direction, unsigned int* sched0,
+                                     unsigned int* sched1, cudaStream_t stream);
 
 int launch_simt_project(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
                         void* a, void* b, cudaStream_t stream);
@@ -60,7 +84,7 @@ int launch_simt_finalize(const void* o, const void* z, const void* mask,
                          const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
 
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
-                           void* a, void* b, cudaStream_t stream);
+                           void* a, void* b, unsigned int* sched, cudaStream_t stream);
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
                             const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
 

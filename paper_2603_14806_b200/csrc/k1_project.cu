@@ -162,7 +162,6 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::tma_load_2d(dst, &tmap_z, zfull(s), 0, row0);
         ptx::tma_load_2d(dst + kHalfBox, &tmap_z, zfull(s), 64, row0);
       }
-      ring.drain(prm.sched, gridDim.x);
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
@@ -458,7 +457,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
 
 bool k1_tanh_sigmoid() {
   static const bool v = [] {
-    const char* e = getenv("FOLDCP_K1_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
+    const char* e = debug_env("FOLDCP_K1_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
     return !(e && e[0] == 'e');
   }();
   return v;
@@ -467,7 +466,7 @@ bool k1_tanh_sigmoid() {
 }  // namespace
 
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
-                           void* a, void* b, cudaStream_t stream) {
+                           void* a, void* b, unsigned int* sched, cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   const uint64_t R = static_cast<uint64_t>(N) * N;
@@ -501,8 +500,7 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   prm.eps = p->ln_eps;
   prm.R = static_cast<long long>(R);
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
-  prm.sched = next_sched_slot();
-  if (prm.sched == nullptr) return FOLDCP_ERR_CUDA;
+  prm.sched = sched;
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k1_tanh_sigmoid();
   auto kern = tanh_sig ? k1_project_kernel<true> : k1_project_kernel<false>;

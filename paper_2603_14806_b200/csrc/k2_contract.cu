@@ -55,7 +55,7 @@ struct K2Params {
   int num_kb;      // ceil(N / 64)
   int l2_hints;    // 1: evict_last loads / evict_first stores
   int panel_n;     // tile rasterisation: n-tiles per column panel (>= 1)
-  unsigned int* sched;   // [0] next tile index, [1] number of CTA groups that have drained
+  unsigned int* sched;   // next tile index: launch-private, zeroed on the stream before the launch
 };
 
 // Tile rasterisation inside one channel: column panels of `panel_n` n-tiles, m fastest-varying
@@ -107,7 +107,6 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const int lane = threadIdx.x & 31;
   const uint32_t cta_rank = (kCtaGroup == 2) ? ptx::cluster_ctarank() : 0u;
   const bool is_leader = cta_rank == 0;
-  const int num_groups = gridDim.x / kCtaGroup;
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmap_a);
@@ -240,15 +239,6 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
             stage = 0;
             phase ^= 1u;
           }
-        }
-      }
-      if (is_leader) {
-        // the last pair to run dry re-arms the scheduler words for a later launch
-        const unsigned int drained = atomicAdd(prm.sched + 1, 1u);
-        if (drained == static_cast<unsigned int>(num_groups) - 1u) {
-          prm.sched[0] = 0u;
-          prm.sched[1] = 0u;
-          __threadfence();
         }
       }
     }
@@ -408,11 +398,11 @@ int g_k2_cta_group = 2;
 // i.e. d[c][m][n] = sum_k X(m, k) Y(n, k).  The forward contraction uses (0,0) / (1,1); its
 // gradients also need the mixed (0,1) form.
 int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn,
-                        cudaStream_t stream) {
+                        unsigned int* sched, cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   static const int cta_group = [] {
-    const char* e = getenv("FOLDCP_K2_CTA_GROUP");
+    const char* e = debug_env("FOLDCP_K2_CTA_GROUP");
     return (e && e[0] == '1') ? 1 : g_k2_cta_group;
   }();
   const uint64_t n = static_cast<uint64_t>(N);
@@ -433,12 +423,12 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
   prm.num_tiles = kChannels * prm.tiles_m * prm.tiles_n;
   prm.num_kb = (N + kBlockK - 1) / kBlockK;
   static const int l2_hints = [] {
-    const char* e = getenv("FOLDCP_K2_L2_HINTS");
+    const char* e = debug_env("FOLDCP_K2_L2_HINTS");
     return e ? atoi(e) : 0;   // 1: loads evict_last + stores evict_first; 2: stores only
   }();
   prm.l2_hints = l2_hints;
   static const int panel = [] {
-    const char* e = getenv("FOLDCP_K2_PANEL");
+    const char* e = debug_env("FOLDCP_K2_PANEL");
     return e ? atoi(e) : 0;
   }();
   // Default rasterisation (measured with the in-order scheduler): plain row-major while one row
@@ -447,8 +437,7 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
   // narrow B panel (N = 8192: 104 GB instead of 554 GB, 105 instead of 132 ms).
   const int auto_panel = prm.tiles_n <= 16 ? prm.tiles_n : 8;
   prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : auto_panel;
-  prm.sched = next_sched_slot();
-  if (prm.sched == nullptr) return FOLDCP_ERR_CUDA;
+  prm.sched = sched;
   const int sms = dev.sm_count;
   if (cta_group == 2) {
     if (x_mn) return y_mn ? launch_variant<2, true, true>(ta, tb, to, prm, sms, stream)
@@ -463,9 +452,9 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
 }
 
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            cudaStream_t stream) {
+                            unsigned int* sched, cudaStream_t stream) {
   const bool inc = direction == FOLDCP_INCOMING;
-  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, stream);
+  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, sched, stream);
 }
 
 // Gradients of the contraction (oracle/trimul_oracle.py contraction_backward):
@@ -474,14 +463,17 @@ int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int di
 //   incoming: d_a = B dO^T     -> X = B (K-major),  Y = dO (K-major)
 //             d_b = A dO       -> X = A (K-major),  Y = dO (MN-major)
 int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void* b, void* d_a,
-                                     void* d_b, int N, int direction, cudaStream_t stream) {
+                                     void* d_b, int N, int direction, unsigned int* sched0,
+                                     unsigned int* sched1, cudaStream_t stream) {
   int st;
   if (direction == FOLDCP_OUTGOING) {
-    if ((st = launch_k2_gemm_bf16(d_o, b, d_a, N, false, true, stream)) != FOLDCP_OK) return st;
-    return launch_k2_gemm_bf16(d_o, a, d_b, N, true, true, stream);
+    if ((st = launch_k2_gemm_bf16(d_o, b, d_a, N, false, true, sched0, stream)) != FOLDCP_OK)
+      return st;
+    return launch_k2_gemm_bf16(d_o, a, d_b, N, true, true, sched1, stream);
   }
-  if ((st = launch_k2_gemm_bf16(b, d_o, d_a, N, false, false, stream)) != FOLDCP_OK) return st;
-  return launch_k2_gemm_bf16(a, d_o, d_b, N, false, true, stream);
+  if ((st = launch_k2_gemm_bf16(b, d_o, d_a, N, false, false, sched0, stream)) != FOLDCP_OK)
+    return st;
+  return launch_k2_gemm_bf16(a, d_o, d_b, N, false, true, sched1, stream);
 }
 
 }  // namespace foldcp

@@ -448,7 +448,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
 
 bool k3_tanh_sigmoid() {
   static const bool v = [] {
-    const char* e = getenv("FOLDCP_K3_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
+    const char* e = debug_env("FOLDCP_K3_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
     return !(e && e[0] == 'e');
   }();
   return v;

@@ -8,8 +8,8 @@
 // would, but to persistent CTAs -- keeps the window of tiles in flight compact.  Every tile is
 // computed the same way whichever pair gets it, so results stay bitwise reproducible.
 //
-// The scheduler words live in a pool in global memory ({next tile, drained CTA groups} per
-// launch); the last group to run dry re-arms its pair for a later launch (k2_contract.cu).
+// The counter is launch-private: one 32-bit word in caller-owned device memory (workspace tail /
+// stage scratch), zeroed on the caller's stream ahead of the launch (api.cu arm_sched_words).
 // K1's tiles share nothing, but its a / b stores are 128-byte rows 32 MB apart: adjacent tiles fill
 // the same DRAM pages only if they are written at about the same time, and the in-order scheduler
 // (TileRing below) made K1 13-15 % faster.  K3 keeps the static assignment: the same scheduler
@@ -19,9 +19,6 @@
 #include "ptx.cuh"
 
 namespace foldcp {
-
-// host side (api.cu): a pair of zeroed scheduler words for one launch; nullptr on CUDA error
-unsigned int* next_sched_slot();
 
 // Single-CTA flavour: one thread draws tile indices and publishes them in a ring in shared memory;
 // every other role waits on the entry's "full" mbarrier, reads it and releases it on "empty".
@@ -46,14 +43,6 @@ struct TileRing {
     ptx::sts32(slot(s), static_cast<uint32_t>(tile));
     ptx::mbar_arrive(full(s));
     return tile;
-  }
-  __device__ __forceinline__ void drain(unsigned int* sched, unsigned int num_ctas) const {
-    const unsigned int drained = atomicAdd(sched + 1, 1u);
-    if (drained == num_ctas - 1u) {
-      sched[0] = 0u;
-      sched[1] = 0u;
-      __threadfence();
-    }
   }
   __device__ __forceinline__ int consume(int i) const {
     const int s = i % kDepth;

@@ -34,9 +34,9 @@ def test_version_and_strings(lib):
 
 
 def test_workspace_bytes(lib):
-    assert B.workspace_bytes(4096, 128, 128, B.BF16) == 3 * 128 * 4096 * 4096 * 2   # 12 GiB
-    assert B.workspace_bytes(8192, 128, 128, B.BF16) == 48 * 2 ** 30
-    assert B.workspace_bytes(64, 128, 128, B.F32) == 3 * 128 * 64 * 64 * 4
+    assert B.workspace_bytes(4096, 128, 128, B.BF16) == 3 * 128 * 4096 * 4096 * 2 + 256   # 12 GiB + counters
+    assert B.workspace_bytes(8192, 128, 128, B.BF16) == 48 * 2 ** 30 + B.SCHED_SCRATCH_BYTES
+    assert B.workspace_bytes(64, 128, 128, B.F32) == 3 * 128 * 64 * 64 * 4 + 256
     assert B.workspace_bytes(12, 128, 128, B.BF16) == 0      # N % 8 != 0 in bf16
     assert B.workspace_bytes(12, 128, 128, B.F32) > 0
     assert B.workspace_bytes(64, 64, 128, B.BF16) == 0       # c_z != 128
@@ -111,6 +111,39 @@ def test_host_side_rejections(lib):
     assert _call(lib, _params(lib, ws=big, ws_bytes=need), z=0x100000, out=0x100000) == ALIAS
     assert _call(lib, _params(lib, ws=big, ws_bytes=need), out=big + 4096) == ALIAS
     assert _call(lib, _params(lib, ws=big, ws_bytes=need), z=big + 256) == ALIAS
+
+
+def test_stage_entry_points_reject_aliasing_and_missing_scratch(lib):
+    """The persistent kernels store tiles while later tiles still read the operands, so an in-place
+    stage call must be refused on the host; bf16 stage calls need the tile-counter scratch."""
+    WS, ALIGN, ALIAS = 4, 3, 5
+    s = _params(lib)
+    X, Y, Zp, SC = 0x10000000, 0x20000000, 0x30000000, 0x50000000
+    by = ctypes.byref(s)
+    assert lib.foldcp_trimul_project(X, None, by, 64, 128, 128, X, Y, SC, None) == ALIAS        # a == z
+    assert lib.foldcp_trimul_project(X, None, by, 64, 128, 128, Y, Y + 4096, SC, None) == ALIAS  # a, b overlap
+    assert lib.foldcp_trimul_project(X, None, by, 64, 128, 128, Y, Zp, None, None) == WS
+    assert lib.foldcp_trimul_project(X, None, by, 64, 128, 128, Y, Zp, SC + 8, None) == ALIGN
+    assert lib.foldcp_trimul_contract(X, Y, 64, 128, B.BF16, 0, X, SC, None) == ALIAS           # o == a
+    assert lib.foldcp_trimul_contract(X, Y, 64, 128, B.BF16, 1, Y + 256, SC, None) == ALIAS      # o inside b
+    assert lib.foldcp_trimul_contract(X, Y, 64, 128, B.BF16, 0, Zp, None, None) == WS
+    assert lib.foldcp_trimul_contract_backward(X, Y, Zp, 64, 128, B.BF16, 0, 0x60000000, 0x70000000,
+                                               None, None) == WS
+    assert lib.foldcp_trimul_finalize(X, Y, None, by, 64, 128, 128, X, None) == ALIAS            # out == o
+    assert lib.foldcp_trimul_finalize(X, Y, None, by, 64, 128, 128, Y, None) == ALIAS            # out == z
+
+
+def test_library_has_no_device_global_state_and_reads_no_environment():
+    """no __device__ global scheduler pool, no getenv dispatch in the shipped
+    build (the A/B knobs exist only under -DFOLDCP_DEBUG_KNOBS)."""
+    csrc = os.path.join(ROOT, "paper_2603_14806_b200", "csrc")
+    for name in os.listdir(csrc):
+        src = open(os.path.join(csrc, name)).read()
+        assert "__device__ unsigned int g_" not in src, name
+        for line in src.splitlines():
+            if "getenv(" in line:
+                assert name == "common.h" and "return getenv(name);" in line, (name, line)
+    assert "-DFOLDCP_DEBUG_KNOBS" not in " ".join(builder.NVCC_FLAGS)
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):

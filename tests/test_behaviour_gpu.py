@@ -98,16 +98,30 @@ def test_I2_token_permutation_equivariance():
 
 
 def test_non_default_stream_is_asynchronous_and_correct():
+    """SURVEY 8(b): the call only enqueues.  A long spin kernel is queued on a side stream first;
+    foldcp_trimul must return while that kernel is still running (an event recorded right after
+    the call is not yet complete), i.e. it neither synchronises the stream nor the device."""
     z, M, p = inputs(264)
     ref = B.trimul(z, M, p, OUT)
+    ws = torch.empty(B.workspace_bytes(264), dtype=torch.uint8, device=DEV)
+    out = torch.empty_like(z)
     torch.cuda.synchronize()
     s = torch.cuda.Stream()
     with torch.cuda.stream(s):
-        got = B.trimul(z, M, p, OUT)
-        ev = torch.cuda.Event()
-        ev.record(s)
-    ev.synchronize()
-    assert torch.equal(got, ref)
+        torch.cuda._sleep(int(2.0e9))              # ~1 s of device time at ~2 GHz
+        before = torch.cuda.Event()
+        before.record(s)
+        B.trimul(z, M, p, OUT, out=out, workspace=ws)
+        after = torch.cuda.Event()
+        after.record(s)
+    # the host is back although nothing behind the spin kernel can have started
+    assert not before.query(), "the spin kernel finished before the call returned: cannot tell"
+    assert not after.query()
+    # the default stream is not blocked by it either (no device-wide synchronisation happened)
+    torch.ones(8, device=DEV).sum().item()
+    assert not after.query()
+    after.synchronize()
+    assert torch.equal(out, ref)
 
 
 def test_two_host_threads_two_streams():
@@ -220,19 +234,121 @@ def test_fully_masked_input_gives_exact_zero():
     assert torch.count_nonzero(out) == 0 and torch.isfinite(out).all()
 
 
-def test_scheduler_slots_are_rearmed_after_wrap_around():
-    """K1 and K2 draw their tiles from a pool of 1024 scheduler-word pairs handed out round robin;
-    every launch must leave its pair zeroed for the launch that re-uses it.  More launches than
-    slots, results bitwise identical throughout."""
+def test_deep_queue_on_one_stream_plus_second_stream_bitwise():
+    """VERDICT r1 item 7 / ADVICE: the tile counters are per call (workspace tail), not a process-wide
+    pool.  1200 calls are queued on stream A without any synchronisation (2400 scheduler-using
+    launches outstanding) while stream B keeps launching; every result is bitwise the reference."""
     z, M, p = inputs(136)
     ref = B.trimul(z, M, p, OUT)
     torch.cuda.synchronize()
-    ws = torch.empty(B.workspace_bytes(136), dtype=torch.uint8, device=DEV)
-    out = torch.empty_like(z)
-    for i in range(700):                      # 2 scheduler-using launches per call -> 1400 draws
-        B.trimul(z, M, p, OUT, out=out, workspace=ws)
-        if i % 100 == 99:
-            torch.cuda.synchronize()
-            assert torch.equal(out, ref), f"call {i}"
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    need = B.workspace_bytes(136)
+    ws_a, ws_b = (torch.empty(need, dtype=torch.uint8, device=DEV) for _ in range(2))
+    outs_a = [torch.empty_like(z) for _ in range(8)]
+    outs_b = [torch.empty_like(z) for _ in range(8)]
+    with torch.cuda.stream(sa):
+        torch.cuda._sleep(int(4.0e8))              # hold stream A back so that its queue is deep
+    for i in range(1200):
+        with torch.cuda.stream(sa):
+            B.trimul(z, M, p, OUT, out=outs_a[i % 8], workspace=ws_a)
+        if i % 10 == 0:
+            with torch.cuda.stream(sb):
+                B.trimul(z, M, p, OUT, out=outs_b[(i // 10) % 8], workspace=ws_b)
     torch.cuda.synchronize()
-    assert torch.equal(out, ref)
+    for o in outs_a + outs_b:
+        assert torch.equal(o, ref)
+
+
+def test_cuda_graph_replays_are_bitwise_and_overlap_with_eager_calls():
+    """A captured call carries its own counter memset: replays (also while eager calls run on another
+    stream with another workspace) reproduce the eager result bit for bit."""
+    z, M, p = inputs(136, INC)
+    ref = B.trimul(z, M, p, INC)
+    torch.cuda.synchronize()
+    need = B.workspace_bytes(136)
+    ws_g, ws_e = (torch.empty(need, dtype=torch.uint8, device=DEV) for _ in range(2))
+    out_g, out_e = torch.empty_like(z), torch.empty_like(z)
+    g = torch.cuda.CUDAGraph()
+    cap = torch.cuda.Stream()
+    with torch.cuda.stream(cap):
+        with torch.cuda.graph(g, stream=cap):
+            B.trimul(z, M, p, INC, out=out_g, workspace=ws_g)
+    se = torch.cuda.Stream()
+    for _ in range(20):
+        g.replay()
+        with torch.cuda.stream(se):
+            B.trimul(z, M, p, INC, out=out_e, workspace=ws_e)
+    torch.cuda.synchronize()
+    assert torch.equal(out_g, ref) and torch.equal(out_e, ref)
+
+
+# ---------------------------------------------------------------- numeric preconditions of the bf16 mode
+def test_saturated_gates_parity():
+    """trained gates saturate.  Gate biases of -6 / +6 and gate weights scaled x4 push
+    sigmoid towards 0 and 1, where the relative accuracy of the gate matters (a, b are summed over k
+    in K2).  Full oracle, both directions; the result is recorded like every other parity number."""
+    cfg = synth.CONFIGS[1]
+    N = 264
+    for direction, shift in ((OUT, -6.0), (INC, 6.0), (OUT, 0.0)):
+        z, _, p = synth.make_inputs(cfg, direction, "cpu", N=N)
+        M = synth.pair_mask(synth.make_token_mask("tail", N, cfg.seed), cfg.dtype)
+        p = dict(p)
+        for k in ("w_a_gate", "w_b_gate", "w_g"):
+            p[k] = (p[k].float() * 4.0).to(torch.bfloat16)
+        for k in ("b_a_gate", "b_b_gate", "b_g"):
+            p[k] = p[k] + shift
+        ref = U.oracle_full(z, M, p, direction)
+        out = B.trimul(z.to(DEV), M.to(DEV), {k: v.to(DEV) for k, v in p.items()}, direction)
+        torch.cuda.synchronize()
+        U.assert_parity(U.np64(out), ref, "bf16", f"saturated gates (x4 weights, bias {shift:+.0f}) N={N} dir={direction}")
+
+
+def test_fp16_operand_tile_preconditions_at_the_edges():
+    """include/foldcp_trimul.h "Numeric preconditions": the gamma-folded weights live on chip as fp16.
+    Inside the range (|gamma w| up to ~1e4, and down to ~2e-4 for a whole matrix) parity holds;
+    beyond 65504 the weights saturate: the output stays finite but is no longer the oracle's."""
+    cfg = synth.CONFIGS[1]
+    N = 136
+    z, _, p0 = synth.make_inputs(cfg, OUT, "cpu", N=N)
+    M = synth.pair_mask(synth.make_token_mask("tail", N, cfg.seed), cfg.dtype)
+
+    def run(scale):
+        p = dict(p0)
+        p["w_a"] = (p0["w_a"].float() * scale).to(torch.bfloat16)
+        ref = U.oracle_full(z, M, p, OUT)
+        out = B.trimul(z.to(DEV), M.to(DEV), {k: v.to(DEV) for k, v in p.items()}, OUT)
+        torch.cuda.synchronize()
+        assert torch.isfinite(out).all()
+        return U.errors(U.np64(out), ref)
+
+    for scale in (2.0 ** 15, 2.0 ** -9):           # max |gamma w| ~ 1.5e4 / whole matrix ~ 2e-4
+        e = run(scale)
+        U.record_parity(f"fp16 operand tiles, W_a scaled by {scale:g} (inside the precondition)", e, "bf16", N=N)
+        assert e["rel_fro"] <= 1e-2 and e["max_over_rms"] <= 5e-2
+    e = run(2.0 ** 19)                              # max |gamma w| ~ 2e5 > 65504: saturates
+    print(f"[precondition] W_a scaled by 2^19 (|gamma w| > 65504): rel_fro {e['rel_fro']:.3e} (finite, documented)")
+    assert e["rel_fro"] > 1e-2
+
+
+def test_layernorm_fp32_range_precondition():
+    """|z| up to ~1e17 is normalised like the oracle does; beyond ~1e18 the fp32 variance overflows
+    (documented precondition): the result stays finite -- LayerNorm degenerates to beta -- but is not
+    the oracle's."""
+    cfg = synth.CONFIGS[1]
+    N = 72
+    z, _, p = synth.make_inputs(cfg, OUT, "cpu", N=N)
+    M = synth.pair_mask(synth.make_token_mask("ones", N, cfg.seed), cfg.dtype)
+    pd = {k: v.to(DEV) for k, v in p.items()}
+    zf = z.float()
+    zf[5] *= 1.0e17
+    zb = zf.to(torch.bfloat16)
+    out = B.trimul(zb.to(DEV), M.to(DEV), pd, OUT)
+    torch.cuda.synchronize()
+    U.assert_parity(U.np64(out), U.oracle_full(zb, M, p, OUT), "bf16", "|z| ~ 1e17 rows")
+    zf[5] *= 1.0e4                                  # ~1e21: variance ~1e42 overflows fp32
+    zb = zf.to(torch.bfloat16)
+    out = B.trimul(zb.to(DEV), M.to(DEV), pd, OUT)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out).all()
+    e = U.errors(U.np64(out), U.oracle_full(zb, M, p, OUT))
+    print(f"[precondition] |z| ~ 1e21 rows: rel_fro {e['rel_fro']:.3e} (finite, outside the documented range)")

@@ -477,6 +477,94 @@ def test_rowblock_null_mask_and_single_row():
             assert relerr(row[0], full[i]) < 1e-13
 
 
+# ----------------------------------------------------------------------------------------
+# backward pass: finite differences of the forward
+# oracle for every input and parameter, the adjoint identity, scalar-loop LayerNorm Jacobian
+# ----------------------------------------------------------------------------------------
+def _fd(f, x, idx, h=1e-6):
+    """central difference of the scalar function f with respect to x[idx]"""
+    old = x[idx]
+    x[idx] = old + h
+    fp = f()
+    x[idx] = old - h
+    fm = f()
+    x[idx] = old
+    return (fp - fm) / (2 * h)
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("mask_output,bias", [(True, True), (False, False)])
+def test_backward_against_finite_differences(direction, mask_output, bias):
+    rng = np.random.default_rng(900 + 10 * direction + int(bias))
+    N, c_z, c = 4, 6, 5
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.25).astype(np.float64)
+    M[1, 2] = 0.5                                               # a soft mask value too (A22)
+    p = rand_params(rng, c_z, c, bias=bias)
+    d_out = rng.standard_normal((N, N, c_z))
+    loss = lambda: float((d_out * orc.trimul(z, M, p, direction, mask_output=mask_output)).sum())
+    d_z, grads = orc.trimul_backward(d_out, z, M, p, direction, mask_output=mask_output)
+    assert set(grads) == set(p)                                 # every parameter has a gradient
+    # d_z: every element
+    for idx in np.ndindex(z.shape):
+        assert abs(_fd(loss, z, idx) - d_z[idx]) < 2e-7 * max(1.0, abs(d_z[idx])), ("z", idx)
+    # parameters: every element of the vectors, a seeded sample of the matrices
+    for name, arr in p.items():
+        gr = grads[name]
+        assert gr.shape == arr.shape, name
+        idxs = list(np.ndindex(arr.shape))
+        if arr.ndim == 2:
+            idxs = [idxs[k] for k in rng.choice(len(idxs), size=12, replace=False)]
+        for idx in idxs:
+            assert abs(_fd(loss, arr, idx) - gr[idx]) < 2e-7 * max(1.0, abs(gr[idx])), (name, idx)
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_backward_adjoint_identity_and_residual(direction):
+    """<d_out, J u> = <J^T d_out, u> with J u from a central difference along a random direction u
+    of ALL inputs at once (z and every parameter); the residual form adds d_out to d_z."""
+    rng = np.random.default_rng(77 + direction)
+    N, c_z, c = 6, 8, 4
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)
+    p = rand_params(rng, c_z, c)
+    d_out = rng.standard_normal((N, N, c_z))
+    uz = rng.standard_normal(z.shape)
+    up = {k: rng.standard_normal(v.shape) for k, v in p.items()}
+    h = 1e-6
+    shift = lambda t: (z + t * uz, {k: v + t * up[k] for k, v in p.items()})
+    zp_, pp_ = shift(h)
+    zm_, pm_ = shift(-h)
+    Ju = (orc.trimul(zp_, M, pp_, direction) - orc.trimul(zm_, M, pm_, direction)) / (2 * h)
+    d_z, grads = orc.trimul_backward(d_out, z, M, p, direction)
+    lhs = float((d_out * Ju).sum())
+    rhs = float((d_z * uz).sum()) + sum(float((grads[k] * up[k]).sum()) for k in p)
+    assert abs(lhs - rhs) < 1e-6 * max(1.0, abs(lhs))
+    d_z_res, grads_res = orc.trimul_backward(d_out, z, M, p, direction, residual=True)
+    assert np.array_equal(d_z_res, d_z + d_out)
+    assert all(np.array_equal(grads_res[k], grads[k]) for k in grads)
+
+
+def test_layer_norm_backward_against_scalar_jacobian():
+    """d_x of the LayerNorm from its Jacobian written out element by element in Python floats:
+    dy_t/dx_s = gamma_t * rstd * (delta_ts - 1/n - xh_t xh_s / n)."""
+    rng = np.random.default_rng(3)
+    n, eps = 7, 1e-3
+    x = rng.standard_normal(n).tolist()
+    gamma = (1 + 0.3 * rng.standard_normal(n)).tolist()
+    dy = rng.standard_normal(n).tolist()
+    mu = sum(x) / n
+    var = sum((v - mu) ** 2 for v in x) / n
+    rstd = 1.0 / math.sqrt(var + eps)
+    xh = [(v - mu) * rstd for v in x]
+    dx = [sum(dy[t] * gamma[t] * rstd * ((1.0 if t == s_ else 0.0) - 1.0 / n - xh[t] * xh[s_] / n)
+              for t in range(n)) for s_ in range(n)]
+    got_dx, got_dg, got_db = orc.layer_norm_backward(np.array([dy]), np.array([x]), np.array(gamma), eps)
+    assert np.allclose(got_dx[0], dx, rtol=0, atol=1e-13)
+    assert np.allclose(got_dg, [dy[t] * xh[t] for t in range(n)], rtol=0, atol=1e-13)
+    assert np.allclose(got_db, dy, rtol=0, atol=1e-15)
+
+
 def test_flop_count_matches_baseline_md():
     # BASELINE.md section 4: 17.592 + 2.749 + 0.550 = 20.891 TFLOP at N=4096, c=c_z=128
     assert abs(orc.flops(4096, 128, 128) / 1e12 - 20.891) < 1e-3
