@@ -24,7 +24,32 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 C = 128
-K2_DRAM_BYTES_PER_LAUNCH_N4096 = 9.06e9 + 4.28e9   # ncu, profiles/r1_k2_contract_ncu_full.txt
+
+
+def k2_traffic_from_profile():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k2_contract launch at N = 4096, parsed from
+    the newest committed ncu --set full summary (profiles/r<round>_k2_contract_ncu_full.txt).
+    Returns (bytes or None, file name or None): nothing is hard-coded here."""
+    import glob
+    import re
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r[0-9]*_k2_contract_ncu_full.txt")),
+                   key=lambda f: int(re.match(r"r(\d+)", os.path.basename(f)).group(1)))
+    if not files:
+        return None, None
+    rd = wr = None
+    with open(files[-1]) as f:
+        for line in f:
+            m = re.match(r"dram__bytes_(read|write)\.sum \[(\w+)\]:\s*([0-9.eE+-]+)", line)
+            if m:
+                unit = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}[m.group(2)]
+                v = float(m.group(3)) * unit
+                if m.group(1) == "read":
+                    rd = v
+                else:
+                    wr = v
+    if rd is None or wr is None:
+        return None, os.path.basename(files[-1])
+    return rd + wr, os.path.basename(files[-1])
 
 
 def counted_flops(N: int) -> float:
@@ -149,12 +174,115 @@ def oracle_sample_step(N: int, rows: int, seed: int, direction: int):
     return dt
 
 
+def host_info():
+    """CPU model string, cores this process may run on, and the thread count numpy's BLAS really uses."""
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    blas_threads = None
+    try:
+        import numpy  # noqa: F401  (load the BLAS before asking)
+        from threadpoolctl import threadpool_info
+        blas = [d for d in threadpool_info() if d.get("user_api") == "blas"]
+        if blas:
+            blas_threads = max(int(d.get("num_threads", 0)) for d in blas)
+    except Exception:
+        pass
+    return {"cpu_model": model, "cores_available": cores, "blas_threads": blas_threads or cores}
+
+
+def oracle_full_op(N: int, direction: int, threads=None, split=False):
+    """Wall-clock of the oracle's full op (orc.trimul as it stands) on the headline-shaped problem at N
+    tokens (z ~ N(0,1) rounded to bf16, all-ones mask).  threads=1 pins the BLAS to one thread.
+    split=True also times orc.contraction alone on the same a, b (for the labelled extrapolation)."""
+    import contextlib
+    import numpy as np
+    from oracle import trimul_oracle as orc
+    from paper_2603_14806_b200 import synth
+    z = synth.make_z(7, N, C, "bf16", "cpu").double().numpy()
+    p = {k: v.double().numpy() for k, v in synth.make_params(14 + direction, C, C, "bf16").items()}
+    ctx = contextlib.nullcontext()
+    if threads is not None:
+        from threadpoolctl import threadpool_limits
+        ctx = threadpool_limits(limits=threads)
+    with ctx:
+        t0 = time.perf_counter()
+        out = orc.trimul(z, None, p, direction)
+        dt = time.perf_counter() - t0
+        assert np.all(np.isfinite(out))
+        del out
+        t_c = None
+        if split:
+            a, b = orc.projections(z, None, p)
+            t0 = time.perf_counter()
+            orc.contraction(a, b, direction)
+            t_c = time.perf_counter() - t0
+    return dt, t_c
+
+
+def cpu_baseline_protocol(N_headline: int, budget_s: float):
+    """SURVEY 8(d) "Oracle timed beside it": the oracle's FULL op wall-clocked at N = 64, 512 and 2048
+    (N = 2048 once, and only if the N = 512 timing predicts it fits the budget and the host has the
+    memory; otherwise N = 1024 and said so), one single-thread figure at N = 512, and the N = 4096
+    figure as a LABELLED extrapolation (contraction ~ N^3, the rest ~ N^2)."""
+    import psutil
+    info = host_info()
+    fl = lambda n: counted_flops(n)
+    res = {"host": info, "full_op": {}}
+    split512 = None
+    for n in (64, 512):
+        t_out, t_c = oracle_full_op(n, 0, split=(n == 512))
+        t_in, _ = oracle_full_op(n, 1)
+        if n == 512:
+            split512 = (t_out, t_c)
+        res["full_op"][f"N={n}"] = {"seconds_outgoing": t_out, "seconds_incoming": t_in,
+                                     "tflops": 2 * fl(n) / (t_out + t_in) / 1e12,
+                                     "threads": info["blas_threads"]}
+    t1, _ = oracle_full_op(512, 0, threads=1)
+    res["single_thread"] = {"N": 512, "direction": "outgoing", "seconds": t1, "tflops": fl(512) / t1 / 1e12}
+    # largest of N = 2048 / 1024 whose predicted time (contraction ~ N^3, the rest ~ N^2, from the
+    # N = 512 split) fits the budget and whose fp64 working set (~12 arrays of N*N*128 doubles) fits
+    predict = lambda n: split512[1] * (n / 512) ** 3 + (split512[0] - split512[1]) * (n / 512) ** 2
+    big = 1024
+    if predict(2048) <= budget_s and psutil.virtual_memory().available > 12 * 2048 * 2048 * C * 8 * 1.2:
+        big = 2048
+    t_big, t_contr = oracle_full_op(big, 0, split=True)
+    res["full_op"][f"N={big}"] = {"seconds_outgoing": t_big, "seconds_contraction_alone": t_contr,
+                                   "tflops": fl(big) / t_big / 1e12, "threads": info["blas_threads"],
+                                   "note": "timed once (outgoing)" + ("" if big == 2048 else
+                                           f"; N=2048 was predicted at {predict(2048):.0f} s, over the "
+                                           f"{budget_s:.0f} s budget of the default run (--cpu-budget)")}
+    r = N_headline / big
+    t_head = t_contr * r ** 3 + (t_big - t_contr) * r ** 2
+    res["extrapolated"] = {"N": N_headline, "seconds_per_call": t_head, "tflops": fl(N_headline) / t_head / 1e12,
+                           "label": f"EXTRAPOLATION from the measured N={big} full op: contraction x{r:g}^3, "
+                                    f"the rest x{r:g}^2 -- not measured"}
+    res["value"] = res["full_op"][f"N={big}"]["tflops"]
+    res["unit"] = "TFLOP/s"
+    res["cores"] = info["blas_threads"]
+    res["kind"] = "oracle"
+    res["sample"] = (f"fp64 numpy oracle, FULL op at N={big} (outgoing, timed once) on {info['blas_threads']} BLAS "
+                     f"threads of {info['cpu_model']}; full-op timings at N=64 / 512 (both directions), a "
+                     f"single-thread figure at N=512 and a labelled extrapolation to N={N_headline} beside it")
+    return res
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     N, rows = args.n, args.ref_rows
-    for _ in range(min(args.warmup, 1)):
+    # the oracle has no caches or lazy initialisation worth more than one untimed call: ONE warm-up
+    # sample whatever --warmup says (stated in the line as warmup_run)
+    warm = min(args.warmup, 1)
+    for _ in range(warm):
         oracle_sample_step(N, rows, 0, 0)
     times = []
     for s in range(args.steps):
@@ -162,13 +290,15 @@ def run_reference(args):
     total = sum(times)
     fl = 2 * subgrid_flops(N, rows, rows) * args.steps
     val = fl / total / 1e12
-    cores = os.cpu_count()
+    info = host_info()
+    cores = info["blas_threads"]
     sample = (f"sub-grid oracle, {rows}x{rows} sampled output pairs of the N={N} problem (exact full-k "
               f"sums), outgoing+incoming per step; TFLOP/s on the sample's own counted FLOPs")
     line = {
         "impl": "reference", "metric": "triangle-mult TFLOP/s at N=4096 c=128 bf16 (outgoing+incoming)",
         "value": val, "unit": "TFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
+        "warmup": args.warmup, "warmup_run": warm, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "host": info,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"BASELINE configs[3]: trimul outgoing+incoming N={N} c_z=c=128 all-ones mask",
                    "sample": sample},
@@ -274,6 +404,18 @@ def run_ours(args):
         stage_ms["k1"] += ev[0].elapsed_time(ev[1])
         stage_ms["k2_out" if d == 0 else "k2_in"] += ev[1].elapsed_time(ev[2])
         stage_ms["k3"] += ev[2].elapsed_time(ev[3])
+    # ---- per-direction ms: events around each foldcp_trimul call, same loop length
+    dir_ev = []
+    for it in range(K):
+        for d in (0, 1):
+            e_a, e_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e_a.record()
+            B.trimul(z, M, ps[d], d, out=outs[d], workspace=ws)
+            e_b.record()
+            dir_ev.append((d, e_a, e_b))
+    torch.cuda.synchronize()
+    per_direction = {"outgoing": sum(a.elapsed_time(b) for d, a, b in dir_ev if d == 0) / K,
+                     "incoming": sum(a.elapsed_time(b) for d, a, b in dir_ev if d == 1) / K}
     clocks = sampler.stop() if rank == 0 else None
     stage_ms["k1"] /= 2 * K
     stage_ms["k3"] /= 2 * K
@@ -281,7 +423,82 @@ def run_ours(args):
     stage_ms["k2_in"] /= K
     return dict(torch=torch, dist=dist, B=B, synth=synth, rank=rank, world=world, dev=dev, N=N, K=K,
                 W=W, z=z, M=M, ps=ps, ws=ws, outs=outs, ms_per_step=ms_per_step, value=value,
-                stage_ms=stage_ms, clocks=clocks, flops_step=flops_step)
+                stage_ms=stage_ms, clocks=clocks, flops_step=flops_step, per_direction=per_direction)
+
+
+def run_backward(ctx, steps):
+    """NEXT-2: the full backward pass (foldcp_trimul_backward) at the headline size, both directions,
+    CUDA events around each call.  FLOPs counted: the forward recomputation (one forward call), the
+    two contraction-gradient GEMMs (2 x 2cN^3) and the 12 projection-sized GEMMs of the tail
+    (6 data gradients + 6 weight gradients, 2 N^2 c^2 each)."""
+    torch, B = ctx["torch"], ctx["B"]
+    z, M, ps, dev, N = ctx["z"], ctx["M"], ctx["ps"], ctx["dev"], ctx["N"]
+    ws = torch.empty(B.backward_workspace_bytes(N), dtype=torch.uint8, device=dev)
+    g = torch.Generator(device=dev).manual_seed(77)
+    d_out = torch.empty_like(z)
+    for r0 in range(0, N, 256):
+        d_out[r0:r0 + 256] = torch.randn(min(256, N - r0), N, C, generator=g, device=dev).to(z.dtype)
+    res = {}
+    for d, name in ((0, "outgoing"), (1, "incoming")):
+        B.trimul_backward(d_out, z, M, ps[d], d, workspace=ws)          # warm-up
+        torch.cuda.synchronize()
+        evs = []
+        for _ in range(steps):
+            e_a, e_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e_a.record()
+            B.trimul_backward(d_out, z, M, ps[d], d, workspace=ws)
+            e_b.record()
+            evs.append((e_a, e_b))
+        torch.cuda.synchronize()
+        res[name] = sum(a.elapsed_time(b) for a, b in evs) / steps
+    fl = counted_flops(N) + 2 * 2.0 * C * N ** 3 + 12 * 2.0 * N * N * C * C
+    ms = 0.5 * (res["outgoing"] + res["incoming"])
+    del ws, d_out
+    torch.cuda.empty_cache()
+    return {"ms_per_call": res, "counted_tflop_per_call": fl / 1e12, "tflops": fl / (ms * 1e-3) / 1e12,
+            "steps": steps, "workspace_bytes": B.backward_workspace_bytes(N),
+            "note": "forward recomputation + contraction gradients on tcgen05; LayerNorm / gate / projection "
+                    "backward and weight gradients on fp32 CUDA-core kernels (first correct path)"}
+
+
+def run_n8192(ctx, steps=3):
+    """BASELINE configs[4] (N = 8192, 5 % of tokens masked) in a single call per direction: 3 timed
+    calls each, CUDA events; peak HBM bytes from torch's allocator."""
+    torch, B, synth = ctx["torch"], ctx["B"], ctx["synth"]
+    dev, ps = ctx["dev"], ctx["ps"]
+    free, _ = torch.cuda.mem_get_info()
+    N = 8192
+    need = 2 * N * N * C * 2 + B.workspace_bytes(N)
+    if free < need + (4 << 30):
+        return {"skipped": f"needs {need / 2**30:.0f} GiB of free HBM, {free / 2**30:.0f} GiB free"}
+    cfg = synth.CONFIGS[4]
+    torch.cuda.reset_peak_memory_stats(dev)
+    base = torch.cuda.memory_allocated(dev)
+    z = synth.make_z(cfg.seed, N, C, "bf16", dev)
+    M = synth.pair_mask(synth.make_token_mask(cfg.mask_kind, N, cfg.seed), "bf16", dev)
+    ws = torch.empty(B.workspace_bytes(N), dtype=torch.uint8, device=dev)
+    out = torch.empty_like(z)
+    res = {}
+    for d, name in ((0, "outgoing"), (1, "incoming")):
+        B.trimul(z, M, ps[d], d, out=out, workspace=ws)                   # warm-up
+        torch.cuda.synchronize()
+        evs = []
+        for _ in range(steps):
+            e_a, e_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e_a.record()
+            B.trimul(z, M, ps[d], d, out=out, workspace=ws)
+            e_b.record()
+            evs.append((e_a, e_b))
+        torch.cuda.synchronize()
+        res[name] = sum(a.elapsed_time(b) for a, b in evs) / steps
+    peak = torch.cuda.max_memory_allocated(dev) - base
+    ms = 0.5 * (res["outgoing"] + res["incoming"])
+    del z, M, ws, out
+    torch.cuda.empty_cache()
+    return {"workload": "BASELINE configs[4]: N=8192, 5 % of tokens masked, single call per direction",
+            "ms_per_call": res, "tflops": counted_flops(N) / (ms * 1e-3) / 1e12,
+            "counted_tflop_per_call": counted_flops(N) / 1e12, "steps": steps,
+            "peak_hbm_bytes": int(peak), "peak_hbm_GiB": peak / 2 ** 30}
 
 
 def run_e2e(ctx, steps):
@@ -353,6 +570,10 @@ def main():
     ap.add_argument("--n", type=int, default=4096, help="tokens (default: BASELINE configs[3])")
     ap.add_argument("--ref-rows", type=int, default=128,
                     help="sub-grid size of the oracle sample (128: ~12 s of CPU work per step)")
+    ap.add_argument("--cpu-budget", type=float, default=90.0,
+                    help="seconds the N=2048 full-op oracle timing may take (else N=1024 is timed)")
+    ap.add_argument("--no-n8192", action="store_true")
+    ap.add_argument("--no-backward", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -363,6 +584,14 @@ def main():
     ctx = run_ours(args)
     N, K, world = ctx["N"], ctx["K"], ctx["world"]
     e2e = None if args.no_e2e else run_e2e(ctx, max(4, min(K, 6)))
+    single = world == 1 and ctx["rank"] == 0
+    bwd = run_backward(ctx, 2) if (single and not args.no_backward) else None
+    n8192 = None
+    if single and not args.no_n8192:
+        for k in ("z", "M", "ws", "outs"):
+            ctx[k] = None
+        ctx["torch"].cuda.empty_cache()
+        n8192 = run_n8192(ctx)
     if ctx["rank"] != 0:
         if world > 1:
             ctx["dist"].barrier()
@@ -373,6 +602,7 @@ def main():
     k2_ms = 0.5 * (sm["k2_out"] + sm["k2_in"])
     k2_tf = 2.0 * C * N ** 3 / (k2_ms * 1e-3) / 1e12
     step_sum = 2 * sm["k1"] + sm["k2_out"] + sm["k2_in"] + 2 * sm["k3"]
+    traffic, traffic_file = k2_traffic_from_profile()
     roofline = {
         "bound": "tensor", "kernel": "k2_contract_kernel (mean of outgoing and incoming launches)",
         "achieved": k2_tf, "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
@@ -383,11 +613,10 @@ def main():
         "algorithmic_flops_per_launch": 2.0 * C * N ** 3,
         "ms_per_launch": {"outgoing": sm["k2_out"], "incoming": sm["k2_in"]},
         "share_of_step": (sm["k2_out"] + sm["k2_in"]) / step_sum,
-        # dram__bytes_read.sum + dram__bytes_write.sum of one k2_contract launch at N=4096, from the
-        # ncu --set full capture summarised in profiles/ (9.06 GB read + 4.28 GB written; the
-        # algorithmic bytes are 8.59 GB read + 4.29 GB written)
-        "traffic": K2_DRAM_BYTES_PER_LAUNCH_N4096 if N == 4096 else None,
-        "traffic_source": "profiles/r1_k2_contract_ncu_full.txt",
+        # dram__bytes_read.sum + dram__bytes_write.sum of one k2_contract launch at N=4096, parsed
+        # from the newest ncu --set full summary under profiles/ (null if there is none)
+        "traffic": traffic if N == 4096 else None,
+        "traffic_source": None if traffic_file is None else "profiles/" + traffic_file,
         "algorithmic_bytes_per_launch": 3.0 * C * N * N * 2,
         "other_kernels": {
             "k1_project": {"ms": sm["k1"], "bound": "hbm",
@@ -400,12 +629,7 @@ def main():
     }
     cpu = None
     if not args.no_cpu_baseline:
-        rows = args.ref_rows
-        t = oracle_sample_step(N, rows, 1, 0) + oracle_sample_step(N, rows, 1, 1)
-        cpu = {"value": 2 * subgrid_flops(N, rows, rows) / t / 1e12, "unit": "TFLOP/s",
-               "cores": os.cpu_count(), "kind": "oracle", "seconds": t,
-               "sample": f"sub-grid oracle, {rows}x{rows} sampled output pairs of the N={N} problem, "
-                         f"outgoing+incoming (exact full-k sums), fp64 numpy"}
+        cpu = cpu_baseline_protocol(N, args.cpu_budget)
     line = {
         "metric": "triangle-mult TFLOP/s at N=4096 c=128 bf16 (outgoing+incoming)",
         "value": ctx["value"], "unit": "TFLOP/s", "n_gpus": world, "steps": K, "warmup": ctx["W"],
@@ -422,6 +646,10 @@ def main():
                          "datasheet_2250": ctx["value"] / world / 2250.0},
         "clocks": ctx["clocks"], "e2e": e2e, "gpu_launches": 3 * 2 * K,
         "roofline": roofline, "cpu_baseline": cpu,
+        "per_direction": {"ms_per_call": ctx["per_direction"],
+                          "tflops": {k: counted_flops(N) / (v * 1e-3) / 1e12
+                                     for k, v in ctx["per_direction"].items()}},
+        "n8192": n8192, "backward": bwd,
     }
     print(json.dumps(line), flush=True)
     if world > 1:

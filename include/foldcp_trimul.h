@@ -41,6 +41,11 @@
  *     operand tiles (11-bit significand instead of bf16's 8): |gamma_k * W[r][k]| must be
  *     <= 65504 (larger values saturate to +-65504) and values below 2^-14 in magnitude are stored
  *     as fp16 subnormals (absolute error <= 2^-25).  tests/test_behaviour_gpu.py shows both edges.
+ *   - intermediates: in bf16 mode the gated projections a and b are stored as IEEE fp16
+ *     (11-bit significand: their rounding was the largest term of the bf16 pipeline's error
+ *     budget), so |a|, |b| must stay <= 65504 -- i.e. |W_a z' + b_a| and
+ *     |W_b z' + b_b| <= 65504, far above anything LayerNorm-ed inputs and sane weights give;
+ *     larger values saturate.  o, out and all gradients are bf16 (no range limit beyond fp32's).
  * No exceptions cross this boundary; every failure is a status code and, when detected on the
  * host, leaves `out` untouched.
  */
@@ -70,7 +75,13 @@ typedef enum { FOLDCP_OUTGOING = 0, FOLDCP_INCOMING = 1 } foldcp_direction_t;
 /* dtype of z, mask, out and of the six weight matrices.  FOLDCP_F32 is the exact mode
  * (plain fp32 FFMA arithmetic, tolerance 1e-5 relative); FOLDCP_BF16 is the tensor-core mode
  * (bf16 operands, fp32 accumulation in tensor memory). */
-typedef enum { FOLDCP_F32 = 0, FOLDCP_BF16 = 1 } foldcp_dtype_t;
+typedef enum {
+  FOLDCP_F32 = 0,
+  FOLDCP_BF16 = 1,
+  /* only for foldcp_trimul_contract: a and b are IEEE fp16 -- what foldcp_trimul_project writes in
+   * bf16 mode (see "intermediates" below) -- and o is bf16 */
+  FOLDCP_BF16_F16AB = 2
+} foldcp_dtype_t;
 
 typedef struct {
   uint32_t struct_size; /* = sizeof(foldcp_trimul_params); ABI versioning                          */
@@ -141,9 +152,12 @@ size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
  * roofline and by callers that keep a / b / o).  All tensors are device pointers.
  *
  *   foldcp_trimul_project : step a1+a2 -- LayerNorm + gated projections + mask
- *        a, b  [c_hidden][N][N]  channel-major ("[channel][row][col]" of the pair index), dtype
+ *        a, b  [c_hidden][N][N]  channel-major ("[channel][row][col]" of the pair index);
+ *              fp32 in FOLDCP_F32 mode, IEEE fp16 in FOLDCP_BF16 mode
  *   foldcp_trimul_contract: step a4 -- Eq. 2 / Eq. 3 per channel
- *        o     [c_hidden][N][N]  channel-major, dtype
+ *        o     [c_hidden][N][N]  channel-major; dtype = FOLDCP_F32 (a, b, o fp32), FOLDCP_BF16
+ *              (a, b, o bf16) or FOLDCP_BF16_F16AB (a, b fp16 as the project stage writes them,
+ *              o bf16)
  *   foldcp_trimul_finalize: step a3+a5 -- LayerNorm(o) + output projection + sigmoid gate + mask
  *
  *   scratch: FOLDCP_SCHED_SCRATCH_BYTES of caller-owned device memory, 16-byte aligned, contents
@@ -172,6 +186,57 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
                            const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
                            void* out, void* stream);
 
+/*
+ * Full backward pass.  PAPER.md lines 92-96 (section 3.1): every Fold-CP
+ * module hand-writes its backward with the same algorithm as its forward.  Given d_out = dL/d(out)
+ * of one foldcp_trimul call (same z, mask, params, direction; params->add_residual and
+ * params->mask_output as in the forward), computes
+ *     d_z   [N][N][c_z]  device, dtype = params->dtype     gradient with respect to z
+ *     grads              gradients of all 16 parameters, fp32 in both modes, each [same shape as
+ *                        the parameter]; any pointer may be NULL (that gradient is not written)
+ * by the chain rule through the definition at the top of this header, in reverse order:
+ *     d_y = d_out [M] g, d_g = d_out [M] y            -> dW_o, db_o, dW_g, db_g
+ *     d_o = LayerNorm-backward(d_y W_o)               -> dgamma_out, dbeta_out
+ *     d_a, d_b = gradients of Eq. 2-3 (foldcp_trimul_contract_backward, on tcgen05 in bf16 mode)
+ *     d_z' = sum over the five projections of (their pre-activation gradient) W
+ *                                                     -> dW_a, db_a, dW_a_gate, ... (8 tensors)
+ *     d_z = LayerNorm-backward(d_z') [+ d_out when add_residual]   -> dgamma_in, dbeta_in
+ * Nothing is kept from the forward call: a, b and o are recomputed (by the forward kernels) into
+ * params->workspace, which must hold foldcp_trimul_backward_workspace_bytes() bytes.  d_z must not
+ * overlap d_out, z or the workspace.  Deterministic: per-block partial sums of the parameter
+ * gradients are reduced in a fixed order.  Asynchronous like foldcp_trimul.
+ */
+typedef struct {
+  uint32_t struct_size;      /* = sizeof(foldcp_trimul_grads) */
+  uint32_t reserved0;        /* must be 0 */
+  float* ln_in_gamma;        /* [c_z] */
+  float* ln_in_beta;         /* [c_z] */
+  float* w_a;                /* [c_hidden][c_z] row-major, like the parameter */
+  float* w_a_gate;
+  float* w_b;
+  float* w_b_gate;
+  float* b_a;                /* [c_hidden] */
+  float* b_a_gate;
+  float* b_b;
+  float* b_b_gate;
+  float* w_g;                /* [c_z][c_z] */
+  float* b_g;                /* [c_z] */
+  float* ln_out_gamma;       /* [c_hidden] */
+  float* ln_out_beta;
+  float* w_o;                /* [c_z][c_hidden] */
+  float* b_o;                /* [c_z] */
+} foldcp_trimul_grads;
+
+int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
+                           const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
+                           int direction, void* d_z, const foldcp_trimul_grads* grads,
+                           void* stream);
+
+/* Device scratch of foldcp_trimul_backward: a, b, o (d_o in place), d_a, d_b in the tensor dtype,
+ * the fp32 accumulator of d_z', staged fp32 weights and per-block partial sums, tile counters.
+ * 0 if the shape / dtype is unsupported. */
+size_t foldcp_trimul_backward_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
+
 /* Number of kernels one foldcp_trimul call launches for this dtype (for launch accounting). */
 int foldcp_trimul_launches_per_call(int dtype);
 
@@ -179,7 +244,7 @@ const char* foldcp_status_string(int status);
 /* major * 100 + minor * 10; 110 added params->add_residual, foldcp_trimul_batched and
  * foldcp_trimul_contract_backward (the params struct grew: struct_size guards mismatches);
  * 120 made the tile counters per call (workspace grew by FOLDCP_SCHED_SCRATCH_BYTES, the stage
- * entry points take `scratch`). */
+ * entry points take `scratch`) and added foldcp_trimul_backward. */
 int foldcp_version(void);
 
 #ifdef __cplusplus

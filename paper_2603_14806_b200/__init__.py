@@ -6,4 +6,4 @@ its CUDA sources (csrc/), the build step (build.py), a ctypes binding with the s
 """
 from . import binding, synth  # noqa: F401
 from .binding import (BF16, F32, INCOMING, OUTGOING, FoldcpError, contract, finalize,  # noqa: F401
-                      project, trimul, workspace_bytes)
+                      project, trimul, trimul_backward, workspace_bytes)

@@ -16,6 +16,7 @@ OUTGOING = 0
 INCOMING = 1
 F32 = 0
 BF16 = 1
+BF16_F16AB = 2     # foldcp_trimul_contract only: a, b fp16 (as the project stage writes them), o bf16
 
 _LIB_NAME = "libfoldcp_trimul.so"
 _lib = None
@@ -23,6 +24,7 @@ _lib = None
 EXPORTS = (
     "foldcp_trimul", "foldcp_trimul_batched", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
     "foldcp_trimul_contract", "foldcp_trimul_contract_backward", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
+    "foldcp_trimul_backward", "foldcp_trimul_backward_workspace_bytes",
     "foldcp_status_string", "foldcp_version",
 )
 
@@ -48,6 +50,15 @@ class _Params(ctypes.Structure):
         ("w_o", ctypes.c_void_p), ("b_o", ctypes.c_void_p),
         ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
     ]
+
+
+PARAM_NAMES = ("ln_in_gamma", "ln_in_beta", "w_a", "w_a_gate", "w_b", "w_b_gate", "b_a", "b_a_gate",
+               "b_b", "b_b_gate", "w_g", "b_g", "ln_out_gamma", "ln_out_beta", "w_o", "b_o")
+
+
+class _Grads(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_uint32), ("reserved0", ctypes.c_uint32)] + \
+               [(name, ctypes.c_void_p) for name in PARAM_NAMES]
 
 
 def lib_path() -> str:
@@ -80,6 +91,11 @@ def load() -> ctypes.CDLL:
     lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp, vp]
     lib.foldcp_trimul_finalize.restype = ci
     lib.foldcp_trimul_finalize.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_backward.restype = ci
+    lib.foldcp_trimul_backward.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, ci, vp,
+                                           ctypes.POINTER(_Grads), vp]
+    lib.foldcp_trimul_backward_workspace_bytes.restype = ctypes.c_size_t
+    lib.foldcp_trimul_backward_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.foldcp_trimul_launches_per_call.restype = ci
     lib.foldcp_trimul_launches_per_call.argtypes = [ci]
     lib.foldcp_status_string.restype = ctypes.c_char_p
@@ -108,6 +124,10 @@ def dtype_code(t: torch.Tensor) -> int:
 
 def workspace_bytes(N: int, c_z: int = 128, c_hidden: int = 128, dtype: int = BF16) -> int:
     return int(load().foldcp_trimul_workspace_bytes(N, c_z, c_hidden, dtype))
+
+
+def backward_workspace_bytes(N: int, c_z: int = 128, c_hidden: int = 128, dtype: int = BF16) -> int:
+    return int(load().foldcp_trimul_backward_workspace_bytes(N, c_z, c_hidden, dtype))
 
 
 def launches_per_call(dtype: int = BF16) -> int:
@@ -226,7 +246,9 @@ def project(z, mask, p, eps: float = 1e-5):
     N, c_z = z.shape[0], z.shape[2]
     c_hidden = p["w_a"].shape[0]
     _check_tensors(z, p, (mask,))
-    a = torch.empty(c_hidden, N, N, dtype=z.dtype, device=z.device)
+    # bf16 mode stores the intermediates a, b as fp16 (include/foldcp_trimul.h, numeric preconditions)
+    ab_dtype = torch.float16 if z.dtype == torch.bfloat16 else z.dtype
+    a = torch.empty(c_hidden, N, N, dtype=ab_dtype, device=z.device)
     b = torch.empty_like(a)
     s = make_params(p, dtype_code(z), eps)
     st = lib.foldcp_trimul_project(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
@@ -239,13 +261,19 @@ def project(z, mask, p, eps: float = 1e-5):
 
 def contract(a: torch.Tensor, b: torch.Tensor, direction: int,
              o: Optional[torch.Tensor] = None) -> torch.Tensor:
-    """Stage a4 (Eq. 2-3): a, b [c, N, N] channel-major -> o [c, N, N]."""
+    """Stage a4 (Eq. 2-3): a, b [c, N, N] channel-major -> o [c, N, N].  a, b may be fp32, bf16 or
+    fp16 (the project stage's output in bf16 mode; o is then bf16)."""
     lib = load()
     c, N = a.shape[0], a.shape[1]
+    assert a.dtype == b.dtype
+    if a.dtype == torch.float16:
+        code, o_dtype = BF16_F16AB, torch.bfloat16
+    else:
+        code, o_dtype = dtype_code(a), a.dtype
     if o is None:
-        o = torch.empty_like(a)
+        o = torch.empty(a.shape, dtype=o_dtype, device=a.device)
     _check_tensors(a, {}, (b, o))
-    st = lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, c, dtype_code(a),
+    st = lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, c, code,
                                     int(direction), o.data_ptr(),
                                     stage_scratch(a.device).data_ptr(), _stream())
     if st != 0:
@@ -282,3 +310,35 @@ def finalize(o, z, mask, p, eps: float = 1e-5, mask_output: bool = True,
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_finalize")
     return out
+
+
+def trimul_backward(d_out: torch.Tensor, z: torch.Tensor, mask: Optional[torch.Tensor],
+                    p: Dict[str, Optional[torch.Tensor]], direction: int, eps: float = 1e-5,
+                    mask_output: bool = True, residual: bool = False,
+                    workspace: Optional[torch.Tensor] = None):
+    """Full backward of one trimul call: returns (d_z, grads) with grads a dict of fp32 tensors, one
+    per parameter present in `p` (same shapes).  Asynchronous on the current stream."""
+    lib = load()
+    _check_tensors(z, p, (d_out, mask, workspace))
+    assert z.dim() == 3 and z.shape[0] == z.shape[1] and d_out.shape == z.shape and d_out.dtype == z.dtype
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = p["w_a"].shape[0]
+    dt = dtype_code(z)
+    if workspace is None:
+        workspace = torch.empty(max(backward_workspace_bytes(N, c_z, c_hidden, dt), 1),
+                                dtype=torch.uint8, device=z.device)
+    s = make_params(p, dt, eps, mask_output, workspace, residual)
+    d_z = torch.empty_like(z)
+    grads = {k: torch.empty(v.shape, dtype=torch.float32, device=z.device)
+             for k, v in p.items() if v is not None}
+    g = _Grads()
+    g.struct_size = ctypes.sizeof(_Grads)
+    g.reserved0 = 0
+    for name in PARAM_NAMES:
+        setattr(g, name, _ptr(grads.get(name)))
+    st = lib.foldcp_trimul_backward(d_out.data_ptr(), z.data_ptr(), _ptr(mask), ctypes.byref(s), N,
+                                    c_z, c_hidden, int(direction), d_z.data_ptr(), ctypes.byref(g),
+                                    _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_backward")
+    return d_z, grads

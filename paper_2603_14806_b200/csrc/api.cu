@@ -7,11 +7,6 @@
 
 #include "common.h"
 
-// default implementation of the three bf16 stages: bit0 K1, bit1 K2, bit2 K3 on tcgen05
-#ifndef FOLDCP_DEFAULT_TC_STAGES
-#define FOLDCP_DEFAULT_TC_STAGES 7
-#endif
-
 namespace foldcp {
 
 // ----------------------------------------------------------------------------- device info
@@ -173,16 +168,13 @@ int check_arch() {
   return (d.cc_major == 10 && d.cc_minor == 0) ? FOLDCP_OK : FOLDCP_ERR_ARCH;   // sm_100a cubin only
 }
 
-// Which implementation runs a bf16 stage: bit0 = K1, bit1 = K2, bit2 = K3 on tcgen05.  The shipped
-// library has ONE path per dtype (bf16 -> the tcgen05 kernels, fp32 -> the FFMA kernels); only a
-// -DFOLDCP_DEBUG_KNOBS build can re-route bf16 stages to the FFMA kernels for bring-up A/B runs
-// (FOLDCP_FORCE_SIMT=1, FOLDCP_TC_STAGES=<mask>).
-int bf16_stage_mask() {
-  static const int v = [] {
+// The shipped library has ONE path per dtype: bf16 -> the tcgen05 kernels, fp32 -> the FFMA
+// kernels.  Only a -DFOLDCP_DEBUG_KNOBS build can send the bf16 mode through the FFMA kernels
+// (FOLDCP_FORCE_SIMT=1, all three stages; a and b are then bf16) for bring-up cross-checks.
+bool bf16_on_tensor_cores() {
+  static const bool v = [] {
     const char* f = debug_env("FOLDCP_FORCE_SIMT");
-    if (f && f[0] == '1') return 0;
-    const char* e = debug_env("FOLDCP_TC_STAGES");
-    return e ? atoi(e) : FOLDCP_DEFAULT_TC_STAGES;
+    return !(f && f[0] == '1');
   }();
   return v;
 }
@@ -213,22 +205,23 @@ int prepare_scratch(void* scratch, int dtype, cudaStream_t s) {
 }  // namespace
 
 namespace {
-// the stage bodies: arguments already validated, scheduler words already zeroed on the stream
+// the stage bodies: arguments already validated, scheduler words already zeroed on the stream.
+// ab_f16: in bf16 mode the intermediates a, b are IEEE fp16 (forward path) rather than bf16.
 int project_stage(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
-                  void* a, void* b, void* sched_area, cudaStream_t s) {
-  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 1))
-    return launch_k1_project_bf16(z, mask, params, N, a, b, sched_word(sched_area, 0), s);
+                  void* a, void* b, bool ab_f16, void* sched_area, cudaStream_t s) {
+  if (params->dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
+    return launch_k1_project_bf16(z, mask, params, N, a, b, ab_f16, sched_word(sched_area, 0), s);
   return launch_simt_project(z, mask, params, N, a, b, s);
 }
 int contract_stage(const void* a, const void* b, int N, int dtype, int direction, void* o,
-                   void* sched_area, int word, cudaStream_t s) {
-  if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
-    return launch_k2_contract_bf16(a, b, o, N, direction, sched_word(sched_area, word), s);
+                   bool ab_f16, void* sched_area, int word, cudaStream_t s) {
+  if (dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
+    return launch_k2_contract_bf16(a, b, o, N, direction, ab_f16, sched_word(sched_area, word), s);
   return launch_simt_contract(a, b, o, N, dtype, direction, s);
 }
 int finalize_stage(const void* o, const void* z, const void* mask,
                    const foldcp_trimul_params* params, int N, void* out, cudaStream_t s) {
-  if (params->dtype == FOLDCP_BF16 && (bf16_stage_mask() & 4))
+  if (params->dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
     return launch_k3_finalize_bf16(o, z, mask, params, N, out, s);
   return launch_simt_finalize(o, z, mask, params, N, out, s);
 }
@@ -250,11 +243,16 @@ int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_p
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((st = prepare_scratch(scratch, params->dtype, s)) != FOLDCP_OK) return st;
-  return project_stage(z, mask, params, N, a, b, scratch, s);
+  return project_stage(z, mask, params, N, a, b, /*ab_f16=*/true, scratch, s);
 }
 
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
                            int direction, void* o, void* scratch, void* stream) {
+  const bool ab_f16 = dtype == FOLDCP_BF16_F16AB;     // a, b fp16 (what K1 writes), o bf16
+  if (ab_f16) {
+    if (!bf16_on_tensor_cores()) return FOLDCP_ERR_UNSUPPORTED;
+    dtype = FOLDCP_BF16;
+  }
   int st = check_shape(N, kChannels, c_hidden, dtype);
   if (st != FOLDCP_OK) return st;
   if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
@@ -266,7 +264,7 @@ int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, in
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
-  return contract_stage(a, b, N, dtype, direction, o, scratch, 0, s);
+  return contract_stage(a, b, N, dtype, direction, o, ab_f16, scratch, 0, s);
 }
 
 int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* b, int N,
@@ -287,7 +285,7 @@ int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* 
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
-  if (dtype == FOLDCP_BF16 && (bf16_stage_mask() & 2))
+  if (dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
     return launch_k2_contract_backward_bf16(d_o, a, b, d_a, d_b, N, direction,
                                             sched_word(scratch, 0), sched_word(scratch, 1), s);
   return launch_simt_contract_backward(d_o, a, b, d_a, d_b, N, dtype, direction, s);
@@ -334,10 +332,85 @@ int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* p
   void* sched_area = ws + 3 * tensor_bytes;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (params->dtype == FOLDCP_BF16 && (st = arm_sched_words(sched_area, s)) != FOLDCP_OK) return st;
-  if ((st = project_stage(z, mask, params, N, a, b, sched_area, s)) != FOLDCP_OK) return st;
-  if ((st = contract_stage(a, b, N, params->dtype, direction, o, sched_area, 1, s)) != FOLDCP_OK)
+  if ((st = project_stage(z, mask, params, N, a, b, true, sched_area, s)) != FOLDCP_OK) return st;
+  if ((st = contract_stage(a, b, N, params->dtype, direction, o, true, sched_area, 1, s)) !=
+      FOLDCP_OK)
     return st;
   return finalize_stage(o, z, mask, params, N, out, s);
+}
+
+size_t foldcp_trimul_backward_workspace_bytes(int N, int c_z, int c_hidden, int dtype) {
+  if (check_shape(N, c_z, c_hidden, dtype) != FOLDCP_OK) return 0;
+  const size_t pairs = static_cast<size_t>(N) * N;
+  return 5 * pairs * kChannels * elem_bytes(dtype)            // a, b, o / d_o, d_a, d_b
+         + pairs * kChannels * sizeof(float)                  // d_z' accumulator
+         + backward_scratch_floats(kMaxBackwardBlocks) * sizeof(float) + kSchedScratchBytes;
+}
+
+int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
+                           const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
+                           int direction, void* d_z, const foldcp_trimul_grads* grads,
+                           void* stream) {
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if (!grads || grads->struct_size != sizeof(foldcp_trimul_grads) || grads->reserved0 != 0)
+    return FOLDCP_ERR_INVALID_ARG;
+  if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
+  if (!d_out || !z || !d_z) return FOLDCP_ERR_INVALID_ARG;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (!aligned16(d_out) || !aligned16(z) || !aligned16(d_z) || (mask && !aligned16(mask)))
+    return FOLDCP_ERR_ALIGNMENT;
+  float* const gp[] = {grads->ln_in_gamma, grads->ln_in_beta, grads->w_a, grads->w_a_gate,
+                       grads->w_b, grads->w_b_gate, grads->b_a, grads->b_a_gate, grads->b_b,
+                       grads->b_b_gate, grads->w_g, grads->b_g, grads->ln_out_gamma,
+                       grads->ln_out_beta, grads->w_o, grads->b_o};
+  for (const float* q : gp)
+    if (q && (reinterpret_cast<uintptr_t>(q) & 3u) != 0) return FOLDCP_ERR_ALIGNMENT;
+  const size_t need = foldcp_trimul_backward_workspace_bytes(N, c_z, c_hidden, params->dtype);
+  if (!params->workspace || params->workspace_bytes < need) return FOLDCP_ERR_WORKSPACE;
+  if ((reinterpret_cast<uintptr_t>(params->workspace) & 255u) != 0) return FOLDCP_ERR_ALIGNMENT;
+  const size_t tb = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
+  if (overlaps(d_z, tb, z, tb) || overlaps(d_z, tb, d_out, tb) ||
+      overlaps(d_z, tb, params->workspace, need) || overlaps(z, tb, params->workspace, need) ||
+      overlaps(d_out, tb, params->workspace, need))
+    return FOLDCP_ERR_ALIAS;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+
+  // workspace: a | b | o -> d_o | d_a | d_b | d_z' (fp32) | staged weights + partials | counters
+  uint8_t* ws = static_cast<uint8_t*>(params->workspace);
+  void* a = ws;
+  void* b = ws + tb;
+  void* o = ws + 2 * tb;
+  void* d_a = ws + 3 * tb;
+  void* d_b = ws + 4 * tb;
+  float* dzp = reinterpret_cast<float*>(ws + 5 * tb);
+  float* scratch = dzp + static_cast<size_t>(N) * N * kChannels;
+  void* sched_area = scratch + backward_scratch_floats(kMaxBackwardBlocks);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int dt = params->dtype;
+  if (dt == FOLDCP_BF16 && (st = arm_sched_words(sched_area, s)) != FOLDCP_OK) return st;
+  // recompute the forward intermediates with the forward kernels; a and b as bf16 here, because
+  // the gradient GEMMs below pair them with the bf16 d_o (one operand format per tcgen05.mma)
+  if ((st = project_stage(z, mask, params, N, a, b, false, sched_area, s)) != FOLDCP_OK) return st;
+  if ((st = contract_stage(a, b, N, dt, direction, o, false, sched_area, 1, s)) != FOLDCP_OK)
+    return st;
+  // K3-backward: o -> d_o in place
+  if ((st = launch_simt_tail_backward(0, d_out, z, mask, params, N, o, nullptr, nullptr, dzp,
+                                      scratch, grads, d_z, s)) != FOLDCP_OK)
+    return st;
+  // gradients of Eq. 2-3
+  if (dt == FOLDCP_BF16 && bf16_on_tensor_cores())
+    st = launch_k2_contract_backward_bf16(o, a, b, d_a, d_b, N, direction,
+                                          sched_word(sched_area, 2), sched_word(sched_area, 3), s);
+  else
+    st = launch_simt_contract_backward(o, a, b, d_a, d_b, N, dt, direction, s);
+  if (st != FOLDCP_OK) return st;
+  // K1-backward for a, then for b (closing with the LayerNorm(z) backward)
+  if ((st = launch_simt_tail_backward(1, d_out, z, mask, params, N, o, d_a, d_b, dzp, scratch,
+                                      grads, d_z, s)) != FOLDCP_OK)
+    return st;
+  return launch_simt_tail_backward(2, d_out, z, mask, params, N, o, d_a, d_b, dzp, scratch, grads,
+                                   d_z, s);
 }
 
 int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_params* params,

@@ -67,8 +67,9 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
 
 // ----- stage launchers (device pointers; return foldcp_status_t) -----
 // `sched`: zeroed tile-scheduler counter(s) of this launch (see kSchedScratchBytes)
+// ab_f16: a and b hold IEEE fp16 (forward path) instead of bf16; o is bf16 either way
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            unsigned int* sched, cudaStream_t stream);
+                            bool ab_f16, unsigned int* sched, cudaStream_t stream);
 
 int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void* b, void* d_a,
                                      void* d_b, int N, int direction, unsigned int* sched0,
@@ -84,9 +85,20 @@ int launch_simt_finalize(const void* o, const void* z, const void* mask,
                          const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
 
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
-                           void* a, void* b, unsigned int* sched, cudaStream_t stream);
+                           void* a, void* b, bool ab_f16, unsigned int* sched,
+                           cudaStream_t stream);
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
                             const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
+
+// Backward pass around the contraction (simt_backward.cu): phase 0 = K3-backward (o -> d_o in
+// place, dzp written), 1 = K1-backward for a, 2 = K1-backward for b + LayerNorm(z) backward.
+// `scratch`: backward_scratch_floats(blocks) floats; at most kMaxBackwardBlocks persistent blocks.
+constexpr int kMaxBackwardBlocks = 160;
+size_t backward_scratch_floats(int blocks);
+int launch_simt_tail_backward(int phase, const void* d_out, const void* z, const void* mask,
+                              const foldcp_trimul_params* p, int N, void* o_io, const void* d_a,
+                              const void* d_b, float* dzp, float* scratch,
+                              const foldcp_trimul_grads* g, void* d_z, cudaStream_t s);
 
 // Opt a kernel in to `bytes` of dynamic shared memory, once per (kernel, device); thread-safe.
 // Returns FOLDCP_OK or FOLDCP_ERR_CUDA.

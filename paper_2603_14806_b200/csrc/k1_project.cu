@@ -5,8 +5,8 @@
 //   z'  = LN(z; gamma_in, beta_in, eps)                     per pair, over the 128 channels
 //   a   = M * sigmoid(W_ga z' + b_ga) * (W_a z' + b_a)      b likewise
 //
-// z is [R = N*N][128] channel-last bf16; a and b are written channel-major [128][R] bf16, which
-// is the layout K2's TMA boxes want for both directions.
+// z is [R = N*N][128] channel-last bf16; a and b are written channel-major [128][R] as fp16 (or
+// bf16, see kOutF16), which is the layout K2's TMA boxes want for both directions.
 //
 // The GEMM is oriented so that the OUTPUT CHANNEL is the MMA M dimension (TMEM lane) and the
 // PAIR is the MMA N dimension (TMEM column):   D[ch][pair] = W[ch][k] * z'[pair][k]^T.
@@ -91,7 +91,10 @@ struct K1Params {
   unsigned int* sched;
 };
 
-template <bool kTanhSigmoid>
+// kOutF16: a and b are written as IEEE fp16 (the forward path: 11-bit significand, see the header's
+// numerics notes) instead of bf16 (the backward pass's recomputation, whose contraction-gradient
+// GEMMs pair a / b with bf16 gradients -- tcgen05 kind::f16 wants both operands in one format)
+template <bool kTanhSigmoid, bool kOutF16>
 __global__ void __launch_bounds__(kThreads, 1)
 k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
                   const __grid_constant__ CUtensorMap tmap_a,
@@ -363,7 +366,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
             if (masked) pj = ptx::mul2(pj, m2[e2]);
             ptx::upk2(ptx::mul2(pj, ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1))), v0, v1);
           }
-          packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
+          packed[j4 * 2 + e2] = ptx::pack_norm<kOutF16>(v0, v1);
         }
       }
     };
@@ -466,7 +469,8 @@ bool k1_tanh_sigmoid() {
 }  // namespace
 
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
-                           void* a, void* b, unsigned int* sched, cudaStream_t stream) {
+                           void* a, void* b, bool ab_f16, unsigned int* sched,
+                           cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   const uint64_t R = static_cast<uint64_t>(N) * N;
@@ -503,7 +507,8 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   prm.sched = sched;
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k1_tanh_sigmoid();
-  auto kern = tanh_sig ? k1_project_kernel<true> : k1_project_kernel<false>;
+  auto kern = tanh_sig ? (ab_f16 ? k1_project_kernel<true, true> : k1_project_kernel<true, false>)
+                       : (ab_f16 ? k1_project_kernel<false, true> : k1_project_kernel<false, false>);
   if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), kSmemBytes) != FOLDCP_OK)
     return FOLDCP_ERR_CUDA;
   kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, ta, tb, prm);

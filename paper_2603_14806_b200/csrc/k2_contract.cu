@@ -3,7 +3,9 @@
 //   outgoing  o[c][i][j] = sum_k a[c][i][k] * b[c][j][k]      O_c = A_c  B_c^T   (operands K-major)
 //   incoming  o[c][i][j] = sum_k a[c][k][i] * b[c][k][j]      O_c = A_c^T B_c    (operands MN-major)
 //
-// a, b, o are channel-major bf16 [c][N][N]; c independent N x N x N GEMMs with fp32 accumulation.
+// a, b, o are channel-major 16-bit [c][N][N]; c independent N x N x N GEMMs with fp32 accumulation.
+// a and b are fp16 on the forward path and bf16 in the gradient GEMMs (K2Params::ab_fmt, a field of
+// the instruction descriptor); o / the gradients are written as bf16.
 // "The outgoing and incoming variants differ only in which operand is transposed" (PAPER.md line
 // 132): here that is literally one bit per operand in the tcgen05 instruction descriptor plus the
 // TMA box coordinates -- the data is never moved.
@@ -47,6 +49,19 @@ struct Cfg {
   static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kEpiBufBytes + kBarBytes + 1024;
 };
 
+#ifdef FOLDCP_K2_PROBE
+// bring-up instrumentation (never in the product build): cycles the MMA issuer / producer spend
+// waiting, per CTA pair: [0] issuer total, [1] issuer wait full (operands), [2] issuer wait tempty
+// (accumulator hand-back), [3] issuer wait tile ring, [4] producer total, [5] producer wait empty,
+// [6] tiles, [7] epilogue wait tfull (warp 4)
+__device__ unsigned long long g_k2_probe[128][8];
+#define K2_PROBE_T0(var) const long long var = clock64()
+#define K2_PROBE_ADD(acc, t0) acc += clock64() - (t0)
+#else
+#define K2_PROBE_T0(var)
+#define K2_PROBE_ADD(acc, t0)
+#endif
+
 struct K2Params {
   int N;
   int tiles_m;
@@ -56,6 +71,7 @@ struct K2Params {
   int l2_hints;    // 1: evict_last loads / evict_first stores
   int panel_n;     // tile rasterisation: n-tiles per column panel (>= 1)
   unsigned int* sched;   // next tile index: launch-private, zeroed on the stream before the launch
+  uint32_t ab_fmt;       // operand format of both inputs: ptx::kFmtBF16 or ptx::kFmtF16
 };
 
 // Tile rasterisation inside one channel: column panels of `panel_n` n-tiles, m fastest-varying
@@ -189,6 +205,10 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       const uint64_t pol_ld = prm.l2_hints == 1 ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
       int stage = 0;
       uint32_t phase = 0;
+#ifdef FOLDCP_K2_PROBE
+      long long pr_wait = 0;
+      const long long pr_t0 = clock64();
+#endif
       // the leader draws one tile ahead, so the atomic's round trip never stalls the load pipeline
       int tnext = is_leader ? produce_tile(0) : consume_tile(0);
       for (int it = 0;; ++it) {
@@ -202,7 +222,9 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
         const int m0 = tm * C::kTileM + static_cast<int>(cta_rank) * 128;
         const int n0 = tn * kTileN + static_cast<int>(cta_rank) * (kTileN / kCtaGroup);
         for (int kb = 0; kb < prm.num_kb; ++kb) {
+          K2_PROBE_T0(tw);
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+          K2_PROBE_ADD(pr_wait, tw);
           const uint32_t sa = stage_base + stage * C::kStageBytes;
           const uint32_t sb = sa + C::kABytes;
           const int k0 = kb * kBlockK;
@@ -241,11 +263,18 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
           }
         }
       }
+#ifdef FOLDCP_K2_PROBE
+      if (is_leader) {
+        g_k2_probe[blockIdx.x / kCtaGroup][4] = clock64() - pr_t0;
+        g_k2_probe[blockIdx.x / kCtaGroup][5] = pr_wait;
+      }
+#endif
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA only) =====================
     if (is_leader && ptx::elect_one()) {
-      constexpr uint32_t idesc = ptx::make_idesc_bf16(C::kTileM, kTileN, kAMn ? 1 : 0, kBMn ? 1 : 0);
+      const uint32_t idesc = ptx::make_idesc_f16kind(C::kTileM, kTileN, prm.ab_fmt, prm.ab_fmt,
+                                                     kAMn ? 1 : 0, kBMn ? 1 : 0);
       // K-major : rows of 128 B, 8-row atoms 1024 B apart (SBO); one UMMA_K = 32 B along the row
       // MN-major: 64-element MN groups kBoxBytes apart (LBO), 8-k atoms 1024 B apart (SBO);
       //           one UMMA_K = two 8-k atoms = 2048 B
@@ -254,15 +283,29 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
       constexpr uint32_t kstep_a = kAMn ? 2048 : 32, kstep_b = kBMn ? 2048 : 32;
       int stage = 0;
       uint32_t phase = 0;
+#ifdef FOLDCP_K2_PROBE
+      long long w_full = 0, w_tempty = 0, w_ring = 0, ntiles = 0;
+      const long long is_t0 = clock64();
+#endif
       for (int it = 0;; ++it) {
-        if (consume_tile(it) < 0) break;
+        K2_PROBE_T0(tr);
+        const int tcur = consume_tile(it);
+        K2_PROBE_ADD(w_ring, tr);
+        if (tcur < 0) break;
         const int as = it & 1;
         const uint32_t aphase = (it >> 1) & 1;
+        K2_PROBE_T0(te);
         ptx::mbar_wait_cluster(tempty_bar(as), aphase ^ 1u);
+        K2_PROBE_ADD(w_tempty, te);
+#ifdef FOLDCP_K2_PROBE
+        ++ntiles;
+#endif
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kAccumCols;
         for (int kb = 0; kb < prm.num_kb; ++kb) {
+          K2_PROBE_T0(tf);
           ptx::mbar_wait(full_bar(stage), phase);
+          K2_PROBE_ADD(w_full, tf);
           ptx::tc_fence_after();
           const uint32_t sa = stage_base + stage * C::kStageBytes;
           const uint32_t sb = sa + C::kABytes;
@@ -280,6 +323,13 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
         }
         ptx::umma_commit<kCtaGroup>(tfull_bar(as));        // accumulator ready for the epilogue
       }
+#ifdef FOLDCP_K2_PROBE
+      g_k2_probe[blockIdx.x / kCtaGroup][0] = clock64() - is_t0;
+      g_k2_probe[blockIdx.x / kCtaGroup][1] = w_full;
+      g_k2_probe[blockIdx.x / kCtaGroup][2] = w_tempty;
+      g_k2_probe[blockIdx.x / kCtaGroup][3] = w_ring;
+      g_k2_probe[blockIdx.x / kCtaGroup][6] = ntiles;
+#endif
     }
   } else if (warp >= 4) {
     // ===================== epilogue: TMEM -> bf16 -> smem -> TMA store =====================
@@ -398,7 +448,7 @@ int g_k2_cta_group = 2;
 // i.e. d[c][m][n] = sum_k X(m, k) Y(n, k).  The forward contraction uses (0,0) / (1,1); its
 // gradients also need the mixed (0,1) form.
 int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn,
-                        unsigned int* sched, cudaStream_t stream) {
+                        bool xy_f16, unsigned int* sched, cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   static const int cta_group = [] {
@@ -438,6 +488,7 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
   const int auto_panel = prm.tiles_n <= 16 ? prm.tiles_n : 8;
   prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : auto_panel;
   prm.sched = sched;
+  prm.ab_fmt = xy_f16 ? ptx::kFmtF16 : ptx::kFmtBF16;
   const int sms = dev.sm_count;
   if (cta_group == 2) {
     if (x_mn) return y_mn ? launch_variant<2, true, true>(ta, tb, to, prm, sms, stream)
@@ -452,9 +503,9 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
 }
 
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            unsigned int* sched, cudaStream_t stream) {
+                            bool ab_f16, unsigned int* sched, cudaStream_t stream) {
   const bool inc = direction == FOLDCP_INCOMING;
-  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, sched, stream);
+  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, ab_f16, sched, stream);
 }
 
 // Gradients of the contraction (oracle/trimul_oracle.py contraction_backward):
@@ -467,13 +518,20 @@ int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void*
                                      unsigned int* sched1, cudaStream_t stream) {
   int st;
   if (direction == FOLDCP_OUTGOING) {
-    if ((st = launch_k2_gemm_bf16(d_o, b, d_a, N, false, true, sched0, stream)) != FOLDCP_OK)
+    if ((st = launch_k2_gemm_bf16(d_o, b, d_a, N, false, true, false, sched0, stream)) != FOLDCP_OK)
       return st;
-    return launch_k2_gemm_bf16(d_o, a, d_b, N, true, true, sched1, stream);
+    return launch_k2_gemm_bf16(d_o, a, d_b, N, true, true, false, sched1, stream);
   }
-  if ((st = launch_k2_gemm_bf16(b, d_o, d_a, N, false, false, sched0, stream)) != FOLDCP_OK)
+  if ((st = launch_k2_gemm_bf16(b, d_o, d_a, N, false, false, false, sched0, stream)) != FOLDCP_OK)
     return st;
-  return launch_k2_gemm_bf16(a, d_o, d_b, N, false, true, sched1, stream);
+  return launch_k2_gemm_bf16(a, d_o, d_b, N, false, true, false, sched1, stream);
 }
 
 }  // namespace foldcp
+
+#ifdef FOLDCP_K2_PROBE
+extern "C" int foldcp_debug_k2_probe_read(unsigned long long* host_out) {
+  return static_cast<int>(cudaMemcpyFromSymbol(host_out, foldcp::g_k2_probe,
+                                               sizeof(unsigned long long) * 128 * 8));
+}
+#endif

@@ -128,51 +128,80 @@ def _host_workers(bytes_per_worker):
     return max(1, min(cores, int(0.6 * avail // max(bytes_per_worker, 1))))
 
 
-def oracle_projections_whole(z, M, p, eps=1e-5, chunk_rows=16):
-    """(a, b) of the whole z as fp64 views [N, N, c] over channel-major storage (the layout in which
-    trimul_rowblock's per-channel matmuls read contiguous matrices).  z / M may live on the GPU."""
+def _projections_cm(z_sel, M_sel, p, keep, eps=1e-5, chunk_rows=16):
+    """orc.projections over a [R1, R2, c_z] selection of z (device or host tensor), slice by slice on
+    host threads; returns the kept tensors ("a", "b" or "ab") as fp64 [R1, R2, c] views over
+    channel-major storage (the layout in which trimul_rowblock's per-channel matmuls read contiguous
+    matrices)."""
     from concurrent.futures import ThreadPoolExecutor
     from threadpoolctl import threadpool_limits
-    N, c_z = z.shape[0], z.shape[2]
+    R1, R2, c_z = z_sel.shape
     q = params64(p)
     c = q["w_a"].shape[0]
-    a_cm = np.empty((c, N, N), np.float64)
-    b_cm = np.empty((c, N, N), np.float64)
+    store = {k: np.empty((c, R1, R2), np.float64) for k in keep}
 
     def work(r0):
-        r1 = min(N, r0 + chunk_rows)
-        zc = np64(z[r0:r1]).reshape(-1, c_z)
-        mc = None if M is None else np64(M[r0:r1]).reshape(-1)
+        r1 = min(R1, r0 + chunk_rows)
+        zc = np64(z_sel[r0:r1]).reshape(-1, c_z)
+        mc = None if M_sel is None else np64(M_sel[r0:r1]).reshape(-1)
         a, b = orc.projections(zc, mc, q, eps)
-        a_cm[:, r0:r1, :] = a.reshape(r1 - r0, N, c).transpose(2, 0, 1)
-        b_cm[:, r0:r1, :] = b.reshape(r1 - r0, N, c).transpose(2, 0, 1)
+        for k, v in (("a", a), ("b", b)):
+            if k in store:
+                store[k][:, r0:r1, :] = v.reshape(r1 - r0, R2, c).transpose(2, 0, 1)
 
-    workers = _host_workers(chunk_rows * N * c_z * 8 * 12)
+    workers = _host_workers(chunk_rows * R2 * c_z * 8 * 12)
     with threadpool_limits(limits=1):
         with ThreadPoolExecutor(workers) as ex:
-            list(ex.map(work, range(0, N, chunk_rows)))
-    return a_cm.transpose(1, 2, 0), b_cm.transpose(1, 2, 0)
+            list(ex.map(work, range(0, R1, chunk_rows)))
+    return tuple(store[k].transpose(1, 2, 0) for k in keep)
+
+
+def oracle_projections_whole(z, M, p, eps=1e-5, chunk_rows=16):
+    """(a, b) of the whole z as fp64 [N, N, c] views (channel-major storage)."""
+    return _projections_cm(z, M, p, "ab", eps, chunk_rows)
 
 
 def whole_tensor_errors(out, z, M, p, direction, row_blocks=None, block_rows=32, mask_output=True,
-                        eps=1e-5, ab=None):
+                        eps=1e-5, ab=None, rows=None):
     """Errors of `out` (device or host tensor [N, N, c_z]) against the oracle over the given row
     blocks (default: every row, i.e. the WHOLE tensor).  Returns rel_fro, max_over_rms (rms over the
-    compared oracle outputs), the arg-max location and the number of outputs compared."""
+    compared oracle outputs), the arg-max location and the number of outputs compared.
+
+    rows = sorted index array: only those output rows are compared (all columns).  Then b is
+    evaluated for the whole z but a only where Eq. 2-3 need it -- rows `rows` (outgoing) or columns
+    `rows` (incoming) -- and handed to trimul_rowblock in compacted form (N = 8192: a and b whole
+    would be 137 GB in fp64)."""
     from concurrent.futures import ThreadPoolExecutor
     from threadpoolctl import threadpool_limits
+    import torch
     N, c_z = z.shape[0], z.shape[2]
     q = params64(p)
     c = q["w_a"].shape[0]
-    a, b = ab if ab is not None else oracle_projections_whole(z, M, p, eps)
-    if row_blocks is None:
-        row_blocks = [(i0, min(N, i0 + block_rows)) for i0 in range(0, N, block_rows)]
+    if rows is not None:
+        rows = np.asarray(rows, dtype=np.int64)
+        rt = torch.as_tensor(rows, device=z.device)
+        (b,) = _projections_cm(z, M, p, "b", eps)
+        if direction == orc.OUTGOING:
+            (a,) = _projections_cm(z[rt], None if M is None else M[rt], p, "a", eps)
+        else:
+            (a,) = _projections_cm(z[:, rt], None if M is None else M[:, rt], p, "a", eps)
+        nsel = rows.size
+        if row_blocks is None:
+            row_blocks = [(i0, min(nsel, i0 + block_rows)) for i0 in range(0, nsel, block_rows)]
+        sel = lambda t, i0, i1: t[torch.as_tensor(rows[i0:i1], device=t.device)]
+        row_of = lambda i: int(rows[i])
+    else:
+        a, b = ab if ab is not None else oracle_projections_whole(z, M, p, eps)
+        if row_blocks is None:
+            row_blocks = [(i0, min(N, i0 + block_rows)) for i0 in range(0, N, block_rows)]
+        sel = lambda t, i0, i1: t[i0:i1]
+        row_of = lambda i: i
 
     def work(blk):
         i0, i1 = blk
-        ref = orc.trimul_rowblock(a, b, np64(z[i0:i1]), None if M is None else np64(M[i0:i1]), q,
-                                  direction, i0, i1, eps=eps, mask_output=mask_output)
-        got = np64(out[i0:i1])
+        ref = orc.trimul_rowblock(a, b, np64(sel(z, i0, i1)), None if M is None else np64(sel(M, i0, i1)),
+                                  q, direction, i0, i1, eps=eps, mask_output=mask_output)
+        got = np64(sel(out, i0, i1))
         d = np.abs(got - ref)
         k = int(np.argmax(d))
         return (float((d * d).sum()), float((ref * ref).sum()), float(d.flat[k]),
@@ -189,5 +218,5 @@ def whole_tensor_errors(out, z, M, p, direction, row_blocks=None, block_rows=32,
     worst = max(res, key=lambda r: r[2])
     rms = (sr / n) ** 0.5
     return dict(rel_fro=(sd / max(sr, 1e-300)) ** 0.5, max_over_rms=worst[2] / max(rms, 1e-300),
-                rms=rms, max_abs=worst[2], argmax=[worst[4] + worst[3][0], worst[3][1], worst[3][2]],
+                rms=rms, max_abs=worst[2], argmax=[row_of(worst[4] + worst[3][0]), worst[3][1], worst[3][2]],
                 outputs=n, finite=all(r[6] for r in res), host_workers=workers)

@@ -58,13 +58,17 @@ def test_fp32_odd_sizes(N, direction):
 # ---------------------------------------------------------------- stage-level parity
 @pytest.mark.parametrize("direction", [OUT, INC])
 @pytest.mark.parametrize("N", [64, 328, 520])
-def test_contract_stage_bf16(direction, N):
+@pytest.mark.parametrize("ab_dtype", [torch.bfloat16, torch.float16])
+def test_contract_stage_bf16(direction, N, ab_dtype):
+    """a, b as bf16 (the gradient GEMMs' format) and as fp16 (what the project stage writes on the
+    forward path); o is bf16 in both cases."""
     from oracle import trimul_oracle as orc
     g = torch.Generator().manual_seed(N + direction)
-    a = torch.randn(128, N, N, generator=g).to(torch.bfloat16)
-    b = torch.randn(128, N, N, generator=g).to(torch.bfloat16)
+    a = torch.randn(128, N, N, generator=g).to(ab_dtype)
+    b = torch.randn(128, N, N, generator=g).to(ab_dtype)
     o = B.contract(a.to(DEV), b.to(DEV), direction)
     torch.cuda.synchronize()
+    assert o.dtype == torch.bfloat16
     ref = orc.contraction(np.transpose(U.np64(a), (1, 2, 0)), np.transpose(U.np64(b), (1, 2, 0)), direction)
     got = np.transpose(U.np64(o), (1, 2, 0))
     # only the final bf16 rounding of o (2^-9 relative) plus fp32 accumulation
@@ -78,13 +82,15 @@ def test_project_stage_bf16():
     z, M, p = synth.make_inputs(cfg, OUT, "cpu", N=136)
     a, b = B.project(z.to(DEV), M.to(DEV), to_dev(p))
     torch.cuda.synchronize()
+    assert a.dtype == torch.float16 and b.dtype == torch.float16     # fp16 intermediates in bf16 mode
     q = U.params64(p)
     zp = orc.layer_norm(U.np64(z), q["ln_in_gamma"], q["ln_in_beta"], 1e-5)
     ra = orc.gated_projection(zp, U.np64(M), q["w_a"], q["b_a"], q["w_a_gate"], q["b_a_gate"])
     rb = orc.gated_projection(zp, U.np64(M), q["w_b"], q["b_b"], q["w_b_gate"], q["b_b_gate"])
     for got, ref in ((a, ra), (b, rb)):
         e = U.errors(np.transpose(U.np64(got), (1, 2, 0)), ref)
-        assert e["rel_fro"] < 1e-2 and e["max_over_rms"] < 5e-2
+        # fp16 storage (2^-12 relative) + fp16 operand tiles + tanh.approx gates
+        assert e["rel_fro"] < 2e-3 and e["max_over_rms"] < 2e-2, e
 
 
 @pytest.mark.parametrize("mask_output", [True, False])

@@ -32,5 +32,11 @@ def test_block_walk_equals_direct_comparison(direction, tmp_path, monkeypatch):
     rows = np.r_[3:9, 30:40]
     assert e2["outputs"] == ref[rows].size
     assert abs(e2["rel_fro"] - np.linalg.norm(d[rows]) / np.linalg.norm(ref[rows])) < 1e-12
+    # a sorted row subset through the compacted-a path (the N = 8192 form)
+    sel = np.array([1, 4, 5, 17, 22, 39])
+    e3 = U.whole_tensor_errors(torch.from_numpy(got), z, M, p, direction, rows=sel, block_rows=4)
+    assert e3["outputs"] == ref[sel].size and e3["argmax"] == [17, 5, 99]
+    assert abs(e3["rel_fro"] - np.linalg.norm(d[sel]) / np.linalg.norm(ref[sel])) < 1e-12
+    assert abs(e3["max_over_rms"] - np.abs(d[sel]).max() / np.sqrt(np.mean(ref[sel] ** 2))) < 1e-9
     rec = U.record_parity("harness", e, "bf16", N=N)
     assert rec["margin_max_over_rms"] < 0 and (tmp_path / "rec.jsonl").read_text().count("\n") == 1
