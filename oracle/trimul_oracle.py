@@ -323,6 +323,96 @@ def trimul_backward(d_out: np.ndarray, z: np.ndarray, mask: Optional[np.ndarray]
     return d_z, grads
 
 
+# ------------------------------------------------------------------------------------------------
+# The paper's distributed form.  PAPER.md lines 132-134, section 3.3 "Sharding
+# and algorithm": "The pair representation is tiled as (N/sqrt(P))^2 blocks.  One operand is
+# transposed across the 2D grid to align the contracted index with the ring shift direction.  The
+# algorithm then proceeds in a Cannon-style ring: in each of sqrt(P) steps, ranks perform a local
+# batched matrix multiplication between resident blocks of a and b while simultaneously initiating
+# asynchronous P2P transfers to circulate a along rows and b along columns.  Partial results
+# accumulate into the output block.  The outgoing and incoming variants differ only in which operand
+# is transposed" (Fig. 2b; Table 1, line 83).
+#
+# Written out step by step on a simulated g x g grid (rank (r, c) owns block (r, c) of every pair
+# tensor).  The paper names Cannon's algorithm without restating its initial alignment; the reading
+# taken (A23) is the textbook one: after the grid transpose, the row-circulating operand
+# of grid row r is pre-shifted by r and the column-circulating operand of grid column c by c, so
+# that in step s rank (r, c) multiplies the two blocks with contracted block index
+# q = (r + c + s) mod g; then both circulate by one position per step.
+# ------------------------------------------------------------------------------------------------
+def cannon_schedule(grid: int, direction: int):
+    """Which blocks rank (r, c) multiplies in step s.  Returns a dict
+    {(r, c): [((ar, ac), (br, bc)) for s in range(grid)]} of block coordinates of a and of b.
+      outgoing: o_rc = sum_q a_(r,q) b_(c,q)^T   -> b is the operand transposed across the grid
+      incoming: o_rc = sum_q a_(q,r)^T b_(q,c)   -> a is the operand transposed across the grid"""
+    sched = {}
+    for r in range(grid):
+        for c in range(grid):
+            steps = []
+            for s_ in range(grid):
+                q = (r + c + s_) % grid
+                steps.append((((r, q), (c, q)) if direction == OUTGOING else ((q, r), (q, c))))
+            sched[(r, c)] = steps
+    return sched
+
+
+def contraction_cannon(a: np.ndarray, b: np.ndarray, direction: int, grid: int) -> np.ndarray:
+    """Eq. 2-3 computed the paper's way on a simulated grid x grid mesh; equals `contraction`.
+    a, b [N, N, c] with N divisible by grid (the paper's tiling).  Every data movement of the
+    algorithm is carried out explicitly on per-rank block dictionaries."""
+    a = np.asarray(a, _F)
+    b = np.asarray(b, _F)
+    N = a.shape[0]
+    g = int(grid)
+    if direction not in (OUTGOING, INCOMING):
+        raise ValueError("direction must be 0 (outgoing) or 1 (incoming)")
+    if N % g != 0:
+        raise ValueError("N must be divisible by the grid size")
+    nb = N // g
+    blk = lambda t, r, c: t[r * nb:(r + 1) * nb, c * nb:(c + 1) * nb]
+    ranks = [(r, c) for r in range(g) for c in range(g)]
+    # 0. tiling: rank (r, c) owns block (r, c) of a and of b
+    A = {rc: blk(a, *rc).copy() for rc in ranks}
+    Bm = {rc: blk(b, *rc).copy() for rc in ranks}
+    # 1. one operand is transposed across the grid: rank (r, c) receives the block of rank (c, r)
+    if direction == OUTGOING:
+        Bm = {(r, c): Bm[(c, r)] for (r, c) in ranks}       # rank (r, c) now holds b_(c, r)
+    else:
+        A = {(r, c): A[(c, r)] for (r, c) in ranks}         # rank (r, c) now holds a_(c, r)
+    # 2. Cannon's initial alignment (reading A23).  After step 1, in BOTH directions the contracted
+    #    block index of the a block a rank holds varies along its grid row and that of its b block
+    #    along its grid column:
+    #      outgoing: rank (r, c) holds a_(r, c) and b_(c, r)    (contracted index: c for a, r for b)
+    #      incoming: rank (r, c) holds a_(c, r) and b_(r, c)    (contracted index: c for a, r for b)
+    #    which is why "a circulates along rows and b along columns" whatever the direction.
+    A = {(r, c): A[(r, (c + r) % g)] for (r, c) in ranks}   # row r of the grid pre-shifted by r
+    Bm = {(r, c): Bm[((r + c) % g, c)] for (r, c) in ranks} # column c of the grid pre-shifted by c
+    out = {rc: np.zeros((nb, nb, a.shape[2]), _F) for rc in ranks}
+    for _step in range(g):
+        # local batched matrix multiplication between the resident blocks, accumulated
+        for rc in ranks:
+            out[rc] += contraction(A[rc], Bm[rc], direction)
+        # circulate a along rows and b along columns by one position
+        A = {(r, c): A[(r, (c + 1) % g)] for (r, c) in ranks}
+        Bm = {(r, c): Bm[((r + 1) % g, c)] for (r, c) in ranks}
+    o = np.empty_like(a)
+    for (r, c) in ranks:
+        o[r * nb:(r + 1) * nb, c * nb:(c + 1) * nb] = out[(r, c)]
+    return o
+
+
+def trimul_cannon(z: np.ndarray, mask: Optional[np.ndarray], p: Dict[str, np.ndarray],
+                  direction: int, grid: int, eps: float = 1e-5, mask_output: bool = True) -> np.ndarray:
+    """The full op with the contraction done the paper's distributed way.  LayerNorm, projections,
+    gates and the output stage act on each pair independently, so every rank applies them to its own
+    block of z; only Eq. 2-3 need the ring."""
+    z = np.asarray(z, _F)
+    zp = layer_norm(z, p["ln_in_gamma"], p["ln_in_beta"], eps)
+    a, b = projections(z, mask, p, eps)
+    o = contraction_cannon(a, b, direction, grid)
+    return output_stage(o, zp, mask, p, eps, mask_output)
+
+
 def flops(N: int, c_z: int, c_hidden: int) -> float:
     """Counted FLOPs of one call: contraction 2 c N^3 + five
     projections 2 N^2 c_z (4c + c_z) + output projection 2 N^2 c c_z."""

@@ -565,6 +565,64 @@ def test_layer_norm_backward_against_scalar_jacobian():
     assert np.allclose(got_db, dy, rtol=0, atol=1e-15)
 
 
+# ----------------------------------------------------------------------------------------
+# the paper's Cannon-style distributed contraction, simulated grid
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("grid", [1, 2, 3, 4])
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_cannon_contraction_equals_definition(grid, direction):
+    rng = np.random.default_rng(50 + grid)
+    N, c = 12, 3
+    a = rng.standard_normal((N, N, c))
+    b = rng.standard_normal((N, N, c))
+    got = orc.contraction_cannon(a, b, direction, grid)
+    # against the scalar definition of Eq. 2-3 written out here, not against orc.contraction
+    ref = np.zeros((N, N, c))
+    for i in range(N):
+        for j in range(N):
+            for k in range(N):
+                ref[i, j] += (a[i, k] * b[j, k]) if direction == OUT else (a[k, i] * b[k, j])
+    assert relerr(got, ref) < 1e-13
+
+
+@pytest.mark.parametrize("grid", [2, 3, 4])
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_cannon_schedule_is_a_ring(grid, direction):
+    """Every rank meets every contracted block index exactly once; between consecutive steps the a
+    block it needs is the one its right-hand neighbour (r, c+1) just used and the b block the one
+    its lower neighbour (r+1, c) just used: one nearest-neighbour shift along rows / columns per
+    step, as PAPER.md lines 132-134 describe."""
+    sched = orc.cannon_schedule(grid, direction)
+    for (r, c), steps in sched.items():
+        qs = [(ab[0][1] if direction == OUT else ab[0][0]) for ab in steps]
+        assert sorted(qs) == list(range(grid))
+        for s_ in range(grid):
+            ablk, bblk = steps[s_]
+            # the two blocks share the contracted block index, and they are the blocks the
+            # definition pairs: a_(r,q) b_(c,q) (outgoing), a_(q,r) b_(q,c) (incoming)
+            if direction == OUT:
+                assert ablk[0] == r and bblk[0] == c and ablk[1] == bblk[1]
+            else:
+                assert ablk[1] == r and bblk[1] == c and ablk[0] == bblk[0]
+            if s_ + 1 < grid:
+                assert sched[(r, (c + 1) % grid)][s_][0] == steps[s_ + 1][0]      # a arrives from the right
+                assert sched[((r + 1) % grid, c)][s_][1] == steps[s_ + 1][1]      # b arrives from below
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_trimul_cannon_equals_serial_op(direction):
+    """The paper's own validation: the distributed result equals the serial one (lines 23, 221)."""
+    rng = np.random.default_rng(8 + direction)
+    N, c_z, c = 6, 8, 5
+    z = rng.standard_normal((N, N, c_z))
+    M = (rng.random((N, N)) > 0.3).astype(np.float64)
+    p = rand_params(rng, c_z, c)
+    for grid in (2, 3):
+        assert relerr(orc.trimul_cannon(z, M, p, direction, grid), orc.trimul(z, M, p, direction)) < 1e-13
+    with pytest.raises(ValueError):
+        orc.contraction_cannon(np.zeros((5, 5, 1)), np.zeros((5, 5, 1)), direction, 2)
+
+
 def test_flop_count_matches_baseline_md():
     # BASELINE.md section 4: 17.592 + 2.749 + 0.550 = 20.891 TFLOP at N=4096, c=c_z=128
     assert abs(orc.flops(4096, 128, 128) / 1e12 - 20.891) < 1e-3
