@@ -172,6 +172,26 @@ int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_p
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
                            int direction, void* o, void* scratch, void* stream);
 /*
+ * Blocked contraction -- one rank's share of the paper's Cannon-style distributed triangle
+ * multiplication (z is tiled as (N / sqrt(P))^2 blocks
+ * on a sqrt(P) x sqrt(P) grid, "in each of sqrt(P) steps, ranks perform a local batched matrix
+ * multiplication between resident blocks of a and b ... Partial results accumulate into the output
+ * block"):
+ *     o_block = sum over q < nblocks of Eq. 2 / Eq. 3 applied to (a_blocks[q], b_blocks[q])
+ * where rank (r, c) passes, for ring step q,  a_(r, q') and b_(c, q')  (outgoing) or  a_(q', r) and
+ * b_(q', c)  (incoming), q' = (r + c + q) mod sqrt(P) (the Cannon order, which spreads the reads
+ * over the peers).  Every block is a dense [c_hidden][nb][nb] channel-major tensor of `dtype`
+ * (FOLDCP_F32, FOLDCP_BF16 or FOLDCP_BF16_F16AB as for foldcp_trimul_contract).  a_blocks and
+ * b_blocks are HOST arrays of nblocks (1..4) DEVICE pointers; a pointer may address a peer GPU's
+ * memory that is mapped into this process (cudaDeviceEnablePeerAccess / cuMemMap): on an NVLink /
+ * NVSwitch node the ring shifts then become direct TMA reads inside one kernel whose accumulator
+ * never leaves tensor memory.  One launch; o_block must not overlap any input block.
+ */
+int foldcp_trimul_contract_blocks(const void* const* a_blocks, const void* const* b_blocks,
+                                  int nblocks, int nb, int c_hidden, int dtype, int direction,
+                                  void* o_block, void* scratch, void* stream);
+
+/*
  * Backward of step a4 (the O(N^3) part of training; the paper hand-writes
  * every backward with the forward's algorithm).  Given d_o = dL/do:
  *     outgoing  d_a[i][k] = sum_j d_o[i][j] b[j][k]     d_b[j][k] = sum_i d_o[i][j] a[i][k]

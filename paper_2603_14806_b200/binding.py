@@ -24,7 +24,7 @@ _lib = None
 EXPORTS = (
     "foldcp_trimul", "foldcp_trimul_batched", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
     "foldcp_trimul_contract", "foldcp_trimul_contract_backward", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
-    "foldcp_trimul_backward", "foldcp_trimul_backward_workspace_bytes",
+    "foldcp_trimul_backward", "foldcp_trimul_backward_workspace_bytes", "foldcp_trimul_contract_blocks",
     "foldcp_status_string", "foldcp_version",
 )
 
@@ -91,6 +91,9 @@ def load() -> ctypes.CDLL:
     lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp, vp]
     lib.foldcp_trimul_finalize.restype = ci
     lib.foldcp_trimul_finalize.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_contract_blocks.restype = ci
+    lib.foldcp_trimul_contract_blocks.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(vp), ci, ci, ci, ci, ci,
+                                                  vp, vp, vp]
     lib.foldcp_trimul_backward.restype = ci
     lib.foldcp_trimul_backward.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, ci, vp,
                                            ctypes.POINTER(_Grads), vp]
@@ -279,6 +282,32 @@ def contract(a: torch.Tensor, b: torch.Tensor, direction: int,
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_contract")
     return o
+
+
+def contract_blocks(a_blocks, b_blocks, direction: int, o_block: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Blocked (Cannon) contraction: o_block = sum_q contraction(a_blocks[q], b_blocks[q]); every
+    block a contiguous [c, nb, nb] channel-major tensor (fp32 / bf16 / fp16 like `contract`)."""
+    lib = load()
+    a0 = a_blocks[0]
+    c, nb = a0.shape[0], a0.shape[1]
+    assert len(a_blocks) == len(b_blocks) >= 1
+    for t in list(a_blocks) + list(b_blocks):
+        assert t.shape == a0.shape and t.dtype == a0.dtype
+    if a0.dtype == torch.float16:
+        code, o_dtype = BF16_F16AB, torch.bfloat16
+    else:
+        code, o_dtype = dtype_code(a0), a0.dtype
+    if o_block is None:
+        o_block = torch.empty(a0.shape, dtype=o_dtype, device=a0.device)
+    _check_tensors(a0, {}, tuple(a_blocks) + tuple(b_blocks) + (o_block,))
+    n = len(a_blocks)
+    pa = (ctypes.c_void_p * n)(*[t.data_ptr() for t in a_blocks])
+    pb = (ctypes.c_void_p * n)(*[t.data_ptr() for t in b_blocks])
+    st = lib.foldcp_trimul_contract_blocks(pa, pb, n, nb, c, code, int(direction), o_block.data_ptr(),
+                                           stage_scratch(a0.device).data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_contract_blocks")
+    return o_block
 
 
 def contract_backward(d_o: torch.Tensor, a: torch.Tensor, b: torch.Tensor, direction: int):

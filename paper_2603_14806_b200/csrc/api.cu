@@ -267,6 +267,37 @@ int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, in
   return contract_stage(a, b, N, dtype, direction, o, ab_f16, scratch, 0, s);
 }
 
+int foldcp_trimul_contract_blocks(const void* const* a_blocks, const void* const* b_blocks,
+                                  int nblocks, int nb, int c_hidden, int dtype, int direction,
+                                  void* o_block, void* scratch, void* stream) {
+  const bool ab_f16 = dtype == FOLDCP_BF16_F16AB;
+  if (ab_f16) {
+    if (!bf16_on_tensor_cores()) return FOLDCP_ERR_UNSUPPORTED;
+    dtype = FOLDCP_BF16;
+  }
+  int st = check_shape(nb, kChannels, c_hidden, dtype);
+  if (st != FOLDCP_OK) return st;
+  if (direction != FOLDCP_OUTGOING && direction != FOLDCP_INCOMING) return FOLDCP_ERR_INVALID_ARG;
+  if (!a_blocks || !b_blocks || !o_block || nblocks < 1) return FOLDCP_ERR_INVALID_ARG;
+  if (nblocks > kMaxContractBlocks) return FOLDCP_ERR_UNSUPPORTED;
+  if (!aligned16(o_block)) return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(nb) * nb * kChannels * elem_bytes(dtype);
+  for (int q = 0; q < nblocks; ++q) {
+    if (!a_blocks[q] || !b_blocks[q]) return FOLDCP_ERR_INVALID_ARG;
+    if (!aligned16(a_blocks[q]) || !aligned16(b_blocks[q])) return FOLDCP_ERR_ALIGNMENT;
+    if (overlaps(o_block, bytes, a_blocks[q], bytes) || overlaps(o_block, bytes, b_blocks[q], bytes))
+      return FOLDCP_ERR_ALIAS;
+  }
+  if ((st = check_scratch(scratch, dtype)) != FOLDCP_OK) return st;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
+  if (dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
+    return launch_k2_contract_blocks_bf16(a_blocks, b_blocks, nblocks, o_block, nb, direction,
+                                          ab_f16, sched_word(scratch, 0), s);
+  return launch_simt_contract_blocks(a_blocks, b_blocks, nblocks, o_block, nb, dtype, direction, s);
+}
+
 int foldcp_trimul_contract_backward(const void* d_o, const void* a, const void* b, int N,
                                     int c_hidden, int dtype, int direction, void* d_a, void* d_b,
                                     void* scratch, void* stream) {

@@ -71,6 +71,15 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
                             bool ab_f16, unsigned int* sched, cudaStream_t stream);
 
+// blocked (Cannon) form: o_block[c][nb][nb] = sum_q contraction(a_blocks[q], b_blocks[q]), each
+// block a dense [c][nb][nb] tensor, nq <= kMaxContractBlocks; accumulator resident in TMEM
+constexpr int kMaxContractBlocks = 4;
+int launch_k2_contract_blocks_bf16(const void* const* a_blocks, const void* const* b_blocks, int nq,
+                                   void* o_block, int nb, int direction, bool ab_f16,
+                                   unsigned int* sched, cudaStream_t stream);
+int launch_simt_contract_blocks(const void* const* a_blocks, const void* const* b_blocks, int nq,
+                                void* o_block, int nb, int dtype, int direction, cudaStream_t s);
+
 int launch_k2_contract_backward_bf16(const void* d_o, const void* a, const void* b, void* d_a,
                                      void* d_b, int N, int direction, unsigned int* sched0,
                                      unsigned int* sched1, cudaStream_t stream);

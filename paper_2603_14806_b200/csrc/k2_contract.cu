@@ -62,8 +62,24 @@ __device__ unsigned long long g_k2_probe[128][8];
 #define K2_PROBE_ADD(acc, t0)
 #endif
 
+// Operand blocks of one launch.  A launch contracts nq pairs of operand blocks into ONE output
+// block,  D = sum_q op(X_q) op(Y_q)^T,  with the accumulator resident in tensor memory across all of
+// them.  nq = 1 is the single-GPU op (whole tensors); nq = sqrt(P) is one rank's share of the
+// paper's Cannon-style distributed contraction: the q-th pair are the
+// blocks the rank multiplies in ring step q, each behind its own tensor map -- local memory or, on
+// an NVLink / NVSwitch node, a peer GPU's memory mapped into this address space (every peer is one
+// hop away, so the ring's store-and-forward shifts become direct TMA reads and "partial results
+// accumulate into the output block" without ever leaving TMEM).
+constexpr int kMaxBlocks = 4;   // a 4 x 4 context-parallel grid
+struct K2Maps {
+  CUtensorMap a[kMaxBlocks];
+  CUtensorMap b[kMaxBlocks];
+  CUtensorMap o;
+};
+
 struct K2Params {
   int N;
+  int nq;          // operand block pairs contracted by this launch (1 .. kMaxBlocks)
   int tiles_m;
   int tiles_n;
   int num_tiles;   // channels * tiles_m * tiles_n
@@ -96,9 +112,7 @@ __device__ __forceinline__ void decode_tile(const K2Params& prm, int r, int* tm,
 
 template <int kCtaGroup, bool kAMn, bool kBMn>
 __global__ void __launch_bounds__(kThreads, 1)
-k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
-                   const __grid_constant__ CUtensorMap tmap_b,
-                   const __grid_constant__ CUtensorMap tmap_o, const K2Params prm) {
+k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
   using C = Cfg<kCtaGroup>;
   extern __shared__ uint8_t smem_raw[];
   // 128-byte swizzle needs 1024-byte aligned tiles
@@ -124,9 +138,12 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
   const uint32_t cta_rank = (kCtaGroup == 2) ? ptx::cluster_ctarank() : 0u;
   const bool is_leader = cta_rank == 0;
 
+  const CUtensorMap& tmap_o = maps.o;
   if (warp == 0 && lane == 0) {
-    ptx::prefetch_tmap(&tmap_a);
-    ptx::prefetch_tmap(&tmap_b);
+    for (int q = 0; q < prm.nq; ++q) {
+      ptx::prefetch_tmap(&maps.a[q]);
+      ptx::prefetch_tmap(&maps.b[q]);
+    }
     ptx::prefetch_tmap(&tmap_o);
   }
   if (warp == 1 && lane == 0) {
@@ -221,6 +238,9 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
         decode_tile(prm, r, &tm, &tn);
         const int m0 = tm * C::kTileM + static_cast<int>(cta_rank) * 128;
         const int n0 = tn * kTileN + static_cast<int>(cta_rank) * (kTileN / kCtaGroup);
+        for (int q = 0; q < prm.nq; ++q) {
+        const CUtensorMap& tmap_a = maps.a[q];
+        const CUtensorMap& tmap_b = maps.b[q];
         for (int kb = 0; kb < prm.num_kb; ++kb) {
           K2_PROBE_T0(tw);
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
@@ -262,6 +282,7 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
             phase ^= 1u;
           }
         }
+        }
       }
 #ifdef FOLDCP_K2_PROBE
       if (is_leader) {
@@ -302,7 +323,8 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
 #endif
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kAccumCols;
-        for (int kb = 0; kb < prm.num_kb; ++kb) {
+        const int total_kb = prm.num_kb * prm.nq;      // the accumulator lives across all blocks
+        for (int kb = 0; kb < total_kb; ++kb) {
           K2_PROBE_T0(tf);
           ptx::mbar_wait(full_bar(stage), phase);
           K2_PROBE_ADD(w_full, tf);
@@ -414,8 +436,7 @@ k2_contract_kernel(const __grid_constant__ CUtensorMap tmap_a,
 }
 
 template <int kCtaGroup, bool kAMn, bool kBMn>
-int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& to,
-                   const K2Params& prm, int sm_count, cudaStream_t stream) {
+int launch_variant(const K2Maps& maps, const K2Params& prm, int sm_count, cudaStream_t stream) {
   using C = Cfg<kCtaGroup>;
   auto kern = k2_contract_kernel<kCtaGroup, kAMn, kBMn>;
   if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), C::kSmemBytes) != FOLDCP_OK)
@@ -434,7 +455,7 @@ int launch_variant(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorM
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  if (cudaLaunchKernelEx(&cfg, kern, ta, tb, to, prm) != cudaSuccess) return FOLDCP_ERR_CUDA;
+  if (cudaLaunchKernelEx(&cfg, kern, maps, prm) != cudaSuccess) return FOLDCP_ERR_CUDA;
   return FOLDCP_OK;
 }
 
@@ -442,13 +463,16 @@ int g_k2_cta_group = 2;
 
 }  // namespace
 
-// D_c = op(X_c) op(Y_c)^T per channel for the four operand layouts:
+// D_c = sum_q op(X_q,c) op(Y_q,c)^T per channel for the four operand layouts:
 //   x_mn = 0: X_c is [m][k] (k contiguous, K-major)    x_mn = 1: X_c is [k][m] (m contiguous)
 //   y_mn = 0: Y_c is [n][k]                            y_mn = 1: Y_c is [k][n]
-// i.e. d[c][m][n] = sum_k X(m, k) Y(n, k).  The forward contraction uses (0,0) / (1,1); its
-// gradients also need the mixed (0,1) form.
-int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn,
-                        bool xy_f16, unsigned int* sched, cudaStream_t stream) {
+// i.e. d[c][m][n] = sum_q sum_k X_q(m, k) Y_q(n, k); every block is a dense [c][N][N] tensor.  The
+// forward contraction uses (0,0) / (1,1); its gradients also need the mixed (0,1) form; nq > 1 is
+// the blocked (Cannon) form.
+int launch_k2_gemm_blocks_bf16(const void* const* x, const void* const* y, int nq, void* d, int N,
+                               bool x_mn, bool y_mn, bool xy_f16, unsigned int* sched,
+                               cudaStream_t stream) {
+  if (nq < 1 || nq > kMaxBlocks) return FOLDCP_ERR_UNSUPPORTED;
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   static const int cta_group = [] {
@@ -460,13 +484,20 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
   const uint64_t strides[2] = {n * 2, n * n * 2};
   const uint32_t box_ld[3] = {64, 64, 1};
   const uint32_t box_st[3] = {64, 128, 1};
-  CUtensorMap ta, tb, to;
+  K2Maps maps;
   int st;
-  if ((st = encode_tensor_map(&ta, x, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
-  if ((st = encode_tensor_map(&tb, y, 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK) return st;
-  if ((st = encode_tensor_map(&to, d, 2, 3, dims, strides, box_st, true)) != FOLDCP_OK) return st;
+  for (int q = 0; q < kMaxBlocks; ++q) {
+    const int src = q < nq ? q : 0;     // unused slots repeat block 0: never read, but well-formed
+    if ((st = encode_tensor_map(&maps.a[q], x[src], 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK)
+      return st;
+    if ((st = encode_tensor_map(&maps.b[q], y[src], 2, 3, dims, strides, box_ld, true)) != FOLDCP_OK)
+      return st;
+  }
+  if ((st = encode_tensor_map(&maps.o, d, 2, 3, dims, strides, box_st, true)) != FOLDCP_OK)
+    return st;
   K2Params prm;
   prm.N = N;
+  prm.nq = nq;
   const int tile_m = 128 * cta_group;
   prm.tiles_m = (N + tile_m - 1) / tile_m;
   prm.tiles_n = (N + kTileN - 1) / kTileN;
@@ -491,15 +522,30 @@ int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn,
   prm.ab_fmt = xy_f16 ? ptx::kFmtF16 : ptx::kFmtBF16;
   const int sms = dev.sm_count;
   if (cta_group == 2) {
-    if (x_mn) return y_mn ? launch_variant<2, true, true>(ta, tb, to, prm, sms, stream)
-                          : launch_variant<2, true, false>(ta, tb, to, prm, sms, stream);
-    return y_mn ? launch_variant<2, false, true>(ta, tb, to, prm, sms, stream)
-                : launch_variant<2, false, false>(ta, tb, to, prm, sms, stream);
+    if (x_mn) return y_mn ? launch_variant<2, true, true>(maps, prm, sms, stream)
+                          : launch_variant<2, true, false>(maps, prm, sms, stream);
+    return y_mn ? launch_variant<2, false, true>(maps, prm, sms, stream)
+                : launch_variant<2, false, false>(maps, prm, sms, stream);
   }
-  if (x_mn) return y_mn ? launch_variant<1, true, true>(ta, tb, to, prm, sms, stream)
-                        : launch_variant<1, true, false>(ta, tb, to, prm, sms, stream);
-  return y_mn ? launch_variant<1, false, true>(ta, tb, to, prm, sms, stream)
-              : launch_variant<1, false, false>(ta, tb, to, prm, sms, stream);
+  if (x_mn) return y_mn ? launch_variant<1, true, true>(maps, prm, sms, stream)
+                        : launch_variant<1, true, false>(maps, prm, sms, stream);
+  return y_mn ? launch_variant<1, false, true>(maps, prm, sms, stream)
+              : launch_variant<1, false, false>(maps, prm, sms, stream);
+}
+
+int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn,
+                        bool xy_f16, unsigned int* sched, cudaStream_t stream) {
+  return launch_k2_gemm_blocks_bf16(&x, &y, 1, d, N, x_mn, y_mn, xy_f16, sched, stream);
+}
+
+// One rank's share of the Cannon-style distributed contraction: o_block = sum_q of Eq. 2 / Eq. 3 on
+// the block pairs (a_blocks[q], b_blocks[q]).
+int launch_k2_contract_blocks_bf16(const void* const* a_blocks, const void* const* b_blocks, int nq,
+                                   void* o_block, int nb, int direction, bool ab_f16,
+                                   unsigned int* sched, cudaStream_t stream) {
+  const bool inc = direction == FOLDCP_INCOMING;
+  return launch_k2_gemm_blocks_bf16(a_blocks, b_blocks, nq, o_block, nb, inc, inc, ab_f16, sched,
+                                    stream);
 }
 
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,

@@ -114,18 +114,27 @@ simt_project_kernel(const T* __restrict__ z, const T* __restrict__ mask, const T
 // stage 2: per-channel contraction, 64 x 64 output tile per block, 16 x 16 threads, 4 x 4 each
 //   outgoing: o[i][j] = sum_k A[i][k] B[j][k]      incoming: o[i][j] = sum_k A[k][i] B[k][j]
 // ---------------------------------------------------------------------------------------------
+// nq operand block pairs are contracted into one output block (nq = 1: whole tensors; nq > 1: one
+// rank's share of the Cannon-style distributed contraction)
+struct BlockPtrs {
+  const void* a[kMaxContractBlocks];
+  const void* b[kMaxContractBlocks];
+  int nq;
+};
+
 template <typename T, bool kXMn, bool kYMn>
 __global__ void __launch_bounds__(256)
-simt_contract_kernel(const T* __restrict__ a, const T* __restrict__ b, T* __restrict__ o, int N) {
+simt_contract_kernel(const BlockPtrs blocks, T* __restrict__ o, int N) {
   constexpr int TS = 64, KS = 16;
   __shared__ float As[KS][TS + 1];
   __shared__ float Bs[KS][TS + 1];
   const long long chan = static_cast<long long>(blockIdx.z) * N * N;
-  const T* A = a + chan;
-  const T* B = b + chan;
   const int i0 = blockIdx.y * TS, j0 = blockIdx.x * TS;
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
   float acc[4][4] = {};
+  for (int q = 0; q < blocks.nq; ++q) {
+  const T* A = static_cast<const T*>(blocks.a[q]) + chan;
+  const T* B = static_cast<const T*>(blocks.b[q]) + chan;
   for (int k0 = 0; k0 < N; k0 += KS) {
     for (int e = threadIdx.x; e < TS * KS; e += 256) {
       // each operand is read along its contiguous index: [k][mn] when MN-major, [mn][k] otherwise
@@ -165,6 +174,7 @@ simt_contract_kernel(const T* __restrict__ a, const T* __restrict__ b, T* __rest
         for (int v = 0; v < 4; ++v) acc[u][v] = fmaf(ar[u], br[v], acc[u][v]);
     }
     __syncthreads();
+  }
   }
 #pragma unroll
   for (int u = 0; u < 4; ++u)
@@ -245,17 +255,28 @@ int project_t(const void* z, const void* mask, const foldcp_trimul_params* p, in
 
 // d[c][m][n] = sum_k X(m, k) Y(n, k); x_mn / y_mn: the operand is stored [k][m] / [k][n]
 template <typename T>
-int gemm_t(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn, cudaStream_t s) {
+int gemm_blocks_t(const void* const* x, const void* const* y, int nq, void* d, int N, bool x_mn,
+                  bool y_mn, cudaStream_t s) {
+  if (nq < 1 || nq > kMaxContractBlocks) return FOLDCP_ERR_UNSUPPORTED;
   const unsigned t = (N + 63) / 64;
   dim3 grid(t, t, C);
-  const T* X = static_cast<const T*>(x);
-  const T* Y = static_cast<const T*>(y);
+  BlockPtrs bp;
+  bp.nq = nq;
+  for (int q = 0; q < kMaxContractBlocks; ++q) {
+    bp.a[q] = x[q < nq ? q : 0];
+    bp.b[q] = y[q < nq ? q : 0];
+  }
   T* D = static_cast<T*>(d);
-  if (x_mn && y_mn) simt_contract_kernel<T, true, true><<<grid, 256, 0, s>>>(X, Y, D, N);
-  else if (x_mn) simt_contract_kernel<T, true, false><<<grid, 256, 0, s>>>(X, Y, D, N);
-  else if (y_mn) simt_contract_kernel<T, false, true><<<grid, 256, 0, s>>>(X, Y, D, N);
-  else simt_contract_kernel<T, false, false><<<grid, 256, 0, s>>>(X, Y, D, N);
+  if (x_mn && y_mn) simt_contract_kernel<T, true, true><<<grid, 256, 0, s>>>(bp, D, N);
+  else if (x_mn) simt_contract_kernel<T, true, false><<<grid, 256, 0, s>>>(bp, D, N);
+  else if (y_mn) simt_contract_kernel<T, false, true><<<grid, 256, 0, s>>>(bp, D, N);
+  else simt_contract_kernel<T, false, false><<<grid, 256, 0, s>>>(bp, D, N);
   return check_launch();
+}
+
+template <typename T>
+int gemm_t(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn, cudaStream_t s) {
+  return gemm_blocks_t<T>(&x, &y, 1, d, N, x_mn, y_mn, s);
 }
 
 template <typename T>
@@ -301,6 +322,13 @@ int launch_simt_contract(const void* a, const void* b, void* o, int N, int dtype
                          cudaStream_t s) {
   return dtype == FOLDCP_F32 ? contract_t<float>(a, b, o, N, direction, s)
                              : contract_t<__nv_bfloat16>(a, b, o, N, direction, s);
+}
+int launch_simt_contract_blocks(const void* const* a_blocks, const void* const* b_blocks, int nq,
+                                void* o_block, int nb, int dtype, int direction, cudaStream_t s) {
+  const bool inc = direction == FOLDCP_INCOMING;
+  return dtype == FOLDCP_F32
+             ? gemm_blocks_t<float>(a_blocks, b_blocks, nq, o_block, nb, inc, inc, s)
+             : gemm_blocks_t<__nv_bfloat16>(a_blocks, b_blocks, nq, o_block, nb, inc, inc, s);
 }
 int launch_simt_contract_backward(const void* d_o, const void* a, const void* b, void* d_a,
                                   void* d_b, int N, int dtype, int direction, cudaStream_t s) {
