@@ -370,12 +370,20 @@ int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* p
   return finalize_stage(o, z, mask, params, N, out, s);
 }
 
+namespace {
+// staged weights + per-block partial sums: the larger of the CUDA-core and the tcgen05 tail's needs
+size_t backward_scratch_bytes() {
+  const size_t a = backward_scratch_floats(kMaxBackwardBlocks), b = backward_tc_scratch_floats();
+  return ((a > b ? a : b) * sizeof(float) + 255) & ~static_cast<size_t>(255);
+}
+}  // namespace
+
 size_t foldcp_trimul_backward_workspace_bytes(int N, int c_z, int c_hidden, int dtype) {
   if (check_shape(N, c_z, c_hidden, dtype) != FOLDCP_OK) return 0;
   const size_t pairs = static_cast<size_t>(N) * N;
   return 5 * pairs * kChannels * elem_bytes(dtype)            // a, b, o / d_o, d_a, d_b
          + pairs * kChannels * sizeof(float)                  // d_z' accumulator
-         + backward_scratch_floats(kMaxBackwardBlocks) * sizeof(float) + kSchedScratchBytes;
+         + backward_scratch_bytes() + kSchedScratchBytes;
 }
 
 int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
@@ -416,7 +424,7 @@ int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
   void* d_b = ws + 4 * tb;
   float* dzp = reinterpret_cast<float*>(ws + 5 * tb);
   float* scratch = dzp + static_cast<size_t>(N) * N * kChannels;
-  void* sched_area = scratch + backward_scratch_floats(kMaxBackwardBlocks);
+  void* sched_area = reinterpret_cast<uint8_t*>(scratch) + backward_scratch_bytes();
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const int dt = params->dtype;
   if (dt == FOLDCP_BF16 && (st = arm_sched_words(sched_area, s)) != FOLDCP_OK) return st;
@@ -425,23 +433,26 @@ int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
   if ((st = project_stage(z, mask, params, N, a, b, false, sched_area, s)) != FOLDCP_OK) return st;
   if ((st = contract_stage(a, b, N, dt, direction, o, false, sched_area, 1, s)) != FOLDCP_OK)
     return st;
+  // the tail around the contraction: tcgen05 kernels in bf16 mode, CUDA-core kernels in fp32 mode
+  const bool tc = dt == FOLDCP_BF16 && bf16_on_tensor_cores();
+  auto tail = [&](int phase) {
+    return tc ? launch_tc_tail_backward(phase, d_out, z, mask, params, N, o, d_a, d_b, dzp, scratch,
+                                        grads, d_z, s)
+              : launch_simt_tail_backward(phase, d_out, z, mask, params, N, o, d_a, d_b, dzp,
+                                          scratch, grads, d_z, s);
+  };
   // K3-backward: o -> d_o in place
-  if ((st = launch_simt_tail_backward(0, d_out, z, mask, params, N, o, nullptr, nullptr, dzp,
-                                      scratch, grads, d_z, s)) != FOLDCP_OK)
-    return st;
+  if ((st = tail(0)) != FOLDCP_OK) return st;
   // gradients of Eq. 2-3
-  if (dt == FOLDCP_BF16 && bf16_on_tensor_cores())
+  if (tc)
     st = launch_k2_contract_backward_bf16(o, a, b, d_a, d_b, N, direction,
                                           sched_word(sched_area, 2), sched_word(sched_area, 3), s);
   else
     st = launch_simt_contract_backward(o, a, b, d_a, d_b, N, dt, direction, s);
   if (st != FOLDCP_OK) return st;
   // K1-backward for a, then for b (closing with the LayerNorm(z) backward)
-  if ((st = launch_simt_tail_backward(1, d_out, z, mask, params, N, o, d_a, d_b, dzp, scratch,
-                                      grads, d_z, s)) != FOLDCP_OK)
-    return st;
-  return launch_simt_tail_backward(2, d_out, z, mask, params, N, o, d_a, d_b, dzp, scratch, grads,
-                                   d_z, s);
+  if ((st = tail(1)) != FOLDCP_OK) return st;
+  return tail(2);
 }
 
 int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_params* params,

@@ -109,6 +109,14 @@ int launch_simt_tail_backward(int phase, const void* d_out, const void* z, const
                               const void* d_b, float* dzp, float* scratch,
                               const foldcp_trimul_grads* g, void* d_z, cudaStream_t s);
 
+// The same three phases on tcgen05 (k_backward.cu, bf16 mode); phase 2 also assembles all
+// parameter gradients.  `scratch`: backward_tc_scratch_floats() floats.
+size_t backward_tc_scratch_floats();
+int launch_tc_tail_backward(int phase, const void* d_out, const void* z, const void* mask,
+                            const foldcp_trimul_params* p, int N, void* o_io, const void* d_a,
+                            const void* d_b, float* dzp, float* scratch,
+                            const foldcp_trimul_grads* g, void* d_z, cudaStream_t s);
+
 // Opt a kernel in to `bytes` of dynamic shared memory, once per (kernel, device); thread-safe.
 // Returns FOLDCP_OK or FOLDCP_ERR_CUDA.
 int ensure_dynamic_smem(const void* kernel, int bytes);

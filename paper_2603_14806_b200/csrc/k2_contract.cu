@@ -45,8 +45,9 @@ struct Cfg {
   static constexpr int kBBytes = kBBoxes * kBoxBytes;
   static constexpr int kStageBytes = kABytes + kBBytes;          // 48 KB or 32 KB
   static constexpr int kStages = kCtaGroup == 1 ? 4 : 6;
+  static constexpr int kEpiBytes = 2 * kEpiBufBytes;
   static constexpr int kBarBytes = 1024;
-  static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kEpiBufBytes + kBarBytes + 1024;
+  static constexpr int kSmemBytes = kStages * kStageBytes + kEpiBytes + kBarBytes + 1024;
 };
 
 #ifdef FOLDCP_K2_PROBE
@@ -119,7 +120,7 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t stage_base = smem_base;
   const uint32_t epi_base = smem_base + C::kStages * C::kStageBytes;
-  const uint32_t bar_base = epi_base + 2 * kEpiBufBytes;
+  const uint32_t bar_base = epi_base + C::kEpiBytes;
   // barrier layout (8 bytes each)
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (C::kStages + s); };
@@ -154,6 +155,7 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
     for (int s = 0; s < kRing; ++s) {
       ptx::mbar_init(tsfull_bar(s), 1);
       ptx::mbar_init(tsempty_bar(s), 5 * kCtaGroup);   // every consumer of both CTAs, see below
+      ptx::sts32(tile_slot(s), 0xfffffffeu);           // sentinel: "nothing published yet"
     }
     for (int s = 0; s < 2; ++s) {
       ptx::mbar_init(tfull_bar(s), 1);
@@ -186,32 +188,62 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
   // pair under the hardware scheduler).  In-order dispatch keeps the window of tiles in flight
   // compact.  Every tile is computed the same way whichever pair gets it: results stay bitwise
   // reproducible.
-  // The leader's producer thread draws the index and writes it into a 4-deep ring in both CTAs;
+  // The leader's producer thread draws the index (draw_tile / publish_tile below) and writes it into
+  // a 4-deep ring in both CTAs;
   // every other consumer (peer producer, MMA issuer, epilogue warps) waits on its local "full"
   // barrier, reads it and releases the entry on the leader's "empty" barrier.  -1 = no more tiles.
+  //
+  // No cluster-scope release / acquire anywhere on this path: ptxas turns
+  // mbarrier.arrive.release.cluster into MEMBAR.ALL.GPU + ERRBAR + CGAERRBAR (~3000 cycles), and
+  // one of those per tile in the MMA issuer (measured: 8.5 % of its time at N = 4096) and in the
+  // peer's producer drained the operand pipeline at every tile boundary.  Instead:
+  //   leader CTA   slot + "full" barrier in its own shared memory: CTA-scope release / acquire;
+  //   peer CTA     the leader stores the index into the peer's slot with a plain st.shared::cluster
+  //                and the peer's consumers poll the word itself (volatile load) until it differs
+  //                from the value they saw in that slot one ring round earlier -- tile indices only
+  //                grow within a launch and -1 ends it, so the value is its own flag;
+  //   "empty"      consumers signal with a relaxed arrive (remote for the peer): they publish
+  //                nothing, they only report that the slot has been read.
+  // last_seen[s]: the value this thread consumed from ring slot s (peer only); starts at the
+  // sentinel the slots are initialised with.
+  constexpr uint32_t kSlotSentinel = 0xfffffffeu;
+  uint32_t last_seen[kRing];
+#pragma unroll
+  for (int s = 0; s < kRing; ++s) last_seen[s] = kSlotSentinel;
   auto consume_tile = [&](int i) -> int {
     const int s = i % kRing;
-    ptx::mbar_wait_cluster(tsfull_bar(s), (i / kRing) & 1);
     uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(tile_slot(s)) : "memory");
-    if constexpr (kCtaGroup == 2) {
-      ptx::mbar_arrive_cluster(ptx::mapa(tsempty_bar(s), 0));
-    } else {
+    if (is_leader) {
+      ptx::mbar_wait(tsfull_bar(s), (i / kRing) & 1);
+      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(tile_slot(s)) : "memory");
       ptx::mbar_arrive(tsempty_bar(s));
+    } else {
+      uint32_t seen = kSlotSentinel;
+#pragma unroll
+      for (int k = 0; k < kRing; ++k) seen = (k == s) ? last_seen[k] : seen;
+      do {
+        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(tile_slot(s)) : "memory");
+      } while (v == seen);
+#pragma unroll
+      for (int k = 0; k < kRing; ++k) last_seen[k] = (k == s) ? v : last_seen[k];
+      ptx::mbar_arrive_relaxed_cluster(ptx::mapa(tsempty_bar(s), 0));
     }
     return static_cast<int>(v);
   };
-  auto produce_tile = [&](int i) -> int {
+  // Drawing and publishing are split: the atomic is issued at the start of a tile's loads and its
+  // result is only needed when that tile's loads have all been issued, so its ~1 us round trip to
+  // L2 overlaps the producer's own work instead of holding back the first loads of the tile.
+  auto draw_tile = [&](int i) -> unsigned int {
+    ptx::mbar_wait(tsempty_bar(i % kRing), ((i / kRing) & 1) ^ 1u);
+    return atomicAdd(prm.sched, 1u);
+  };
+  auto publish_tile = [&](int i, unsigned int drawn) -> int {
     const int s = i % kRing;
-    ptx::mbar_wait_cluster(tsempty_bar(s), ((i / kRing) & 1) ^ 1u);
-    const unsigned int drawn = atomicAdd(prm.sched, 1u);
     const int tile = drawn < static_cast<unsigned int>(prm.num_tiles) ? static_cast<int>(drawn) : -1;
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(tile_slot(s)), "r"(tile) : "memory");
-    ptx::mbar_arrive_release_cluster_local(tsfull_bar(s));
-    if constexpr (kCtaGroup == 2) {
+    ptx::mbar_arrive(tsfull_bar(s));
+    if constexpr (kCtaGroup == 2)
       ptx::st_shared_cluster_u32(ptx::mapa(tile_slot(s), 1), static_cast<uint32_t>(tile));
-      ptx::mbar_arrive_cluster(ptx::mapa(tsfull_bar(s), 1));
-    }
     return tile;
   };
 
@@ -226,12 +258,13 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
       long long pr_wait = 0;
       const long long pr_t0 = clock64();
 #endif
-      // the leader draws one tile ahead, so the atomic's round trip never stalls the load pipeline
-      int tnext = is_leader ? produce_tile(0) : consume_tile(0);
+      // the leader draws the next tile while it issues this tile's loads and publishes it afterwards
+      int tnext = is_leader ? publish_tile(0, draw_tile(0)) : consume_tile(0);
       for (int it = 0;; ++it) {
         const int t = tnext;
         if (t < 0) break;
-        tnext = is_leader ? produce_tile(it + 1) : consume_tile(it + 1);
+        unsigned int drawn = 0;
+        if (is_leader) drawn = draw_tile(it + 1);
         const int ch = t / tiles_per_ch;
         const int r = t - ch * tiles_per_ch;
         int tm, tn;
@@ -283,6 +316,7 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
           }
         }
         }
+        tnext = is_leader ? publish_tile(it + 1, drawn) : consume_tile(it + 1);
       }
 #ifdef FOLDCP_K2_PROBE
       if (is_leader) {
@@ -316,7 +350,7 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
         const int as = it & 1;
         const uint32_t aphase = (it >> 1) & 1;
         K2_PROBE_T0(te);
-        ptx::mbar_wait_cluster(tempty_bar(as), aphase ^ 1u);
+        ptx::mbar_wait(tempty_bar(as), aphase ^ 1u);
         K2_PROBE_ADD(w_tempty, te);
 #ifdef FOLDCP_K2_PROBE
         ++ntiles;
@@ -392,10 +426,12 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
           ptx::tc_fence_before();
           __syncwarp();
           if (lane == 0) {
-            if constexpr (kCtaGroup == 2) {
-              ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(as), 0));
-            } else {
+            // (tcgen05.wait::ld + fence::before_thread_sync above order the TMEM reads; the
+            // arrive itself publishes nothing, so it is relaxed when it goes to the leader CTA)
+            if (is_leader) {
               ptx::mbar_arrive(tempty_bar(as));
+            } else {
+              ptx::mbar_arrive_relaxed_cluster(ptx::mapa(tempty_bar(as), 0));
             }
           }
         }

@@ -80,7 +80,14 @@ struct K3Params {
   float eps;
   long long R;
   int num_tiles;
+  int dbg_skip;                // debug builds only: 1 skip LN(z) math, 2 skip LN(o) math, 4 skip epilogue math
 };
+
+#ifdef FOLDCP_DEBUG_KNOBS
+#define K3_DBG_SKIP(bit) ((prm.dbg_skip & (bit)) != 0)
+#else
+#define K3_DBG_SKIP(bit) false
+#endif
 
 template <bool kTanhSigmoid>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -261,7 +268,8 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      layernorm_rows_inplace<kNormFp16, false, 1, kLnzWarps * 32>(smem + kOffStage + s * kStageBytes, kHalfBox,
+      if (!K3_DBG_SKIP(1))
+        layernorm_rows_inplace<kNormFp16, false, 1, kLnzWarps * 32>(smem + kOffStage + s * kStageBytes, kHalfBox,
                                                        r, 0, 0, prm.eps);
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
@@ -292,6 +300,11 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const int s = it & 1;
       ptx::mbar_wait(full(s), (it >> 1) & 1);
       const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes;
+      if (K3_DBG_SKIP(2)) {
+        ptx::fence_proxy_async_smem();
+        ptx::mbar_arrive(oready(s));
+        continue;
+      }
       uint32_t w[32];
 #pragma unroll
       for (uint32_t g = 0; g < 4; ++g)
@@ -396,6 +409,10 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           if (lane == 0) ptx::mbar_arrive(tempty(slot));
         }
         uint32_t packed[8];
+        if (K3_DBG_SKIP(4)) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) packed[i] = vo[2 * i] ^ vg[2 * i + 1];
+        } else {
 #pragma unroll
         for (int j4 = 0; j4 < 4; ++j4) {
           ptx::f32x2 bg2[2], bo2[2];
@@ -420,6 +437,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
             }
             packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
           }
+        }
         }
         if (chunk == 0) {
           if (store_thread) ptx::tma_store_wait_read<0>();
@@ -498,6 +516,11 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   prm.eps = p->ln_eps;
   prm.R = static_cast<long long>(R);
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
+  static const int dbg_skip = [] {
+    const char* e = debug_env("FOLDCP_K3_SKIP");
+    return e ? atoi(e) : 0;
+  }();
+  prm.dbg_skip = dbg_skip;
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k3_tanh_sigmoid();
   auto kern = tanh_sig ? k3_finalize_kernel<true> : k3_finalize_kernel<false>;
