@@ -85,7 +85,8 @@ struct K2Params {
   int tiles_n;
   int num_tiles;   // channels * tiles_m * tiles_n
   int num_kb;      // ceil(N / 64)
-  int l2_hints;    // 1: evict_last loads / evict_first stores
+  int l2_hints;    // 1: evict_last loads / evict_first stores; 2: stores only; 3: B evict_last, o evict_first
+  int serpentine;  // 1: odd column panels sweep their m-tiles downwards
   int panel_n;     // tile rasterisation: n-tiles per column panel (>= 1)
   unsigned int* sched;   // next tile index: launch-private, zeroed on the stream before the launch
   uint32_t ab_fmt;       // operand format of both inputs: ptx::kFmtBF16 or ptx::kFmtF16
@@ -101,8 +102,10 @@ __device__ __forceinline__ void decode_tile(const K2Params& prm, int r, int* tm,
   if (r < in_full) {
     const int p = r / (prm.tiles_m * w);
     const int q = r - p * prm.tiles_m * w;
-    *tm = q / w;
-    *tn = p * w + (q - (q / w) * w);
+    const int row = q / w;
+    // serpentine: the A row blocks the previous panel touched last are the first ones of this panel
+    *tm = (prm.serpentine && (p & 1)) ? prm.tiles_m - 1 - row : row;
+    *tn = p * w + (q - row * w);
   } else {
     const int q = r - in_full;
     const int wl = prm.tiles_n - full * w;
@@ -252,6 +255,7 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
     if (ptx::elect_one()) {
       // a_c / b_c are re-read by every tile of channel c: keep them in L2, stream o past them
       const uint64_t pol_ld = prm.l2_hints == 1 ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
+      const uint64_t pol_ld_b = (prm.l2_hints == 1 || prm.l2_hints == 3) ? ptx::kL2EvictLast : ptx::kL2EvictNormal;
       int stage = 0;
       uint32_t phase = 0;
 #ifdef FOLDCP_K2_PROBE
@@ -305,9 +309,9 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
             const int c0 = kBMn ? mn : k0;
             const int c1 = kBMn ? k0 : mn;
             if constexpr (kCtaGroup == 2) {
-              ptx::tma_load_3d_2sm_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld);
+              ptx::tma_load_3d_2sm_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld_b);
             } else {
-              ptx::tma_load_3d_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld);
+              ptx::tma_load_3d_hint(sb + bx * kBoxBytes, &tmap_b, bar, c0, c1, ch, pol_ld_b);
             }
           }
           if (++stage == C::kStages) {
@@ -551,9 +555,18 @@ int launch_k2_gemm_blocks_bf16(const void* const* x, const void* const* y, int n
   // Default rasterisation (measured with the in-order scheduler): plain row-major while one row
   // of tiles spans at most 16 n-tiles (N <= 4096: 9 GB of DRAM reads for 8.6 GB of operands);
   // beyond that, column panels of 8 n-tiles, so that the ~74 tiles in flight keep sharing one
-  // narrow B panel (N = 8192: 104 GB instead of 554 GB, 105 instead of 132 ms).
+  // narrow B panel (N = 8192: 104 GB instead of 554 GB, 105 instead of 132 ms).  Wider panels
+  // read MORE (12: 127 GB, 16: 162 GB, 24: 232 GB, also with evict_last on the B loads): a 64 MB
+  // panel does not stay resident in the 126 MB L2 next to the streaming A blocks and o stores.
   const int auto_panel = prm.tiles_n <= 16 ? prm.tiles_n : 8;
   prm.panel_n = (panel >= 1 && panel < prm.tiles_n) ? panel : auto_panel;
+  // odd panels sweep their m-tiles downwards, so the A row blocks still in L2 from the end of the
+  // previous sweep are re-used first (N = 8192: 107 instead of 115 GB of DRAM reads, time neutral)
+  static const int serp = [] {
+    const char* e = debug_env("FOLDCP_K2_SERP");
+    return e ? atoi(e) : 1;
+  }();
+  prm.serpentine = serp;
   prm.sched = sched;
   prm.ab_fmt = xy_f16 ? ptx::kFmtF16 : ptx::kFmtBF16;
   const int sms = dev.sm_count;

@@ -88,6 +88,23 @@ __device__ __forceinline__ uint32_t tile_addr(uint32_t tile, uint32_t row, uint3
   return tile + box * kHalfBox + row * 128u + ((((c >> 3) ^ (row & 7u))) << 4) + (c & 7u) * 2u;
 }
 
+// All elements (row = 0..127) of ONE column of such a tile: the eight swizzle phases are folded into
+// eight per-thread offsets once, so that an access costs one add (row = 8 g + j -> g * 1024 + off[j]).
+struct ColAccess {
+  uint32_t base;
+  uint32_t off[8];
+  __device__ __forceinline__ ColAccess(uint32_t tile, uint32_t col) {
+    const uint32_t c = col & 63u;
+    base = tile + (col >> 6) * kHalfBox + (c & 7u) * 2u;
+#pragma unroll
+    for (uint32_t j = 0; j < 8; ++j) off[j] = j * 128u + (((c >> 3) ^ j) << 4);
+  }
+  // row must be a compile-time expression modulo 8 for the offset to stay in a register
+  __device__ __forceinline__ uint32_t addr(uint32_t row) const {
+    return base + (row >> 3) * 1024u + off[row & 7u];
+  }
+};
+
 __device__ __forceinline__ float lds_bf16(uint32_t addr) {
   unsigned short v;
   asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
@@ -140,9 +157,11 @@ __device__ __forceinline__ void normalise_rows(uint32_t tile, int tid, float eps
 // ROWS for every column.  Thread = 1 pair x 64 channels (two threads per pair).
 __device__ __forceinline__ void normalise_cols(uint32_t tile, int tid, float eps, float* rstd_out) {
   const uint32_t p = static_cast<uint32_t>(tid & 127), h = static_cast<uint32_t>(tid >> 7);
+  const ColAccess col(tile, p);
+  const uint32_t hb = h * 64u * 128u;                 // rows 64 h ..: 64 rows of 128 bytes
   float x[64];
 #pragma unroll
-  for (uint32_t i = 0; i < 64; ++i) x[i] = lds_bf16(tile_addr(tile, h * 64u + i, p));
+  for (uint32_t i = 0; i < 64; ++i) x[i] = lds_bf16(col.addr(i) + hb);
   float s = 0.f;
 #pragma unroll
   for (int i = 0; i < 64; ++i) s += x[i];
@@ -158,8 +177,9 @@ __device__ __forceinline__ void normalise_cols(uint32_t tile, int tid, float eps
   __syncthreads();
   const float rstd = rsqrtf((xch[1][0][p] + xch[1][1][p]) * (1.0f / kC) + eps);
   if (h == 0) rstd_out[p] = rstd;
+  const float nm = -mu * rstd;
 #pragma unroll
-  for (uint32_t i = 0; i < 64; ++i) sts_bf16(tile_addr(tile, h * 64u + i, p), (x[i] - mu) * rstd);
+  for (uint32_t i = 0; i < 64; ++i) sts_bf16(col.addr(i) + hb, fmaf(x[i], rstd, nm));
 }
 
 // D[tmem] (+)= A * B for 128 x 128 x 128 operand tiles of the four layouts used here.
@@ -319,6 +339,8 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
     // ---------------- epilogue 1: chain rule through gate / projection; thread = (pair r, half h)
     {
       const float mv = msk[r];
+      const ColAccess xcol(XT, static_cast<uint32_t>(r));
+      (void)xcol;
 #pragma unroll 1
       for (int chunk = 0; chunk < 4; ++chunk) {
         const int c0 = h * 64 + chunk * 16;
@@ -340,7 +362,8 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
           }
         } else {
 #pragma unroll
-          for (int j = 0; j < 16; ++j) up[j] = lds_bf16(tile_addr(XT, c0 + j, r)) * mv;
+          for (int j = 0; j < 16; ++j)
+            up[j] = lds_bf16(xcol.addr(j) + static_cast<uint32_t>(c0) * 128u) * mv;   // c0 % 16 == 0
         }
         uint32_t pg[8], ph[8];
 #pragma unroll
@@ -393,12 +416,14 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
     }
     // bias gradients: column sums of GT (threads 0..127) and HT (128..255) over the tile's pairs
     {
-      const uint32_t tile = tid < 128 ? GT : HT;
-      const uint32_t col = static_cast<uint32_t>(tid & 127);
-      float s = 0.f;
-#pragma unroll 8
-      for (uint32_t p = 0; p < 128; ++p) s += lds_bf16(tile_addr(tile, p, col));
-      db_acc += s;
+      const ColAccess col(tid < 128 ? GT : HT, static_cast<uint32_t>(tid & 127));
+      float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+      for (uint32_t p = 0; p < 128; p += 2) {
+        s0 += lds_bf16(col.addr(p));
+        s1 += lds_bf16(col.addr(p + 1));
+      }
+      db_acc += s0 + s1;
     }
     ptx::mbar_wait(mma_bar, mma_phase);
     mma_phase ^= 1u;
@@ -408,16 +433,18 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
       if (warp < 4) {
         // d_o = rstd (d_ohat - mean(d_ohat) - ohat mean(d_ohat ohat)), written over ohat [k][p]
         float m1 = 0.f, m2 = 0.f;
+        const ColAccess ocol(XT, static_cast<uint32_t>(r));
 #pragma unroll 1
         for (int chunk = 0; chunk < 4; ++chunk) {
           uint32_t v[32];
           ptx::tmem_ld_32x32(lane_base + kTmemD0 + chunk * 32, v);
           ptx::tmem_ld_wait();
+          const uint32_t cb = static_cast<uint32_t>(chunk) * 4096u;     // 32 rows of 128 bytes
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             const float d = __uint_as_float(v[j]);
             m1 += d;
-            m2 = fmaf(d, lds_bf16(tile_addr(XT, chunk * 32 + j, r)), m2);
+            m2 = fmaf(d, lds_bf16(ocol.addr(j) + cb), m2);
           }
         }
         m1 *= (1.0f / kC);
@@ -428,9 +455,10 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
           uint32_t v[32];
           ptx::tmem_ld_32x32(lane_base + kTmemD0 + chunk * 32, v);
           ptx::tmem_ld_wait();
+          const uint32_t cb = static_cast<uint32_t>(chunk) * 4096u;
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
-            const uint32_t a = tile_addr(XT, chunk * 32 + j, r);
+            const uint32_t a = ocol.addr(j) + cb;
             sts_bf16(a, rs * (__uint_as_float(v[j]) - m1 - lds_bf16(a) * m2));
           }
         }
@@ -485,11 +513,25 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
         } else {
           // total d_zhat, then d_z = rstd (d_zhat - mean(d_zhat) - zhat mean(d_zhat zhat)) [+ d_out]
           float m1 = 0.f, m2 = 0.f;
+          auto load_xhat = [&](int chunk, float (&xh)[32]) {
+#pragma unroll
+            for (int c8 = 0; c8 < 4; ++c8) {
+              uint32_t w[4];
+              ptx::lds128(tile_addr(ZT, r, chunk * 32 + c8 * 8), w);
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                xh[c8 * 8 + 2 * e] = ptx::bf16_lo(w[e]);
+                xh[c8 * 8 + 2 * e + 1] = ptx::bf16_hi(w[e]);
+              }
+            }
+          };
 #pragma unroll 1
           for (int chunk = 0; chunk < 4; ++chunk) {
             uint32_t v[32];
             ptx::tmem_ld_32x32(lane_base + kTmemD0 + chunk * 32, v);
             ptx::tmem_ld_wait();
+            float xh[32];
+            load_xhat(chunk, xh);
             const float4* src = reinterpret_cast<const float4*>(prm.dzp + p * kC + chunk * 32);
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -499,7 +541,7 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
 #pragma unroll
               for (int e = 0; e < 4; ++e) {
                 m1 += d[e];
-                m2 = fmaf(d[e], lds_bf16(tile_addr(ZT, r, chunk * 32 + 4 * j + e)), m2);
+                m2 = fmaf(d[e], xh[4 * j + e], m2);
               }
             }
           }
@@ -512,19 +554,20 @@ tail_backward_kernel(const __grid_constant__ CUtensorMap tmap_z,     // z   [R][
             ptx::tmem_ld_32x32(lane_base + kTmemD0 + chunk * 32, v);
             ptx::tmem_ld_wait();
             if (live) {
+              float xh[32];
+              load_xhat(chunk, xh);
               const float4* src = reinterpret_cast<const float4*>(prm.dzp + p * kC + chunk * 32);
               uint4* dst = reinterpret_cast<uint4*>(prm.d_z + p * kC + chunk * 32);
               const uint4* res = reinterpret_cast<const uint4*>(prm.d_out + p * kC + chunk * 32);
 #pragma unroll
               for (int j8 = 0; j8 < 4; ++j8) {
+                const float4 c0 = src[2 * j8], c1 = src[2 * j8 + 1];
+                const float cur[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
                 float o[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                   const int k = j8 * 8 + e;
-                  const float4 cur = src[k >> 2];
-                  const float c = (k & 3) == 0 ? cur.x : (k & 3) == 1 ? cur.y : (k & 3) == 2 ? cur.z : cur.w;
-                  const float d = c + __uint_as_float(v[k]);
-                  o[e] = rs * (d - m1 - lds_bf16(tile_addr(ZT, r, chunk * 32 + k)) * m2);
+                  o[e] = rs * (cur[e] + __uint_as_float(v[k]) - m1 - xh[k] * m2);
                 }
                 if (prm.add_residual) {
                   const uint4 rv = __ldg(res + j8);
