@@ -374,8 +374,9 @@ def run_ours(args):
 
     # ---- per-stage durations inside a timed region (stage entry points, same kernels, same stream)
     tb = C * N * N * 2
-    a = ws[:tb].view(torch.bfloat16).view(C, N, N)
-    b = ws[tb: 2 * tb].view(torch.bfloat16).view(C, N, N)
+    # the project stage writes a, b as fp16 in bf16 mode; the contract stage is told so (BF16_F16AB)
+    a = ws[:tb].view(torch.float16).view(C, N, N)
+    b = ws[tb: 2 * tb].view(torch.float16).view(C, N, N)
     o = ws[2 * tb: 3 * tb].view(torch.bfloat16).view(C, N, N)
     scratch = B.stage_scratch(dev)
     import ctypes
@@ -391,7 +392,7 @@ def run_ours(args):
             st = lib.foldcp_trimul_project(z.data_ptr(), M.data_ptr(), ctypes.byref(prm), N, C, C,
                                            a.data_ptr(), b.data_ptr(), scratch.data_ptr(), stream)
             ev[1].record()
-            st |= lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, C, B.BF16, d,
+            st |= lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, C, B.BF16_F16AB, d,
                                              o.data_ptr(), scratch.data_ptr(), stream)
             ev[2].record()
             st |= lib.foldcp_trimul_finalize(o.data_ptr(), z.data_ptr(), M.data_ptr(),
