@@ -220,9 +220,10 @@ int contract_stage(const void* a, const void* b, int N, int dtype, int direction
   return launch_simt_contract(a, b, o, N, dtype, direction, s);
 }
 int finalize_stage(const void* o, const void* z, const void* mask,
-                   const foldcp_trimul_params* params, int N, void* out, cudaStream_t s) {
+                   const foldcp_trimul_params* params, int N, void* out, bool o_f16, float o_scale,
+                   cudaStream_t s) {
   if (params->dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
-    return launch_k3_finalize_bf16(o, z, mask, params, N, out, s);
+    return launch_k3_finalize_bf16(o, z, mask, params, N, out, o_f16, o_scale, s);
   return launch_simt_finalize(o, z, mask, params, N, out, s);
 }
 }  // namespace
@@ -334,7 +335,7 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
   const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
   if (overlaps(out, bytes, z, bytes) || overlaps(out, bytes, o, bytes)) return FOLDCP_ERR_ALIAS;
   if ((st = check_arch()) != FOLDCP_OK) return st;
-  return finalize_stage(o, z, mask, params, N, out, static_cast<cudaStream_t>(stream));
+  return finalize_stage(o, z, mask, params, N, out, false, 1.0f, static_cast<cudaStream_t>(stream));
 }
 
 int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
@@ -367,7 +368,7 @@ int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* p
   if ((st = contract_stage(a, b, N, params->dtype, direction, o, true, sched_area, 1, s)) !=
       FOLDCP_OK)
     return st;
-  return finalize_stage(o, z, mask, params, N, out, s);
+  return finalize_stage(o, z, mask, params, N, out, false, 1.0f, s);
 }
 
 namespace {

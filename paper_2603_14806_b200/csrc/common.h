@@ -96,8 +96,11 @@ int launch_simt_finalize(const void* o, const void* z, const void* mask,
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
                            void* a, void* b, bool ab_f16, unsigned int* sched,
                            cudaStream_t stream);
+// o_f16: o holds fp16 values scaled by the power of two o_scale (the fused path, see
+// contract_o_scale); otherwise bf16 with o_scale = 1 (stage entry point, backward recomputation)
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
-                            const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
+                            const foldcp_trimul_params* p, int N, void* out, bool o_f16,
+                            float o_scale, cudaStream_t stream);
 
 // Backward pass around the contraction (simt_backward.cu): phase 0 = K3-backward (o -> d_o in
 // place, dzp written), 1 = K1-backward for a, 2 = K1-backward for b + LayerNorm(z) backward.

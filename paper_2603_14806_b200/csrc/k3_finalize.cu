@@ -4,35 +4,57 @@
 //   g   = sigmoid(W_g LN(z; gamma_in, beta_in) + b_g)          recomputed from z, never stored
 //   out = [M *] g * (W_o LN(o; gamma_out, beta_out) + b_o)     written bf16, channel-last
 //
-// o is channel-major [128][R] bf16 (K2's output), z and out are [R][128] channel-last bf16.
-// Recomputing g here instead of materialising it in K1 keeps the workspace at a + b + o
-// (N = 8192 fits) and keeps g in fp32 (a bf16 round trip of g costs accuracy -- SURVEY 8(c)).
+// o is channel-major [128][R] (K2's output: bf16, or fp16 scaled by a power of two on the fused
+// path), z and out are [R][128] channel-last bf16.  Recomputing g here instead of materialising it
+// in K1 keeps the workspace at a + b + o (N = 8192 fits) and keeps g in fp32.
+//
+// WHAT BOUNDS THIS KERNEL.  Inside the step the SM clock sits at the power cap (1.1 - 1.3 GHz) and
+// K3 is bound by SHARED-MEMORY BANDWIDTH (128 B / clock / SM), not by HBM and not by issue slots:
+// ncu on the r1 kernel and its successors showed LSU + tensor-operand + TMA wavefronts adding up to
+// ~96 % of the elapsed cycles (profiles/r2_k3_notes.md).  A 128-pair tile unavoidably costs the TMA
+// fill (512 wavefronts), the operand fetch of two 128 x 128 x 128 MMAs (~780), staging + TMA store
+// of the output (512) and one read of each tile for the statistics (512).  Everything else had to go:
+//
+//  * The LayerNorms are NOT applied to the tiles (r1 rewrote both in place: 1024 more wavefronts and
+//    a proxy fence on the MMA's critical path).  With x a pair's 128 raw channels, mean / rstd its
+//    statistics and W' = W diag(gamma) the folded weight,
+//        W LN(x) + b  =  rstd * [ W' x  -  mean (W' 1)  +  (1 / rstd) (W beta + b) ]
+//    the tensor core multiplies the tiles exactly as TMA delivered them, and the two rank-one terms
+//    are ALSO given to the tensor core: one more MMA of K = 16 per GEMM whose A operand holds, per
+//    pair, -mean and 1/rstd and whose B operand holds, per channel, s = W' 1 and t = W beta + b,
+//    each split into three pieces of the operand format (bf16: 3 x 8 bits, fp16: 3 x 11 bits) so
+//    that the products carry fp32 precision (six cross terms per product, twelve of the sixteen
+//    K slots).  s is summed from the ROUNDED folded weights, so D - mean s = sum_k w'_k (x_k - mean)
+//    holds for the weights the tensor core really uses: a row's common offset cancels.
+//  * The epilogue then needs NO per-channel constant at all -- out = rstd-scaled accumulators through
+//    the gate -- where the row-per-thread form loaded four constants per output (2048 wavefronts of
+//    broadcast loads per tile, as much as everything else together).
 //
 // GEMM orientation: the PAIR is the MMA M dimension (TMEM lane), the OUTPUT CHANNEL the N
-// dimension (TMEM column), so an epilogue thread owns a contiguous run of one pair's output row:
-//   D_g[pair][ch] = z'[pair][k]      * W_g[ch][k]^T     A K-major  (z tile as TMA delivers it)
-//   D_o[pair][ch] = LN(o)[k][pair]^T * W_o[ch][k]^T     A MN-major (o tile is [k][pair], pairs
-//                                                       contiguous: the transposition K2's
-//                                                       channel-major output needs is done by the
-//                                                       tensor core's operand fetch, not by us)
+// dimension (TMEM column):
+//   D_g[pair][ch] = z[pair][k]    * W_g'[ch][k]^T     A K-major  (bf16 z tile; W_g' rounded to bf16)
+//   D_o[pair][ch] = o[k][pair]^T  * W_o'[ch][k]^T     A MN-major (the o tile is [k][pair], pairs
+//                                                     contiguous: the transposition K2's
+//                                                     channel-major output needs is done by the
+//                                                     tensor core's operand fetch, not by us)
+//   D_*          += X_*[pair][16] * Y_*[ch][16]^T     the rank-one corrections (K-major, unswizzled)
+// tcgen05 kind::f16 wants both operands of an MMA in one format: W_o' is fp16 when o is fp16
+// (fused path: no rounding of o beyond K2's own 2^-12) and bf16 when o is bf16 (stage entry point).
 //
-// Both LayerNorm affines are folded into the GEMMs once per CTA (W LN(x) + b =
-// (W diag(gamma)) n + (W beta + b), n = (x - mean) * rstd): gamma goes into the resident weights
-// while they are converted to the operand format of the normalised tiles (fp16, see common.h),
-// beta into per-channel fp32 biases in shared memory.  The LayerNorm warps only normalise.
-//
-// Persistent kernel, one CTA per SM, 24 warps, tile = 128 pairs:
+// Persistent kernel, one CTA per SM, 28 warps, tile = 128 pairs:
 //   warp 0       TMA producer : W_g, W_o once (resident), then (z tile, o tile) into a 2-deep ring
-//   warp 1       MMA issuer   : two MMAs (M=128 pairs, N=128 ch, K=128) into a 256-column TMEM
-//                               slot; two slots, so the epilogue overlaps the next tile's MMAs
+//   warp 1       MMA issuer   : 16 MMAs on the raw tiles the moment they land, then the two
+//                               correction MMAs once the statistics are in; 256-column TMEM slot,
+//                               two slots, so the epilogue overlaps the next tile's MMAs
 //   warp 2       TMEM allocator
-//   warps 4-7    LayerNorm(z) : ln_rows.cuh (rows in registers, two-pass statistics, in place)
-//   warps 8-15   LayerNorm(o) : thread = 2 pairs x 32 channels of the [k][pair] tile, held in
-//                               registers, exact two-pass statistics combined across the four
-//                               channel quarters with shuffles, in place
-//   warps 16-23  epilogue     : tcgen05.ld -> bias, sigmoid gate, mask in packed fp32 -> bf16 ->
-//                               swizzled smem -> TMA store [128 pairs][64 ch]
+//   warps 4-11   epilogue     : tcgen05.ld (fragment shape 16x256b) -> rstd, sigmoid gate, mask in
+//                               packed fp32 -> bf16 -> swizzled smem -> TMA store [128 pairs][64 ch]
+//   warps 12-19  statistics of o : thread = 2 pairs x 32 channels of the [k][pair] tile
+//   warps 20-27  statistics of z : ln_rows.cuh layernorm_rows_stats (4 lanes per pair row)
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <type_traits>
 
 #include "common.h"
 #include "ln_rows.cuh"
@@ -43,27 +65,36 @@ namespace {
 
 constexpr int kC = kChannels;
 constexpr int kTilePairs = 128;
-// warp roles: 0 TMA, 1 MMA, 2 TMEM allocator, 3 idle, then LayerNorm(z), LayerNorm(o), epilogue
-#ifndef FOLDCP_K3_LNZ_WARPS
-#define FOLDCP_K3_LNZ_WARPS 4
-#endif
-constexpr int kLnzWarps = FOLDCP_K3_LNZ_WARPS;       // 4 or 8
-constexpr int kWarpLnz = 4;
-constexpr int kWarpLno = kWarpLnz + kLnzWarps;       // 8 warps
-constexpr int kWarpEpi = kWarpLno + 8;               // 8 warps; a multiple of 4 (TMEM lane quadrants)
-constexpr int kThreads = (kWarpEpi + 8) * 32;
-static_assert(kLnzWarps == 4 || kLnzWarps == 8, "LayerNorm(z) runs on 4 or 8 warps");
+// warp roles: 0 TMA, 1 MMA, 2 TMEM allocator, 3 idle, then epilogue, statistics(o), statistics(z).
+// The order matters: the issue arbiter favours higher warp ids, and the statistics sit on the
+// critical path (statistics -> correction MMAs -> accumulator ready -> epilogue) while the epilogue
+// only has to keep up.
+constexpr int kEpiWarps = 8;
+constexpr int kLnoWarps = 8;
+constexpr int kLnzWarps = 8;
+constexpr int kWarpEpi = 4;                          // a multiple of 4 (TMEM lane quadrants)
+constexpr int kWarpLno = kWarpEpi + kEpiWarps;
+constexpr int kWarpLnz = kWarpLno + kLnoWarps;
+constexpr int kThreads = (kWarpLnz + kLnzWarps) * 32;
+static_assert(kWarpEpi % 4 == 0, "epilogue warps must start at a TMEM lane-quadrant boundary");
+// 28 warps leave 72 registers per thread at launch; the twenty control / statistics warps give
+// some up (setmaxnreg, per aligned group of four warps) for the eight epilogue warps
+constexpr int kRegsOther = 56;
+constexpr int kRegsEpi = 104;
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box (128 rows x 128 bytes)
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB
 constexpr int kStages = 2;
 constexpr int kStageBytes = 2 * kMatBytes;      // z tile + o tile
+constexpr int kXBytes = 128 * 16 * 2;           // 4 KB: a [128][16] correction operand
 
-constexpr int kOffW = 0;                                   // W_g, W_o
+constexpr int kOffW = 0;                                   // W_g', W_o'
 constexpr int kOffStage = kOffW + 2 * kMatBytes;           // ring: [z | o] per stage
-constexpr int kOffOut = kOffStage + kStages * kStageBytes; // 2 staging buffers [128 pairs][64 ch]
-constexpr int kOffVec = kOffOut + 2 * kHalfBox;            // folded biases t_g[128], t_o[128] (fp32)
-constexpr int kOffBar = kOffVec + 2 * kC * 4;
-constexpr int kSmemBytes = kOffBar + 128;
+constexpr int kOffOut = kOffStage + kStages * kStageBytes; // ONE staging buffer [128 pairs][64 ch]
+constexpr int kOffY = kOffOut + kHalfBox;                  // Y_g, Y_o: per-channel side, resident
+constexpr int kOffX = kOffY + 2 * kXBytes;                 // X_z, X_o: per-pair side, one tile
+constexpr int kOffRstd = kOffX + 2 * kXBytes;              // per stage: float2[128] (rstd_z, rstd_o)
+constexpr int kOffBar = kOffRstd + kStages * kTilePairs * 8;
+constexpr int kSmemBytes = kOffBar + 256;
 static_assert(kSmemBytes <= 232448, "K3 shared memory exceeds 227 KB");
 
 struct K3Params {
@@ -77,10 +108,12 @@ struct K3Params {
   const __nv_bfloat16* w_o;
   const float* bias_g;         // may be nullptr
   const float* bias_o;         // may be nullptr
-  float eps;
+  float eps_z;                 // LayerNorm epsilon of z
+  float eps_o;                 // of o: eps * o_scale^2 when o arrives scaled (LN(s o; s^2 eps) = LN(o; eps))
   long long R;
   int num_tiles;
-  int dbg_skip;                // debug builds only: 1 skip LN(z) math, 2 skip LN(o) math, 4 skip epilogue math
+  int dbg_skip;                // debug builds only: 1 skip z statistics, 2 skip o statistics, 4 skip epilogue math,
+                               // 8 no wait for the previous store's read (timing only), 16 no stores
 };
 
 #ifdef FOLDCP_DEBUG_KNOBS
@@ -89,7 +122,97 @@ struct K3Params {
 #define K3_DBG_SKIP(bit) false
 #endif
 
-template <bool kTanhSigmoid>
+#ifdef FOLDCP_K3_PROBE
+// bring-up instrumentation (never in the product build): cycles per CTA.  [0] producer total,
+// [1] producer wait sempty, [2] issuer wait tempty, [3] issuer wait full, [4] z-stats wait full,
+// [5] z-stats work, [6] o-stats wait full, [7] o-stats work, [8] epilogue wait sready,
+// [9] epilogue wait tfull, [10] epilogue barrier 1 (+ store-read wait), [11] epilogue barrier 2,
+// [12] epilogue total, [13] tiles, [14] epilogue tcgen05.ld + wait, [15] issuer wait sready
+__device__ unsigned long long g_k3_probe[160][16];
+#define K3_PROBE_T0(var) const long long var = clock64()
+#define K3_PROBE_ADD(acc, t0) acc += clock64() - (t0)
+#define K3_PROBE_DECL(var) long long var = 0
+#define K3_PROBE_PUT(idx, val) g_k3_probe[blockIdx.x][idx] = static_cast<unsigned long long>(val)
+#else
+#define K3_PROBE_T0(var)
+#define K3_PROBE_ADD(acc, t0)
+#define K3_PROBE_DECL(var)
+#define K3_PROBE_PUT(idx, val)
+#endif
+
+// the folded weight  0.5 w gamma  as the tensor core will see it (the factor 1/2 belongs to the tanh
+// form of the sigmoid, below): ONE expression, used both to build the resident operand and to sum s
+template <bool kF16>
+__device__ __forceinline__ uint32_t fold_pack(uint32_t w2, float g_lo, float g_hi) {
+  return ptx::pack_norm<kF16>(0.5f * ptx::bf16_lo(w2) * g_lo, 0.5f * ptx::bf16_hi(w2) * g_hi);
+}
+template <bool kF16>
+__device__ __forceinline__ float packed_sum(uint32_t v) {
+  if constexpr (kF16) {
+    const __half2 h = *reinterpret_cast<const __half2*>(&v);
+    return __low2float(h) + __high2float(h);
+  } else {
+    return ptx::bf16_lo(v) + ptx::bf16_hi(v);
+  }
+}
+// 16-bit pair word of the o tile -> fp32x2 (exact)
+template <bool kF16>
+__device__ __forceinline__ ptx::f32x2 o2_to_f32x2(uint32_t v) {
+  if constexpr (kF16) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&v));
+    return ptx::pk2(f.x, f.y);
+  } else {
+    return ptx::bf16x2_to_f32x2(v);
+  }
+}
+
+// x = x1 + x2 + x3 with every piece representable in the operand format (round to nearest each
+// time; the remainders are exact in fp32): 24 bits of x from bf16 pieces, more from fp16 ones
+template <bool kF16>
+__device__ __forceinline__ void split3(float x, uint32_t (&p)[3]) {
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    if constexpr (kF16) {
+      const __half h = __float2half_rn(x);
+      p[i] = static_cast<uint32_t>(__half_as_ushort(h));
+      x -= __half2float(h);
+    } else {
+      const __nv_bfloat16 h = __float2bfloat16_rn(x);
+      p[i] = static_cast<uint32_t>(__bfloat16_as_ushort(h));
+      x -= __bfloat162float(h);
+    }
+  }
+}
+// One row of a correction operand: the sixteen K slots that pair  (u, v)  on the per-pair side with
+// (s, t)  on the per-channel side so that the MMA adds  u s + v t  with all cross terms down to
+// 2^-24:   per-pair side     u1 u1 u2 u1 u2 u3 | v1 v1 v2 v1 v2 v3 | 0 0 0 0
+//          per-channel side  s1 s2 s1 s3 s2 s1 | t1 t2 t1 t3 t2 t1 | 0 0 0 0
+// Unswizzled K-major layout (ptx::make_smem_desc_noswizzle, lbo 128, sbo 256): slots 0..7 of row r
+// at (r / 8) * 256 + (r % 8) * 16, slots 8..15 another 128 bytes on.
+__device__ __forceinline__ uint32_t x_row_addr(uint32_t base, uint32_t r) {
+  return base + (r >> 3) * 256u + (r & 7u) * 16u;
+}
+template <bool kF16>
+__device__ __forceinline__ void write_pair_side(uint32_t base, uint32_t r, float u, float v) {
+  uint32_t a[3], b[3];
+  split3<kF16>(u, a);
+  split3<kF16>(v, b);
+  const uint32_t addr = x_row_addr(base, r);
+  ptx::sts128(addr, a[0] | (a[0] << 16), a[1] | (a[0] << 16), a[1] | (a[2] << 16), b[0] | (b[0] << 16));
+  ptx::sts128(addr + 128, b[1] | (b[0] << 16), b[1] | (b[2] << 16), 0u, 0u);
+}
+template <bool kF16>
+__device__ __forceinline__ void write_channel_side(uint32_t base, uint32_t r, float s, float t) {
+  uint32_t a[3], b[3];
+  split3<kF16>(s, a);
+  split3<kF16>(t, b);
+  const uint32_t addr = x_row_addr(base, r);
+  ptx::sts128(addr, a[0] | (a[1] << 16), a[0] | (a[2] << 16), a[1] | (a[0] << 16), b[0] | (b[1] << 16));
+  ptx::sts128(addr + 128, b[0] | (b[2] << 16), b[1] | (b[0] << 16), 0u, 0u);
+}
+
+// kOF16: the o tile (and therefore W_o') is fp16; kResidual: out = z + update
+template <bool kOF16, bool kResidual>
 __global__ void __launch_bounds__(kThreads, 1)
 k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
                    const __grid_constant__ CUtensorMap tmap_o,
@@ -102,13 +225,14 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
 
   const uint32_t bar = smem + kOffBar;
   const uint32_t wfull = bar;
-  auto full = [&](int s) { return bar + 8u * (1 + s); };
+  auto full = [&](int s) { return bar + 8u * (1 + s); };        // tile landed (TMA)
+  // stage reusable: MMAs retired + statistics warps done reading + epilogue has taken its rstd
   auto sempty = [&](int s) { return bar + 8u * (3 + s); };
-  auto zready = [&](int s) { return bar + 8u * (5 + s); };
-  auto oready = [&](int s) { return bar + 8u * (7 + s); };
-  auto tfull = [&](int u) { return bar + 8u * (9 + u); };
-  auto tempty = [&](int u) { return bar + 8u * (11 + u); };
-  const uint32_t tmem_slot = bar + 8u * 13;
+  auto tfull = [&](int u) { return bar + 8u * (5 + u); };       // accumulators complete
+  auto tempty = [&](int u) { return bar + 8u * (7 + u); };      // accumulators read
+  auto sready = [&](int s) { return bar + 8u * (9 + s); };      // statistics of the tile in stage s written
+  const uint32_t xfree = bar + 8u * 11;                          // correction MMAs have read X_z, X_o
+  const uint32_t tmem_slot = bar + 8u * 12;
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -122,31 +246,35 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::mbar_init(wfull, 1);
     for (int s = 0; s < kStages; ++s) {
       ptx::mbar_init(full(s), 1);
-      ptx::mbar_init(sempty(s), 1);
-      ptx::mbar_init(zready(s), kLnzWarps * 32);
-      ptx::mbar_init(oready(s), 256);
+      ptx::mbar_init(sempty(s), 1 + kLnzWarps + kLnoWarps + kEpiWarps);
+      ptx::mbar_init(sready(s), kLnzWarps + kLnoWarps);
     }
     for (int u = 0; u < 2; ++u) {
       ptx::mbar_init(tfull(u), 1);
-      ptx::mbar_init(tempty(u), 8);
+      ptx::mbar_init(tempty(u), kEpiWarps);
     }
+    ptx::mbar_init(xfree, 1);
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc<1>(tmem_slot, 512);
   if (threadIdx.x >= 128 && threadIdx.x < 384) {
-    // Fold the LayerNorm shifts into the biases:  W LN(x) + b = (W diag(gamma)) n + (W beta + b)
-    // with n = (x - mean) * rstd.  Thread -> (matrix, output channel); fp32, from the bf16 weights.
+    // Per output channel of each GEMM:  t = 0.5 (W beta + b)  (exact fold of the LayerNorm shift,
+    // fp32 from the bf16 weights) and  s = sum_k w'_k  over the ROUNDED folded weights; both go,
+    // split, into the channel's row of the resident correction operand Y.
     const int id = threadIdx.x - 128;
     const int m = id >> 7, ch = id & 127;
     const uint4* wrow = reinterpret_cast<const uint4*>((m ? prm.w_o : prm.w_g) + ch * kC);
     const float* beta = m ? prm.b_out : prm.b_in;
+    const float* gam = m ? prm.g_out : prm.g_in;
     const float* bias = m ? prm.bias_o : prm.bias_g;
-    float acc = 0.f;
+    float acc = 0.f, ssum = 0.f;
 #pragma unroll 4
     for (int kc = 0; kc < 16; ++kc) {
       const uint4 wv = __ldg(wrow + kc);
       const float4 b0 = __ldg(reinterpret_cast<const float4*>(beta + kc * 8));
       const float4 b1 = __ldg(reinterpret_cast<const float4*>(beta + kc * 8 + 4));
+      const float4 g0 = __ldg(reinterpret_cast<const float4*>(gam + kc * 8));
+      const float4 g1 = __ldg(reinterpret_cast<const float4*>(gam + kc * 8 + 4));
       acc = fmaf(ptx::bf16_lo(wv.x), b0.x, acc);
       acc = fmaf(ptx::bf16_hi(wv.x), b0.y, acc);
       acc = fmaf(ptx::bf16_lo(wv.y), b0.z, acc);
@@ -155,11 +283,26 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       acc = fmaf(ptx::bf16_hi(wv.z), b1.y, acc);
       acc = fmaf(ptx::bf16_lo(wv.w), b1.z, acc);
       acc = fmaf(ptx::bf16_hi(wv.w), b1.w, acc);
+      if (m == 0 || !kOF16) {
+        ssum += packed_sum<false>(fold_pack<false>(wv.x, g0.x, g0.y));
+        ssum += packed_sum<false>(fold_pack<false>(wv.y, g0.z, g0.w));
+        ssum += packed_sum<false>(fold_pack<false>(wv.z, g1.x, g1.y));
+        ssum += packed_sum<false>(fold_pack<false>(wv.w, g1.z, g1.w));
+      } else {
+        ssum += packed_sum<true>(fold_pack<true>(wv.x, g0.x, g0.y));
+        ssum += packed_sum<true>(fold_pack<true>(wv.y, g0.z, g0.w));
+        ssum += packed_sum<true>(fold_pack<true>(wv.z, g1.x, g1.y));
+        ssum += packed_sum<true>(fold_pack<true>(wv.w, g1.z, g1.w));
+      }
     }
     // tanh form: out = M sigma(g) y = M (tanh(g/2) + 1) (y/2): both factors 1/2 are folded into
-    // the weights and these biases (exact: a power of two)
-    reinterpret_cast<float*>(smem_raw + kOffVec)[id] =
-        (kTanhSigmoid ? 0.5f : 1.0f) * (acc + (bias ? bias[ch] : 0.f));
+    // the weights (fold_pack) and t (exact: a power of two)
+    const float t = 0.5f * (acc + (bias ? bias[ch] : 0.f));
+    if (m == 0 || !kOF16) {
+      write_channel_side<false>(smem + kOffY + m * kXBytes, ch, ssum, t);
+    } else {
+      write_channel_side<true>(smem + kOffY + m * kXBytes, ch, ssum, t);
+    }
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -176,9 +319,9 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::tma_load_2d(smem + kOffW + kMatBytes + kHalfBox, &tmap_wo, wfull, 64, 0);
   }
   {
-    // The resident weights become  W diag(gamma)  in the operand format of the normalised tiles
-    // (fp16 unless FOLDCP_NORM_FP16=0), in place: elementwise apart from the gamma index, which
-    // follows from the position under the 128-byte swizzle.
+    // The resident weights become  W' = 0.5 W diag(gamma)  in the format of the tile they multiply
+    // (bf16 for the gate; fp16 or bf16 for the output projection), in place: elementwise apart from
+    // the gamma index, which follows from the position under the 128-byte swizzle.
     ptx::mbar_wait(wfull, 0);
     for (int off = threadIdx.x * 16; off < 2 * kMatBytes; off += kThreads * 16) {
       const int m = off / kMatBytes, rem = off % kMatBytes;
@@ -187,30 +330,40 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const float* gam = (m ? prm.g_out : prm.g_in) + k0;
       const float4 g0 = __ldg(reinterpret_cast<const float4*>(gam));
       const float4 g1 = __ldg(reinterpret_cast<const float4*>(gam + 4));
-      constexpr float ws = kTanhSigmoid ? 0.5f : 1.0f;
       uint32_t v[4];
       ptx::lds128(smem + kOffW + off, v);
-      v[0] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[0]) * g0.x, ws * ptx::bf16_hi(v[0]) * g0.y);
-      v[1] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[1]) * g0.z, ws * ptx::bf16_hi(v[1]) * g0.w);
-      v[2] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[2]) * g1.x, ws * ptx::bf16_hi(v[2]) * g1.y);
-      v[3] = ptx::pack_norm<kNormFp16>(ws * ptx::bf16_lo(v[3]) * g1.z, ws * ptx::bf16_hi(v[3]) * g1.w);
+      if (m == 0 || !kOF16) {
+        v[0] = fold_pack<false>(v[0], g0.x, g0.y);
+        v[1] = fold_pack<false>(v[1], g0.z, g0.w);
+        v[2] = fold_pack<false>(v[2], g1.x, g1.y);
+        v[3] = fold_pack<false>(v[3], g1.z, g1.w);
+      } else {
+        v[0] = fold_pack<true>(v[0], g0.x, g0.y);
+        v[1] = fold_pack<true>(v[1], g0.z, g0.w);
+        v[2] = fold_pack<true>(v[2], g1.x, g1.y);
+        v[3] = fold_pack<true>(v[3], g1.z, g1.w);
+      }
       ptx::sts128(smem + kOffW + off, v[0], v[1], v[2], v[3]);
     }
-    ptx::fence_proxy_async_smem();
+    ptx::fence_proxy_async_smem();     // also covers the Y rows written above
     __syncthreads();
   }
 
   const int first = blockIdx.x;
   const int stride = gridDim.x;
 
-
+  if (warp < kWarpEpi) ptx::setmaxnreg_dec<kRegsOther>();
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
       int it = 0;
+      K3_PROBE_DECL(pw);
+      K3_PROBE_T0(p0t);
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
         const int s = it & 1;
+        K3_PROBE_T0(tw);
         ptx::mbar_wait(sempty(s), ((it >> 1) & 1) ^ 1u);
+        K3_PROBE_ADD(pw, tw);
         ptx::mbar_arrive_expect_tx(full(s), kStageBytes);
         const uint32_t zdst = smem + kOffStage + s * kStageBytes;
         const uint32_t odst = zdst + kMatBytes;
@@ -220,23 +373,38 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::tma_load_2d(odst, &tmap_o, full(s), p0, 0);             // [128 ch][pairs 0..63]
         ptx::tma_load_2d(odst + kHalfBox, &tmap_o, full(s), p0 + 64, 0);
       }
+      K3_PROBE_PUT(0, clock64() - p0t);
+      K3_PROBE_PUT(1, pw);
+      K3_PROBE_PUT(13, it);
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (ptx::elect_one()) {
-      constexpr uint32_t kNormFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
-      constexpr uint32_t idesc_g = ptx::make_idesc_f16kind(128, kC, kNormFmt, kNormFmt, 0, 0);
-      // A = LN(o), MN-major
-      constexpr uint32_t idesc_o = ptx::make_idesc_f16kind(128, kC, kNormFmt, kNormFmt, 1, 0);
-      ptx::mbar_wait(wfull, 0);
+      constexpr uint32_t kOFmt = kOF16 ? ptx::kFmtF16 : ptx::kFmtBF16;
+      constexpr uint32_t idesc_g = ptx::make_idesc_f16kind(128, kC, ptx::kFmtBF16, ptx::kFmtBF16, 0, 0);
+      // A = o, MN-major
+      constexpr uint32_t idesc_o = ptx::make_idesc_f16kind(128, kC, kOFmt, kOFmt, 1, 0);
+      // the correction MMA of the o GEMM: both operands K-major
+      constexpr uint32_t idesc_ox = ptx::make_idesc_f16kind(128, kC, kOFmt, kOFmt, 0, 0);
+      const uint64_t dxz = ptx::make_smem_desc_noswizzle(smem + kOffX, 128, 256);
+      const uint64_t dxo = ptx::make_smem_desc_noswizzle(smem + kOffX + kXBytes, 128, 256);
+      const uint64_t dyg = ptx::make_smem_desc_noswizzle(smem + kOffY, 128, 256);
+      const uint64_t dyo = ptx::make_smem_desc_noswizzle(smem + kOffY + kXBytes, 128, 256);
+      K3_PROBE_DECL(iw_t);
+      K3_PROBE_DECL(iw_f);
+      K3_PROBE_DECL(iw_s);
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
         const int s = it & 1;
         const int slot = it & 1;
         const uint32_t zb = smem + kOffStage + s * kStageBytes;
         const uint32_t ob = zb + kMatBytes;
+        K3_PROBE_T0(t1);
         ptx::mbar_wait(tempty(slot), ((it >> 1) & 1) ^ 1u);
-        ptx::mbar_wait(zready(s), (it >> 1) & 1);
+        K3_PROBE_ADD(iw_t, t1);
+        K3_PROBE_T0(t2);
+        ptx::mbar_wait(full(s), (it >> 1) & 1);
+        K3_PROBE_ADD(iw_f, t2);
         ptx::tc_fence_after();
         const uint32_t d_g = tmem_base + slot * 256;
 #pragma unroll
@@ -246,8 +414,6 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           const uint64_t db = ptx::make_smem_desc_sw128(smem + kOffW + off, 16, 1024);
           ptx::umma_bf16<1>(d_g, da, db, idesc_g, k != 0 ? 1u : 0u);
         }
-        ptx::mbar_wait(oready(s), (it >> 1) & 1);
-        ptx::tc_fence_after();
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           // A MN-major: 64-pair groups kHalfBox apart (LBO), 8-channel atoms 1024 B apart (SBO),
@@ -257,30 +423,65 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           const uint64_t db = ptx::make_smem_desc_sw128(smem + kOffW + kMatBytes + off, 16, 1024);
           ptx::umma_bf16<1>(d_g + 128, da, db, idesc_o, k != 0 ? 1u : 0u);
         }
+        // the rank-one corrections, once this tile's statistics are in X_z / X_o
+        K3_PROBE_T0(t3);
+        ptx::mbar_wait(sready(s), (it >> 1) & 1);
+        K3_PROBE_ADD(iw_s, t3);
+        ptx::tc_fence_after();
+        ptx::umma_bf16<1>(d_g, dxz, dyg, idesc_g, 1u);
+        ptx::umma_bf16<1>(d_g + 128, dxo, dyo, idesc_ox, 1u);
+        ptx::umma_commit<1>(xfree);
         ptx::umma_commit<1>(tfull(slot));
         ptx::umma_commit<1>(sempty(s));
       }
+      K3_PROBE_PUT(2, iw_t);
+      K3_PROBE_PUT(3, iw_f);
+      K3_PROBE_PUT(15, iw_s);
     }
-  } else if (warp >= kWarpLnz && warp < kWarpLno) {
-    // ===================== LayerNorm(z) (4 lanes per pair row) =====================
-    const int r = threadIdx.x - 128;
+  } else if (warp >= kWarpLnz) {
+    // ===================== statistics of the z tile (4 lanes per pair row) =====================
+    ptx::setmaxnreg_dec<kRegsOther>();
+    const int r = threadIdx.x - kWarpLnz * 32;
+    K3_PROBE_DECL(zw);
+    K3_PROBE_DECL(zc);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
+      K3_PROBE_T0(t1);
       ptx::mbar_wait(full(s), (it >> 1) & 1);
+      // X_z still feeds the previous tile's correction MMA until that has retired (long ago by now)
+      if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
+      K3_PROBE_ADD(zw, t1);
+      K3_PROBE_T0(t2);
+      const uint32_t rstd_base = smem + kOffRstd + s * kTilePairs * 8;
       if (!K3_DBG_SKIP(1))
-        layernorm_rows_inplace<kNormFp16, false, 1, kLnzWarps * 32>(smem + kOffStage + s * kStageBytes, kHalfBox,
-                                                       r, 0, 0, prm.eps);
+        layernorm_rows_stats<1, kLnzWarps * 32>(smem + kOffStage + s * kStageBytes, kHalfBox, r,
+                                [&](uint32_t row, float mean, float var) {
+                                  const float ve = var + prm.eps_z;
+                                  const float rstd = rsqrtf(ve);
+                                  write_pair_side<false>(smem + kOffX, row, -mean, ve * rstd);
+                                  ptx::sts32(rstd_base + row * 8u, __float_as_uint(rstd));
+                                });
       ptx::fence_proxy_async_smem();
-      ptx::mbar_arrive(zready(s));
+      __syncwarp();
+      if (lane == 0) {
+        ptx::mbar_arrive(sready(s));
+        ptx::mbar_arrive(sempty(s));
+      }
+      K3_PROBE_ADD(zc, t2);
     }
-  } else if (warp >= kWarpLno && warp < kWarpEpi) {
-    // ===================== LayerNorm(o) on the [channel][pair] tile =====================
+    if (threadIdx.x == kWarpLnz * 32) {
+      K3_PROBE_PUT(4, zw);
+      K3_PROBE_PUT(5, zc);
+    }
+  } else if (warp >= kWarpLno && warp < kWarpLnz) {
+    // ===================== statistics of the o tile, [channel][pair] =====================
+    ptx::setmaxnreg_dec<kRegsOther>();
     // Warp w8 owns 16 pairs; lane = (channel quarter cq = 32 channels, pair-pair pl).  One
-    // ld.shared.b32 = 2 adjacent pairs of one channel, and the thread's 32 words stay in registers
-    // (one pass over shared memory, exact two-pass statistics).  The four quarters visit their
-    // rows in the order i ^ 2cq, which puts their 32-byte segments under four different swizzle
-    // phases: conflict-free.  Statistics combine across the quarters with two shuffles.
+    // ld.shared.b32 = 2 adjacent pairs of one channel.  The four quarters visit their rows in the
+    // order i ^ 2cq, which puts their 32-byte segments under four different swizzle phases:
+    // conflict-free.  Shifted one-sweep accumulation as in layernorm_rows_stats (the shift is the
+    // pair's channel-0 value); the quarters combine with two shuffles.
     const int w8 = warp - kWarpLno;
     const uint32_t cq = static_cast<uint32_t>(lane >> 3);
     const uint32_t pl = static_cast<uint32_t>(lane & 7);
@@ -295,165 +496,225 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const uint32_t k7 = jj ^ (2u * cq);
       toff[jj] = box * kHalfBox + (cq * 32u + k7) * 128u + ((c16 ^ k7) << 4) + within;
     }
+    const uint32_t pair0 = box * 64u + static_cast<uint32_t>(w8 & 3) * 16u + pl * 2u;
+    K3_PROBE_DECL(ow);
+    K3_PROBE_DECL(oc);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
+      K3_PROBE_T0(t1);
       ptx::mbar_wait(full(s), (it >> 1) & 1);
+      if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
+      K3_PROBE_ADD(ow, t1);
+      K3_PROBE_T0(t2);
       const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes;
-      if (K3_DBG_SKIP(2)) {
-        ptx::fence_proxy_async_smem();
-        ptx::mbar_arrive(oready(s));
-        continue;
+      if (!K3_DBG_SKIP(2)) {
+        uint32_t w[32];
+#pragma unroll
+        for (uint32_t g = 0; g < 4; ++g)
+#pragma unroll
+          for (uint32_t jj = 0; jj < 8; ++jj) w[g * 8 + jj] = ptx::lds32(tile + toff[jj] + g * 1024u);
+        // shift: the word the cq = 0 lane loaded first (channel 0 of both pairs)
+        const uint32_t cw = __shfl_sync(0xffffffffu, w[0], static_cast<int>(pl));
+        float c0, c1;
+        ptx::upk2(o2_to_f32x2<kOF16>(cw), c0, c1);
+        const ptx::f32x2 nc = ptx::pk2(-c0, -c1);
+        ptx::f32x2 a0 = ptx::pk2(0.f, 0.f), a1 = a0, b0 = a0, b1 = a0;
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+          const ptx::f32x2 d0 = ptx::add2(o2_to_f32x2<kOF16>(w[i]), nc);
+          const ptx::f32x2 d1 = ptx::add2(o2_to_f32x2<kOF16>(w[i + 1]), nc);
+          a0 = ptx::add2(a0, d0);
+          a1 = ptx::add2(a1, d1);
+          b0 = ptx::fma2(d0, d0, b0);
+          b1 = ptx::fma2(d1, d1, b1);
+        }
+        float s10, s11, s20, s21;
+        ptx::upk2(ptx::add2(a0, a1), s10, s11);
+        ptx::upk2(ptx::add2(b0, b1), s20, s21);
+        s10 += __shfl_xor_sync(0xffffffffu, s10, 8);
+        s11 += __shfl_xor_sync(0xffffffffu, s11, 8);
+        s20 += __shfl_xor_sync(0xffffffffu, s20, 8);
+        s21 += __shfl_xor_sync(0xffffffffu, s21, 8);
+        s10 += __shfl_xor_sync(0xffffffffu, s10, 16);
+        s11 += __shfl_xor_sync(0xffffffffu, s11, 16);
+        s20 += __shfl_xor_sync(0xffffffffu, s20, 16);
+        s21 += __shfl_xor_sync(0xffffffffu, s21, 16);
+        if (cq == 0) {
+          const float md0 = s10 * (1.0f / kC), md1 = s11 * (1.0f / kC);
+          const float ve0 = fmaxf(fmaf(-md0, md0, s20 * (1.0f / kC)), 0.f) + prm.eps_o;
+          const float ve1 = fmaxf(fmaf(-md1, md1, s21 * (1.0f / kC)), 0.f) + prm.eps_o;
+          const float r0 = rsqrtf(ve0), r1 = rsqrtf(ve1);
+          write_pair_side<kOF16>(smem + kOffX + kXBytes, pair0, -(c0 + md0), ve0 * r0);
+          write_pair_side<kOF16>(smem + kOffX + kXBytes, pair0 + 1, -(c1 + md1), ve1 * r1);
+          const uint32_t ra = smem + kOffRstd + s * kTilePairs * 8 + pair0 * 8u + 4u;
+          ptx::sts32(ra, __float_as_uint(r0));
+          ptx::sts32(ra + 8, __float_as_uint(r1));
+        }
       }
-      uint32_t w[32];
-#pragma unroll
-      for (uint32_t g = 0; g < 4; ++g)
-#pragma unroll
-        for (uint32_t jj = 0; jj < 8; ++jj) w[g * 8 + jj] = ptx::lds32(tile + toff[jj] + g * 1024u);
-      ptx::f32x2 sa = ptx::bf16x2_to_f32x2(w[0]), sb = ptx::bf16x2_to_f32x2(w[1]);
-#pragma unroll
-      for (int i = 2; i < 32; i += 2) {
-        sa = ptx::add2(sa, ptx::bf16x2_to_f32x2(w[i]));
-        sb = ptx::add2(sb, ptx::bf16x2_to_f32x2(w[i + 1]));
-      }
-      float s0, s1;
-      ptx::upk2(ptx::add2(sa, sb), s0, s1);
-      s0 += __shfl_xor_sync(0xffffffffu, s0, 8);
-      s1 += __shfl_xor_sync(0xffffffffu, s1, 8);
-      s0 += __shfl_xor_sync(0xffffffffu, s0, 16);
-      s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
-      const float m0 = s0 * (1.0f / kC), m1 = s1 * (1.0f / kC);
-      const ptx::f32x2 nm = ptx::pk2(-m0, -m1);
-      ptx::f32x2 qa = ptx::pk2(0.f, 0.f), qb = qa;
-#pragma unroll
-      for (int i = 0; i < 32; i += 2) {
-        const ptx::f32x2 d0 = ptx::add2(ptx::bf16x2_to_f32x2(w[i]), nm);
-        const ptx::f32x2 d1 = ptx::add2(ptx::bf16x2_to_f32x2(w[i + 1]), nm);
-        qa = ptx::fma2(d0, d0, qa);
-        qb = ptx::fma2(d1, d1, qb);
-      }
-      float q0, q1;
-      ptx::upk2(ptx::add2(qa, qb), q0, q1);
-      q0 += __shfl_xor_sync(0xffffffffu, q0, 8);
-      q1 += __shfl_xor_sync(0xffffffffu, q1, 8);
-      q0 += __shfl_xor_sync(0xffffffffu, q0, 16);
-      q1 += __shfl_xor_sync(0xffffffffu, q1, 16);
-      const float r0 = rsqrtf(q0 * (1.0f / kC) + prm.eps), r1 = rsqrtf(q1 * (1.0f / kC) + prm.eps);
-      const ptx::f32x2 rr = ptx::pk2(r0, r1);
-      const ptx::f32x2 nn = ptx::pk2(-m0 * r0, -m1 * r1);
-#pragma unroll
-      for (uint32_t g = 0; g < 4; ++g)
-#pragma unroll
-        for (uint32_t jj = 0; jj < 8; ++jj)
-          ptx::sts32(tile + toff[jj] + g * 1024u,
-                     ptx::pack_norm2<kNormFp16>(
-                         ptx::fma2(ptx::bf16x2_to_f32x2(w[g * 8 + jj]), rr, nn)));
       ptx::fence_proxy_async_smem();
-      ptx::mbar_arrive(oready(s));
+      __syncwarp();
+      if (lane == 0) {
+        ptx::mbar_arrive(sready(s));
+        ptx::mbar_arrive(sempty(s));
+      }
+      K3_PROBE_ADD(oc, t2);
     }
-  } else if (warp >= kWarpEpi) {
-    // ===================== epilogue (thread = pair, 64 output channels) =====================
+    if (threadIdx.x == kWarpLno * 32) {
+      K3_PROBE_PUT(6, ow);
+      K3_PROBE_PUT(7, oc);
+    }
+  } else if (warp >= kWarpEpi && warp < kWarpLno) {
+    // ===================== epilogue =====================
+    ptx::setmaxnreg_inc<kRegsEpi>();
+    // tcgen05.ld in the fragment shape 16x256b: a thread holds COLUMN PAIRS (two adjacent output
+    // channels = one bf16x2 word of the output) of four pairs, see ptx::tmem_ld_16x256b_x4.
+    // Warp = (lane quadrant q) x (32-channel part e of the 64 channels in flight); the tile's two
+    // channel halves go one after the other through ONE [128 pairs][64 ch] staging buffer, a half's
+    // outputs being computed into registers first so that the wait for the previous TMA store to
+    // have read the buffer is covered by arithmetic.
     const int q = warp & 3;                       // TMEM lane quadrant (hardware: warp % 4)
-    const int h = (warp - kWarpEpi) >> 2;               // channel half
-    const int r = q * 32 + lane;                  // pair within the tile
-    const uint32_t stage_buf = smem + kOffOut + h * kHalfBox;
-    const uint32_t row_addr = stage_buf + r * 128;
-    const uint32_t sw = static_cast<uint32_t>(r & 7);
-    const bool store_thread = (q == 0 && lane == 0);
-    const uint32_t bar_id = 1 + h;
-    constexpr float kLog2e = 1.4426950408889634f;
-    constexpr float kGateScale = kTanhSigmoid ? 0.5f : -kLog2e;
-    const ptx::f32x2 gscale2 = ptx::pk2(kGateScale, kGateScale);
-    const ptx::f32x2 one2 = ptx::pk2(1.0f, 1.0f);
-    (void)gscale2;
-    (void)one2;
-    // folded biases (fp32) of this thread's 64 channels
-    const uint32_t tg_addr = smem + kOffVec + h * 64 * 4, to_addr = tg_addr + kC * 4;
+    const int e = (warp - kWarpEpi) >> 2;         // which 32 of the 64 channels
+    const uint32_t t4 = static_cast<uint32_t>(lane & 3), r8 = static_cast<uint32_t>(lane >> 2);
+    // this thread's four pairs: row(lh, ab) = q * 32 + lh * 16 + ab * 8 + r8
+    const uint32_t row0 = static_cast<uint32_t>(q) * 32u + r8;
+    const uint32_t stage_buf = smem + kOffOut;
+    const uint32_t row_addr = stage_buf + row0 * 128u + t4 * 4u;    // swizzle phase = row & 7 = r8
+    const bool store_thread = (warp == kWarpEpi && lane == 0);
+    constexpr uint32_t kEpiBar = 1;
     // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
-    auto load_mask = [&](int t) -> unsigned short {
-      if (prm.mask == nullptr) return static_cast<unsigned short>(0x3f80);   // bf16 1.0
-      if (t >= prm.num_tiles) return static_cast<unsigned short>(0);
-      const long long p = static_cast<long long>(t) * kTilePairs + r;
-      return p < prm.R ? __ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)
-                       : static_cast<unsigned short>(0);
+    auto load_mask = [&](int t, uint32_t i) -> uint32_t {
+      if (prm.mask == nullptr) return 0x3f80u;   // bf16 1.0
+      if (t >= prm.num_tiles) return 0u;
+      const long long p = static_cast<long long>(t) * kTilePairs + row0 + i * 8u;
+      return p < prm.R ? static_cast<uint32_t>(__ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)) : 0u;
     };
-    unsigned short mnext = load_mask(first);
+    uint32_t mnext[4];
+#pragma unroll
+    for (uint32_t i = 0; i < 4; ++i) mnext[i] = load_mask(first, i);
+    K3_PROBE_DECL(ew_s);
+    K3_PROBE_DECL(ew_t);
+    K3_PROBE_DECL(ew_b1);
+    K3_PROBE_DECL(ew_b2);
+    K3_PROBE_DECL(ew_ld);
+    K3_PROBE_T0(e0t);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+      const int s = it & 1;
       const int slot = it & 1;
-      const unsigned short mraw = mnext;
-      mnext = load_mask(t + stride);
-      ptx::mbar_wait(tfull(slot), (it >> 1) & 1);
+      float mval[4];
+      bool ones = true;
+#pragma unroll
+      for (uint32_t i = 0; i < 4; ++i) {
+        mval[i] = __uint_as_float(mnext[i] << 16);
+        ones = ones && mnext[i] == 0x3f80u;
+        mnext[i] = load_mask(t + stride, i);
+      }
+      const bool masked = !__all_sync(0xffffffffu, ones);   // warp-uniform
+      K3_PROBE_T0(t2);
+      ptx::mbar_wait(sready(s), (it >> 1) & 1);             // rstd of this tile (long complete:
+      ptx::mbar_wait(tfull(slot), (it >> 1) & 1);           // the correction MMAs waited for it)
+      K3_PROBE_ADD(ew_t, t2);
       ptx::tc_fence_after();
-      const float mval = __uint_as_float(static_cast<uint32_t>(mraw) << 16);
-      const ptx::f32x2 mval2 = ptx::pk2(mval, mval);
-      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + h * 64;
-      const long long p = static_cast<long long>(t) * kTilePairs + r;
+      // (rstd_z, rstd_o) of this thread's four pairs; then the stage may be refilled
+      float rz[4], ro[4];
 #pragma unroll
-      for (int chunk = 0; chunk < 4; ++chunk) {
-        // residual: this pair's 16 raw z channels (the tile was just read by TMA: an L2 hit)
-        uint4 zr0 = make_uint4(0u, 0u, 0u, 0u), zr1 = zr0;
-        if (prm.z_res != nullptr && p < prm.R) {
-          const uint4* zp = reinterpret_cast<const uint4*>(prm.z_res + p * kC + h * 64 + chunk * 16);
-          zr0 = __ldg(zp);
-          zr1 = __ldg(zp + 1);
-        }
-        const uint32_t zr[8] = {zr0.x, zr0.y, zr0.z, zr0.w, zr1.x, zr1.y, zr1.z, zr1.w};
-        uint32_t vg[16], vo[16];
-        ptx::tmem_ld_32x16(taddr + chunk * 16, vg);
-        ptx::tmem_ld_32x16(taddr + 128 + chunk * 16, vo);
-        ptx::tmem_ld_wait();
-        if (chunk == 3) {
-          ptx::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) ptx::mbar_arrive(tempty(slot));
-        }
-        uint32_t packed[8];
-        if (K3_DBG_SKIP(4)) {
+      for (uint32_t i = 0; i < 4; ++i)
+        ptx::upk2(ptx::lds64x(smem + kOffRstd + s * kTilePairs * 8 + (row0 + i * 8u) * 8u), rz[i], ro[i]);
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(sempty(s));
+      const uint32_t tbase = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + e * 32;
+      const long long p0 = static_cast<long long>(t) * kTilePairs + row0;
 #pragma unroll
-          for (int i = 0; i < 8; ++i) packed[i] = vo[2 * i] ^ vg[2 * i + 1];
-        } else {
+      for (int h = 0; h < 2; ++h) {
+        uint32_t packed[16];
 #pragma unroll
-        for (int j4 = 0; j4 < 4; ++j4) {
-          ptx::f32x2 bg2[2], bo2[2];
-          ptx::lds128x2(tg_addr + (chunk * 16 + j4 * 4) * 4, bg2);
-          ptx::lds128x2(to_addr + (chunk * 16 + j4 * 4) * 4, bo2);
+        for (int lh = 0; lh < 2; ++lh) {
+          uint32_t vg[16], vo[16];
+          const uint32_t ta = tbase + (static_cast<uint32_t>(lh * 16) << 16) + h * 64;
+          K3_PROBE_T0(t5);
+          ptx::tmem_ld_16x256b_x4(ta, vg);
+          ptx::tmem_ld_16x256b_x4(ta + 128, vo);
+          ptx::tmem_ld_wait();
+          K3_PROBE_ADD(ew_ld, t5);
+          if (h == 1 && lh == 1) {
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(tempty(slot));
+          }
+          auto chunk = [&](auto masked_tag) {
+            constexpr bool kMasked = decltype(masked_tag)::value;
 #pragma unroll
-          for (int e2 = 0; e2 < 2; ++e2) {
-            const int j = j4 * 4 + e2 * 2;
-            const ptx::f32x2 zres = ptx::bf16x2_to_f32x2(zr[j4 * 2 + e2]);   // 0 without residual
-            const ptx::f32x2 y = ptx::mul2(ptx::add2(ptx::pk2u(vo[j], vo[j + 1]), bo2[e2]), mval2);
-            float g0, g1, v0, v1;
-            if constexpr (kTanhSigmoid) {
-              // y and the gate pre-activation arrive halved: out = (tanh(g/2) + 1) (y/2) [+ z]
-              ptx::upk2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bg2[e2]), g0, g1);
-              ptx::upk2(ptx::fma2(y, ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1)),
-                                  ptx::add2(y, zres)), v0, v1);
-            } else {
-              float d0, d1;
-              ptx::upk2(ptx::mul2(ptx::add2(ptx::pk2u(vg[j], vg[j + 1]), bg2[e2]), gscale2), g0, g1);
-              ptx::upk2(ptx::add2(ptx::pk2(ptx::ex2_approx(g0), ptx::ex2_approx(g1)), one2), d0, d1);
-              ptx::upk2(ptx::fma2(y, ptx::pk2(ptx::rcp_approx(d0), ptx::rcp_approx(d1)), zres), v0, v1);
+            for (int k = 0; k < 4; ++k) {
+#pragma unroll
+              for (int ab = 0; ab < 2; ++ab) {
+                const int j = 4 * k + 2 * ab;
+                const int ri = lh * 2 + ab;
+                // g/2 = rstd_z D_g ,  y/2 = rstd_o D_o  (everything else is already in D)
+                const ptx::f32x2 gx = ptx::mul2(ptx::pk2u(vg[j], vg[j + 1]), ptx::pk2(rz[ri], rz[ri]));
+                const ptx::f32x2 y = ptx::mul2(ptx::pk2u(vo[j], vo[j + 1]), ptx::pk2(ro[ri], ro[ri]));
+                float g0, g1, v0, v1;
+                ptx::upk2(gx, g0, g1);
+                const ptx::f32x2 th = K3_DBG_SKIP(32) ? gx : ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1));
+                // out = M (tanh(g/2) + 1) (y/2) [+ z]; the same roundings with and without the
+                // mask, so that M = 1 gives the unmasked bits
+                ptx::f32x2 v = ptx::fma2(y, th, y);
+                if constexpr (kResidual) {
+                  uint32_t zw = 0u;
+                  const long long p = p0 + lh * 16 + ab * 8;
+                  const int ch = h * 64 + e * 32 + k * 8;
+                  if (p < prm.R) zw = __ldg(reinterpret_cast<const uint32_t*>(prm.z_res + p * kC + ch) + t4);
+                  const ptx::f32x2 zres = ptx::bf16x2_to_f32x2(zw);
+                  if constexpr (kMasked) v = ptx::fma2(v, ptx::pk2(mval[ri], mval[ri]), zres);
+                  else v = ptx::add2(v, zres);
+                } else {
+                  if constexpr (kMasked) v = ptx::mul2(v, ptx::pk2(mval[ri], mval[ri]));
+                }
+                ptx::upk2(v, v0, v1);
+                packed[lh * 8 + k * 2 + ab] = K3_DBG_SKIP(64) ? (__float_as_uint(v0) ^ __float_as_uint(v1)) : ptx::pack_bf16x2(v0, v1);
+              }
             }
-            packed[j4 * 2 + e2] = ptx::pack_bf16x2(v0, v1);
+          };
+          if (K3_DBG_SKIP(4)) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) packed[lh * 8 + i] = vo[2 * i] ^ vg[2 * i + 1];
+          } else if (masked) {
+            chunk(std::true_type{});
+          } else {
+            chunk(std::false_type{});
           }
         }
+        // the previous store out of the staging buffer has read it
+        K3_PROBE_T0(t3);
+        if (store_thread && !K3_DBG_SKIP(8)) ptx::tma_store_wait_read<0>();
+        ptx::named_bar_sync(kEpiBar, kEpiWarps * 32);
+        K3_PROBE_ADD(ew_b1, t3);
+#pragma unroll
+        for (int lh = 0; lh < 2; ++lh)
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int ab = 0; ab < 2; ++ab)
+              ptx::sts32(row_addr + (lh * 16 + ab * 8) * 128 +
+                             ((static_cast<uint32_t>(e * 4 + k) ^ r8) << 4),
+                         packed[lh * 8 + k * 2 + ab]);
+        ptx::fence_proxy_async_smem();
+        K3_PROBE_T0(t4);
+        ptx::named_bar_sync(kEpiBar, kEpiWarps * 32);
+        K3_PROBE_ADD(ew_b2, t4);
+        if (store_thread && !K3_DBG_SKIP(16)) {
+          ptx::tma_store_2d(&tmap_out, stage_buf, h * 64, t * kTilePairs);
+          ptx::tma_store_commit();
         }
-        if (chunk == 0) {
-          if (store_thread) ptx::tma_store_wait_read<0>();
-          ptx::named_bar_sync(bar_id, 128);
-        }
-        ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2) ^ sw) << 4), packed[0], packed[1],
-                    packed[2], packed[3]);
-        ptx::sts128(row_addr + ((static_cast<uint32_t>(chunk * 2 + 1) ^ sw) << 4), packed[4],
-                    packed[5], packed[6], packed[7]);
       }
-      ptx::fence_proxy_async_smem();
-      ptx::named_bar_sync(bar_id, 128);
-      if (store_thread) {
-        ptx::tma_store_2d(&tmap_out, stage_buf, h * 64, t * kTilePairs);
-        ptx::tma_store_commit();
-      }
+    }
+    if (store_thread) {
+      K3_PROBE_PUT(8, ew_s);
+      K3_PROBE_PUT(9, ew_t);
+      K3_PROBE_PUT(10, ew_b1);
+      K3_PROBE_PUT(11, ew_b2);
+      K3_PROBE_PUT(12, clock64() - e0t);
+      K3_PROBE_PUT(14, ew_ld);
     }
     if (store_thread) ptx::tma_store_wait<0>();
   }
@@ -464,18 +725,13 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
 }
 
-bool k3_tanh_sigmoid() {
-  static const bool v = [] {
-    const char* e = debug_env("FOLDCP_K3_SIGMOID");   // "exp" = ex2+rcp (2 MUFU), default tanh (1 MUFU)
-    return !(e && e[0] == 'e');
-  }();
-  return v;
-}
-
 }  // namespace
 
+// o_f16: o holds IEEE fp16 values scaled by o_scale (a power of two; K2 on the fused path), else
+// bf16 unscaled (o_scale = 1)
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
-                            const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream) {
+                            const foldcp_trimul_params* p, int N, void* out, bool o_f16,
+                            float o_scale, cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   const uint64_t R = static_cast<uint64_t>(N) * N;
@@ -513,7 +769,8 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   prm.w_o = static_cast<const __nv_bfloat16*>(p->w_o);
   prm.bias_g = p->b_g;
   prm.bias_o = p->b_o;
-  prm.eps = p->ln_eps;
+  prm.eps_z = p->ln_eps;
+  prm.eps_o = p->ln_eps * o_scale * o_scale;
   prm.R = static_cast<long long>(R);
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
   static const int dbg_skip = [] {
@@ -522,8 +779,9 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   }();
   prm.dbg_skip = dbg_skip;
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
-  const bool tanh_sig = k3_tanh_sigmoid();
-  auto kern = tanh_sig ? k3_finalize_kernel<true> : k3_finalize_kernel<false>;
+  const bool res = p->add_residual != 0;
+  auto kern = o_f16 ? (res ? k3_finalize_kernel<true, true> : k3_finalize_kernel<true, false>)
+                    : (res ? k3_finalize_kernel<false, true> : k3_finalize_kernel<false, false>);
   if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), kSmemBytes) != FOLDCP_OK)
     return FOLDCP_ERR_CUDA;
   kern<<<grid, kThreads, kSmemBytes, stream>>>(tz, to, twg, two, tout, prm);
@@ -531,3 +789,10 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
 }
 
 }  // namespace foldcp
+
+#ifdef FOLDCP_K3_PROBE
+extern "C" int foldcp_debug_k3_probe_read(unsigned long long* host_out) {
+  return static_cast<int>(cudaMemcpyFromSymbol(host_out, foldcp::g_k3_probe,
+                                               sizeof(unsigned long long) * 160 * 16));
+}
+#endif

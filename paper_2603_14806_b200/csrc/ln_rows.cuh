@@ -125,4 +125,77 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
   }
 }
 
+// LayerNorm STATISTICS of the same tile, nothing written back to it: per pair row r, mean and
+// biased variance over the 128 channels, handed to `emit(row, mean, var)` by ONE lane per row (a
+// consumer then applies the normalisation after the GEMM, see k3_finalize.cu).  One sweep over the
+// row with a shifted accumulation: d = x - c with c the row's own first channel, S1 = sum d,
+// S2 = sum d^2, mean = c + S1 / 128, var = S2 / 128 - (S1 / 128)^2.  The shift is a sample of the
+// row, so |mean - c| is of the order of the row's spread and the subtraction cancels nothing that
+// matters, whatever the row's common offset (|mean| >> sigma is as safe as with two passes).
+// kLnThreads (128 or 256) threads, four adjacent lanes per row, kRows rows per thread in flight.
+template <int kRows, int kLnThreads, typename Emit>
+__device__ __forceinline__ void layernorm_rows_stats(uint32_t tile, uint32_t box_stride, int tid,
+                                                     Emit&& emit) {
+  const uint32_t j = static_cast<uint32_t>(tid & 3);
+  const uint32_t box = j >> 1;
+  const uint32_t cbase = (j & 1u) * 4u;
+  constexpr int kRowStep = kLnThreads / 4;                    // rows between a thread's rows in flight
+  constexpr int kRowsPerPass = kRowStep * kRows;
+  static_assert(128 % kRowsPerPass == 0 && kRowStep % 8 == 0, "unsupported LayerNorm shape");
+#pragma unroll 1
+  for (int pass = 0; pass < 128 / kRowsPerPass; ++pass) {
+    const uint32_t r0 = static_cast<uint32_t>(pass * kRowsPerPass + (tid >> 2));
+    const uint32_t sw = r0 & 7u;                              // (r0 + kRowStep) & 7 is the same
+    const uint32_t row0 = tile + box * box_stride + r0 * 128u;
+    uint32_t w[kRows][4][4];
+#pragma unroll
+    for (uint32_t q = 0; q < kRows; ++q)
+#pragma unroll
+      for (uint32_t t = 0; t < 4; ++t)
+        ptx::lds128(row0 + q * (kRowStep * 128u) + (((cbase + (t ^ j)) ^ sw) << 4), w[q][t]);
+    float s1[kRows], s2[kRows], c[kRows];
+#pragma unroll
+    for (int q = 0; q < kRows; ++q) {
+      // the shift: the first channel lane 0 of the row's quad loaded -- any channel would do
+      c[q] = __shfl_sync(0xffffffffu, ptx::bf16_lo(w[q][0][0]), tid & 28);
+      const ptx::f32x2 nc = ptx::pk2(-c[q], -c[q]);
+      ptx::f32x2 a0 = ptx::pk2(0.f, 0.f), a1 = a0, b0 = a0, b1 = a0;
+#pragma unroll
+      for (int t = 0; t < 4; ++t)
+#pragma unroll
+        for (int e = 0; e < 4; e += 2) {
+          const ptx::f32x2 d0 = ptx::add2(ptx::bf16x2_to_f32x2(w[q][t][e]), nc);
+          const ptx::f32x2 d1 = ptx::add2(ptx::bf16x2_to_f32x2(w[q][t][e + 1]), nc);
+          a0 = ptx::add2(a0, d0);
+          a1 = ptx::add2(a1, d1);
+          b0 = ptx::fma2(d0, d0, b0);
+          b1 = ptx::fma2(d1, d1, b1);
+        }
+      float lo, hi;
+      ptx::upk2(ptx::add2(a0, a1), lo, hi);
+      s1[q] = lo + hi;
+      ptx::upk2(ptx::add2(b0, b1), lo, hi);
+      s2[q] = lo + hi;
+    }
+#pragma unroll
+    for (int q = 0; q < kRows; ++q) {
+      s1[q] += __shfl_xor_sync(0xffffffffu, s1[q], 1);
+      s2[q] += __shfl_xor_sync(0xffffffffu, s2[q], 1);
+    }
+#pragma unroll
+    for (int q = 0; q < kRows; ++q) {
+      s1[q] += __shfl_xor_sync(0xffffffffu, s1[q], 2);
+      s2[q] += __shfl_xor_sync(0xffffffffu, s2[q], 2);
+    }
+    if (j == 0) {
+#pragma unroll
+      for (uint32_t q = 0; q < kRows; ++q) {
+        const float md = s1[q] * (1.0f / 128.0f);
+        const float var = fmaxf(fmaf(-md, md, s2[q] * (1.0f / 128.0f)), 0.f);
+        emit(r0 + q * kRowStep, c[q] + md, var);
+      }
+    }
+  }
+}
+
 }  // namespace foldcp

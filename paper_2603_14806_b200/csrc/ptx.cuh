@@ -331,6 +331,32 @@ __device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t (&v)[16])
       : "r"(taddr)
       : "memory");
 }
+// TMEM -> registers in the matrix-fragment shape 16x256b (measured on sm_100a): the warp reads 16
+// lanes (the lane field of taddr: this warp's quadrant base, +0 or +16) x 16 consecutive fp32
+// columns; thread T gets, for k = 0, 1:
+//   v[4k + 0], v[4k + 1] = lane T/4,     columns 8k + 2 (T%4), + 1
+//   v[4k + 2], v[4k + 3] = lane T/4 + 8, the same two columns
+// i.e. a thread owns column PAIRS of a few rows instead of one whole row: per-column constants are
+// then needed for 4 columns per thread and load, not 16.
+__device__ __forceinline__ void tmem_ld_16x256b_x2(uint32_t taddr, uint32_t (&v)[8]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
+        "=r"(v[7])
+      : "r"(taddr)
+      : "memory");
+}
+// the same shape over 32 columns (k = 0..3)
+__device__ __forceinline__ void tmem_ld_16x256b_x4(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.16x256b.x4.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
+        "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]),
+        "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr)
+      : "memory");
+}
 // registers -> TMEM: this warp's 32 lanes x 32 consecutive 32-bit columns
 __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&v)[32]) {
   asm volatile(
@@ -375,6 +401,19 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr, uin
   d |= static_cast<uint64_t>((sbo_bytes >> 4) & 0x3FFF) << 32;
   d |= static_cast<uint64_t>(1) << 46;
   d |= static_cast<uint64_t>(2) << 61;
+  return d;
+}
+
+// The same descriptor without swizzle (layout type 0): 8-row x 16-byte core matrices, each 128
+// contiguous bytes.  K-major operand: element (row r, k) of a 16-bit type sits at
+//   (r / 8) * sbo + (k / 8) * lbo + (r % 8) * 16 + (k % 8) * 2.
+__device__ __forceinline__ uint64_t make_smem_desc_noswizzle(uint32_t smem_addr, uint32_t lbo_bytes,
+                                                             uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= static_cast<uint64_t>((smem_addr & 0x3FFFF) >> 4);
+  d |= static_cast<uint64_t>((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= static_cast<uint64_t>((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= static_cast<uint64_t>(1) << 46;
   return d;
 }
 
@@ -530,6 +569,11 @@ __device__ __forceinline__ uint32_t pack_norm2(f32x2 v) {
   float lo, hi;
   upk2(v, lo, hi);
   return pack_norm<kF16>(lo, hi);
+}
+__device__ __forceinline__ f32x2 lds64x(uint32_t addr) {
+  f32x2 v;
+  asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+  return v;
 }
 __device__ __forceinline__ void lds128x2(uint32_t addr, f32x2 (&v)[2]) {
   asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v[0]), "=l"(v[1]) : "r"(addr));
