@@ -184,11 +184,20 @@ bool bf16_on_tensor_cores() {
 
 using namespace foldcp;
 
+namespace {
+// (mean, rstd) of LayerNorm(z) per pair, handed from K1 to K3 in bf16 mode; a multiple of 256 bytes
+size_t z_stats_bytes(int N, int dtype) {
+  if (dtype != FOLDCP_BF16) return 0;
+  return (static_cast<size_t>(N) * N * sizeof(float2) + 255) & ~static_cast<size_t>(255);
+}
+}  // namespace
+
 extern "C" {
 
 size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype) {
   if (check_shape(N, c_z, c_hidden, dtype) != FOLDCP_OK) return 0;
-  return 3 * static_cast<size_t>(kChannels) * N * N * elem_bytes(dtype) + kSchedScratchBytes;
+  return 3 * static_cast<size_t>(kChannels) * N * N * elem_bytes(dtype) + z_stats_bytes(N, dtype) +
+         kSchedScratchBytes;
 }
 
 namespace {
@@ -208,22 +217,24 @@ namespace {
 // the stage bodies: arguments already validated, scheduler words already zeroed on the stream.
 // ab_f16: in bf16 mode the intermediates a, b are IEEE fp16 (forward path) rather than bf16.
 int project_stage(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
-                  void* a, void* b, bool ab_f16, void* sched_area, cudaStream_t s) {
+                  void* a, void* b, bool ab_f16, void* z_stats, void* sched_area, cudaStream_t s) {
   if (params->dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
-    return launch_k1_project_bf16(z, mask, params, N, a, b, ab_f16, sched_word(sched_area, 0), s);
+    return launch_k1_project_bf16(z, mask, params, N, a, b, ab_f16, z_stats,
+                                  sched_word(sched_area, 0), s);
   return launch_simt_project(z, mask, params, N, a, b, s);
 }
 int contract_stage(const void* a, const void* b, int N, int dtype, int direction, void* o,
-                   bool ab_f16, void* sched_area, int word, cudaStream_t s) {
+                   bool ab_f16, float o_f16_scale, void* sched_area, int word, cudaStream_t s) {
   if (dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
-    return launch_k2_contract_bf16(a, b, o, N, direction, ab_f16, sched_word(sched_area, word), s);
+    return launch_k2_contract_bf16(a, b, o, N, direction, ab_f16, o_f16_scale,
+                                   sched_word(sched_area, word), s);
   return launch_simt_contract(a, b, o, N, dtype, direction, s);
 }
 int finalize_stage(const void* o, const void* z, const void* mask,
                    const foldcp_trimul_params* params, int N, void* out, bool o_f16, float o_scale,
-                   cudaStream_t s) {
+                   const void* z_stats, cudaStream_t s) {
   if (params->dtype == FOLDCP_BF16 && bf16_on_tensor_cores())
-    return launch_k3_finalize_bf16(o, z, mask, params, N, out, o_f16, o_scale, s);
+    return launch_k3_finalize_bf16(o, z, mask, params, N, out, o_f16, o_scale, z_stats, s);
   return launch_simt_finalize(o, z, mask, params, N, out, s);
 }
 }  // namespace
@@ -244,7 +255,7 @@ int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_p
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((st = prepare_scratch(scratch, params->dtype, s)) != FOLDCP_OK) return st;
-  return project_stage(z, mask, params, N, a, b, /*ab_f16=*/true, scratch, s);
+  return project_stage(z, mask, params, N, a, b, /*ab_f16=*/true, nullptr, scratch, s);
 }
 
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
@@ -265,7 +276,7 @@ int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, in
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
-  return contract_stage(a, b, N, dtype, direction, o, ab_f16, scratch, 0, s);
+  return contract_stage(a, b, N, dtype, direction, o, ab_f16, 0.f, scratch, 0, s);
 }
 
 int foldcp_trimul_contract_blocks(const void* const* a_blocks, const void* const* b_blocks,
@@ -335,7 +346,8 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
   const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
   if (overlaps(out, bytes, z, bytes) || overlaps(out, bytes, o, bytes)) return FOLDCP_ERR_ALIAS;
   if ((st = check_arch()) != FOLDCP_OK) return st;
-  return finalize_stage(o, z, mask, params, N, out, false, 1.0f, static_cast<cudaStream_t>(stream));
+  return finalize_stage(o, z, mask, params, N, out, false, 1.0f, nullptr,
+                        static_cast<cudaStream_t>(stream));
 }
 
 int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
@@ -356,19 +368,24 @@ int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* p
     return FOLDCP_ERR_ALIAS;
   if ((st = check_arch()) != FOLDCP_OK) return st;
 
-  // workspace: a | b | o (channel-major) | tile counters of this call
+  // workspace: a | b | o (channel-major) | LayerNorm(z) statistics (bf16 mode) | tile counters
   uint8_t* ws = static_cast<uint8_t*>(params->workspace);
   void* a = ws;
   void* b = ws + tensor_bytes;
   void* o = ws + 2 * tensor_bytes;
-  void* sched_area = ws + 3 * tensor_bytes;
+  const bool tc = params->dtype == FOLDCP_BF16 && bf16_on_tensor_cores();
+  void* z_stats = tc ? ws + 3 * tensor_bytes : nullptr;
+  void* sched_area = ws + 3 * tensor_bytes + z_stats_bytes(N, params->dtype);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (params->dtype == FOLDCP_BF16 && (st = arm_sched_words(sched_area, s)) != FOLDCP_OK) return st;
-  if ((st = project_stage(z, mask, params, N, a, b, true, sched_area, s)) != FOLDCP_OK) return st;
-  if ((st = contract_stage(a, b, N, params->dtype, direction, o, true, sched_area, 1, s)) !=
+  if ((st = project_stage(z, mask, params, N, a, b, true, z_stats, sched_area, s)) != FOLDCP_OK)
+    return st;
+  // bf16 mode: o travels from K2 to K3 as fp16 scaled by ~1/sqrt(N) (see contract_o_scale)
+  const float o_scale = tc ? contract_o_scale(N) : 0.f;
+  if ((st = contract_stage(a, b, N, params->dtype, direction, o, true, o_scale, sched_area, 1, s)) !=
       FOLDCP_OK)
     return st;
-  return finalize_stage(o, z, mask, params, N, out, false, 1.0f, s);
+  return finalize_stage(o, z, mask, params, N, out, tc, tc ? o_scale : 1.0f, z_stats, s);
 }
 
 namespace {
@@ -431,8 +448,9 @@ int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
   if (dt == FOLDCP_BF16 && (st = arm_sched_words(sched_area, s)) != FOLDCP_OK) return st;
   // recompute the forward intermediates with the forward kernels; a and b as bf16 here, because
   // the gradient GEMMs below pair them with the bf16 d_o (one operand format per tcgen05.mma)
-  if ((st = project_stage(z, mask, params, N, a, b, false, sched_area, s)) != FOLDCP_OK) return st;
-  if ((st = contract_stage(a, b, N, dt, direction, o, false, sched_area, 1, s)) != FOLDCP_OK)
+  if ((st = project_stage(z, mask, params, N, a, b, false, nullptr, sched_area, s)) != FOLDCP_OK)
+    return st;
+  if ((st = contract_stage(a, b, N, dt, direction, o, false, 0.f, sched_area, 1, s)) != FOLDCP_OK)
     return st;
   // the tail around the contraction: tcgen05 kernels in bf16 mode, CUDA-core kernels in fp32 mode
   const bool tc = dt == FOLDCP_BF16 && bf16_on_tensor_cores();

@@ -67,9 +67,20 @@ int encode_tensor_map(CUtensorMap* map, const void* base, int elem_bytes, int ra
 
 // ----- stage launchers (device pointers; return foldcp_status_t) -----
 // `sched`: zeroed tile-scheduler counter(s) of this launch (see kSchedScratchBytes)
-// ab_f16: a and b hold IEEE fp16 (forward path) instead of bf16; o is bf16 either way
+// ab_f16: a and b hold IEEE fp16 (forward path) instead of bf16.
+// o_f16_scale: 0 = o is written as bf16; otherwise o is written as IEEE fp16 after multiplication
+// by this power of two (the fused forward path: K3's LayerNorm(o) absorbs the scale exactly through
+// eps * scale^2, and fp16 carries 11 significant bits where bf16 carries 8)
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            bool ab_f16, unsigned int* sched, cudaStream_t stream);
+                            bool ab_f16, float o_f16_scale, unsigned int* sched,
+                            cudaStream_t stream);
+// the scale of the fused path: 2^-ceil(log2(N) / 2), i.e. about 1 / sqrt(N) -- o is a sum of N
+// products a b, typically sqrt(N) sigma_a sigma_b, at worst N max|a b|; fp16 holds up to 65504
+inline float contract_o_scale(int N) {
+  int lg = 0;
+  while ((1 << lg) < N) ++lg;
+  return 1.0f / static_cast<float>(1 << ((lg + 1) / 2));
+}
 
 // blocked (Cannon) form: o_block[c][nb][nb] = sum_q contraction(a_blocks[q], b_blocks[q]), each
 // block a dense [c][nb][nb] tensor, nq <= kMaxContractBlocks; accumulator resident in TMEM
@@ -93,14 +104,16 @@ int launch_simt_contract_backward(const void* d_o, const void* a, const void* b,
 int launch_simt_finalize(const void* o, const void* z, const void* mask,
                          const foldcp_trimul_params* p, int N, void* out, cudaStream_t stream);
 
+// z_stats: [N*N] float2 (mean, rstd) of LayerNorm(z) written for K3 (fused path), or nullptr
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
-                           void* a, void* b, bool ab_f16, unsigned int* sched,
+                           void* a, void* b, bool ab_f16, void* z_stats, unsigned int* sched,
                            cudaStream_t stream);
 // o_f16: o holds fp16 values scaled by the power of two o_scale (the fused path, see
 // contract_o_scale); otherwise bf16 with o_scale = 1 (stage entry point, backward recomputation)
+// z_stats: what K1 wrote (see above), or nullptr: K3 then computes the statistics of z itself
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
                             const foldcp_trimul_params* p, int N, void* out, bool o_f16,
-                            float o_scale, cudaStream_t stream);
+                            float o_scale, const void* z_stats, cudaStream_t stream);
 
 // Backward pass around the contraction (simt_backward.cu): phase 0 = K3-backward (o -> d_o in
 // place, dzp written), 1 = K1-backward for a, 2 = K1-backward for b + LayerNorm(z) backward.

@@ -89,6 +89,7 @@ struct K1Params {
   long long R;                 // number of pairs
   int num_tiles;
   unsigned int* sched;
+  float2* stats;               // [R] (mean, rstd) of every pair's LayerNorm(z), or nullptr: K3 re-uses them
 };
 
 // kOutF16: a and b are written as IEEE fp16 (the forward path: 11-bit significand, see the header's
@@ -261,7 +262,11 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       mnext = load_mask(tnext);
       ptx::mbar_wait(zfull(s), (it / kZStages) & 1);
       layernorm_rows_inplace<kNormFp16, false, kLnWarps == 4 ? 2 : 1, kLnWarps * 32>(
-          smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0, prm.eps);
+          smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0, prm.eps,
+          [&](uint32_t row, float mean, float rstd) {
+            const long long p = static_cast<long long>(t) * kTilePairs + row;
+            if (prm.stats != nullptr && p < prm.R) prm.stats[p] = make_float2(mean, rstd);
+          });
       const int ms = it & (kMaskSlots - 1);
       if (r < kTilePairs) {   // warp-uniform: the first four LayerNorm warps stage mask and flag
         reinterpret_cast<float*>(smem_raw + kOffMask)[ms * kTilePairs + r] =
@@ -469,7 +474,7 @@ bool k1_tanh_sigmoid() {
 }  // namespace
 
 int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_params* p, int N,
-                           void* a, void* b, bool ab_f16, unsigned int* sched,
+                           void* a, void* b, bool ab_f16, void* z_stats, unsigned int* sched,
                            cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
@@ -505,6 +510,7 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   prm.R = static_cast<long long>(R);
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
   prm.sched = sched;
+  prm.stats = static_cast<float2*>(z_stats);
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k1_tanh_sigmoid();
   auto kern = tanh_sig ? (ab_f16 ? k1_project_kernel<true, true> : k1_project_kernel<true, false>)

@@ -22,6 +22,8 @@
 // (K, K) and (MN, MN), the gradients of the contraction also the mixed (K, MN) form.
 // Tiles are not assigned statically: the leader's producer thread draws them in index order from
 // a global counter (tile_sched.cuh) and publishes them to the other roles through a small ring.
+#include <type_traits>
+
 #include "common.h"
 #include "ptx.cuh"
 #include "tile_sched.cuh"
@@ -90,6 +92,9 @@ struct K2Params {
   int panel_n;     // tile rasterisation: n-tiles per column panel (>= 1)
   unsigned int* sched;   // next tile index: launch-private, zeroed on the stream before the launch
   uint32_t ab_fmt;       // operand format of both inputs: ptx::kFmtBF16 or ptx::kFmtF16
+  int o_f16;             // 1: the result is written as IEEE fp16 after scaling by o_scale (the fused
+                         // forward path: K3 normalises o anyway, see contract_o_scale); 0: bf16
+  float o_scale;         // a power of two
 };
 
 // Tile rasterisation inside one channel: column panels of `panel_n` n-tiles, m fastest-varying
@@ -440,18 +445,25 @@ k2_contract_kernel(const __grid_constant__ K2Maps maps, const K2Params prm) {
           }
         }
         const uint32_t row_addr = buf + row * 128;
+        auto store_chunks = [&](auto f16_tag) {
+          constexpr bool kF16 = decltype(f16_tag)::value;
+          const float sc = prm.o_scale;
 #pragma unroll
-        for (int cchunk = 0; cchunk < 8; ++cchunk) {
-          const uint32_t* src = (cchunk < 4) ? &v0[cchunk * 8] : &v1[(cchunk - 4) * 8];
-          const uint32_t p0 = ptx::pack_bf16x2(__uint_as_float(src[0]), __uint_as_float(src[1]));
-          const uint32_t p1 = ptx::pack_bf16x2(__uint_as_float(src[2]), __uint_as_float(src[3]));
-          const uint32_t p2 = ptx::pack_bf16x2(__uint_as_float(src[4]), __uint_as_float(src[5]));
-          const uint32_t p3 = ptx::pack_bf16x2(__uint_as_float(src[6]), __uint_as_float(src[7]));
-          const uint32_t dst = row_addr + ((cchunk ^ (row & 7)) << 4);
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(p0), "r"(p1),
-                       "r"(p2), "r"(p3)
-                       : "memory");
-        }
+          for (int cchunk = 0; cchunk < 8; ++cchunk) {
+            const uint32_t* src = (cchunk < 4) ? &v0[cchunk * 8] : &v1[(cchunk - 4) * 8];
+            uint32_t pk[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float lo = __uint_as_float(src[2 * i]), hi = __uint_as_float(src[2 * i + 1]);
+              pk[i] = kF16 ? ptx::pack_f16x2(lo * sc, hi * sc) : ptx::pack_bf16x2(lo, hi);
+            }
+            const uint32_t dst = row_addr + ((cchunk ^ (row & 7)) << 4);
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(pk[0]), "r"(pk[1]),
+                         "r"(pk[2]), "r"(pk[3])
+                         : "memory");
+          }
+        };
+        if (prm.o_f16) store_chunks(std::true_type{}); else store_chunks(std::false_type{});
         ptx::fence_proxy_async_smem();
         ptx::named_bar_sync(1, 128);
         if (store_thread) {
@@ -511,7 +523,7 @@ int g_k2_cta_group = 2;
 // the blocked (Cannon) form.
 int launch_k2_gemm_blocks_bf16(const void* const* x, const void* const* y, int nq, void* d, int N,
                                bool x_mn, bool y_mn, bool xy_f16, unsigned int* sched,
-                               cudaStream_t stream) {
+                               cudaStream_t stream, float d_f16_scale = 0.f) {
   if (nq < 1 || nq > kMaxBlocks) return FOLDCP_ERR_UNSUPPORTED;
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
@@ -569,6 +581,8 @@ int launch_k2_gemm_blocks_bf16(const void* const* x, const void* const* y, int n
   prm.serpentine = serp;
   prm.sched = sched;
   prm.ab_fmt = xy_f16 ? ptx::kFmtF16 : ptx::kFmtBF16;
+  prm.o_f16 = d_f16_scale != 0.f ? 1 : 0;       // 0 = bf16 result, unscaled
+  prm.o_scale = d_f16_scale != 0.f ? d_f16_scale : 1.f;
   const int sms = dev.sm_count;
   if (cta_group == 2) {
     if (x_mn) return y_mn ? launch_variant<2, true, true>(maps, prm, sms, stream)
@@ -583,8 +597,9 @@ int launch_k2_gemm_blocks_bf16(const void* const* x, const void* const* y, int n
 }
 
 int launch_k2_gemm_bf16(const void* x, const void* y, void* d, int N, bool x_mn, bool y_mn,
-                        bool xy_f16, unsigned int* sched, cudaStream_t stream) {
-  return launch_k2_gemm_blocks_bf16(&x, &y, 1, d, N, x_mn, y_mn, xy_f16, sched, stream);
+                        bool xy_f16, unsigned int* sched, cudaStream_t stream,
+                        float d_f16_scale = 0.f) {
+  return launch_k2_gemm_blocks_bf16(&x, &y, 1, d, N, x_mn, y_mn, xy_f16, sched, stream, d_f16_scale);
 }
 
 // One rank's share of the Cannon-style distributed contraction: o_block = sum_q of Eq. 2 / Eq. 3 on
@@ -598,9 +613,10 @@ int launch_k2_contract_blocks_bf16(const void* const* a_blocks, const void* cons
 }
 
 int launch_k2_contract_bf16(const void* a, const void* b, void* o, int N, int direction,
-                            bool ab_f16, unsigned int* sched, cudaStream_t stream) {
+                            bool ab_f16, float o_f16_scale, unsigned int* sched,
+                            cudaStream_t stream) {
   const bool inc = direction == FOLDCP_INCOMING;
-  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, ab_f16, sched, stream);
+  return launch_k2_gemm_bf16(a, b, o, N, inc, inc, ab_f16, sched, stream, o_f16_scale);
 }
 
 // Gradients of the contraction (oracle/trimul_oracle.py contraction_backward):

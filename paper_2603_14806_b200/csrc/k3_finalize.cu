@@ -56,6 +56,11 @@
 
 #include <type_traits>
 
+// 28 warps, most of them waiting on an mbarrier most of the time: their try_wait loops would take
+// every fifth issue slot of the SM partition; with a suspend-time hint a waiting warp sleeps
+#ifndef FOLDCP_MBAR_HINT_NS
+#define FOLDCP_MBAR_HINT_NS 4000
+#endif
 #include "common.h"
 #include "ln_rows.cuh"
 #include "ptx.cuh"
@@ -79,13 +84,17 @@ constexpr int kThreads = (kWarpLnz + kLnzWarps) * 32;
 static_assert(kWarpEpi % 4 == 0, "epilogue warps must start at a TMEM lane-quadrant boundary");
 // 28 warps leave 72 registers per thread at launch; the twenty control / statistics warps give
 // some up (setmaxnreg, per aligned group of four warps) for the eight epilogue warps
-constexpr int kRegsOther = 56;
-constexpr int kRegsEpi = 104;
+constexpr int kRegsOther = 64;
+constexpr int kRegsEpi = 88;
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box (128 rows x 128 bytes)
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB
 constexpr int kStages = 2;
 constexpr int kStageBytes = 2 * kMatBytes;      // z tile + o tile
 constexpr int kXBytes = 128 * 16 * 2;           // 4 KB: a [128][16] correction operand
+// an overflowed fp32 variance (|x| beyond ~1e18, outside the documented range) must not turn into
+// 0 * inf: the variance is capped, so rstd >= 1e-19 and 1 / rstd stays finite
+constexpr float kMaxVar = 1.0e38f;
+constexpr float kMinRstd = 1.0e-19f;
 
 constexpr int kOffW = 0;                                   // W_g', W_o'
 constexpr int kOffStage = kOffW + 2 * kMatBytes;           // ring: [z | o] per stage
@@ -100,6 +109,7 @@ static_assert(kSmemBytes <= 232448, "K3 shared memory exceeds 227 KB");
 struct K3Params {
   const __nv_bfloat16* mask;   // [R] or nullptr (also nullptr when mask_output == 0)
   const __nv_bfloat16* z_res;  // z [R][128] when out = z + update (add_residual), else nullptr
+  const float2* z_stats;       // [R] (mean, rstd) of LayerNorm(z) from K1, or nullptr: computed here
   const float* g_in;
   const float* b_in;
   const float* g_out;
@@ -226,13 +236,16 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   const uint32_t bar = smem + kOffBar;
   const uint32_t wfull = bar;
   auto full = [&](int s) { return bar + 8u * (1 + s); };        // tile landed (TMA)
-  // stage reusable: MMAs retired + statistics warps done reading + epilogue has taken its rstd
+  // stage reusable: the MMAs on the tiles have retired and the statistics warps have read them.
+  // (Nothing else holds a stage: HBM latency under load is ~4 us, the two stages are all the bytes
+  // this SM keeps in flight, so every cycle a stage waits for arithmetic is bandwidth lost.)
   auto sempty = [&](int s) { return bar + 8u * (3 + s); };
   auto tfull = [&](int u) { return bar + 8u * (5 + u); };       // accumulators complete
   auto tempty = [&](int u) { return bar + 8u * (7 + u); };      // accumulators read
   auto sready = [&](int s) { return bar + 8u * (9 + s); };      // statistics of the tile in stage s written
   const uint32_t xfree = bar + 8u * 11;                          // correction MMAs have read X_z, X_o
-  const uint32_t tmem_slot = bar + 8u * 12;
+  auto rfree = [&](int b) { return bar + 8u * (12 + b); };      // epilogue has taken rstd buffer b
+  const uint32_t tmem_slot = bar + 8u * 14;
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -246,7 +259,9 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     ptx::mbar_init(wfull, 1);
     for (int s = 0; s < kStages; ++s) {
       ptx::mbar_init(full(s), 1);
-      ptx::mbar_init(sempty(s), 1 + kLnzWarps + kLnoWarps + kEpiWarps);
+      // (with K1's statistics the z warps never touch the tile)
+      ptx::mbar_init(sempty(s), 1 + kLnoWarps + (prm.z_stats != nullptr ? 0 : kLnzWarps));
+      ptx::mbar_init(rfree(s), kEpiWarps);
       ptx::mbar_init(sready(s), kLnzWarps + kLnoWarps);
     }
     for (int u = 0; u < 2; ++u) {
@@ -423,6 +438,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           const uint64_t db = ptx::make_smem_desc_sw128(smem + kOffW + kMatBytes + off, 16, 1024);
           ptx::umma_bf16<1>(d_g + 128, da, db, idesc_o, k != 0 ? 1u : 0u);
         }
+        ptx::umma_commit<1>(sempty(s));      // the tiles themselves are not needed beyond this point
         // the rank-one corrections, once this tile's statistics are in X_z / X_o
         K3_PROBE_T0(t3);
         ptx::mbar_wait(sready(s), (it >> 1) & 1);
@@ -432,7 +448,6 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::umma_bf16<1>(d_g + 128, dxo, dyo, idesc_ox, 1u);
         ptx::umma_commit<1>(xfree);
         ptx::umma_commit<1>(tfull(slot));
-        ptx::umma_commit<1>(sempty(s));
       }
       K3_PROBE_PUT(2, iw_t);
       K3_PROBE_PUT(3, iw_f);
@@ -442,6 +457,33 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // ===================== statistics of the z tile (4 lanes per pair row) =====================
     ptx::setmaxnreg_dec<kRegsOther>();
     const int r = threadIdx.x - kWarpLnz * 32;
+    if (prm.z_stats != nullptr) {
+      // K1 normalised the same rows and left (mean, rstd) in the workspace: only turn them into the
+      // correction operand X_z (one row per thread of the first four warps), one tile ahead
+      auto load_stats = [&](int t) -> float2 {
+        const long long p = static_cast<long long>(t) * kTilePairs + r;
+        return (r < kTilePairs && t < prm.num_tiles && p < prm.R) ? __ldg(prm.z_stats + p)
+                                                                     : make_float2(0.f, 1.f);
+      };
+      float2 st_next = load_stats(first);
+      int it = 0;
+      for (int t = first; t < prm.num_tiles; t += stride, ++it) {
+        const int s = it & 1;
+        const float2 st = st_next;
+        st_next = load_stats(t + stride);
+        if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
+        if (it > 1) ptx::mbar_wait(rfree(s), ((it >> 1) - 1) & 1);
+        if (r < kTilePairs) {
+          // (rstd = 0 only when the fp32 variance overflowed, |z| beyond ~1e18: stay finite)
+          const float rstd = fmaxf(st.y, kMinRstd);
+          write_pair_side<false>(smem + kOffX, static_cast<uint32_t>(r), -st.x, __frcp_rn(rstd));
+          ptx::sts32(smem + kOffRstd + s * kTilePairs * 8 + r * 8, __float_as_uint(rstd));
+        }
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(sready(s));
+      }
+    } else {
     K3_PROBE_DECL(zw);
     K3_PROBE_DECL(zc);
     int it = 0;
@@ -449,30 +491,41 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const int s = it & 1;
       K3_PROBE_T0(t1);
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      // X_z still feeds the previous tile's correction MMA until that has retired (long ago by now)
-      if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
       K3_PROBE_ADD(zw, t1);
       K3_PROBE_T0(t2);
       const uint32_t rstd_base = smem + kOffRstd + s * kTilePairs * 8;
+      bool released = false;
       if (!K3_DBG_SKIP(1))
-        layernorm_rows_stats<1, kLnzWarps * 32>(smem + kOffStage + s * kStageBytes, kHalfBox, r,
-                                [&](uint32_t row, float mean, float var) {
-                                  const float ve = var + prm.eps_z;
-                                  const float rstd = rsqrtf(ve);
-                                  write_pair_side<false>(smem + kOffX, row, -mean, ve * rstd);
-                                  ptx::sts32(rstd_base + row * 8u, __float_as_uint(rstd));
-                                });
+        layernorm_rows_stats<2, kLnzWarps * 32>(
+            smem + kOffStage + s * kStageBytes, kHalfBox, r,
+            [&]() {
+              // the rows are in registers: hand the stage back before the arithmetic
+              __syncwarp();
+              if (lane == 0) ptx::mbar_arrive(sempty(s));
+              released = true;
+              // X_z still feeds the previous tile's correction MMA until that has retired, and the
+              // rstd buffer the epilogue of two tiles ago (both long done by now)
+              if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
+              if (it > 1) ptx::mbar_wait(rfree(s), ((it >> 1) - 1) & 1);
+            },
+            [&](uint32_t row, float mean, float var) {
+              const float ve = fminf(var + prm.eps_z, kMaxVar);
+              const float rstd = rsqrtf(ve);
+              write_pair_side<false>(smem + kOffX, row, -mean, ve * rstd);
+              ptx::sts32(rstd_base + row * 8u, __float_as_uint(rstd));
+            });
       ptx::fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) {
+        if (!released) ptx::mbar_arrive(sempty(s));
         ptx::mbar_arrive(sready(s));
-        ptx::mbar_arrive(sempty(s));
       }
       K3_PROBE_ADD(zc, t2);
     }
     if (threadIdx.x == kWarpLnz * 32) {
       K3_PROBE_PUT(4, zw);
       K3_PROBE_PUT(5, zc);
+    }
     }
   } else if (warp >= kWarpLno && warp < kWarpLnz) {
     // ===================== statistics of the o tile, [channel][pair] =====================
@@ -504,7 +557,6 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const int s = it & 1;
       K3_PROBE_T0(t1);
       ptx::mbar_wait(full(s), (it >> 1) & 1);
-      if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
       K3_PROBE_ADD(ow, t1);
       K3_PROBE_T0(t2);
       const uint32_t tile = smem + kOffStage + s * kStageBytes + kMatBytes;
@@ -532,6 +584,11 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         float s10, s11, s20, s21;
         ptx::upk2(ptx::add2(a0, a1), s10, s11);
         ptx::upk2(ptx::add2(b0, b1), s20, s21);
+        // the tile has been consumed: hand the stage back before the reductions
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(sempty(s));
+        if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
+        if (it > 1) ptx::mbar_wait(rfree(s), ((it >> 1) - 1) & 1);
         s10 += __shfl_xor_sync(0xffffffffu, s10, 8);
         s11 += __shfl_xor_sync(0xffffffffu, s11, 8);
         s20 += __shfl_xor_sync(0xffffffffu, s20, 8);
@@ -542,8 +599,8 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         s21 += __shfl_xor_sync(0xffffffffu, s21, 16);
         if (cq == 0) {
           const float md0 = s10 * (1.0f / kC), md1 = s11 * (1.0f / kC);
-          const float ve0 = fmaxf(fmaf(-md0, md0, s20 * (1.0f / kC)), 0.f) + prm.eps_o;
-          const float ve1 = fmaxf(fmaf(-md1, md1, s21 * (1.0f / kC)), 0.f) + prm.eps_o;
+          const float ve0 = fminf(fmaxf(fmaf(-md0, md0, s20 * (1.0f / kC)), 0.f) + prm.eps_o, kMaxVar);
+          const float ve1 = fminf(fmaxf(fmaf(-md1, md1, s21 * (1.0f / kC)), 0.f) + prm.eps_o, kMaxVar);
           const float r0 = rsqrtf(ve0), r1 = rsqrtf(ve1);
           write_pair_side<kOF16>(smem + kOffX + kXBytes, pair0, -(c0 + md0), ve0 * r0);
           write_pair_side<kOF16>(smem + kOffX + kXBytes, pair0 + 1, -(c1 + md1), ve1 * r1);
@@ -551,13 +608,13 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           ptx::sts32(ra, __float_as_uint(r0));
           ptx::sts32(ra + 8, __float_as_uint(r1));
         }
+      } else {
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(sempty(s));
       }
       ptx::fence_proxy_async_smem();
       __syncwarp();
-      if (lane == 0) {
-        ptx::mbar_arrive(sready(s));
-        ptx::mbar_arrive(sempty(s));
-      }
+      if (lane == 0) ptx::mbar_arrive(sready(s));
       K3_PROBE_ADD(oc, t2);
     }
     if (threadIdx.x == kWarpLno * 32) {
@@ -565,33 +622,32 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       K3_PROBE_PUT(7, oc);
     }
   } else if (warp >= kWarpEpi && warp < kWarpLno) {
-    // ===================== epilogue =====================
-    ptx::setmaxnreg_inc<kRegsEpi>();
-    // tcgen05.ld in the fragment shape 16x256b: a thread holds COLUMN PAIRS (two adjacent output
-    // channels = one bf16x2 word of the output) of four pairs, see ptx::tmem_ld_16x256b_x4.
+    // ===================== epilogue (thread = pair) =====================
+    // With the LayerNorm terms inside the accumulators the epilogue needs no per-channel constant:
+    //   out = M (tanh(rstd_z D_g) + 1) (rstd_o D_o) [+ z]
     // Warp = (lane quadrant q) x (32-channel part e of the 64 channels in flight); the tile's two
     // channel halves go one after the other through ONE [128 pairs][64 ch] staging buffer, a half's
-    // outputs being computed into registers first so that the wait for the previous TMA store to
-    // have read the buffer is covered by arithmetic.
+    // 32 outputs being computed into registers first so that the wait for the previous TMA store to
+    // have read the buffer is covered by arithmetic.  Row-per-thread tcgen05.ld (32x32b) keeps the
+    // staging stores 16 bytes wide: the MUFU, conversion and shared-memory instructions all go
+    // through the same issue queue, so fewer, wider shared-memory instructions matter.
+    ptx::setmaxnreg_inc<kRegsEpi>();
     const int q = warp & 3;                       // TMEM lane quadrant (hardware: warp % 4)
     const int e = (warp - kWarpEpi) >> 2;         // which 32 of the 64 channels
-    const uint32_t t4 = static_cast<uint32_t>(lane & 3), r8 = static_cast<uint32_t>(lane >> 2);
-    // this thread's four pairs: row(lh, ab) = q * 32 + lh * 16 + ab * 8 + r8
-    const uint32_t row0 = static_cast<uint32_t>(q) * 32u + r8;
+    const int r = q * 32 + lane;                  // pair within the tile
     const uint32_t stage_buf = smem + kOffOut;
-    const uint32_t row_addr = stage_buf + row0 * 128u + t4 * 4u;    // swizzle phase = row & 7 = r8
+    const uint32_t row_addr = stage_buf + r * 128;
+    const uint32_t sw = static_cast<uint32_t>(r & 7);
     const bool store_thread = (warp == kWarpEpi && lane == 0);
     constexpr uint32_t kEpiBar = 1;
     // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
-    auto load_mask = [&](int t, uint32_t i) -> uint32_t {
+    auto load_mask = [&](int t) -> uint32_t {
       if (prm.mask == nullptr) return 0x3f80u;   // bf16 1.0
       if (t >= prm.num_tiles) return 0u;
-      const long long p = static_cast<long long>(t) * kTilePairs + row0 + i * 8u;
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
       return p < prm.R ? static_cast<uint32_t>(__ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)) : 0u;
     };
-    uint32_t mnext[4];
-#pragma unroll
-    for (uint32_t i = 0; i < 4; ++i) mnext[i] = load_mask(first, i);
+    uint32_t mnext = load_mask(first);
     K3_PROBE_DECL(ew_s);
     K3_PROBE_DECL(ew_t);
     K3_PROBE_DECL(ew_b1);
@@ -602,42 +658,44 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       const int slot = it & 1;
-      float mval[4];
-      bool ones = true;
-#pragma unroll
-      for (uint32_t i = 0; i < 4; ++i) {
-        mval[i] = __uint_as_float(mnext[i] << 16);
-        ones = ones && mnext[i] == 0x3f80u;
-        mnext[i] = load_mask(t + stride, i);
-      }
-      const bool masked = !__all_sync(0xffffffffu, ones);   // warp-uniform
+      const uint32_t mraw = mnext;
+      mnext = load_mask(t + stride);
+      const bool masked = !__all_sync(0xffffffffu, mraw == 0x3f80u);   // warp-uniform
+      const float mval = __uint_as_float(mraw << 16);
       K3_PROBE_T0(t2);
       ptx::mbar_wait(sready(s), (it >> 1) & 1);             // rstd of this tile (long complete:
       ptx::mbar_wait(tfull(slot), (it >> 1) & 1);           // the correction MMAs waited for it)
       K3_PROBE_ADD(ew_t, t2);
       ptx::tc_fence_after();
-      // (rstd_z, rstd_o) of this thread's four pairs; then the stage may be refilled
-      float rz[4], ro[4];
-#pragma unroll
-      for (uint32_t i = 0; i < 4; ++i)
-        ptx::upk2(ptx::lds64x(smem + kOffRstd + s * kTilePairs * 8 + (row0 + i * 8u) * 8u), rz[i], ro[i]);
+      float rz, ro;
+      ptx::upk2(ptx::lds64x(smem + kOffRstd + s * kTilePairs * 8 + r * 8), rz, ro);
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(sempty(s));
+      if (lane == 0) ptx::mbar_arrive(rfree(s));            // the rstd buffer may be rewritten
       const uint32_t tbase = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + slot * 256 + e * 32;
-      const long long p0 = static_cast<long long>(t) * kTilePairs + row0;
+      const long long p = static_cast<long long>(t) * kTilePairs + r;
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         uint32_t packed[16];
 #pragma unroll
-        for (int lh = 0; lh < 2; ++lh) {
+        for (int c = 0; c < 2; ++c) {
           uint32_t vg[16], vo[16];
-          const uint32_t ta = tbase + (static_cast<uint32_t>(lh * 16) << 16) + h * 64;
+          const int ch0 = h * 64 + e * 32 + c * 16;          // first of this chunk's 16 channels
           K3_PROBE_T0(t5);
-          ptx::tmem_ld_16x256b_x4(ta, vg);
-          ptx::tmem_ld_16x256b_x4(ta + 128, vo);
+          ptx::tmem_ld_32x16(tbase + h * 64 + c * 16, vg);
+          ptx::tmem_ld_32x16(tbase + 128 + h * 64 + c * 16, vo);
+          // residual: this pair's 16 raw z channels (the tile was just read by TMA: an L2 hit)
+          uint32_t zr[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+          if constexpr (kResidual) {
+            if (p < prm.R) {
+              const uint4* zp = reinterpret_cast<const uint4*>(prm.z_res + p * kC + ch0);
+              const uint4 zr0 = __ldg(zp), zr1 = __ldg(zp + 1);
+              zr[0] = zr0.x; zr[1] = zr0.y; zr[2] = zr0.z; zr[3] = zr0.w;
+              zr[4] = zr1.x; zr[5] = zr1.y; zr[6] = zr1.z; zr[7] = zr1.w;
+            }
+          }
           ptx::tmem_ld_wait();
           K3_PROBE_ADD(ew_ld, t5);
-          if (h == 1 && lh == 1) {
+          if (h == 1 && c == 1) {
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(tempty(slot));
@@ -645,39 +703,30 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           auto chunk = [&](auto masked_tag) {
             constexpr bool kMasked = decltype(masked_tag)::value;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-#pragma unroll
-              for (int ab = 0; ab < 2; ++ab) {
-                const int j = 4 * k + 2 * ab;
-                const int ri = lh * 2 + ab;
-                // g/2 = rstd_z D_g ,  y/2 = rstd_o D_o  (everything else is already in D)
-                const ptx::f32x2 gx = ptx::mul2(ptx::pk2u(vg[j], vg[j + 1]), ptx::pk2(rz[ri], rz[ri]));
-                const ptx::f32x2 y = ptx::mul2(ptx::pk2u(vo[j], vo[j + 1]), ptx::pk2(ro[ri], ro[ri]));
-                float g0, g1, v0, v1;
-                ptx::upk2(gx, g0, g1);
-                const ptx::f32x2 th = K3_DBG_SKIP(32) ? gx : ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1));
-                // out = M (tanh(g/2) + 1) (y/2) [+ z]; the same roundings with and without the
-                // mask, so that M = 1 gives the unmasked bits
-                ptx::f32x2 v = ptx::fma2(y, th, y);
-                if constexpr (kResidual) {
-                  uint32_t zw = 0u;
-                  const long long p = p0 + lh * 16 + ab * 8;
-                  const int ch = h * 64 + e * 32 + k * 8;
-                  if (p < prm.R) zw = __ldg(reinterpret_cast<const uint32_t*>(prm.z_res + p * kC + ch) + t4);
-                  const ptx::f32x2 zres = ptx::bf16x2_to_f32x2(zw);
-                  if constexpr (kMasked) v = ptx::fma2(v, ptx::pk2(mval[ri], mval[ri]), zres);
-                  else v = ptx::add2(v, zres);
-                } else {
-                  if constexpr (kMasked) v = ptx::mul2(v, ptx::pk2(mval[ri], mval[ri]));
-                }
-                ptx::upk2(v, v0, v1);
-                packed[lh * 8 + k * 2 + ab] = K3_DBG_SKIP(64) ? (__float_as_uint(v0) ^ __float_as_uint(v1)) : ptx::pack_bf16x2(v0, v1);
+            for (int j = 0; j < 16; j += 2) {
+              // g/2 = rstd_z D_g ,  y/2 = rstd_o D_o  (everything else is already in D)
+              const ptx::f32x2 gx = ptx::mul2(ptx::pk2u(vg[j], vg[j + 1]), ptx::pk2(rz, rz));
+              const ptx::f32x2 y = ptx::mul2(ptx::pk2u(vo[j], vo[j + 1]), ptx::pk2(ro, ro));
+              float g0, g1, v0, v1;
+              ptx::upk2(gx, g0, g1);
+              const ptx::f32x2 th = K3_DBG_SKIP(32) ? gx : ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1));
+              // out = M (tanh(g/2) + 1) (y/2) [+ z]; the same roundings with and without the
+              // mask, so that M = 1 gives the unmasked bits
+              ptx::f32x2 v = ptx::fma2(y, th, y);
+              if constexpr (kResidual) {
+                const ptx::f32x2 zres = ptx::bf16x2_to_f32x2(zr[j >> 1]);
+                if constexpr (kMasked) v = ptx::fma2(v, ptx::pk2(mval, mval), zres);
+                else v = ptx::add2(v, zres);
+              } else {
+                if constexpr (kMasked) v = ptx::mul2(v, ptx::pk2(mval, mval));
               }
+              ptx::upk2(v, v0, v1);
+              packed[c * 8 + (j >> 1)] = K3_DBG_SKIP(64) ? (__float_as_uint(v0) ^ __float_as_uint(v1)) : ptx::pack_bf16x2(v0, v1);
             }
           };
           if (K3_DBG_SKIP(4)) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) packed[lh * 8 + i] = vo[2 * i] ^ vg[2 * i + 1];
+            for (int i = 0; i < 8; ++i) packed[c * 8 + i] = vo[2 * i] ^ vg[2 * i + 1];
           } else if (masked) {
             chunk(std::true_type{});
           } else {
@@ -690,14 +739,9 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::named_bar_sync(kEpiBar, kEpiWarps * 32);
         K3_PROBE_ADD(ew_b1, t3);
 #pragma unroll
-        for (int lh = 0; lh < 2; ++lh)
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-#pragma unroll
-            for (int ab = 0; ab < 2; ++ab)
-              ptx::sts32(row_addr + (lh * 16 + ab * 8) * 128 +
-                             ((static_cast<uint32_t>(e * 4 + k) ^ r8) << 4),
-                         packed[lh * 8 + k * 2 + ab]);
+        for (int i = 0; i < 4; ++i)
+          ptx::sts128(row_addr + ((static_cast<uint32_t>(e * 4 + i) ^ sw) << 4), packed[4 * i],
+                      packed[4 * i + 1], packed[4 * i + 2], packed[4 * i + 3]);
         ptx::fence_proxy_async_smem();
         K3_PROBE_T0(t4);
         ptx::named_bar_sync(kEpiBar, kEpiWarps * 32);
@@ -731,7 +775,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
 // bf16 unscaled (o_scale = 1)
 int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
                             const foldcp_trimul_params* p, int N, void* out, bool o_f16,
-                            float o_scale, cudaStream_t stream) {
+                            float o_scale, const void* z_stats, cudaStream_t stream) {
   DeviceInfo dev;
   if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   const uint64_t R = static_cast<uint64_t>(N) * N;
@@ -761,6 +805,7 @@ int launch_k3_finalize_bf16(const void* o, const void* z, const void* mask,
   K3Params prm;
   prm.mask = p->mask_output ? static_cast<const __nv_bfloat16*>(mask) : nullptr;
   prm.z_res = p->add_residual ? static_cast<const __nv_bfloat16*>(z) : nullptr;
+  prm.z_stats = static_cast<const float2*>(z_stats);
   prm.g_in = p->ln_in_gamma;
   prm.b_in = p->ln_in_beta;
   prm.g_out = p->ln_out_gamma;

@@ -23,9 +23,16 @@ namespace foldcp {
 // weights and biases of the GEMM that consumes the tile (gaddr / baddr unused).
 // kRows = rows per thread in flight (2 = more latency hiding, ~100 registers; 1 = ~60 registers).
 // kLnThreads = threads of the LayerNorm group (128 or 256; 256 only with kRows = 1).
-template <bool kF16, bool kAffine = true, int kRows = 2, int kLnThreads = 128>
+// `emit(row, mean, rstd)` is called by one lane per row with the row's statistics (K1 hands them
+// to K3 through the workspace, which then does not recompute them).
+struct NoRowStats {
+  __device__ __forceinline__ void operator()(uint32_t, float, float) const {}
+};
+template <bool kF16, bool kAffine = true, int kRows = 2, int kLnThreads = 128,
+          typename Emit = NoRowStats>
 __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t box_stride, int tid,
-                                                       uint32_t gaddr, uint32_t baddr, float eps) {
+                                                       uint32_t gaddr, uint32_t baddr, float eps,
+                                                       Emit&& emit = Emit()) {
   const uint32_t j = static_cast<uint32_t>(tid & 3);        // quarter of the row: channels 32j..
   const uint32_t box = j >> 1;
   const uint32_t cbase = (j & 1u) * 4u;                      // first 16-byte chunk inside the box
@@ -98,6 +105,7 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
       rs2[q] = ptx::pk2(rstd[q], rstd[q]);
       const float nmr = -mu[q] * rstd[q];
       nmr2[q] = ptx::pk2(nmr, nmr);
+      if (j == 0) emit(r0 + static_cast<uint32_t>(q) * 32u, mu[q], rstd[q]);
     }
 #pragma unroll
     for (uint32_t t = 0; t < 4; ++t) {
@@ -133,9 +141,11 @@ __device__ __forceinline__ void layernorm_rows_inplace(uint32_t tile, uint32_t b
 // row, so |mean - c| is of the order of the row's spread and the subtraction cancels nothing that
 // matters, whatever the row's common offset (|mean| >> sigma is as safe as with two passes).
 // kLnThreads (128 or 256) threads, four adjacent lanes per row, kRows rows per thread in flight.
-template <int kRows, int kLnThreads, typename Emit>
+// `tile_read()` is called once the thread has consumed everything it loads from the tile (the tile
+// may be handed back to its producer then), before the shuffles and the emits.
+template <int kRows, int kLnThreads, typename TileRead, typename Emit>
 __device__ __forceinline__ void layernorm_rows_stats(uint32_t tile, uint32_t box_stride, int tid,
-                                                     Emit&& emit) {
+                                                     TileRead&& tile_read, Emit&& emit) {
   const uint32_t j = static_cast<uint32_t>(tid & 3);
   const uint32_t box = j >> 1;
   const uint32_t cbase = (j & 1u) * 4u;
@@ -177,6 +187,7 @@ __device__ __forceinline__ void layernorm_rows_stats(uint32_t tile, uint32_t box
       ptx::upk2(ptx::add2(b0, b1), lo, hi);
       s2[q] = lo + hi;
     }
+    if (pass == 128 / kRowsPerPass - 1) tile_read();
 #pragma unroll
     for (int q = 0; q < kRows; ++q) {
       s1[q] += __shfl_xor_sync(0xffffffffu, s1[q], 1);

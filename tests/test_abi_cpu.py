@@ -34,8 +34,9 @@ def test_version_and_strings(lib):
 
 
 def test_workspace_bytes(lib):
-    assert B.workspace_bytes(4096, 128, 128, B.BF16) == 3 * 128 * 4096 * 4096 * 2 + 256   # 12 GiB + counters
-    assert B.workspace_bytes(8192, 128, 128, B.BF16) == 48 * 2 ** 30 + B.SCHED_SCRATCH_BYTES
+    # a, b, o (12 GiB) + the LayerNorm(z) statistics K1 hands to K3 (8 bytes per pair) + counters
+    assert B.workspace_bytes(4096, 128, 128, B.BF16) == 3 * 128 * 4096 * 4096 * 2 + 8 * 4096 * 4096 + 256
+    assert B.workspace_bytes(8192, 128, 128, B.BF16) == 48 * 2 ** 30 + 8 * 8192 * 8192 + B.SCHED_SCRATCH_BYTES
     assert B.workspace_bytes(64, 128, 128, B.F32) == 3 * 128 * 64 * 64 * 4 + 256
     assert B.workspace_bytes(12, 128, 128, B.BF16) == 0      # N % 8 != 0 in bf16
     assert B.workspace_bytes(12, 128, 128, B.F32) > 0
