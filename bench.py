@@ -372,12 +372,14 @@ def run_ours(args):
     flops_step = 2 * counted_flops(N)
     value = whole_job_tflops(flops_step, ms_per_step, world)
 
-    # ---- per-stage durations inside a timed region (stage entry points, same kernels, same stream)
+    # ---- per-stage durations inside a timed region: the stages in the form foldcp_trimul chains them
+    # (project_stats -> contract with fp16 scaled o -> finalize_fused: bitwise the fused call, see
+    # tests/test_parity_gpu.py test_fused_stage_chain_is_the_full_call_bitwise), same stream
     tb = C * N * N * 2
-    # the project stage writes a, b as fp16 in bf16 mode; the contract stage is told so (BF16_F16AB)
     a = ws[:tb].view(torch.float16).view(C, N, N)
     b = ws[tb: 2 * tb].view(torch.float16).view(C, N, N)
-    o = ws[2 * tb: 3 * tb].view(torch.bfloat16).view(C, N, N)
+    o = ws[2 * tb: 3 * tb].view(torch.float16).view(C, N, N)
+    zst = ws[3 * tb: 3 * tb + N * N * 8].view(torch.float32).view(N, N, 2)
     scratch = B.stage_scratch(dev)
     import ctypes
     lib = B.load()
@@ -389,14 +391,15 @@ def run_ours(args):
             prm = B.make_params(ps[d], B.BF16, 1e-5, True)
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
             ev[0].record()
-            st = lib.foldcp_trimul_project(z.data_ptr(), M.data_ptr(), ctypes.byref(prm), N, C, C,
-                                           a.data_ptr(), b.data_ptr(), scratch.data_ptr(), stream)
+            st = lib.foldcp_trimul_project_stats(z.data_ptr(), M.data_ptr(), ctypes.byref(prm), N, C, C,
+                                                 a.data_ptr(), b.data_ptr(), zst.data_ptr(),
+                                                 scratch.data_ptr(), stream)
             ev[1].record()
-            st |= lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, C, B.BF16_F16AB, d,
+            st |= lib.foldcp_trimul_contract(a.data_ptr(), b.data_ptr(), N, C, B.BF16_F16ALL, d,
                                              o.data_ptr(), scratch.data_ptr(), stream)
             ev[2].record()
-            st |= lib.foldcp_trimul_finalize(o.data_ptr(), z.data_ptr(), M.data_ptr(),
-                                             ctypes.byref(prm), N, C, C, outs[d].data_ptr(), stream)
+            st |= lib.foldcp_trimul_finalize_fused(o.data_ptr(), z.data_ptr(), zst.data_ptr(), M.data_ptr(),
+                                                   ctypes.byref(prm), N, C, C, outs[d].data_ptr(), stream)
             ev[3].record()
             assert st == 0
             evs.append((d, ev))

@@ -45,7 +45,14 @@
  *     (11-bit significand: their rounding was the largest term of the bf16 pipeline's error
  *     budget), so |a|, |b| must stay <= 65504 -- i.e. |W_a z' + b_a| and
  *     |W_b z' + b_b| <= 65504, far above anything LayerNorm-ed inputs and sane weights give;
- *     larger values saturate.  o, out and all gradients are bf16 (no range limit beyond fp32's).
+ *     larger values saturate.  Inside foldcp_trimul the contraction o travels to the last kernel as
+ *     fp16 too, multiplied by foldcp_trimul_o_scale(N) = 2^-ceil(log2(N)/2) ~ 1/sqrt(N) (exact: a
+ *     power of two; LayerNorm(o) absorbs it through eps * scale^2): |o| * scale must stay <= 65504,
+ *     i.e. |sum_k a b| <= 65504 sqrt(N).  out and all gradients are bf16.
+ *   - the output gate's folded weight W_g diag(gamma_in) multiplies the raw bf16 z tile and is
+ *     therefore rounded to bf16 (2^-9 relative): invisible at ordinary gate scales, a relative error
+ *     of ~5e-3 on the outputs of nearly closed gates when the gate weights are 4x larger
+ *     (tests/test_behaviour_gpu.py test_saturated_gates_parity).
  * No exceptions cross this boundary; every failure is a status code and, when detected on the
  * host, leaves `out` untouched.
  */
@@ -80,7 +87,10 @@ typedef enum {
   FOLDCP_BF16 = 1,
   /* only for foldcp_trimul_contract: a and b are IEEE fp16 -- what foldcp_trimul_project writes in
    * bf16 mode (see "intermediates" below) -- and o is bf16 */
-  FOLDCP_BF16_F16AB = 2
+  FOLDCP_BF16_F16AB = 2,
+  /* only for foldcp_trimul_contract: a, b fp16 and o ALSO fp16, multiplied by
+   * foldcp_trimul_o_scale(N) -- the form in which o travels inside foldcp_trimul (bf16 mode) */
+  FOLDCP_BF16_F16ALL = 3
 } foldcp_dtype_t;
 
 typedef struct {
@@ -143,7 +153,8 @@ int foldcp_trimul_batched(const void* z, const void* mask, const foldcp_trimul_p
  * argument of the stage entry points. */
 #define FOLDCP_SCHED_SCRATCH_BYTES 256
 
-/* Bytes of device scratch foldcp_trimul needs for this problem (a, b and o, channel-major, plus
+/* Bytes of device scratch foldcp_trimul needs for this problem (a, b and o, channel-major; in bf16
+ * mode 8 bytes per pair of LayerNorm(z) statistics handed from the first kernel to the last; plus
  * FOLDCP_SCHED_SCRATCH_BYTES of tile counters); 0 if the shape / dtype is unsupported.
  * Monotone in N. */
 size_t foldcp_trimul_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
@@ -207,6 +218,26 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
                            void* out, void* stream);
 
 /*
+ * The same stages in the form foldcp_trimul itself chains them in bf16 mode (FOLDCP_BF16 only;
+ * FOLDCP_ERR_UNSUPPORTED otherwise) -- for per-stage timing and per-stage tests of exactly the
+ * kernels the fused call launches:
+ *   foldcp_trimul_project_stats : foldcp_trimul_project that also leaves, per pair, the LayerNorm(z)
+ *        statistics (mean, rstd) as two floats in z_stats [N*N][2] (device, 16-byte aligned)
+ *   foldcp_trimul_contract with dtype FOLDCP_BF16_F16ALL : o is fp16, scaled by
+ *        foldcp_trimul_o_scale(N)
+ *   foldcp_trimul_finalize_fused : o as just described; z_stats from foldcp_trimul_project_stats
+ *        (NULL: the statistics are recomputed from z)
+ */
+int foldcp_trimul_project_stats(const void* z, const void* mask, const foldcp_trimul_params* params,
+                                int N, int c_z, int c_hidden, void* a, void* b, void* z_stats,
+                                void* scratch, void* stream);
+int foldcp_trimul_finalize_fused(const void* o, const void* z, const void* z_stats, const void* mask,
+                                 const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
+                                 void* out, void* stream);
+/* the power of two by which foldcp_trimul scales o between its last two kernels (bf16 mode) */
+float foldcp_trimul_o_scale(int N);
+
+/*
  * Full backward pass.  PAPER.md lines 92-96 (section 3.1): every Fold-CP
  * module hand-writes its backward with the same algorithm as its forward.  Given d_out = dL/d(out)
  * of one foldcp_trimul call (same z, mask, params, direction; params->add_residual and
@@ -264,7 +295,8 @@ const char* foldcp_status_string(int status);
 /* major * 100 + minor * 10; 110 added params->add_residual, foldcp_trimul_batched and
  * foldcp_trimul_contract_backward (the params struct grew: struct_size guards mismatches);
  * 120 made the tile counters per call (workspace grew by FOLDCP_SCHED_SCRATCH_BYTES, the stage
- * entry points take `scratch`) and added foldcp_trimul_backward. */
+ * entry points take `scratch`) and added foldcp_trimul_backward; 130: the workspace holds the
+ * LayerNorm(z) statistics in bf16 mode (8 bytes per pair more), fused-form stage entry points. */
 int foldcp_version(void);
 
 #ifdef __cplusplus

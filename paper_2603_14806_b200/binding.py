@@ -17,6 +17,7 @@ INCOMING = 1
 F32 = 0
 BF16 = 1
 BF16_F16AB = 2     # foldcp_trimul_contract only: a, b fp16 (as the project stage writes them), o bf16
+BF16_F16ALL = 3    # foldcp_trimul_contract only: a, b fp16; o fp16 scaled by o_scale(N) (the fused form)
 
 _LIB_NAME = "libfoldcp_trimul.so"
 _lib = None
@@ -25,6 +26,7 @@ EXPORTS = (
     "foldcp_trimul", "foldcp_trimul_batched", "foldcp_trimul_workspace_bytes", "foldcp_trimul_project",
     "foldcp_trimul_contract", "foldcp_trimul_contract_backward", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
     "foldcp_trimul_backward", "foldcp_trimul_backward_workspace_bytes", "foldcp_trimul_contract_blocks",
+    "foldcp_trimul_project_stats", "foldcp_trimul_finalize_fused", "foldcp_trimul_o_scale",
     "foldcp_status_string", "foldcp_version",
 )
 
@@ -91,6 +93,12 @@ def load() -> ctypes.CDLL:
     lib.foldcp_trimul_contract.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp, vp]
     lib.foldcp_trimul_finalize.restype = ci
     lib.foldcp_trimul_finalize.argtypes = [vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_project_stats.restype = ci
+    lib.foldcp_trimul_project_stats.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp, vp, vp, vp]
+    lib.foldcp_trimul_finalize_fused.restype = ci
+    lib.foldcp_trimul_finalize_fused.argtypes = [vp, vp, vp, vp, ctypes.POINTER(_Params), ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_o_scale.restype = ctypes.c_float
+    lib.foldcp_trimul_o_scale.argtypes = [ci]
     lib.foldcp_trimul_contract_blocks.restype = ci
     lib.foldcp_trimul_contract_blocks.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(vp), ci, ci, ci, ci, ci,
                                                   vp, vp, vp]
@@ -262,16 +270,60 @@ def project(z, mask, p, eps: float = 1e-5):
     return a, b
 
 
+def o_scale(N: int) -> float:
+    """The power of two by which the fused call scales o between its last two kernels."""
+    return float(load().foldcp_trimul_o_scale(int(N)))
+
+
+def project_stats(z, mask, p, eps: float = 1e-5):
+    """Stage a1+a2 in the fused form (bf16 mode): returns (a, b, z_stats) with z_stats [N, N, 2] fp32 =
+    (mean, rstd) of LayerNorm(z) per pair."""
+    lib = load()
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = p["w_a"].shape[0]
+    _check_tensors(z, p, (mask,))
+    a = torch.empty(c_hidden, N, N, dtype=torch.float16, device=z.device)
+    b = torch.empty_like(a)
+    stats = torch.empty(N, N, 2, dtype=torch.float32, device=z.device)
+    s = make_params(p, dtype_code(z), eps)
+    st = lib.foldcp_trimul_project_stats(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
+                                         a.data_ptr(), b.data_ptr(), stats.data_ptr(),
+                                         stage_scratch(z.device).data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_project_stats")
+    return a, b, stats
+
+
+def finalize_fused(o, z, z_stats, mask, p, eps: float = 1e-5, mask_output: bool = True,
+                   residual: bool = False, out: Optional[torch.Tensor] = None):
+    """Stage a3+a5 in the fused form: o [c, N, N] fp16 scaled by o_scale(N); z_stats from
+    project_stats (or None: recomputed)."""
+    lib = load()
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = o.shape[0]
+    assert o.dtype == torch.float16
+    if out is None:
+        out = torch.empty_like(z)
+    _check_tensors(z, p, (o, mask, out, z_stats))
+    s = make_params(p, dtype_code(z), eps, mask_output, None, residual)
+    st = lib.foldcp_trimul_finalize_fused(o.data_ptr(), z.data_ptr(), _ptr(z_stats), _ptr(mask),
+                                          ctypes.byref(s), N, c_z, c_hidden, out.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_finalize_fused")
+    return out
+
+
 def contract(a: torch.Tensor, b: torch.Tensor, direction: int,
-             o: Optional[torch.Tensor] = None) -> torch.Tensor:
+             o: Optional[torch.Tensor] = None, fused_o: bool = False) -> torch.Tensor:
     """Stage a4 (Eq. 2-3): a, b [c, N, N] channel-major -> o [c, N, N].  a, b may be fp32, bf16 or
     fp16 (the project stage's output in bf16 mode; o is then bf16)."""
     lib = load()
     c, N = a.shape[0], a.shape[1]
     assert a.dtype == b.dtype
     if a.dtype == torch.float16:
-        code, o_dtype = BF16_F16AB, torch.bfloat16
+        code, o_dtype = (BF16_F16ALL, torch.float16) if fused_o else (BF16_F16AB, torch.bfloat16)
     else:
+        assert not fused_o
         code, o_dtype = dtype_code(a), a.dtype
     if o is None:
         o = torch.empty(a.shape, dtype=o_dtype, device=a.device)

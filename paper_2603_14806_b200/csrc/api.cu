@@ -260,7 +260,8 @@ int foldcp_trimul_project(const void* z, const void* mask, const foldcp_trimul_p
 
 int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, int dtype,
                            int direction, void* o, void* scratch, void* stream) {
-  const bool ab_f16 = dtype == FOLDCP_BF16_F16AB;     // a, b fp16 (what K1 writes), o bf16
+  const bool o_f16 = dtype == FOLDCP_BF16_F16ALL;     // ... and o fp16, scaled (the fused form)
+  const bool ab_f16 = dtype == FOLDCP_BF16_F16AB || o_f16;   // a, b fp16 (what K1 writes)
   if (ab_f16) {
     if (!bf16_on_tensor_cores()) return FOLDCP_ERR_UNSUPPORTED;
     dtype = FOLDCP_BF16;
@@ -276,7 +277,8 @@ int foldcp_trimul_contract(const void* a, const void* b, int N, int c_hidden, in
   if ((st = check_arch()) != FOLDCP_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((st = prepare_scratch(scratch, dtype, s)) != FOLDCP_OK) return st;
-  return contract_stage(a, b, N, dtype, direction, o, ab_f16, 0.f, scratch, 0, s);
+  return contract_stage(a, b, N, dtype, direction, o, ab_f16, o_f16 ? contract_o_scale(N) : 0.f,
+                        scratch, 0, s);
 }
 
 int foldcp_trimul_contract_blocks(const void* const* a_blocks, const void* const* b_blocks,
@@ -349,6 +351,52 @@ int foldcp_trimul_finalize(const void* o, const void* z, const void* mask,
   return finalize_stage(o, z, mask, params, N, out, false, 1.0f, nullptr,
                         static_cast<cudaStream_t>(stream));
 }
+
+int foldcp_trimul_project_stats(const void* z, const void* mask, const foldcp_trimul_params* params,
+                                int N, int c_z, int c_hidden, void* a, void* b, void* z_stats,
+                                void* scratch, void* stream) {
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (params->dtype != FOLDCP_BF16 || !bf16_on_tensor_cores()) return FOLDCP_ERR_UNSUPPORTED;
+  if (!z || !a || !b || !z_stats) return FOLDCP_ERR_INVALID_ARG;
+  if (!aligned16(z) || !aligned16(a) || !aligned16(b) || !aligned16(z_stats) ||
+      (mask && !aligned16(mask)))
+    return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
+  const size_t sbytes = static_cast<size_t>(N) * N * sizeof(float2);
+  if (overlaps(a, bytes, z, bytes) || overlaps(b, bytes, z, bytes) || overlaps(a, bytes, b, bytes) ||
+      overlaps(z_stats, sbytes, z, bytes) || overlaps(z_stats, sbytes, a, bytes) ||
+      overlaps(z_stats, sbytes, b, bytes))
+    return FOLDCP_ERR_ALIAS;
+  if ((st = check_scratch(scratch, params->dtype)) != FOLDCP_OK) return st;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if ((st = prepare_scratch(scratch, params->dtype, s)) != FOLDCP_OK) return st;
+  return project_stage(z, mask, params, N, a, b, /*ab_f16=*/true, z_stats, scratch, s);
+}
+
+int foldcp_trimul_finalize_fused(const void* o, const void* z, const void* z_stats, const void* mask,
+                                 const foldcp_trimul_params* params, int N, int c_z, int c_hidden,
+                                 void* out, void* stream) {
+  int st = check_params(params);
+  if (st != FOLDCP_OK) return st;
+  if ((st = check_shape(N, c_z, c_hidden, params->dtype)) != FOLDCP_OK) return st;
+  if (params->dtype != FOLDCP_BF16 || !bf16_on_tensor_cores()) return FOLDCP_ERR_UNSUPPORTED;
+  if (!o || !z || !out) return FOLDCP_ERR_INVALID_ARG;
+  if (!aligned16(o) || !aligned16(z) || !aligned16(out) || (mask && !aligned16(mask)) ||
+      (z_stats && !aligned16(z_stats)))
+    return FOLDCP_ERR_ALIGNMENT;
+  const size_t bytes = static_cast<size_t>(N) * N * kChannels * elem_bytes(params->dtype);
+  if (overlaps(out, bytes, z, bytes) || overlaps(out, bytes, o, bytes) ||
+      (z_stats && overlaps(out, bytes, z_stats, static_cast<size_t>(N) * N * sizeof(float2))))
+    return FOLDCP_ERR_ALIAS;
+  if ((st = check_arch()) != FOLDCP_OK) return st;
+  return finalize_stage(o, z, mask, params, N, out, true, contract_o_scale(N), z_stats,
+                        static_cast<cudaStream_t>(stream));
+}
+
+float foldcp_trimul_o_scale(int N) { return N > 0 ? contract_o_scale(N) : 0.f; }
 
 int foldcp_trimul(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
                   int c_z, int c_hidden, int direction, void* out, void* stream) {
@@ -517,6 +565,6 @@ const char* foldcp_status_string(int status) {
   }
 }
 
-int foldcp_version(void) { return 120; }   // 1.2: per-call tile counters (workspace tail / stage scratch)
+int foldcp_version(void) { return 130; }   // 1.3: z statistics in the workspace, fused-form stage entries
 
 }  // extern "C"

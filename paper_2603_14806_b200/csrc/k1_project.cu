@@ -55,9 +55,14 @@ constexpr int kTilePairs = 128;
 constexpr int kTeams = FOLDCP_K1_TEAMS;         // epilogue teams of 4 warps: 2 or 4
 constexpr int kPar = kTeams / 2;                // teams per output tensor (pair-quarter parities)
 constexpr int kLnWarps = kTeams == 2 ? 4 : 8;   // 4 teams leave 72 registers/thread: one row in flight
-constexpr int kWarpLn = 4;
-constexpr int kWarpEpi = kWarpLn + kLnWarps;    // a multiple of 4 (TMEM lane quadrants)
-constexpr int kThreads = (kWarpEpi + 4 * kTeams) * 32;
+// role order: the issue arbiter favours higher warp ids (FOLDCP_K1_LN_HIGH=1 puts the LayerNorm
+// warps, which feed everything else, above the epilogue teams)
+#ifndef FOLDCP_K1_LN_HIGH
+#define FOLDCP_K1_LN_HIGH 0
+#endif
+constexpr int kWarpEpi = FOLDCP_K1_LN_HIGH ? 4 : 4 + kLnWarps;   // a multiple of 4 (TMEM lane quadrants)
+constexpr int kWarpLn = FOLDCP_K1_LN_HIGH ? 4 + 4 * kTeams : 4;
+constexpr int kThreads = (4 + kLnWarps + 4 * kTeams) * 32;
 static_assert(kTeams == 2 || kTeams == 4, "two or four epilogue teams");
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box, 128 rows x 64 bf16
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 16-bit tile (two k-halves)
@@ -239,9 +244,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       }
       ptx::tma_store_wait<0>();
     }
-  } else if (warp >= kWarpLn && warp < kWarpEpi) {
+  } else if (warp >= kWarpLn && warp < kWarpLn + kLnWarps) {
     // ===================== LayerNorm =====================
-    const int r = threadIdx.x - 128;
+    const int r = threadIdx.x - kWarpLn * 32;
     // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
     auto load_mask = [&](int t) -> unsigned short {
       if (prm.mask == nullptr || r >= kTilePairs) return static_cast<unsigned short>(0x3f80);
@@ -279,7 +284,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
     }
-  } else if (warp >= kWarpEpi) {
+  } else if (warp >= kWarpEpi && warp < kWarpEpi + 4 * kTeams) {
     // ===================== epilogue =====================
     // warp -> TMEM lane quadrant q (hardware rule: warp % 4) and team = (tensor h, parity par)
     const int q = warp & 3;

@@ -113,6 +113,90 @@ def test_finalize_stage_bf16(mask_output):
     assert e["rel_fro"] < 3e-3 and e["max_over_rms"] < 5e-2
 
 
+# ---------------------------------------------------------------- the stages in the form the fused call chains them
+def test_project_stats_stage():
+    """foldcp_trimul_project_stats: a, b bitwise those of foldcp_trimul_project, plus (mean, rstd) of
+    LayerNorm(z) per pair against the fp64 definition."""
+    cfg = synth.CONFIGS[1]
+    N = 136
+    z, M, p = synth.make_inputs(cfg, OUT, "cpu", N=N)
+    a0, b0 = B.project(z.to(DEV), M.to(DEV), to_dev(p))
+    a1, b1, st = B.project_stats(z.to(DEV), M.to(DEV), to_dev(p))
+    torch.cuda.synchronize()
+    assert torch.equal(a0, a1) and torch.equal(b0, b1)
+    zz = U.np64(z)
+    mean = zz.mean(axis=-1)
+    rstd = 1.0 / np.sqrt(zz.var(axis=-1) + 1e-5)          # biased variance, eps inside the sqrt (A6)
+    got = U.np64(st)
+    assert np.abs(got[..., 0] - mean).max() <= 1e-6 * max(1.0, np.abs(mean).max())
+    assert np.abs(got[..., 1] / rstd - 1.0).max() <= 1e-5
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+@pytest.mark.parametrize("N", [64, 328])
+def test_contract_stage_fused_o(direction, N):
+    """FOLDCP_BF16_F16ALL: o leaves K2 as fp16, multiplied by foldcp_trimul_o_scale(N) (a power of two
+    ~ 1/sqrt(N)): only fp16's 2^-11 rounding separates it from the fp64 contraction."""
+    from oracle import trimul_oracle as orc
+    g = torch.Generator().manual_seed(N + direction)
+    a = torch.randn(128, N, N, generator=g).to(torch.float16)
+    b = torch.randn(128, N, N, generator=g).to(torch.float16)
+    o = B.contract(a.to(DEV), b.to(DEV), direction, fused_o=True)
+    torch.cuda.synchronize()
+    assert o.dtype == torch.float16
+    sc = B.o_scale(N)
+    assert sc == 2.0 ** -int(np.ceil(np.log2(N) / 2))
+    ref = sc * orc.contraction(np.transpose(U.np64(a), (1, 2, 0)), np.transpose(U.np64(b), (1, 2, 0)), direction)
+    got = np.transpose(U.np64(o), (1, 2, 0))
+    assert np.abs(got - ref).max() <= 2.0 ** -10 * np.abs(ref).max()
+    assert U.errors(got, ref)["rel_fro"] < 5e-4
+
+
+@pytest.mark.parametrize("mask_output", [True, False])
+@pytest.mark.parametrize("with_stats", [True, False])
+def test_finalize_fused_stage(mask_output, with_stats):
+    """K3 as the fused call launches it: o in fp16 scaled by o_scale(N) (LayerNorm(o) must absorb the
+    scale through eps), LayerNorm(z) statistics handed over by K1 or recomputed."""
+    from oracle import trimul_oracle as orc
+    cfg = synth.CONFIGS[1]
+    N = 136
+    z, M, p = synth.make_inputs(cfg, OUT, "cpu", N=N)
+    M = synth.pair_mask(synth.make_token_mask("scatter", N, cfg.seed), cfg.dtype)
+    g = torch.Generator().manual_seed(7)
+    o64 = (torch.randn(128, N, N, generator=g) * 3 + torch.randn(128, 1, 1, generator=g)).double()
+    sc = B.o_scale(N)
+    o16 = (o64 * sc).to(torch.float16)
+    stats = None
+    if with_stats:
+        _, _, stats = B.project_stats(z.to(DEV), M.to(DEV), to_dev(p))
+    out = B.finalize_fused(o16.to(DEV), z.to(DEV), stats, M.to(DEV), to_dev(p), mask_output=mask_output)
+    torch.cuda.synchronize()
+    q = U.params64(p)
+    zp = orc.layer_norm(U.np64(z), q["ln_in_gamma"], q["ln_in_beta"], 1e-5)
+    # the oracle sees the values the kernel was given, unscaled: o16 / sc is exact (power of two)
+    ref = orc.output_stage(np.transpose(o16.double().numpy() / sc, (1, 2, 0)), zp, U.np64(M), q, 1e-5, mask_output)
+    e = U.errors(U.np64(out), ref)
+    U.record_parity(f"finalize_fused stage N={N} mask_output={mask_output} stats={'K1' if with_stats else 'recomputed'}",
+                    e, "bf16", N=N)
+    assert e["rel_fro"] < 3e-3 and e["max_over_rms"] < 5e-2
+
+
+@pytest.mark.parametrize("direction", [OUT, INC])
+def test_fused_stage_chain_is_the_full_call_bitwise(direction):
+    """project_stats -> contract (fp16 scaled o) -> finalize_fused are exactly the three launches of
+    foldcp_trimul in bf16 mode."""
+    cfg = synth.CONFIGS[1]
+    N = 264
+    z, M, p = synth.make_inputs(cfg, direction, "cpu", N=N)
+    zd, Md, pd = z.to(DEV), M.to(DEV), to_dev(p)
+    a, b, st = B.project_stats(zd, Md, pd)
+    o = B.contract(a, b, direction, fused_o=True)
+    out = B.finalize_fused(o, zd, st, Md, pd)
+    full = B.trimul(zd, Md, pd, direction)
+    torch.cuda.synchronize()
+    assert torch.equal(out, full)
+
+
 @pytest.mark.parametrize("direction", [OUT, INC])
 def test_bf16_n1024_full_tensor(direction):
     """Whole-tensor parity at N = 1024 (1.3e8 outputs): the max-abs criterion is the binding one
