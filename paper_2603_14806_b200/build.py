@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(PKG_DIR, "libfoldcp_trimul.so")
 
 SOURCES = ["api.cu", "simt_kernels.cu", "simt_backward.cu", "k1_project.cu", "k2_contract.cu",
            "k3_finalize.cu", "k_backward.cu"]
-HEADERS = ["common.h", "ptx.cuh", "ln_rows.cuh", "tile_sched.cuh"]
+HEADERS = ["common.h", "ptx.cuh", "ln_rows.cuh", "tile_sched.cuh", "rank1.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -54,8 +54,6 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
-#include <type_traits>
-
 // 28 warps, most of them waiting on an mbarrier most of the time: their try_wait loops would take
 // every fifth issue slot of the SM partition; with a suspend-time hint a waiting warp sleeps
 #ifndef FOLDCP_MBAR_HINT_NS
@@ -64,6 +62,7 @@
 #include "common.h"
 #include "ln_rows.cuh"
 #include "ptx.cuh"
+#include "rank1.cuh"
 
 namespace foldcp {
 namespace {
@@ -176,38 +175,17 @@ __device__ __forceinline__ ptx::f32x2 o2_to_f32x2(uint32_t v) {
   }
 }
 
-// x = x1 + x2 + x3 with every piece representable in the operand format (round to nearest each
-// time; the remainders are exact in fp32): 24 bits of x from bf16 pieces, more from fp16 ones
-template <bool kF16>
-__device__ __forceinline__ void split3(float x, uint32_t (&p)[3]) {
-#pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    if constexpr (kF16) {
-      const __half h = __float2half_rn(x);
-      p[i] = static_cast<uint32_t>(__half_as_ushort(h));
-      x -= __half2float(h);
-    } else {
-      const __nv_bfloat16 h = __float2bfloat16_rn(x);
-      p[i] = static_cast<uint32_t>(__bfloat16_as_ushort(h));
-      x -= __bfloat162float(h);
-    }
-  }
-}
 // One row of a correction operand: the sixteen K slots that pair  (u, v)  on the per-pair side with
 // (s, t)  on the per-channel side so that the MMA adds  u s + v t  with all cross terms down to
 // 2^-24:   per-pair side     u1 u1 u2 u1 u2 u3 | v1 v1 v2 v1 v2 v3 | 0 0 0 0
 //          per-channel side  s1 s2 s1 s3 s2 s1 | t1 t2 t1 t3 t2 t1 | 0 0 0 0
-// Unswizzled K-major layout (ptx::make_smem_desc_noswizzle, lbo 128, sbo 256): slots 0..7 of row r
-// at (r / 8) * 256 + (r % 8) * 16, slots 8..15 another 128 bytes on.
-__device__ __forceinline__ uint32_t x_row_addr(uint32_t base, uint32_t r) {
-  return base + (r >> 3) * 256u + (r & 7u) * 16u;
-}
+// (split3 and the unswizzled K-major row layout: rank1.cuh)
 template <bool kF16>
 __device__ __forceinline__ void write_pair_side(uint32_t base, uint32_t r, float u, float v) {
   uint32_t a[3], b[3];
   split3<kF16>(u, a);
   split3<kF16>(v, b);
-  const uint32_t addr = x_row_addr(base, r);
+  const uint32_t addr = rank1_row_addr(base, r);
   ptx::sts128(addr, a[0] | (a[0] << 16), a[1] | (a[0] << 16), a[1] | (a[2] << 16), b[0] | (b[0] << 16));
   ptx::sts128(addr + 128, b[1] | (b[0] << 16), b[1] | (b[2] << 16), 0u, 0u);
 }
@@ -216,7 +194,7 @@ __device__ __forceinline__ void write_channel_side(uint32_t base, uint32_t r, fl
   uint32_t a[3], b[3];
   split3<kF16>(s, a);
   split3<kF16>(t, b);
-  const uint32_t addr = x_row_addr(base, r);
+  const uint32_t addr = rank1_row_addr(base, r);
   ptx::sts128(addr, a[0] | (a[1] << 16), a[0] | (a[2] << 16), a[1] | (a[0] << 16), b[0] | (b[1] << 16));
   ptx::sts128(addr + 128, b[0] | (b[2] << 16), b[1] | (b[0] << 16), 0u, 0u);
 }
@@ -459,18 +437,21 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     const int r = threadIdx.x - kWarpLnz * 32;
     if (prm.z_stats != nullptr) {
       // K1 normalised the same rows and left (mean, rstd) in the workspace: only turn them into the
-      // correction operand X_z (one row per thread of the first four warps), one tile ahead
+      // correction operand X_z (one row per thread of the first four warps)
       auto load_stats = [&](int t) -> float2 {
         const long long p = static_cast<long long>(t) * kTilePairs + r;
         return (r < kTilePairs && t < prm.num_tiles && p < prm.R) ? __ldg(prm.z_stats + p)
                                                                      : make_float2(0.f, 1.f);
       };
-      float2 st_next = load_stats(first);
+      // (three tiles ahead: HBM latency under load exceeds a tile's time)
+      float2 sq0 = load_stats(first), sq1 = load_stats(first + stride), sq2 = load_stats(first + 2 * stride);
       int it = 0;
       for (int t = first; t < prm.num_tiles; t += stride, ++it) {
         const int s = it & 1;
-        const float2 st = st_next;
-        st_next = load_stats(t + stride);
+        const float2 st = sq0;
+        sq0 = sq1;
+        sq1 = sq2;
+        sq2 = load_stats(t + 3 * stride);
         if (it > 0) ptx::mbar_wait(xfree, (it - 1) & 1);
         if (it > 1) ptx::mbar_wait(rfree(s), ((it >> 1) - 1) & 1);
         if (r < kTilePairs) {
@@ -550,11 +531,26 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
       toff[jj] = box * kHalfBox + (cq * 32u + k7) * 128u + ((c16 ^ k7) << 4) + within;
     }
     const uint32_t pair0 = box * 64u + static_cast<uint32_t>(w8 & 3) * 16u + pl * 2u;
+    // The output mask rides on rstd_o (out = (tanh + 1) (M rstd_o D_o) [+ z]: M = 1 leaves the bits
+    // untouched, M = 0 gives exact zeros), so the epilogue never sees it.  Two bf16 mask values per
+    // thread, fetched three tiles ahead: HBM latency under this kernel's own load is ~4 us, longer
+    // than a tile.
+    auto load_mask2 = [&](int t) -> uint32_t {
+      if (prm.mask == nullptr) return 0x3f803f80u;   // bf16 (1.0, 1.0)
+      if (t >= prm.num_tiles) return 0u;
+      const long long p = static_cast<long long>(t) * kTilePairs + pair0;
+      return p < prm.R ? __ldg(reinterpret_cast<const uint32_t*>(prm.mask + p)) : 0u;   // R is even
+    };
+    uint32_t mq0 = load_mask2(first), mq1 = load_mask2(first + stride), mq2 = load_mask2(first + 2 * stride);
     K3_PROBE_DECL(ow);
     K3_PROBE_DECL(oc);
     int it = 0;
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
+      const uint32_t m2 = mq0;
+      mq0 = mq1;
+      mq1 = mq2;
+      mq2 = load_mask2(t + 3 * stride);
       K3_PROBE_T0(t1);
       ptx::mbar_wait(full(s), (it >> 1) & 1);
       K3_PROBE_ADD(ow, t1);
@@ -605,8 +601,8 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
           write_pair_side<kOF16>(smem + kOffX + kXBytes, pair0, -(c0 + md0), ve0 * r0);
           write_pair_side<kOF16>(smem + kOffX + kXBytes, pair0 + 1, -(c1 + md1), ve1 * r1);
           const uint32_t ra = smem + kOffRstd + s * kTilePairs * 8 + pair0 * 8u + 4u;
-          ptx::sts32(ra, __float_as_uint(r0));
-          ptx::sts32(ra + 8, __float_as_uint(r1));
+          ptx::sts32(ra, __float_as_uint(r0 * ptx::bf16_lo(m2)));
+          ptx::sts32(ra + 8, __float_as_uint(r1 * ptx::bf16_hi(m2)));
         }
       } else {
         __syncwarp();
@@ -624,7 +620,7 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
   } else if (warp >= kWarpEpi && warp < kWarpLno) {
     // ===================== epilogue (thread = pair) =====================
     // With the LayerNorm terms inside the accumulators the epilogue needs no per-channel constant:
-    //   out = M (tanh(rstd_z D_g) + 1) (rstd_o D_o) [+ z]
+    //   out = (tanh(rstd_z D_g) + 1) (M rstd_o D_o) [+ z]        (M rides on rstd_o, see there)
     // Warp = (lane quadrant q) x (32-channel part e of the 64 channels in flight); the tile's two
     // channel halves go one after the other through ONE [128 pairs][64 ch] staging buffer, a half's
     // 32 outputs being computed into registers first so that the wait for the previous TMA store to
@@ -640,14 +636,6 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     const uint32_t sw = static_cast<uint32_t>(r & 7);
     const bool store_thread = (warp == kWarpEpi && lane == 0);
     constexpr uint32_t kEpiBar = 1;
-    // the pair mask is fetched one tile ahead so that its latency never sits on the critical path
-    auto load_mask = [&](int t) -> uint32_t {
-      if (prm.mask == nullptr) return 0x3f80u;   // bf16 1.0
-      if (t >= prm.num_tiles) return 0u;
-      const long long p = static_cast<long long>(t) * kTilePairs + r;
-      return p < prm.R ? static_cast<uint32_t>(__ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)) : 0u;
-    };
-    uint32_t mnext = load_mask(first);
     K3_PROBE_DECL(ew_s);
     K3_PROBE_DECL(ew_t);
     K3_PROBE_DECL(ew_b1);
@@ -658,10 +646,6 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
     for (int t = first; t < prm.num_tiles; t += stride, ++it) {
       const int s = it & 1;
       const int slot = it & 1;
-      const uint32_t mraw = mnext;
-      mnext = load_mask(t + stride);
-      const bool masked = !__all_sync(0xffffffffu, mraw == 0x3f80u);   // warp-uniform
-      const float mval = __uint_as_float(mraw << 16);
       K3_PROBE_T0(t2);
       ptx::mbar_wait(sready(s), (it >> 1) & 1);             // rstd of this tile (long complete:
       ptx::mbar_wait(tfull(slot), (it >> 1) & 1);           // the correction MMAs waited for it)
@@ -700,37 +684,24 @@ k3_finalize_kernel(const __grid_constant__ CUtensorMap tmap_z,
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(tempty(slot));
           }
-          auto chunk = [&](auto masked_tag) {
-            constexpr bool kMasked = decltype(masked_tag)::value;
+          if (K3_DBG_SKIP(4)) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) packed[c * 8 + i] = vo[2 * i] ^ vg[2 * i + 1];
+          } else {
 #pragma unroll
             for (int j = 0; j < 16; j += 2) {
-              // g/2 = rstd_z D_g ,  y/2 = rstd_o D_o  (everything else is already in D)
+              // g/2 = rstd_z D_g ,  y/2 = M rstd_o D_o  (everything else is already in D)
               const ptx::f32x2 gx = ptx::mul2(ptx::pk2u(vg[j], vg[j + 1]), ptx::pk2(rz, rz));
               const ptx::f32x2 y = ptx::mul2(ptx::pk2u(vo[j], vo[j + 1]), ptx::pk2(ro, ro));
               float g0, g1, v0, v1;
               ptx::upk2(gx, g0, g1);
               const ptx::f32x2 th = K3_DBG_SKIP(32) ? gx : ptx::pk2(ptx::tanh_approx(g0), ptx::tanh_approx(g1));
-              // out = M (tanh(g/2) + 1) (y/2) [+ z]; the same roundings with and without the
-              // mask, so that M = 1 gives the unmasked bits
+              // out = (tanh(g/2) + 1) (y/2) [+ z]
               ptx::f32x2 v = ptx::fma2(y, th, y);
-              if constexpr (kResidual) {
-                const ptx::f32x2 zres = ptx::bf16x2_to_f32x2(zr[j >> 1]);
-                if constexpr (kMasked) v = ptx::fma2(v, ptx::pk2(mval, mval), zres);
-                else v = ptx::add2(v, zres);
-              } else {
-                if constexpr (kMasked) v = ptx::mul2(v, ptx::pk2(mval, mval));
-              }
+              if constexpr (kResidual) v = ptx::add2(v, ptx::bf16x2_to_f32x2(zr[j >> 1]));
               ptx::upk2(v, v0, v1);
               packed[c * 8 + (j >> 1)] = K3_DBG_SKIP(64) ? (__float_as_uint(v0) ^ __float_as_uint(v1)) : ptx::pack_bf16x2(v0, v1);
             }
-          };
-          if (K3_DBG_SKIP(4)) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) packed[c * 8 + i] = vo[2 * i] ^ vg[2 * i + 1];
-          } else if (masked) {
-            chunk(std::true_type{});
-          } else {
-            chunk(std::false_type{});
           }
         }
         // the previous store out of the staging buffer has read it
