@@ -23,10 +23,12 @@
 //
 // Persistent kernel, one CTA per SM, 28 warps (FOLDCP_K1_TEAMS = 4; 16 warps with 2), tile = 128 pairs:
 //   warp 0       TMA producer : z tiles into a kZStages-deep ring
-//   warp 1       MMA issuer   : per tile eight "units" (pair quarter pq, tensor u in {a, b}); a unit
+//   warps 1, 2   MMA issuers  : per tile eight "units" (pair quarter pq, tensor u in {a, b}); a unit
 //                               = projection + gate MMA (M=128 ch, N=32 pairs, K=128) into one
-//                               64-column TMEM slot; four slots, two per tensor
-//   warp 2       TMEM allocator (512 columns: 256 weights + 4 x 64 accumulators)
+//                               64-column TMEM slot; four slots, two per tensor.  Warp 1 issues
+//                               tensor a's units, warp 2 (after allocating TMEM: 512 columns =
+//                               256 weights + 4 x 64 accumulators) tensor b's: 128 small MMAs per
+//                               tile were one thread's whole instruction budget
 //   LayerNorm    8 warps      : ln_rows.cuh -- z rows -> registers -> two-pass mean/variance in
 //                               fp32 -> n written back in place as the K-major B operand; also
 //                               stage the pair mask and an "all ones" flag per tile
@@ -84,6 +86,23 @@ static_assert((3 * kZStages + 18) * 8 <= 256, "barrier region too small");
 constexpr int kTmemW = 0;        // columns 0..255: four weight matrices, 64 columns each
 constexpr int kTmemAcc = 256;    // columns 256..511: four slots of (projection 32 | gate 32)
 
+#ifdef FOLDCP_K1_PROBE
+// bring-up instrumentation (never in the product build): cycles per CTA.  [0] producer total,
+// [1] producer wait zempty, [2] issuer wait zready, [3] issuer wait tempty, [4] LayerNorm wait zfull,
+// [5] LayerNorm work, [6] epilogue (team 0, quadrant 0) wait tfull, [7] wait oempty, [8] total,
+// [9] store issuer wait ofull, [10] tiles, [11] store issuer wait read
+__device__ unsigned long long g_k1_probe[160][16];
+#define K1_PROBE_T0(var) const long long var = clock64()
+#define K1_PROBE_ADD(acc, t0) acc += clock64() - (t0)
+#define K1_PROBE_DECL(var) long long var = 0
+#define K1_PROBE_PUT(idx, val) g_k1_probe[blockIdx.x][idx] = static_cast<unsigned long long>(val)
+#else
+#define K1_PROBE_T0(var)
+#define K1_PROBE_ADD(acc, t0)
+#define K1_PROBE_DECL(var)
+#define K1_PROBE_PUT(idx, val)
+#endif
+
 struct K1Params {
   const __nv_bfloat16* mask;   // [R] or nullptr
   const __nv_bfloat16* w[4];   // W_a, W_ga, W_b, W_gb: [128][128] row-major
@@ -120,7 +139,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   auto ofull = [&](int b) { return bar + 8u * (3 * kZStages + 10 + b); };    // staging buffer b
   auto oempty = [&](int b) { return bar + 8u * (3 * kZStages + 14 + b); };   // (tensor, group)
   const TileRing<kRingDepth> ring{smem + kOffRing};
-  constexpr uint32_t kRingConsumers = 1 + 1 + kLnWarps + 4 * kTeams;   // MMA, store, LN, epilogue
+  constexpr uint32_t kRingConsumers = 2 + 1 + kLnWarps + 4 * kTeams;   // 2 MMA, store, LN, epilogue
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -133,7 +152,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < kZStages; ++s) {
       ptx::mbar_init(zfull(s), 1);
-      ptx::mbar_init(zempty(s), 1);
+      ptx::mbar_init(zempty(s), 2);        // one commit per MMA issuer
       ptx::mbar_init(zready(s), kLnWarps * 32);
     }
     for (int u = 0; u < 4; ++u) {
@@ -160,42 +179,58 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // ===================== TMA producer =====================
     if (ptx::elect_one()) {
       int it = 0;
+      K1_PROBE_DECL(pw);
+      K1_PROBE_T0(p0);
       for (;; ++it) {
         const int t = ring.produce(it, prm.sched, prm.num_tiles);
         if (t < 0) break;
         const int s = it % kZStages;
+        K1_PROBE_T0(t1);
         ptx::mbar_wait(zempty(s), ((it / kZStages) & 1) ^ 1u);
+        K1_PROBE_ADD(pw, t1);
         ptx::mbar_arrive_expect_tx(zfull(s), kMatBytes);
         const uint32_t dst = smem + kOffZ + s * kMatBytes;
         const int row0 = t * kTilePairs;          // < 2^31: R <= 2^30 (N <= 32768)
         ptx::tma_load_2d(dst, &tmap_z, zfull(s), 0, row0);
         ptx::tma_load_2d(dst + kHalfBox, &tmap_z, zfull(s), 64, row0);
       }
+      K1_PROBE_PUT(0, clock64() - p0);
+      K1_PROBE_PUT(1, pw);
+      K1_PROBE_PUT(10, it);
     }
-  } else if (warp == 1) {
-    // ===================== MMA issuer =====================
+  } else if (warp == 1 || warp == 2) {
+    // ===================== MMA issuers: warp 1 tensor a, warp 2 tensor b =====================
+    // 128 small MMAs per tile (N = 32) cost the issuing thread ~25 cycles each -- with one issuer that
+    // thread's instruction stream was the kernel's critical path at the power-capped clock (probe:
+    // busy 3,200 of 4,200 cycles per tile).  Two issuers on two SM partitions, one per output tensor.
+    const int u = warp - 1;
     if (ptx::elect_one()) {
       // A = folded weights in TMEM, B = n (K-major, 32 pairs), both fp16 (or both bf16)
       constexpr uint32_t kFmt = kNormFp16 ? ptx::kFmtF16 : ptx::kFmtBF16;
       constexpr uint32_t idesc = ptx::make_idesc_f16kind(128, 32, kFmt, kFmt, 0, 0);
       ptx::mbar_wait(wready, 0);
       ptx::tc_fence_after();
+      K1_PROBE_DECL(iw_z);
+      K1_PROBE_DECL(iw_t);
       int it = 0;
       for (;; ++it) {
         if (ring.consume(it) < 0) break;
         const int s = it % kZStages;
+        K1_PROBE_T0(t1);
         ptx::mbar_wait(zready(s), (it / kZStages) & 1);
+        K1_PROBE_ADD(iw_z, t1);
         ptx::tc_fence_after();
         const uint32_t zb = smem + kOffZ + s * kMatBytes;
 #pragma unroll
         for (int pq = 0; pq < 4; ++pq) {
-#pragma unroll
-          for (int u = 0; u < 2; ++u) {
+          {
             // slot 2u + (pq & 1): each tensor's team alternates between its two slots, so this
             // unit's MMAs overlap the team's epilogue of the previous unit
             const uint32_t slot = static_cast<uint32_t>(2 * u + (pq & 1));
             const uint32_t use = static_cast<uint32_t>(it * 2 + (pq >> 1));   // per-slot use count
+            K1_PROBE_T0(t2);
             ptx::mbar_wait(tempty(slot), (use & 1u) ^ 1u);
+            K1_PROBE_ADD(iw_t, t2);
             ptx::tc_fence_after();
 #pragma unroll
             for (int m2 = 0; m2 < 2; ++m2) {
@@ -212,7 +247,11 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
             ptx::umma_commit<1>(tfull(slot));
           }
         }
-        ptx::umma_commit<1>(zempty(s));   // stage reusable once all MMAs of the tile retired
+        ptx::umma_commit<1>(zempty(s));   // stage reusable once all MMAs of the tile (both issuers') retired
+      }
+      if (u == 0) {
+        K1_PROBE_PUT(2, iw_z);
+        K1_PROBE_PUT(3, iw_t);
       }
     }
   } else if (warp == 3) {
@@ -222,6 +261,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // previous store has finished reading shared memory.  No block-wide barrier in the epilogue.
     if (ptx::elect_one()) {
       int it = 0, prev = -1;
+      K1_PROBE_DECL(sw_f);
+      K1_PROBE_DECL(sw_r);
       for (;; ++it) {
         const int t = ring.consume(it);
         if (t < 0) break;
@@ -230,12 +271,16 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
 #pragma unroll
           for (int u = 0; u < 2; ++u) {
             const int b = 2 * u + g;
+            K1_PROBE_T0(t1);
             ptx::mbar_wait(ofull(b), it & 1);
+            K1_PROBE_ADD(sw_f, t1);
             ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, smem + kOffOut + b * kHalfBox,
                               t * kTilePairs + g * 64, 0);
             ptx::tma_store_commit();
             if (prev >= 0) {
+              K1_PROBE_T0(t2);
               ptx::tma_store_wait_read<1>();
+              K1_PROBE_ADD(sw_r, t2);
               ptx::mbar_arrive(oempty(prev));
             }
             prev = b;
@@ -243,6 +288,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         }
       }
       ptx::tma_store_wait<0>();
+      K1_PROBE_PUT(9, sw_f);
+      K1_PROBE_PUT(11, sw_r);
     }
   } else if (warp >= kWarpLn && warp < kWarpLn + kLnWarps) {
     // ===================== LayerNorm =====================
@@ -255,6 +302,8 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       return p < prm.R ? __ldg(reinterpret_cast<const unsigned short*>(prm.mask) + p)
                        : static_cast<unsigned short>(0);
     };
+    K1_PROBE_DECL(lw);
+    K1_PROBE_DECL(lc);
     int tnext = ring.consume_warp(0, lane);
     unsigned short mnext = load_mask(tnext);
     int it = 0;
@@ -265,7 +314,10 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       const unsigned short mraw = mnext;
       tnext = ring.consume_warp(it + 1, lane);
       mnext = load_mask(tnext);
+      K1_PROBE_T0(t1);
       ptx::mbar_wait(zfull(s), (it / kZStages) & 1);
+      K1_PROBE_ADD(lw, t1);
+      K1_PROBE_T0(t2);
       layernorm_rows_inplace<kNormFp16, false, kLnWarps == 4 ? 2 : 1, kLnWarps * 32>(
           smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0, prm.eps,
           [&](uint32_t row, float mean, float rstd) {
@@ -283,6 +335,11 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       }
       ptx::fence_proxy_async_smem();
       ptx::mbar_arrive(zready(s));
+      K1_PROBE_ADD(lc, t2);
+    }
+    if (threadIdx.x == kWarpLn * 32) {
+      K1_PROBE_PUT(4, lw);
+      K1_PROBE_PUT(5, lc);
     }
   } else if (warp >= kWarpEpi && warp < kWarpEpi + 4 * kTeams) {
     // ===================== epilogue =====================
@@ -389,6 +446,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
     // slower), stored once both halves are in.  Tensors a and b are handled independently (own
     // barrier, store thread and staging buffers).
     constexpr bool kPrefetch = kTeams == 2;     // enough registers for a second tcgen05.ld buffer
+    K1_PROBE_DECL(ew_t);
+    K1_PROBE_DECL(ew_o);
+    K1_PROBE_T0(e0);
     int it = 0;
     for (;; ++it) {
       if (ring.consume_warp(it, lane) < 0) break;
@@ -401,7 +461,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         const uint32_t slot = static_cast<uint32_t>(2 * h + (pq & 1));
         const uint32_t use = static_cast<uint32_t>(it * 2 + g);          // per-slot use count
         const int b = 2 * h + g;                                          // staging buffer
+        K1_PROBE_T0(t1);
         ptx::mbar_wait(tfull(slot), use & 1u);
+        K1_PROBE_ADD(ew_t, t1);
         ptx::tc_fence_after();
         if (i == 0) {
           // written by the LayerNorm warps before zready, hence visible after this tile's tfull
@@ -417,7 +479,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::tmem_ld_32x16(taddr, vp[0]);
         ptx::tmem_ld_32x16(taddr + 32, vg[0]);
         // first write of this team into buffer b for this tile: last tile's store has read it
+        K1_PROBE_T0(t2);
         if (kPar == 2 || (pq & 1) == 0) ptx::mbar_wait(oempty(b), (it & 1) ^ 1u);
+        K1_PROBE_ADD(ew_o, t2);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           const int cb = kPrefetch ? k : 0;
@@ -459,6 +523,11 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
           if (lane == 0) ptx::mbar_arrive(ofull(b));
         }
       }
+    }
+    if (threadIdx.x == kWarpEpi * 32) {
+      K1_PROBE_PUT(6, ew_t);
+      K1_PROBE_PUT(7, ew_o);
+      K1_PROBE_PUT(8, clock64() - e0);
     }
   }
 
@@ -527,3 +596,10 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
 }
 
 }  // namespace foldcp
+
+#ifdef FOLDCP_K1_PROBE
+extern "C" int foldcp_debug_k1_probe_read(unsigned long long* host_out) {
+  return static_cast<int>(cudaMemcpyFromSymbol(host_out, foldcp::g_k1_probe,
+                                               sizeof(unsigned long long) * 160 * 16));
+}
+#endif
