@@ -27,6 +27,7 @@ EXPORTS = (
     "foldcp_trimul_contract", "foldcp_trimul_contract_backward", "foldcp_trimul_finalize", "foldcp_trimul_launches_per_call",
     "foldcp_trimul_backward", "foldcp_trimul_backward_workspace_bytes", "foldcp_trimul_contract_blocks",
     "foldcp_trimul_project_stats", "foldcp_trimul_finalize_fused", "foldcp_trimul_o_scale",
+    "foldcp_triattn", "foldcp_triattn_workspace_bytes",
     "foldcp_status_string", "foldcp_version",
 )
 
@@ -56,6 +57,21 @@ class _Params(ctypes.Structure):
 
 PARAM_NAMES = ("ln_in_gamma", "ln_in_beta", "w_a", "w_a_gate", "w_b", "w_b_gate", "b_a", "b_a_gate",
                "b_b", "b_b_gate", "w_g", "b_g", "ln_out_gamma", "ln_out_beta", "w_o", "b_o")
+
+
+class _TriAttnParams(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32), ("dtype", ctypes.c_int32), ("ln_eps", ctypes.c_float),
+        ("n_heads", ctypes.c_int32),
+        ("ln_gamma", ctypes.c_void_p), ("ln_beta", ctypes.c_void_p),
+        ("w_q", ctypes.c_void_p), ("w_k", ctypes.c_void_p), ("w_v", ctypes.c_void_p),
+        ("w_g", ctypes.c_void_p), ("w_t", ctypes.c_void_p), ("w_o", ctypes.c_void_p),
+        ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
+    ]
+
+
+TRIATTN_STARTING = 0
+TRIATTN_ENDING = 1
 
 
 class _Grads(ctypes.Structure):
@@ -109,6 +125,10 @@ def load() -> ctypes.CDLL:
     lib.foldcp_trimul_backward_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.foldcp_trimul_launches_per_call.restype = ci
     lib.foldcp_trimul_launches_per_call.argtypes = [ci]
+    lib.foldcp_triattn.restype = ci
+    lib.foldcp_triattn.argtypes = [vp, vp, ctypes.POINTER(_TriAttnParams), ci, ci, ci, vp, vp]
+    lib.foldcp_triattn_workspace_bytes.restype = ctypes.c_size_t
+    lib.foldcp_triattn_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.foldcp_status_string.restype = ctypes.c_char_p
     lib.foldcp_status_string.argtypes = [ci]
     lib.foldcp_version.restype = ci
@@ -423,3 +443,49 @@ def trimul_backward(d_out: torch.Tensor, z: torch.Tensor, mask: Optional[torch.T
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul_backward")
     return d_z, grads
+
+
+def triattn_workspace_bytes(N: int, c_z: int = 128, n_heads: int = 4, dtype: int = BF16) -> int:
+    return int(load().foldcp_triattn_workspace_bytes(N, c_z, n_heads, dtype))
+
+
+def triattn(z: torch.Tensor, mask: Optional[torch.Tensor], p: Dict[str, torch.Tensor], node: int,
+            n_heads: int = 4, eps: float = 1e-5, out: Optional[torch.Tensor] = None,
+            workspace: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Triangle attention (include/foldcp_triattn.h), starting (rows) or ending (columns) node, on the
+    current CUDA stream.  p: ln_gamma, ln_beta (fp32), w_q, w_k, w_v, w_g [H*c, c_z], w_t [H, c_z],
+    w_o [c_z, H*c] in z's dtype."""
+    lib = load()
+    assert z.dim() == 3 and z.shape[0] == z.shape[1] and z.is_contiguous() and z.is_cuda
+    if z.device.index != torch.cuda.current_device():
+        raise ValueError("z is not on the current CUDA device")
+    N, c_z = z.shape[0], z.shape[2]
+    dt = dtype_code(z)
+    for name in ("w_q", "w_k", "w_v", "w_g", "w_t", "w_o"):
+        t = p[name]
+        if t.dtype != z.dtype or t.device != z.device or not t.is_contiguous():
+            raise TypeError(f"{name}: dtype / device / contiguity must match z")
+    for name in ("ln_gamma", "ln_beta"):
+        if p[name].dtype != torch.float32 or p[name].device != z.device:
+            raise TypeError(f"{name} must be float32 on z's device")
+    if mask is not None:
+        assert mask.dtype == z.dtype and mask.is_contiguous() and mask.shape == z.shape[:-1]
+    if workspace is None:
+        workspace = torch.empty(max(triattn_workspace_bytes(N, c_z, n_heads, dt), 1), dtype=torch.uint8,
+                                device=z.device)
+    if out is None:
+        out = torch.empty_like(z)
+    s = _TriAttnParams()
+    s.struct_size = ctypes.sizeof(_TriAttnParams)
+    s.dtype = dt
+    s.ln_eps = eps
+    s.n_heads = n_heads
+    for name in ("ln_gamma", "ln_beta", "w_q", "w_k", "w_v", "w_g", "w_t", "w_o"):
+        setattr(s, name, p[name].data_ptr())
+    s.workspace = workspace.data_ptr()
+    s.workspace_bytes = workspace.numel()
+    st = lib.foldcp_triattn(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, int(node), out.data_ptr(),
+                            _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_triattn")
+    return out

@@ -19,7 +19,9 @@ def lib():
 
 
 def test_exports_match_header(lib):
-    hdr = open(os.path.join(ROOT, "include", "foldcp_trimul.h")).read()
+    # every entry point declared in include/*.h is exported by the library and bound, and vice versa
+    hdr = "".join(open(os.path.join(ROOT, "include", f)).read()
+                  for f in ("foldcp_trimul.h", "foldcp_triattn.h"))
     declared = set(re.findall(r"\b(foldcp_[a-z_]+)\s*\(", hdr))
     assert declared == set(B.EXPORTS)
     for name in declared:
