@@ -465,6 +465,46 @@ def run_backward(ctx, steps):
                     "backward and weight gradients on fp32 CUDA-core kernels (first correct path)"}
 
 
+def run_triattn(ctx, N=1024, steps=2):
+    """NEXT-4: triangle attention (foldcp_triattn), starting and ending node, bf16 storage, on a
+    synthetic pair tensor of N tokens (mask: last 10 % of tokens padding).  Counted FLOPs: QK^T and PV
+    (4 N^3 H c) plus the projections (oracle/triattn_oracle.py flops())."""
+    torch, B, synth = ctx["torch"], ctx["B"], ctx["synth"]
+    dev = ctx["dev"]
+    g = torch.Generator(device=dev).manual_seed(4242)
+    rn = lambda *s: torch.randn(*s, generator=g, device=dev)
+    z = rn(N, N, C).to(torch.bfloat16)
+    p = dict(ln_gamma=1 + 0.1 * rn(C), ln_beta=0.1 * rn(C))
+    for name, rows in (("w_q", C), ("w_k", C), ("w_v", C), ("w_g", C), ("w_t", 4)):
+        p[name] = (rn(rows, C) / C ** 0.5).to(torch.bfloat16)
+    p["w_o"] = (rn(C, C) / C ** 0.5).to(torch.bfloat16)
+    m = synth.make_token_mask("tail", N, 7)
+    M = synth.pair_mask(m, "bf16", dev)
+    M[:, 0] = 1
+    M[0, :] = 1
+    ws = torch.empty(B.triattn_workspace_bytes(N), dtype=torch.uint8, device=dev)
+    out = torch.empty_like(z)
+    res = {}
+    for node, name in ((B.TRIATTN_STARTING, "starting"), (B.TRIATTN_ENDING, "ending")):
+        B.triattn(z, M, p, node, out=out, workspace=ws)
+        torch.cuda.synchronize()
+        e_a, e_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e_a.record()
+        for _ in range(steps):
+            B.triattn(z, M, p, node, out=out, workspace=ws)
+        e_b.record()
+        torch.cuda.synchronize()
+        res[name] = e_a.elapsed_time(e_b) / steps
+    fl = 4.0 * N ** 3 * C + 2.0 * N * N * C * (4 * C + 4) + 2.0 * N * N * C * C
+    ms = 0.5 * (res["starting"] + res["ending"])
+    del z, M, ws, out
+    torch.cuda.empty_cache()
+    return {"workload": f"triangle attention (PAPER.md Eq. 1), N={N}, c_z=128, 4 heads x 32, bf16 storage",
+            "ms_per_call": res, "counted_tflop_per_call": fl / 1e12, "tflops": fl / (ms * 1e-3) / 1e12,
+            "steps": steps, "gpu_launches_per_call": 3,
+            "note": "first correct CUDA path: CUDA-core kernels, fp32 arithmetic -- not yet on tcgen05"}
+
+
 def run_n8192(ctx, steps=3):
     """BASELINE configs[4] (N = 8192, 5 % of tokens masked) in a single call per direction: 3 timed
     calls each, CUDA events; peak HBM bytes from torch's allocator."""
@@ -578,6 +618,7 @@ def main():
                     help="seconds the N=2048 full-op oracle timing may take (else N=1024 is timed)")
     ap.add_argument("--no-n8192", action="store_true")
     ap.add_argument("--no-backward", action="store_true")
+    ap.add_argument("--no-triattn", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -590,6 +631,7 @@ def main():
     e2e = None if args.no_e2e else run_e2e(ctx, max(4, min(K, 6)))
     single = world == 1 and ctx["rank"] == 0
     bwd = run_backward(ctx, 2) if (single and not args.no_backward) else None
+    triattn = run_triattn(ctx) if (single and not args.no_triattn) else None
     n8192 = None
     if single and not args.no_n8192:
         for k in ("z", "M", "ws", "outs"):
@@ -653,7 +695,7 @@ def main():
         "per_direction": {"ms_per_call": ctx["per_direction"],
                           "tflops": {k: counted_flops(N) / (v * 1e-3) / 1e12
                                      for k, v in ctx["per_direction"].items()}},
-        "n8192": n8192, "backward": bwd,
+        "n8192": n8192, "backward": bwd, "triattn": triattn,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
