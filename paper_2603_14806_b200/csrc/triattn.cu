@@ -10,9 +10,11 @@
 // Layouts: z / out [N][N][128]; workspace q, k, v, g fp32 [N][N][128] (head-major inside: h * 32 + d);
 // t, tT fp32 [H][N][N].
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "../../include/foldcp_triattn.h"
 #include "common.h"
+#include "ptx.cuh"
 
 namespace foldcp {
 namespace {
@@ -35,6 +37,17 @@ template <> __device__ __forceinline__ void stf<__nv_bfloat16>(__nv_bfloat16* p,
   *p = __float2bfloat16_rn(v);
 }
 
+constexpr float kLog2e = 1.4426950408889634f;
+// 16-bit operands of the tensor-core attention (bf16 mode); all nullptr in fp32 mode
+struct TcOut {
+  __half* q16;    // [N*N][128]  q * log2(e) / sqrt(c)
+  __half* k16;    // [N*N][128]
+  __half* vts;    // [N][128][N] v transposed per line, starting node
+  __half* vte;    // [N][128][N] ending node
+  __half* t16s;   // [H][N][N]   t * log2(e), (query position, key position) of the starting node
+  __half* t16e;   // [H][N][N]   transposed: ending node
+};
+
 // block = 128 threads (thread = output channel), 16 consecutive pairs
 template <typename T>
 __global__ void __launch_bounds__(128)
@@ -42,7 +55,7 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
                   const T* __restrict__ w_v, const T* __restrict__ w_g, const T* __restrict__ w_t,
                   const float* __restrict__ gamma, const float* __restrict__ beta, float eps, int N,
                   float* __restrict__ q, float* __restrict__ k, float* __restrict__ v,
-                  float* __restrict__ g, float* __restrict__ t, float* __restrict__ tT) {
+                  float* __restrict__ g, float* __restrict__ t, float* __restrict__ tT, TcOut tc) {
   __shared__ float zs[kPairsPerBlock][C];
   const long long npairs = static_cast<long long>(N) * N;
   const long long p0 = static_cast<long long>(blockIdx.x) * kPairsPerBlock;
@@ -90,10 +103,22 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
   }
   for (int p = 0; p < np; ++p) {
     const long long o = (p0 + p) * C + tid;
-    q[o] = aq[p];
-    k[o] = ak[p];
-    v[o] = av[p];
     g[o] = 1.0f / (1.0f + expf(-ag[p]));
+    if (tc.q16 == nullptr) {
+      q[o] = aq[p];
+      k[o] = ak[p];
+      v[o] = av[p];
+    } else {
+      // operands of the tensor-core attention: q carries 1/sqrt(c) and log2(e) (the softmax runs on
+      // exp2), v is written transposed for both nodes ([line][h][d][key], keys contiguous)
+      const long long pair = p0 + p;
+      const long long i = pair / N, j = pair % N;
+      tc.q16[o] = __float2half_rn(aq[p] * (kLog2e * 0.17677669529663687f));
+      tc.k16[o] = __float2half_rn(ak[p]);
+      const __half vh = __float2half_rn(av[p]);
+      tc.vts[(i * C + tid) * N + j] = vh;      // starting node: line i, key position j
+      tc.vte[(j * C + tid) * N + i] = vh;      // ending node:   line j, key position i
+    }
   }
   // the triangular bias: thread (p, h) for the first 16 * H threads
   if (tid < kPairsPerBlock * kHeads) {
@@ -103,8 +128,14 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
       for (int c = 0; c < C; ++c) acc = fmaf(ldf(w_t + h * C + c), zs[p][c], acc);
       const long long pair = p0 + p;
       const long long i = pair / N, j = pair % N;
-      t[(static_cast<long long>(h) * N + i) * N + j] = acc;
-      tT[(static_cast<long long>(h) * N + j) * N + i] = acc;
+      if (tc.q16 == nullptr) {
+        t[(static_cast<long long>(h) * N + i) * N + j] = acc;
+        tT[(static_cast<long long>(h) * N + j) * N + i] = acc;
+      } else {
+        const __half th = __float2half_rn(acc * kLog2e);
+        tc.t16s[(static_cast<long long>(h) * N + i) * N + j] = th;
+        tc.t16e[(static_cast<long long>(h) * N + j) * N + i] = th;
+      }
     }
   }
 }
@@ -172,6 +203,223 @@ ta_attention_kernel(const float* __restrict__ q, const float* __restrict__ k,
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Tensor-core attention (bf16 mode): one CTA per (128 queries, line, head), key blocks of 128.
+//   S = Q K^T                 tcgen05.mma M=128 (queries) N=128 (keys) K=32, fp16 operands, into TMEM
+//   softmax (4 warps, thread = query row = TMEM lane): S + triangular bias tile + key mask, running
+//                             maximum, p = exp2(s - m) written as fp16 into the P tile
+//   O_blk = P V               tcgen05.mma M=128 N=32 K=128, V^T tile as the K-major B operand
+//   acc = acc * 2^(m_old - m_new) + O_blk   in registers; out = g * acc / l at the end
+// Operand layouts: Q and K tiles [128 rows][32 d] arrive through a 5-D tensor map as unswizzled core
+// matrices ([row / 8][d / 8][row % 8][8 halves]: lbo 128, sbo 512 -- the same descriptor form K3's
+// rank-one operands use); the bias tile, P and V^T are 128-byte-swizzled K-major tiles of two
+// 64-key boxes (K3's z / weight tiles).  The ending node is the same kernel on a tensor map with
+// swapped strides, the transposed bias and the other V^T.
+// ---------------------------------------------------------------------------------------------
+constexpr int kTcThreads = 160;                   // warp 0: TMA + MMA issue; warps 1-4: softmax
+constexpr int kTcOffT = 0;                        // bias tile  [128 q][128 k] fp16, two SW128 boxes
+constexpr int kTcOffP = 32768;                    // P tile     [128 q][128 k] fp16, two SW128 boxes
+constexpr int kTcOffV = 65536;                    // V^T tile   [32 d][128 k]  fp16, two SW128 boxes
+constexpr int kTcOffQ = 73728;                    // Q tile     unswizzled core matrices, 8 KB
+constexpr int kTcOffK = 81920;                    // K tile
+constexpr int kTcOffM = 90112;                    // key mask bias, 128 floats
+constexpr int kTcOffBar = 90624;
+constexpr int kTcSmem = kTcOffBar + 64;
+
+struct TcAttnParams {
+  const float* g;        // [N*N][128]
+  const void* mask;      // bf16 [N][N] or nullptr
+  float* og;             // [N*N][128]  g * o
+  int N;
+  long long ls, xs;      // pair (line, x) = line * ls + x * xs
+};
+
+__global__ void __launch_bounds__(kTcThreads)
+ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
+                       const __grid_constant__ CUtensorMap tmap_k,
+                       const __grid_constant__ CUtensorMap tmap_v,
+                       const __grid_constant__ CUtensorMap tmap_t, const TcAttnParams prm) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t smem = ptx::smem_u32(smem_raw);
+  const uint32_t bar = smem + kTcOffBar;
+  const uint32_t bar_q = bar, bar_kv = bar + 8, bar_s = bar + 16, bar_p = bar + 24, bar_o = bar + 32,
+                 bar_free = bar + 40, tmem_slot = bar + 48;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int N = prm.N;
+  const int pos0 = blockIdx.x * 128, line = blockIdx.y, h = blockIdx.z;
+  const int nblocks = (N + 127) / 128;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      ptx::mbar_init(bar_q, 1);
+      ptx::mbar_init(bar_kv, 1);
+      ptx::mbar_init(bar_s, 1);
+      ptx::mbar_init(bar_p, 4);
+      ptx::mbar_init(bar_o, 1);
+      ptx::mbar_init(bar_free, 4);
+      ptx::fence_mbar_init();
+    }
+    __syncwarp();
+    ptx::tmem_alloc<1>(tmem_slot, 256);
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  const uint32_t tm_s = tmem_base, tm_o = tmem_base + 128;
+
+  if (warp == 0) {
+    if (ptx::elect_one()) {
+      constexpr uint32_t idesc_s = ptx::make_idesc_f16kind(128, 128, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
+      constexpr uint32_t idesc_o = ptx::make_idesc_f16kind(128, 32, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
+      ptx::mbar_arrive_expect_tx(bar_q, 8192);
+      ptx::tma_load_5d(smem + kTcOffQ, &tmap_q, bar_q, 0, 0, h * 4, pos0 / 8, line);
+      ptx::mbar_wait(bar_q, 0);
+      for (int b = 0; b < nblocks; ++b) {
+        const int k0 = b * 128;
+        if (b > 0) ptx::mbar_wait(bar_free, (b - 1) & 1);
+        ptx::mbar_arrive_expect_tx(bar_kv, 8192 + 8192 + 32768);
+        ptx::tma_load_5d(smem + kTcOffK, &tmap_k, bar_kv, 0, 0, h * 4, k0 / 8, line);
+        ptx::tma_load_2d(smem + kTcOffV, &tmap_v, bar_kv, k0, (line * kHeads + h) * kHead);
+        ptx::tma_load_2d(smem + kTcOffV + 4096, &tmap_v, bar_kv, k0 + 64, (line * kHeads + h) * kHead);
+        ptx::tma_load_2d(smem + kTcOffT, &tmap_t, bar_kv, k0, h * N + pos0);
+        ptx::tma_load_2d(smem + kTcOffT + 16384, &tmap_t, bar_kv, k0 + 64, h * N + pos0);
+        ptx::mbar_wait(bar_kv, b & 1);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks)       // K = 32 = two MMAs of K = 16 (two core matrices each)
+          ptx::umma_bf16<1>(tm_s, ptx::make_smem_desc_noswizzle(smem + kTcOffQ + ks * 256, 128, 512),
+                            ptx::make_smem_desc_noswizzle(smem + kTcOffK + ks * 256, 128, 512), idesc_s,
+                            ks ? 1u : 0u);
+        ptx::umma_commit<1>(bar_s);
+        ptx::mbar_wait(bar_p, b & 1);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {     // K = 128 keys
+          const uint32_t offp = (ks >> 2) * 16384 + (ks & 3) * 32;
+          const uint32_t offv = (ks >> 2) * 4096 + (ks & 3) * 32;
+          ptx::umma_bf16<1>(tm_o, ptx::make_smem_desc_sw128(smem + kTcOffP + offp, 16, 1024),
+                            ptx::make_smem_desc_sw128(smem + kTcOffV + offv, 16, 1024), idesc_o,
+                            ks ? 1u : 0u);
+        }
+        ptx::umma_commit<1>(bar_o);
+      }
+    }
+  } else {
+    // ===================== softmax: thread = query row =====================
+    const int quad = warp & 3;
+    const int r = quad * 32 + lane;            // query row of the tile = TMEM lane
+    const int st = threadIdx.x - 32;           // 0..127: the key this thread fetches the mask of
+    const int pos = pos0 + r;
+    const bool active = pos < N;
+    const uint32_t lane_addr = static_cast<uint32_t>(quad * 32) << 16;
+    const uint32_t sw = static_cast<uint32_t>(r & 7);
+    float acc[kHead];
+#pragma unroll
+    for (int d = 0; d < kHead; ++d) acc[d] = 0.f;
+    float m = -INFINITY, l = 0.f;
+    for (int b = 0; b < nblocks; ++b) {
+      const int k0 = b * 128;
+      {
+        // mask bias of key k0 + st (in log2 units); keys beyond N do not exist
+        float mb = 0.f;
+        const int kp = k0 + st;
+        if (kp >= N) {
+          mb = -INFINITY;
+        } else if (prm.mask != nullptr) {
+          const float mv = __bfloat162float(static_cast<const __nv_bfloat16*>(prm.mask)[line * prm.ls + kp * prm.xs]);
+          mb = -1.0e9f * kLog2e * (1.0f - mv);
+        }
+        reinterpret_cast<float*>(smem_raw + kTcOffM)[st] = mb;
+      }
+      ptx::named_bar_sync(1, 128);
+      ptx::mbar_wait(bar_s, b & 1);
+      ptx::tc_fence_after();
+      // pass 1: the block's row maximum
+      float bmax = -INFINITY;
+#pragma unroll 1
+      for (int c = 0; c < 4; ++c) {
+        uint32_t sv[32];
+        ptx::tmem_ld_32x32(tm_s + lane_addr + c * 32, sv);
+        ptx::tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          uint32_t tw[4];
+          ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + ((static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4), tw);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
+            const int kk = c * 32 + i * 8 + e * 2;
+            const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + kk * 4);
+            bmax = fmaxf(bmax, __uint_as_float(sv[i * 8 + e * 2]) + tf.x + mb.x);
+            bmax = fmaxf(bmax, __uint_as_float(sv[i * 8 + e * 2 + 1]) + tf.y + mb.y);
+          }
+        }
+      }
+      const float m_new = fmaxf(m, bmax);
+      const float m_use = m_new == -INFINITY ? 0.f : m_new;     // a row with no key yet: p = 0 everywhere
+      const float resc = ptx::ex2_approx(m - m_use);              // 0 on the first block
+      // pass 2: p = exp2(s - m_new), row sum, P tile
+      float lsum = 0.f;
+#pragma unroll 1
+      for (int c = 0; c < 4; ++c) {
+        uint32_t sv[32];
+        ptx::tmem_ld_32x32(tm_s + lane_addr + c * 32, sv);
+        ptx::tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          uint32_t tw[4], pw[4];
+          const uint32_t chunk = (static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4;
+          ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + chunk, tw);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
+            const int kk = c * 32 + i * 8 + e * 2;
+            const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + kk * 4);
+            const float p0 = ptx::ex2_approx(__uint_as_float(sv[i * 8 + e * 2]) + tf.x + mb.x - m_use);
+            const float p1 = ptx::ex2_approx(__uint_as_float(sv[i * 8 + e * 2 + 1]) + tf.y + mb.y - m_use);
+            lsum += p0 + p1;
+            pw[e] = ptx::pack_f16x2(p0, p1);
+          }
+          ptx::sts128(smem + kTcOffP + (c >> 1) * 16384 + r * 128 + chunk, pw[0], pw[1], pw[2], pw[3]);
+        }
+      }
+      l = l * resc + lsum;
+      m = m_new;
+      ptx::tc_fence_before();
+      ptx::fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar_p);
+      // O_blk = P V, then the running output
+      ptx::mbar_wait(bar_o, b & 1);
+      ptx::tc_fence_after();
+      uint32_t ov[32];
+      ptx::tmem_ld_32x32(tm_o + lane_addr, ov);
+      ptx::tmem_ld_wait();
+#pragma unroll
+      for (int d = 0; d < kHead; ++d) acc[d] = fmaf(acc[d], resc, __uint_as_float(ov[d]));
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar_free);
+    }
+    if (active) {
+      const float inv = 1.0f / l;
+      const long long a = (static_cast<long long>(line) * prm.ls + static_cast<long long>(pos) * prm.xs) * C + h * kHead;
+#pragma unroll
+      for (int d = 0; d < kHead; d += 4) {
+        const float4 gv = *reinterpret_cast<const float4*>(prm.g + a + d);
+        *reinterpret_cast<float4*>(prm.og + a + d) =
+            make_float4(gv.x * acc[d] * inv, gv.y * acc[d + 1] * inv, gv.z * acc[d + 2] * inv, gv.w * acc[d + 3] * inv);
+      }
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 0) ptx::tmem_dealloc<1>(tmem_base, 256);
+}
+
 // block = 128 threads (thread = output channel), 16 consecutive pairs
 template <typename T>
 __global__ void __launch_bounds__(128)
@@ -200,9 +448,18 @@ inline bool overlaps(const void* p, size_t pn, const void* q, size_t qn) {
   return a < b + qn && b < a + pn;
 }
 
-template <typename T>
-int launch_all(const void* z, const void* mask, const foldcp_triattn_params* p, int N, int node,
+// workspace layout (floats first): fp32 mode  q | k | v | g | t | tT ;  bf16 mode  og | g | then halves
+// q16 | k16 | vts | vte | t16s | t16e
+size_t workspace_bytes_for(int N, int dtype) {
+  const size_t np = static_cast<size_t>(N) * N;
+  const size_t b = dtype == FOLDCP_F32 ? np * (4 * C + 2 * kHeads) * sizeof(float)
+                                       : np * (2 * C * sizeof(float) + (4 * C + 2 * kHeads) * sizeof(__half));
+  return (b + 255) & ~static_cast<size_t>(255);
+}
+
+int launch_f32(const void* z, const void* mask, const foldcp_triattn_params* p, int N, int node,
                void* out, cudaStream_t s) {
+  using T = float;
   const long long npairs = static_cast<long long>(N) * N;
   float* ws = static_cast<float*>(p->workspace);
   float* q = ws;
@@ -215,13 +472,76 @@ int launch_all(const void* z, const void* mask, const foldcp_triattn_params* p, 
   ta_project_kernel<T><<<pblocks, 128, 0, s>>>(
       static_cast<const T*>(z), static_cast<const T*>(p->w_q), static_cast<const T*>(p->w_k),
       static_cast<const T*>(p->w_v), static_cast<const T*>(p->w_g), static_cast<const T*>(p->w_t),
-      p->ln_gamma, p->ln_beta, p->ln_eps, N, q, k, v, g, t, tT);
+      p->ln_gamma, p->ln_beta, p->ln_eps, N, q, k, v, g, t, tT, TcOut{});
   const bool starting = node == FOLDCP_TRIATTN_STARTING;
   const dim3 grid((N + kQueries - 1) / kQueries, N, kHeads);
   ta_attention_kernel<T><<<grid, kQueries, 0, s>>>(q, k, v, g, starting ? t : tT,
                                                    static_cast<const T*>(mask), N,
                                                    starting ? N : 1, starting ? 1 : N, q);
   ta_output_kernel<T><<<pblocks, 128, 0, s>>>(q, static_cast<const T*>(p->w_o), npairs,
+                                              static_cast<T*>(out));
+  return check_launch();
+}
+
+int launch_bf16(const void* z, const void* mask, const foldcp_triattn_params* p, int N, int node,
+                void* out, cudaStream_t s) {
+  using T = __nv_bfloat16;
+  const long long npairs = static_cast<long long>(N) * N;
+  float* og = static_cast<float*>(p->workspace);
+  float* g = og + npairs * C;
+  TcOut tc;
+  tc.q16 = reinterpret_cast<__half*>(g + npairs * C);
+  tc.k16 = tc.q16 + npairs * C;
+  tc.vts = tc.k16 + npairs * C;
+  tc.vte = tc.vts + npairs * C;
+  tc.t16s = tc.vte + npairs * C;
+  tc.t16e = tc.t16s + npairs * kHeads;
+  const int pblocks = static_cast<int>((npairs + kPairsPerBlock - 1) / kPairsPerBlock);
+  ta_project_kernel<T><<<pblocks, 128, 0, s>>>(
+      static_cast<const T*>(z), static_cast<const T*>(p->w_q), static_cast<const T*>(p->w_k),
+      static_cast<const T*>(p->w_v), static_cast<const T*>(p->w_g), static_cast<const T*>(p->w_t),
+      p->ln_gamma, p->ln_beta, p->ln_eps, N, nullptr, nullptr, nullptr, g, nullptr, nullptr, tc);
+  const bool starting = node == FOLDCP_TRIATTN_STARTING;
+  const uint64_t n = static_cast<uint64_t>(N);
+  CUtensorMap tq, tk, tv, tt;
+  int st;
+  {
+    // q16 / k16 [N*N][128] as (8 halves, row % 8, d / 8, row / 8 within the line, line): a box of
+    // (8, 8, 4, 16, 1) lands in shared memory as unswizzled 8 x 16-byte core matrices
+    const uint64_t row = C * 2;                                    // bytes of one pair's 128 halves
+    const uint64_t xs = starting ? row : n * row, ls = starting ? n * row : row;
+    const uint64_t dims[5] = {8, 8, C / 8, n / 8, n};
+    const uint64_t strides[4] = {xs, 16, 8 * xs, ls};
+    const uint32_t box[5] = {8, 8, 4, 16, 1};
+    if ((st = encode_tensor_map(&tq, tc.q16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
+    if ((st = encode_tensor_map(&tk, tc.k16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
+  }
+  {
+    const uint64_t dims[2] = {n, n * C};
+    const uint64_t strides[1] = {n * 2};
+    const uint32_t box[2] = {64, kHead};
+    if ((st = encode_tensor_map(&tv, starting ? tc.vts : tc.vte, 2, 2, dims, strides, box, 1)) != FOLDCP_OK)
+      return st;
+  }
+  {
+    const uint64_t dims[2] = {n, n * kHeads};
+    const uint64_t strides[1] = {n * 2};
+    const uint32_t box[2] = {64, 128};
+    if ((st = encode_tensor_map(&tt, starting ? tc.t16s : tc.t16e, 2, 2, dims, strides, box, 1)) != FOLDCP_OK)
+      return st;
+  }
+  TcAttnParams prm;
+  prm.g = g;
+  prm.mask = mask;
+  prm.og = og;
+  prm.N = N;
+  prm.ls = starting ? N : 1;
+  prm.xs = starting ? 1 : N;
+  if (ensure_dynamic_smem(reinterpret_cast<const void*>(ta_attention_tc_kernel), kTcSmem) != FOLDCP_OK)
+    return FOLDCP_ERR_CUDA;
+  const dim3 grid((N + 127) / 128, N, kHeads);
+  ta_attention_tc_kernel<<<grid, kTcThreads, kTcSmem, s>>>(tq, tk, tv, tt, prm);
+  ta_output_kernel<T><<<pblocks, 128, 0, s>>>(og, static_cast<const T*>(p->w_o), npairs,
                                               static_cast<T*>(out));
   return check_launch();
 }
@@ -236,8 +556,8 @@ extern "C" {
 size_t foldcp_triattn_workspace_bytes(int N, int c_z, int n_heads, int dtype) {
   if ((dtype != FOLDCP_F32 && dtype != FOLDCP_BF16) || N <= 0 || c_z != C || n_heads != kHeads)
     return 0;
-  const size_t np = static_cast<size_t>(N) * N;
-  return (np * (4 * C + 2 * kHeads) * sizeof(float) + 255) & ~static_cast<size_t>(255);
+  if (dtype == FOLDCP_BF16 && N % 8 != 0) return 0;     // 16-byte TMA row strides, like foldcp_trimul
+  return workspace_bytes_for(N, dtype);
 }
 
 int foldcp_triattn(const void* z, const void* mask, const foldcp_triattn_params* p, int N, int c_z,
@@ -247,7 +567,7 @@ int foldcp_triattn(const void* z, const void* mask, const foldcp_triattn_params*
   if (N <= 0 || c_z <= 0 || p->n_heads <= 0) return FOLDCP_ERR_INVALID_ARG;
   if (node != FOLDCP_TRIATTN_STARTING && node != FOLDCP_TRIATTN_ENDING) return FOLDCP_ERR_INVALID_ARG;
   if (c_z != C || p->n_heads != kHeads) return FOLDCP_ERR_UNSUPPORTED;
-  if (N > 32768) return FOLDCP_ERR_UNSUPPORTED;
+  if (N > 32768 || (p->dtype == FOLDCP_BF16 && N % 8 != 0)) return FOLDCP_ERR_UNSUPPORTED;
   const void* req[] = {z, out, p->ln_gamma, p->ln_beta, p->w_q, p->w_k, p->w_v, p->w_g, p->w_t, p->w_o};
   for (const void* r : req)
     if (!r) return FOLDCP_ERR_INVALID_ARG;
@@ -265,8 +585,8 @@ int foldcp_triattn(const void* z, const void* mask, const foldcp_triattn_params*
   if (!get_device_info(&d)) return FOLDCP_ERR_CUDA;
   if (!(d.cc_major == 10 && d.cc_minor == 0)) return FOLDCP_ERR_ARCH;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  return p->dtype == FOLDCP_F32 ? launch_all<float>(z, mask, p, N, node, out, s)
-                                : launch_all<__nv_bfloat16>(z, mask, p, N, node, out, s);
+  return p->dtype == FOLDCP_F32 ? launch_f32(z, mask, p, N, node, out, s)
+                                : launch_bf16(z, mask, p, N, node, out, s);
 }
 
 }  // extern "C"
