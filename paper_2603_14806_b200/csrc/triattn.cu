@@ -42,8 +42,7 @@ constexpr float kLog2e = 1.4426950408889634f;
 struct TcOut {
   __half* q16;    // [N*N][128]  q * log2(e) / sqrt(c)
   __half* k16;    // [N*N][128]
-  __half* vts;    // [N][128][N] v transposed per line, starting node
-  __half* vte;    // [N][128][N] ending node
+  __half* v16;    // [N*N][128]
   __half* t16s;   // [H][N][N]   t * log2(e), (query position, key position) of the starting node
   __half* t16e;   // [H][N][N]   transposed: ending node
 };
@@ -109,15 +108,10 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
       k[o] = ak[p];
       v[o] = av[p];
     } else {
-      // operands of the tensor-core attention: q carries 1/sqrt(c) and log2(e) (the softmax runs on
-      // exp2), v is written transposed for both nodes ([line][h][d][key], keys contiguous)
-      const long long pair = p0 + p;
-      const long long i = pair / N, j = pair % N;
+      // operands of the tensor-core attention: q carries 1/sqrt(c) and log2(e) (the softmax runs on exp2)
       tc.q16[o] = __float2half_rn(aq[p] * (kLog2e * 0.17677669529663687f));
       tc.k16[o] = __float2half_rn(ak[p]);
-      const __half vh = __float2half_rn(av[p]);
-      tc.vts[(i * C + tid) * N + j] = vh;      // starting node: line i, key position j
-      tc.vte[(j * C + tid) * N + i] = vh;      // ending node:   line j, key position i
+      tc.v16[o] = __float2half_rn(av[p]);
     }
   }
   // the triangular bias: thread (p, h) for the first 16 * H threads
@@ -209,18 +203,21 @@ ta_attention_kernel(const float* __restrict__ q, const float* __restrict__ k,
 //   S = Q K^T                 tcgen05.mma M=128 (queries) N=128 (keys) K=32, fp16 operands, into TMEM
 //   softmax (4 warps, thread = query row = TMEM lane): S + triangular bias tile + key mask, running
 //                             maximum, p = exp2(s - m) written as fp16 into the P tile
-//   O_blk = P V               tcgen05.mma M=128 N=32 K=128, V^T tile as the K-major B operand
+//   O_blk = P V               tcgen05.mma M=128 N=32 K=128, V tile as an MN-major B operand
 //   acc = acc * 2^(m_old - m_new) + O_blk   in registers; out = g * acc / l at the end
 // Operand layouts: Q and K tiles [128 rows][32 d] arrive through a 5-D tensor map as unswizzled core
 // matrices ([row / 8][d / 8][row % 8][8 halves]: lbo 128, sbo 512 -- the same descriptor form K3's
-// rank-one operands use); the bias tile, P and V^T are 128-byte-swizzled K-major tiles of two
-// 64-key boxes (K3's z / weight tiles).  The ending node is the same kernel on a tensor map with
-// swapped strides, the transposed bias and the other V^T.
+// rank-one operands use), and the V tile [128 keys][32 d] through the same map: for the product P V it
+// is an MN-major operand (d contiguous), the same core matrices read with the roles of lbo / sbo
+// swapped (for an MN-major unswizzled operand lbo is the stride between K-adjacent core matrices and
+// sbo between MN-adjacent ones -- measured: the other assignment fails parity); the bias tile and P are 128-byte-swizzled K-major tiles of two
+// 64-key boxes (K3's z tile).  The ending node is the same kernel on tensor maps with swapped
+// strides and the transposed bias -- no data is moved.
 // ---------------------------------------------------------------------------------------------
 constexpr int kTcThreads = 160;                   // warp 0: TMA + MMA issue; warps 1-4: softmax
 constexpr int kTcOffT = 0;                        // bias tile  [128 q][128 k] fp16, two SW128 boxes
 constexpr int kTcOffP = 32768;                    // P tile     [128 q][128 k] fp16, two SW128 boxes
-constexpr int kTcOffV = 65536;                    // V^T tile   [32 d][128 k]  fp16, two SW128 boxes
+constexpr int kTcOffV = 65536;                    // V tile     unswizzled core matrices, 8 KB
 constexpr int kTcOffQ = 73728;                    // Q tile     unswizzled core matrices, 8 KB
 constexpr int kTcOffK = 81920;                    // K tile
 constexpr int kTcOffM = 90112;                    // key mask bias, 128 floats
@@ -273,7 +270,8 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
   if (warp == 0) {
     if (ptx::elect_one()) {
       constexpr uint32_t idesc_s = ptx::make_idesc_f16kind(128, 128, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
-      constexpr uint32_t idesc_o = ptx::make_idesc_f16kind(128, 32, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
+      // B = V tile [key][d], d contiguous: an MN-major operand
+      constexpr uint32_t idesc_o = ptx::make_idesc_f16kind(128, 32, ptx::kFmtF16, ptx::kFmtF16, 0, 1);
       ptx::mbar_arrive_expect_tx(bar_q, 8192);
       ptx::tma_load_5d(smem + kTcOffQ, &tmap_q, bar_q, 0, 0, h * 4, pos0 / 8, line);
       ptx::mbar_wait(bar_q, 0);
@@ -282,8 +280,7 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (b > 0) ptx::mbar_wait(bar_free, (b - 1) & 1);
         ptx::mbar_arrive_expect_tx(bar_kv, 8192 + 8192 + 32768);
         ptx::tma_load_5d(smem + kTcOffK, &tmap_k, bar_kv, 0, 0, h * 4, k0 / 8, line);
-        ptx::tma_load_2d(smem + kTcOffV, &tmap_v, bar_kv, k0, (line * kHeads + h) * kHead);
-        ptx::tma_load_2d(smem + kTcOffV + 4096, &tmap_v, bar_kv, k0 + 64, (line * kHeads + h) * kHead);
+        ptx::tma_load_5d(smem + kTcOffV, &tmap_v, bar_kv, 0, 0, h * 4, k0 / 8, line);
         ptx::tma_load_2d(smem + kTcOffT, &tmap_t, bar_kv, k0, h * N + pos0);
         ptx::tma_load_2d(smem + kTcOffT + 16384, &tmap_t, bar_kv, k0 + 64, h * N + pos0);
         ptx::mbar_wait(bar_kv, b & 1);
@@ -299,9 +296,10 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {     // K = 128 keys
           const uint32_t offp = (ks >> 2) * 16384 + (ks & 3) * 32;
-          const uint32_t offv = (ks >> 2) * 4096 + (ks & 3) * 32;
+          // V core matrices [key / 8][d / 8][key % 8][8 halves]: key-adjacent 512 B apart (lbo of an
+          // MN-major operand), d-adjacent 128 B apart (sbo); one MMA of K = 16 keys = two key groups
           ptx::umma_bf16<1>(tm_o, ptx::make_smem_desc_sw128(smem + kTcOffP + offp, 16, 1024),
-                            ptx::make_smem_desc_sw128(smem + kTcOffV + offv, 16, 1024), idesc_o,
+                            ptx::make_smem_desc_noswizzle(smem + kTcOffV + ks * 1024, 512, 128), idesc_o,
                             ks ? 1u : 0u);
         }
         ptx::umma_commit<1>(bar_o);
@@ -449,11 +447,11 @@ inline bool overlaps(const void* p, size_t pn, const void* q, size_t qn) {
 }
 
 // workspace layout (floats first): fp32 mode  q | k | v | g | t | tT ;  bf16 mode  og | g | then halves
-// q16 | k16 | vts | vte | t16s | t16e
+// q16 | k16 | v16 | t16s | t16e
 size_t workspace_bytes_for(int N, int dtype) {
   const size_t np = static_cast<size_t>(N) * N;
   const size_t b = dtype == FOLDCP_F32 ? np * (4 * C + 2 * kHeads) * sizeof(float)
-                                       : np * (2 * C * sizeof(float) + (4 * C + 2 * kHeads) * sizeof(__half));
+                                       : np * (2 * C * sizeof(float) + (3 * C + 2 * kHeads) * sizeof(__half));
   return (b + 255) & ~static_cast<size_t>(255);
 }
 
@@ -492,9 +490,8 @@ int launch_bf16(const void* z, const void* mask, const foldcp_triattn_params* p,
   TcOut tc;
   tc.q16 = reinterpret_cast<__half*>(g + npairs * C);
   tc.k16 = tc.q16 + npairs * C;
-  tc.vts = tc.k16 + npairs * C;
-  tc.vte = tc.vts + npairs * C;
-  tc.t16s = tc.vte + npairs * C;
+  tc.v16 = tc.k16 + npairs * C;
+  tc.t16s = tc.v16 + npairs * C;
   tc.t16e = tc.t16s + npairs * kHeads;
   const int pblocks = static_cast<int>((npairs + kPairsPerBlock - 1) / kPairsPerBlock);
   ta_project_kernel<T><<<pblocks, 128, 0, s>>>(
@@ -515,13 +512,7 @@ int launch_bf16(const void* z, const void* mask, const foldcp_triattn_params* p,
     const uint32_t box[5] = {8, 8, 4, 16, 1};
     if ((st = encode_tensor_map(&tq, tc.q16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
     if ((st = encode_tensor_map(&tk, tc.k16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
-  }
-  {
-    const uint64_t dims[2] = {n, n * C};
-    const uint64_t strides[1] = {n * 2};
-    const uint32_t box[2] = {64, kHead};
-    if ((st = encode_tensor_map(&tv, starting ? tc.vts : tc.vte, 2, 2, dims, strides, box, 1)) != FOLDCP_OK)
-      return st;
+    if ((st = encode_tensor_map(&tv, tc.v16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
   }
   {
     const uint64_t dims[2] = {n, n * kHeads};
