@@ -14,6 +14,7 @@
 
 #include "../../include/foldcp_triattn.h"
 #include "common.h"
+#include "ln_rows.cuh"
 #include "ptx.cuh"
 
 namespace foldcp {
@@ -225,9 +226,9 @@ constexpr int kTcOffBar = 90624;
 constexpr int kTcSmem = kTcOffBar + 64;
 
 struct TcAttnParams {
-  const float* g;        // [N*N][128]
+  const __half* g;       // [N*N][128]  sigmoid gate
   const void* mask;      // bf16 [N][N] or nullptr
-  float* og;             // [N*N][128]  g * o
+  __half* og;            // [N*N][128]  g * o: the A operand of the output projection
   int N;
   long long ls, xs;      // pair (line, x) = line * ls + x * xs
 };
@@ -406,16 +407,267 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const float inv = 1.0f / l;
       const long long a = (static_cast<long long>(line) * prm.ls + static_cast<long long>(pos) * prm.xs) * C + h * kHead;
 #pragma unroll
-      for (int d = 0; d < kHead; d += 4) {
-        const float4 gv = *reinterpret_cast<const float4*>(prm.g + a + d);
-        *reinterpret_cast<float4*>(prm.og + a + d) =
-            make_float4(gv.x * acc[d] * inv, gv.y * acc[d + 1] * inv, gv.z * acc[d + 2] * inv, gv.w * acc[d + 3] * inv);
+      for (int d = 0; d < kHead; d += 8) {
+        const uint4 gv = *reinterpret_cast<const uint4*>(prm.g + a + d);
+        const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
+        uint32_t ow[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float2 gf = __half22float2(*reinterpret_cast<const __half2*>(&gw[e]));
+          ow[e] = ptx::pack_f16x2(gf.x * acc[d + 2 * e] * inv, gf.y * acc[d + 2 * e + 1] * inv);
+        }
+        *reinterpret_cast<uint4*>(prm.og + a + d) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
       }
     }
   }
   ptx::tc_fence_before();
   __syncthreads();
   if (warp == 0) ptx::tmem_dealloc<1>(tmem_base, 256);
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Tensor-core projections (bf16 mode).  One persistent kernel, tile = 128 pairs, bulk-synchronous per
+// tile (TMA -> LayerNorm -> MMA -> epilogue -> TMA store): these GEMMs move ~1.3 KB per pair against
+// the attention's O(N) work per pair, so simplicity wins over overlap here.
+//   kProj = true : z tile (bf16) -> LayerNorm with its affine, in place, fp16 -> round A: q, k and the
+//                  triangular bias t (N = 16, four rows used); round B: v, gate.  Outputs q16 (times
+//                  log2(e) / sqrt(c)), k16, v16, g16 = sigmoid as fp16 [pair][128]; t * log2(e) as fp16 in
+//                  both orientations.
+//   kProj = false: og tile (fp16, the attention's gated output) -> out = W_o og as bf16.
+// Operands exactly as in K3 (pairs = MMA M, output channel = MMA N, K-major 128-byte-swizzled tiles);
+// the bf16 weights become fp16 in shared memory once per CTA (exact).
+// ---------------------------------------------------------------------------------------------
+constexpr int kRgThreads = 256;
+constexpr int kRgHalfBox = 128 * 64 * 2;       // 16 KB
+constexpr int kRgMat = 2 * kRgHalfBox;         // 32 KB
+
+template <bool kProj>
+struct RgSmem {
+  static constexpr int kMats = kProj ? 4 : 1;
+  static constexpr int kOffW = 0;
+  static constexpr int kOffWt = kMats * kRgMat;                 // W_t padded to 16 rows: two boxes of 2 KB
+  static constexpr int kOffIn = kOffWt + (kProj ? 4096 : 0);    // input tile
+  static constexpr int kOffStage = kOffIn + kRgMat;             // staging [128 pairs][128 ch] 16-bit
+  static constexpr int kOffVec = kOffStage + kRgMat;            // gamma[128], beta[128] fp32
+  static constexpr int kOffBar = kOffVec + 1024;
+  static constexpr int kBytes = kOffBar + 64;
+};
+
+struct RgParams {
+  const float* gamma;
+  const float* beta;
+  float eps;
+  int N;
+  long long R;
+  int num_tiles;
+  __half* t16s;      // [H][N][N]
+  __half* t16e;
+};
+
+template <bool kProj>
+__global__ void __launch_bounds__(kRgThreads, 1)
+ta_rows_gemm_kernel(const __grid_constant__ CUtensorMap tmap_in,
+                    const __grid_constant__ CUtensorMap tmap_w0,
+                    const __grid_constant__ CUtensorMap tmap_w1,
+                    const __grid_constant__ CUtensorMap tmap_w2,
+                    const __grid_constant__ CUtensorMap tmap_w3,
+                    const __grid_constant__ CUtensorMap tmap_wt,
+                    const __grid_constant__ CUtensorMap tmap_o0,
+                    const __grid_constant__ CUtensorMap tmap_o1,
+                    const __grid_constant__ CUtensorMap tmap_o2,
+                    const __grid_constant__ CUtensorMap tmap_o3, const RgParams prm) {
+  using L = RgSmem<kProj>;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t smem = ptx::smem_u32(smem_raw);
+  const uint32_t bar = smem + L::kOffBar;
+  const uint32_t bar_w = bar, bar_in = bar + 8, bar_mma = bar + 16, tmem_slot = bar + 24;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
+  const CUtensorMap* wmaps[4] = {&tmap_w0, &tmap_w1, &tmap_w2, &tmap_w3};
+  const CUtensorMap* omaps[4] = {&tmap_o0, &tmap_o1, &tmap_o2, &tmap_o3};
+
+  if (tid == 0) {
+    ptx::mbar_init(bar_w, 1);
+    ptx::mbar_init(bar_in, 1);
+    ptx::mbar_init(bar_mma, 1);
+    ptx::fence_mbar_init();
+  }
+  if (warp == 1) ptx::tmem_alloc<1>(tmem_slot, 512);
+  if (kProj && tid < 128) {
+    reinterpret_cast<float*>(smem_raw + L::kOffVec)[tid] = prm.gamma[tid];
+    reinterpret_cast<float*>(smem_raw + L::kOffVec)[128 + tid] = prm.beta[tid];
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  // weights: once per CTA, bf16 -> fp16 in place (exact for |w| in [2^-14, 65504])
+  if (tid == 0) {
+    ptx::mbar_arrive_expect_tx(bar_w, L::kMats * kRgMat + (kProj ? 4096 : 0));
+    for (int m = 0; m < L::kMats; ++m) {
+      ptx::tma_load_2d(smem + L::kOffW + m * kRgMat, wmaps[m], bar_w, 0, 0);
+      ptx::tma_load_2d(smem + L::kOffW + m * kRgMat + kRgHalfBox, wmaps[m], bar_w, 64, 0);
+    }
+    if (kProj) {
+      ptx::tma_load_2d(smem + L::kOffWt, &tmap_wt, bar_w, 0, 0);        // rows 4..15: out of bounds = 0
+      ptx::tma_load_2d(smem + L::kOffWt + 2048, &tmap_wt, bar_w, 64, 0);
+    }
+  }
+  ptx::mbar_wait(bar_w, 0);
+  ptx::smem_bf16_to_f16_inplace(smem + L::kOffW, L::kMats * kRgMat + (kProj ? 4096 : 0), tid, kRgThreads);
+  ptx::fence_proxy_async_smem();
+  __syncthreads();
+
+  constexpr uint32_t idesc128 = ptx::make_idesc_f16kind(128, 128, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
+  constexpr uint32_t idesc16 = ptx::make_idesc_f16kind(128, 16, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
+  const int q4 = warp & 3;                   // TMEM lane quadrant
+  const int half = warp >> 2;                // which 64 output channels
+  const int r = q4 * 32 + lane;              // pair row of the tile
+  const uint32_t lane_addr = static_cast<uint32_t>(q4 * 32) << 16;
+  const uint32_t sw = static_cast<uint32_t>(r & 7);
+  uint32_t mma_phase = 0;
+
+  auto issue_gemm = [&](int m, uint32_t dcol) {       // D[dcol ..] = in_tile * W_m^T
+#pragma unroll
+    for (int ks = 0; ks < 8; ++ks) {
+      const uint32_t off = (ks >> 2) * kRgHalfBox + (ks & 3) * 32;
+      ptx::umma_bf16<1>(tmem_base + dcol, ptx::make_smem_desc_sw128(smem + L::kOffIn + off, 16, 1024),
+                        ptx::make_smem_desc_sw128(smem + L::kOffW + m * kRgMat + off, 16, 1024), idesc128,
+                        ks ? 1u : 0u);
+    }
+  };
+  // epilogue of one matrix: this thread's 64 channels of its pair -> staging -> one TMA store
+  auto epilogue = [&](int m, uint32_t dcol, const CUtensorMap* omap, int tile) {
+    if (tid == 0) ptx::tma_store_wait_read<0>();         // the previous store has read the staging tile
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      uint32_t v[32];
+      ptx::tmem_ld_32x32(tmem_base + lane_addr + dcol + half * 64 + c * 32, v);
+      ptx::tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        uint32_t pw[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          float x0 = __uint_as_float(v[i * 8 + e * 2]), x1 = __uint_as_float(v[i * 8 + e * 2 + 1]);
+          if (kProj) {
+            if (m == 0) {                                // q carries 1/sqrt(c) and log2(e)
+              x0 *= kLog2e * 0.17677669529663687f;
+              x1 *= kLog2e * 0.17677669529663687f;
+            } else if (m == 3) {                         // gate
+              x0 = 1.0f / (1.0f + __expf(-x0));
+              x1 = 1.0f / (1.0f + __expf(-x1));
+            }
+            pw[e] = ptx::pack_f16x2(x0, x1);
+          } else {
+            pw[e] = ptx::pack_bf16x2(x0, x1);
+          }
+        }
+        ptx::sts128(smem + L::kOffStage + half * kRgHalfBox + r * 128 +
+                        ((static_cast<uint32_t>(c * 4 + i) ^ sw) << 4),
+                    pw[0], pw[1], pw[2], pw[3]);
+      }
+    }
+    ptx::tc_fence_before();
+    ptx::fence_proxy_async_smem();
+    __syncthreads();
+    if (tid == 0) {
+      ptx::tma_store_2d(omap, smem + L::kOffStage, 0, tile * 128);
+      ptx::tma_store_2d(omap, smem + L::kOffStage + kRgHalfBox, 64, tile * 128);
+      ptx::tma_store_commit();
+    }
+  };
+
+  int it = 0;
+  if (tid == 0 && static_cast<int>(blockIdx.x) < prm.num_tiles) {
+    ptx::mbar_arrive_expect_tx(bar_in, kRgMat);
+    ptx::tma_load_2d(smem + L::kOffIn, &tmap_in, bar_in, 0, blockIdx.x * 128);
+    ptx::tma_load_2d(smem + L::kOffIn + kRgHalfBox, &tmap_in, bar_in, 64, blockIdx.x * 128);
+  }
+  for (int t = blockIdx.x; t < prm.num_tiles; t += gridDim.x, ++it) {
+    ptx::mbar_wait(bar_in, it & 1);
+    if (kProj) {
+      layernorm_rows_inplace<true, true, 1, kRgThreads>(smem + L::kOffIn, kRgHalfBox, tid, smem + L::kOffVec,
+                                                        smem + L::kOffVec + 512, prm.eps);
+      ptx::fence_proxy_async_smem();
+    }
+    __syncthreads();
+    // ---- round A: q, k, t  (or the only matrix)
+    if (tid == 0) {
+      ptx::tc_fence_after();
+      issue_gemm(0, 0);
+      if (kProj) {
+        issue_gemm(1, 128);
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          const uint32_t off = (ks >> 2) * kRgHalfBox + (ks & 3) * 32;
+          const uint32_t offt = (ks >> 2) * 2048 + (ks & 3) * 32;
+          ptx::umma_bf16<1>(tmem_base + 256, ptx::make_smem_desc_sw128(smem + L::kOffIn + off, 16, 1024),
+                            ptx::make_smem_desc_sw128(smem + L::kOffWt + offt, 16, 1024), idesc16,
+                            ks ? 1u : 0u);
+        }
+      }
+      ptx::umma_commit<1>(bar_mma);
+    }
+    ptx::mbar_wait(bar_mma, mma_phase);
+    mma_phase ^= 1u;
+    ptx::tc_fence_after();
+    epilogue(0, 0, omaps[0], t);
+    if (kProj) {
+      epilogue(1, 128, omaps[1], t);
+      if (half == 0) {
+        // the triangular bias of this thread's pair: four heads, both orientations
+        uint32_t tv[8];
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : "=r"(tv[0]), "=r"(tv[1]), "=r"(tv[2]), "=r"(tv[3]), "=r"(tv[4]), "=r"(tv[5]),
+                       "=r"(tv[6]), "=r"(tv[7])
+                     : "r"(tmem_base + lane_addr + 256)
+                     : "memory");
+        ptx::tmem_ld_wait();
+        const long long pair = static_cast<long long>(t) * 128 + r;
+        if (pair < prm.R) {
+          const long long i = pair / prm.N, j = pair % prm.N;
+#pragma unroll
+          for (int h = 0; h < kHeads; ++h) {
+            const __half th = __float2half_rn(__uint_as_float(tv[h]) * kLog2e);
+            prm.t16s[(static_cast<long long>(h) * prm.N + i) * prm.N + j] = th;
+            prm.t16e[(static_cast<long long>(h) * prm.N + j) * prm.N + i] = th;
+          }
+        }
+      }
+      // ---- round B: v, gate (the accumulators of round A have been read by everybody)
+      ptx::tc_fence_before();
+      __syncthreads();
+      if (tid == 0) {
+        ptx::tc_fence_after();
+        issue_gemm(2, 0);
+        issue_gemm(3, 128);
+        ptx::umma_commit<1>(bar_mma);
+      }
+      ptx::mbar_wait(bar_mma, mma_phase);
+      mma_phase ^= 1u;
+      ptx::tc_fence_after();
+    }
+    // the input tile is free: fetch the next one while the last epilogues run
+    if (tid == 0 && t + static_cast<int>(gridDim.x) < prm.num_tiles) {
+      ptx::mbar_arrive_expect_tx(bar_in, kRgMat);
+      ptx::tma_load_2d(smem + L::kOffIn, &tmap_in, bar_in, 0, (t + gridDim.x) * 128);
+      ptx::tma_load_2d(smem + L::kOffIn + kRgHalfBox, &tmap_in, bar_in, 64, (t + gridDim.x) * 128);
+    }
+    if (kProj) {
+      epilogue(2, 0, omaps[2], t);
+      epilogue(3, 128, omaps[3], t);
+    }
+    ptx::tc_fence_before();
+    __syncthreads();     // accumulators read before the next tile's MMAs overwrite them
+  }
+  if (tid == 0) ptx::tma_store_wait<0>();
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) ptx::tmem_dealloc<1>(tmem_base, 512);
 }
 
 // block = 128 threads (thread = output channel), 16 consecutive pairs
@@ -446,12 +698,12 @@ inline bool overlaps(const void* p, size_t pn, const void* q, size_t qn) {
   return a < b + qn && b < a + pn;
 }
 
-// workspace layout (floats first): fp32 mode  q | k | v | g | t | tT ;  bf16 mode  og | g | then halves
-// q16 | k16 | v16 | t16s | t16e
+// workspace layout: fp32 mode  q | k | v | g | t | tT  (floats);  bf16 mode  q16 | k16 | v16 | g16 | og16 |
+// t16s | t16e  (halves)
 size_t workspace_bytes_for(int N, int dtype) {
   const size_t np = static_cast<size_t>(N) * N;
   const size_t b = dtype == FOLDCP_F32 ? np * (4 * C + 2 * kHeads) * sizeof(float)
-                                       : np * (2 * C * sizeof(float) + (3 * C + 2 * kHeads) * sizeof(__half));
+                                       : np * (5 * C + 2 * kHeads) * sizeof(__half);
   return (b + 255) & ~static_cast<size_t>(255);
 }
 
@@ -483,57 +735,98 @@ int launch_f32(const void* z, const void* mask, const foldcp_triattn_params* p, 
 
 int launch_bf16(const void* z, const void* mask, const foldcp_triattn_params* p, int N, int node,
                 void* out, cudaStream_t s) {
-  using T = __nv_bfloat16;
+  DeviceInfo dev;
+  if (!get_device_info(&dev)) return FOLDCP_ERR_CUDA;
   const long long npairs = static_cast<long long>(N) * N;
-  float* og = static_cast<float*>(p->workspace);
-  float* g = og + npairs * C;
-  TcOut tc;
-  tc.q16 = reinterpret_cast<__half*>(g + npairs * C);
-  tc.k16 = tc.q16 + npairs * C;
-  tc.v16 = tc.k16 + npairs * C;
-  tc.t16s = tc.v16 + npairs * C;
-  tc.t16e = tc.t16s + npairs * kHeads;
-  const int pblocks = static_cast<int>((npairs + kPairsPerBlock - 1) / kPairsPerBlock);
-  ta_project_kernel<T><<<pblocks, 128, 0, s>>>(
-      static_cast<const T*>(z), static_cast<const T*>(p->w_q), static_cast<const T*>(p->w_k),
-      static_cast<const T*>(p->w_v), static_cast<const T*>(p->w_g), static_cast<const T*>(p->w_t),
-      p->ln_gamma, p->ln_beta, p->ln_eps, N, nullptr, nullptr, nullptr, g, nullptr, nullptr, tc);
+  __half* q16 = static_cast<__half*>(p->workspace);
+  __half* k16 = q16 + npairs * C;
+  __half* v16 = k16 + npairs * C;
+  __half* g16 = v16 + npairs * C;
+  __half* og16 = g16 + npairs * C;
+  __half* t16s = og16 + npairs * C;
+  __half* t16e = t16s + npairs * kHeads;
   const bool starting = node == FOLDCP_TRIATTN_STARTING;
-  const uint64_t n = static_cast<uint64_t>(N);
-  CUtensorMap tq, tk, tv, tt;
+  const uint64_t n = static_cast<uint64_t>(N), R = n * n;
   int st;
+  auto rows_map = [&](CUtensorMap* m, const void* base) {   // [R][128] 16-bit, box 64 x 128, SW128
+    const uint64_t dims[2] = {C, R};
+    const uint64_t strides[1] = {C * 2};
+    const uint32_t box[2] = {64, 128};
+    return encode_tensor_map(m, base, 2, 2, dims, strides, box, 1);
+  };
+  auto weight_map = [&](CUtensorMap* m, const void* base, uint64_t rows, uint32_t box_rows) {
+    const uint64_t dims[2] = {C, rows};
+    const uint64_t strides[1] = {C * 2};
+    const uint32_t box[2] = {64, box_rows};
+    return encode_tensor_map(m, base, 2, 2, dims, strides, box, 1);
+  };
+  RgParams rp;
+  rp.gamma = p->ln_gamma;
+  rp.beta = p->ln_beta;
+  rp.eps = p->ln_eps;
+  rp.N = N;
+  rp.R = npairs;
+  rp.num_tiles = static_cast<int>((npairs + 127) / 128);
+  rp.t16s = t16s;
+  rp.t16e = t16e;
+  const int grid_rg = rp.num_tiles < dev.sm_count ? rp.num_tiles : dev.sm_count;
   {
-    // q16 / k16 [N*N][128] as (8 halves, row % 8, d / 8, row / 8 within the line, line): a box of
+    // LayerNorm + q / k / v / gate / triangular-bias projections on the tensor cores
+    CUtensorMap tin, w[4], wt, o[4];
+    if ((st = rows_map(&tin, z)) != FOLDCP_OK) return st;
+    const void* ws[4] = {p->w_q, p->w_k, p->w_v, p->w_g};
+    const void* os[4] = {q16, k16, v16, g16};
+    for (int m = 0; m < 4; ++m) {
+      if ((st = weight_map(&w[m], ws[m], C, 128)) != FOLDCP_OK) return st;
+      if ((st = rows_map(&o[m], os[m])) != FOLDCP_OK) return st;
+    }
+    if ((st = weight_map(&wt, p->w_t, kHeads, 16)) != FOLDCP_OK) return st;
+    auto kern = ta_rows_gemm_kernel<true>;
+    if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), RgSmem<true>::kBytes) != FOLDCP_OK)
+      return FOLDCP_ERR_CUDA;
+    kern<<<grid_rg, kRgThreads, RgSmem<true>::kBytes, s>>>(tin, w[0], w[1], w[2], w[3], wt, o[0], o[1],
+                                                           o[2], o[3], rp);
+  }
+  {
+    CUtensorMap tq, tk, tv, tt;
+    // q16 / k16 / v16 [N*N][128] as (8 halves, row % 8, d / 8, row / 8 within the line, line): a box of
     // (8, 8, 4, 16, 1) lands in shared memory as unswizzled 8 x 16-byte core matrices
     const uint64_t row = C * 2;                                    // bytes of one pair's 128 halves
     const uint64_t xs = starting ? row : n * row, ls = starting ? n * row : row;
     const uint64_t dims[5] = {8, 8, C / 8, n / 8, n};
     const uint64_t strides[4] = {xs, 16, 8 * xs, ls};
     const uint32_t box[5] = {8, 8, 4, 16, 1};
-    if ((st = encode_tensor_map(&tq, tc.q16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
-    if ((st = encode_tensor_map(&tk, tc.k16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
-    if ((st = encode_tensor_map(&tv, tc.v16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
+    if ((st = encode_tensor_map(&tq, q16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
+    if ((st = encode_tensor_map(&tk, k16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
+    if ((st = encode_tensor_map(&tv, v16, 2, 5, dims, strides, box, 0)) != FOLDCP_OK) return st;
+    const uint64_t tdims[2] = {n, n * kHeads};
+    const uint64_t tstrides[1] = {n * 2};
+    const uint32_t tbox[2] = {64, 128};
+    if ((st = encode_tensor_map(&tt, starting ? t16s : t16e, 2, 2, tdims, tstrides, tbox, 1)) != FOLDCP_OK)
+      return st;
+    TcAttnParams prm;
+    prm.g = g16;
+    prm.mask = mask;
+    prm.og = og16;
+    prm.N = N;
+    prm.ls = starting ? N : 1;
+    prm.xs = starting ? 1 : N;
+    if (ensure_dynamic_smem(reinterpret_cast<const void*>(ta_attention_tc_kernel), kTcSmem) != FOLDCP_OK)
+      return FOLDCP_ERR_CUDA;
+    const dim3 grid((N + 127) / 128, N, kHeads);
+    ta_attention_tc_kernel<<<grid, kTcThreads, kTcSmem, s>>>(tq, tk, tv, tt, prm);
   }
   {
-    const uint64_t dims[2] = {n, n * kHeads};
-    const uint64_t strides[1] = {n * 2};
-    const uint32_t box[2] = {64, 128};
-    if ((st = encode_tensor_map(&tt, starting ? tc.t16s : tc.t16e, 2, 2, dims, strides, box, 1)) != FOLDCP_OK)
-      return st;
+    // out = W_o (g * o)
+    CUtensorMap tin, w, o;
+    if ((st = rows_map(&tin, og16)) != FOLDCP_OK) return st;
+    if ((st = weight_map(&w, p->w_o, C, 128)) != FOLDCP_OK) return st;
+    if ((st = rows_map(&o, out)) != FOLDCP_OK) return st;
+    auto kern = ta_rows_gemm_kernel<false>;
+    if (ensure_dynamic_smem(reinterpret_cast<const void*>(kern), RgSmem<false>::kBytes) != FOLDCP_OK)
+      return FOLDCP_ERR_CUDA;
+    kern<<<grid_rg, kRgThreads, RgSmem<false>::kBytes, s>>>(tin, w, w, w, w, w, o, o, o, o, rp);
   }
-  TcAttnParams prm;
-  prm.g = g;
-  prm.mask = mask;
-  prm.og = og;
-  prm.N = N;
-  prm.ls = starting ? N : 1;
-  prm.xs = starting ? 1 : N;
-  if (ensure_dynamic_smem(reinterpret_cast<const void*>(ta_attention_tc_kernel), kTcSmem) != FOLDCP_OK)
-    return FOLDCP_ERR_CUDA;
-  const dim3 grid((N + 127) / 128, N, kHeads);
-  ta_attention_tc_kernel<<<grid, kTcThreads, kTcSmem, s>>>(tq, tk, tv, tt, prm);
-  ta_output_kernel<T><<<pblocks, 128, 0, s>>>(og, static_cast<const T*>(p->w_o), npairs,
-                                              static_cast<T*>(out));
   return check_launch();
 }
 
