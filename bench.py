@@ -502,7 +502,7 @@ def run_triattn(ctx, N=1024, steps=2):
     return {"workload": f"triangle attention (PAPER.md Eq. 1), N={N}, c_z=128, 4 heads x 32, bf16 storage",
             "ms_per_call": res, "counted_tflop_per_call": fl / 1e12, "tflops": fl / (ms * 1e-3) / 1e12,
             "steps": steps, "gpu_launches_per_call": 3,
-            "note": "first correct CUDA path: CUDA-core kernels, fp32 arithmetic -- not yet on tcgen05"}
+            "note": "bf16 mode: projections, QK^T, PV and the output projection on tcgen05 (csrc/triattn.cu)"}
 
 
 def run_n8192(ctx, steps=3):

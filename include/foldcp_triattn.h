@@ -1,5 +1,5 @@
 /*
- * foldcp_triattn.h -- C ABI of triangle attention, a first correct CUDA path.
+ * foldcp_triattn.h -- C ABI of triangle attention.
  *
  * The operation (section 3.2, lines 98-115, Eq. 1):
  *       Q, K, V = proj(z),   output = softmax(Q K^T / sqrt(d) + tri_bias(z) + mask_bias) V
@@ -16,10 +16,12 @@
  *       out_ij  = W_o concat_h(o_ij)            [N,N,c_z]
  *   with mb = -1e9 * (1 - M) for the pair mask M (values 0 or 1; NULL = all ones).
  *
- * State of this path: plain CUDA-core kernels with fp32 arithmetic in both dtypes (projection,
- * online-softmax attention tiled over the keys in shared memory, output projection) -- correct
- * against the fp64 oracle (oracle/triattn_oracle.py), measured, NOT yet on tcgen05.
- * section 8 says what the tensor-core version needs.
+ * FOLDCP_BF16: three tcgen05 launches -- LayerNorm + q / k / v / gate / bias projections as tensor-core
+ * GEMMs, attention with S = Q K^T and O = P V on the tensor cores (softmax on exp2 with a running
+ * maximum; q, k, v, the gate, P and the gated output are held as IEEE fp16, the triangular bias as
+ * fp16), output projection.  Needs N % 8 == 0 (16-byte TMA strides), like foldcp_trimul.
+ * FOLDCP_F32: the exact mode, plain CUDA-core kernels with fp32 arithmetic, any N.
+ * Both are checked element by element against the fp64 oracle (oracle/triattn_oracle.py).
  *
  * Conventions as in foldcp_trimul.h: device pointers owned by the caller, params struct in host
  * memory, asynchronous on `stream`, no allocation, status codes of foldcp_status_t.
@@ -53,7 +55,7 @@ typedef struct {
 } foldcp_triattn_params;
 
 /*
- *   z, out  [N][N][c_z] device, dtype = params->dtype; c_z = 128; any N >= 1
+ *   z, out  [N][N][c_z] device, dtype = params->dtype; c_z = 128; N >= 1 (bf16 mode: N % 8 == 0)
  *   mask    [N][N] device, same dtype, values 0 / 1 (the KEY position's mask enters the softmax as
  *           -1e9; every query row is expected to keep at least one unmasked key)
  *   node    foldcp_triattn_node_t
@@ -62,7 +64,8 @@ typedef struct {
 int foldcp_triattn(const void* z, const void* mask, const foldcp_triattn_params* params, int N,
                    int c_z, int node, void* out, void* stream);
 
-/* q, k, v, g as fp32 [N][N][128] plus the triangular bias in both orientations; 0 if unsupported. */
+/* q, k, v, gate (and, in bf16 mode, the gated output) as [N][N][128] in fp32 / fp16 plus the triangular
+ * bias in both orientations; 0 if the shape / dtype is unsupported. */
 size_t foldcp_triattn_workspace_bytes(int N, int c_z, int n_heads, int dtype);
 
 #ifdef __cplusplus

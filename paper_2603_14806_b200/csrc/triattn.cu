@@ -1,14 +1,19 @@
-// Triangle attention (section 3.2 lines 98-115, Eq. 1; AF3 Alg. 14/15):
-// a first correct CUDA path on the CUDA cores, fp32 arithmetic, for both storage types.
+// Triangle attention (section 3.2 lines 98-115, Eq. 1; AF3 Alg. 14/15).
 //
-//   ta_project_kernel    z' = LN(z);  q, k, v = W z';  g = sigmoid(W_g z');  t = W_t z'  (t also transposed)
-//   ta_attention_kernel  per (line, head): out[pos] = g * softmax_k(q[pos] . k[k] / sqrt(c) + t[pos][k] + mb[k]) v
-//                        -- online softmax over key chunks staged in shared memory; "line" is the row i
-//                        (starting node) or the column j (ending node), "pos" the other pair index, so
-//                        the ending node is the same kernel with swapped strides and the transposed bias
-//   ta_output_kernel     out = W_o (g * o)
-// Layouts: z / out [N][N][128]; workspace q, k, v, g fp32 [N][N][128] (head-major inside: h * 32 + d);
-// t, tT fp32 [H][N][N].
+// bf16 mode -- everything on tcgen05, three launches:
+//   ta_rows_gemm_kernel<true>   z tile -> LayerNorm (with its affine, in place, fp16) -> q, k, v, gate and
+//                               the triangular bias as tensor-core GEMMs; fp16 outputs [pair][128]
+//   ta_attention_tc_kernel      per (128 queries, line, head): S = Q K^T into TMEM, softmax warps (thread =
+//                               query row) add the bias tile and the key mask and write P = exp2(s - m) as
+//                               fp16, O_blk = P V, running output in registers; "line" is the row i
+//                               (starting node) or the column j (ending node) -- the ending node is the
+//                               same kernel on tensor maps with swapped strides and the transposed bias
+//   ta_rows_gemm_kernel<false>  out = W_o (g * o)
+// fp32 mode -- the exact mode (1e-5 relative), plain CUDA-core kernels with the same three stages:
+//   ta_project_kernel, ta_attention_kernel (online softmax over key chunks in shared memory),
+//   ta_output_kernel.
+// Layouts: z / out [N][N][128]; intermediates [N][N][128] (head-major inside: h * 32 + d), fp16 in bf16
+// mode, fp32 in fp32 mode; triangular bias [H][N][N] in both orientations.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
@@ -39,15 +44,6 @@ template <> __device__ __forceinline__ void stf<__nv_bfloat16>(__nv_bfloat16* p,
 }
 
 constexpr float kLog2e = 1.4426950408889634f;
-// 16-bit operands of the tensor-core attention (bf16 mode); all nullptr in fp32 mode
-struct TcOut {
-  __half* q16;    // [N*N][128]  q * log2(e) / sqrt(c)
-  __half* k16;    // [N*N][128]
-  __half* v16;    // [N*N][128]
-  __half* t16s;   // [H][N][N]   t * log2(e), (query position, key position) of the starting node
-  __half* t16e;   // [H][N][N]   transposed: ending node
-};
-
 // block = 128 threads (thread = output channel), 16 consecutive pairs
 template <typename T>
 __global__ void __launch_bounds__(128)
@@ -55,7 +51,7 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
                   const T* __restrict__ w_v, const T* __restrict__ w_g, const T* __restrict__ w_t,
                   const float* __restrict__ gamma, const float* __restrict__ beta, float eps, int N,
                   float* __restrict__ q, float* __restrict__ k, float* __restrict__ v,
-                  float* __restrict__ g, float* __restrict__ t, float* __restrict__ tT, TcOut tc) {
+                  float* __restrict__ g, float* __restrict__ t, float* __restrict__ tT) {
   __shared__ float zs[kPairsPerBlock][C];
   const long long npairs = static_cast<long long>(N) * N;
   const long long p0 = static_cast<long long>(blockIdx.x) * kPairsPerBlock;
@@ -104,16 +100,9 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
   for (int p = 0; p < np; ++p) {
     const long long o = (p0 + p) * C + tid;
     g[o] = 1.0f / (1.0f + expf(-ag[p]));
-    if (tc.q16 == nullptr) {
-      q[o] = aq[p];
-      k[o] = ak[p];
-      v[o] = av[p];
-    } else {
-      // operands of the tensor-core attention: q carries 1/sqrt(c) and log2(e) (the softmax runs on exp2)
-      tc.q16[o] = __float2half_rn(aq[p] * (kLog2e * 0.17677669529663687f));
-      tc.k16[o] = __float2half_rn(ak[p]);
-      tc.v16[o] = __float2half_rn(av[p]);
-    }
+    q[o] = aq[p];
+    k[o] = ak[p];
+    v[o] = av[p];
   }
   // the triangular bias: thread (p, h) for the first 16 * H threads
   if (tid < kPairsPerBlock * kHeads) {
@@ -123,14 +112,8 @@ ta_project_kernel(const T* __restrict__ z, const T* __restrict__ w_q, const T* _
       for (int c = 0; c < C; ++c) acc = fmaf(ldf(w_t + h * C + c), zs[p][c], acc);
       const long long pair = p0 + p;
       const long long i = pair / N, j = pair % N;
-      if (tc.q16 == nullptr) {
-        t[(static_cast<long long>(h) * N + i) * N + j] = acc;
-        tT[(static_cast<long long>(h) * N + j) * N + i] = acc;
-      } else {
-        const __half th = __float2half_rn(acc * kLog2e);
-        tc.t16s[(static_cast<long long>(h) * N + i) * N + j] = th;
-        tc.t16e[(static_cast<long long>(h) * N + j) * N + i] = th;
-      }
+      t[(static_cast<long long>(h) * N + i) * N + j] = acc;
+      tT[(static_cast<long long>(h) * N + j) * N + i] = acc;
     }
   }
 }
@@ -722,7 +705,7 @@ int launch_f32(const void* z, const void* mask, const foldcp_triattn_params* p, 
   ta_project_kernel<T><<<pblocks, 128, 0, s>>>(
       static_cast<const T*>(z), static_cast<const T*>(p->w_q), static_cast<const T*>(p->w_k),
       static_cast<const T*>(p->w_v), static_cast<const T*>(p->w_g), static_cast<const T*>(p->w_t),
-      p->ln_gamma, p->ln_beta, p->ln_eps, N, q, k, v, g, t, tT, TcOut{});
+      p->ln_gamma, p->ln_beta, p->ln_eps, N, q, k, v, g, t, tT);
   const bool starting = node == FOLDCP_TRIATTN_STARTING;
   const dim3 grid((N + kQueries - 1) / kQueries, N, kHeads);
   ta_attention_kernel<T><<<grid, kQueries, 0, s>>>(q, k, v, g, starting ? t : tT,

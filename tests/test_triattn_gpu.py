@@ -87,3 +87,9 @@ def test_triattn_rejects_bad_arguments():
         B.triattn(zd, None, pd, 0, out=zd)
     assert ei.value.status == 5
     assert B.triattn_workspace_bytes(16, 64) == 0 and B.triattn_workspace_bytes(16, 128, 8) == 0
+    # bf16 mode needs N % 8 == 0 (16-byte TMA strides); the fp32 mode takes any N
+    assert B.triattn_workspace_bytes(12, dtype=B.BF16) == 0 and B.triattn_workspace_bytes(12, dtype=B.F32) > 0
+    z12 = torch.zeros(12, 12, 128, dtype=torch.bfloat16, device=DEV)
+    with pytest.raises(B.FoldcpError) as ei:
+        B.triattn(z12, None, pd, 0)
+    assert ei.value.status == 2
