@@ -114,7 +114,14 @@ struct K1Params {
   int num_tiles;
   unsigned int* sched;
   float2* stats;               // [R] (mean, rstd) of every pair's LayerNorm(z), or nullptr: K3 re-uses them
+  int dbg_skip;                // debug builds only: 1 no LayerNorm arithmetic, 2 no epilogue arithmetic, 4 no TMA stores
 };
+
+#ifdef FOLDCP_DEBUG_KNOBS
+#define K1_DBG_SKIP(bit) ((prm.dbg_skip & (bit)) != 0)
+#else
+#define K1_DBG_SKIP(bit) false
+#endif
 
 // kOutF16: a and b are written as IEEE fp16 (the forward path: 11-bit significand, see the header's
 // numerics notes) instead of bf16 (the backward pass's recomputation, whose contraction-gradient
@@ -274,8 +281,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
             K1_PROBE_T0(t1);
             ptx::mbar_wait(ofull(b), it & 1);
             K1_PROBE_ADD(sw_f, t1);
-            ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, smem + kOffOut + b * kHalfBox,
-                              t * kTilePairs + g * 64, 0);
+            if (!K1_DBG_SKIP(4))
+              ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, smem + kOffOut + b * kHalfBox,
+                                t * kTilePairs + g * 64, 0);
             ptx::tma_store_commit();
             if (prev >= 0) {
               K1_PROBE_T0(t2);
@@ -318,6 +326,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
       ptx::mbar_wait(zfull(s), (it / kZStages) & 1);
       K1_PROBE_ADD(lw, t1);
       K1_PROBE_T0(t2);
+      if (!K1_DBG_SKIP(1))
       layernorm_rows_inplace<kNormFp16, false, kLnWarps == 4 ? 2 : 1, kLnWarps * 32>(
           smem + kOffZ + s * kMatBytes, kHalfBox, r, 0, 0, prm.eps,
           [&](uint32_t row, float mean, float rstd) {
@@ -500,7 +509,10 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
             if (lane == 0) ptx::mbar_arrive(tempty(slot));
           }
           uint32_t packed[8];
-          if (masked) {
+          if (K1_DBG_SKIP(2)) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) packed[i] = vp[cb][2 * i] ^ vg[cb][2 * i + 1];
+          } else if (masked) {
             compute_chunk(vp[cb], vg[cb], maddr + k * 64, true, packed);
           } else {
             compute_chunk(vp[cb], vg[cb], maddr + k * 64, false, packed);
@@ -563,7 +575,11 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   }
   {
     const uint64_t dims[2] = {R, kC};
-    const uint64_t strides[1] = {R * 2};
+    static const uint64_t dbg_pad = [] {
+      const char* e = debug_env("FOLDCP_K1_PAD");     // timing experiment: padded channel stride (bytes)
+      return e ? static_cast<uint64_t>(atoll(e)) : 0ull;
+    }();
+    const uint64_t strides[1] = {R * 2 + dbg_pad};
     const uint32_t box[2] = {64, 128};
     if ((st = encode_tensor_map(&ta, a, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
     if ((st = encode_tensor_map(&tb, b, 2, 2, dims, strides, box, true)) != FOLDCP_OK) return st;
@@ -585,6 +601,11 @@ int launch_k1_project_bf16(const void* z, const void* mask, const foldcp_trimul_
   prm.num_tiles = static_cast<int>((R + kTilePairs - 1) / kTilePairs);
   prm.sched = sched;
   prm.stats = static_cast<float2*>(z_stats);
+  static const int dbg_skip = [] {
+    const char* e = debug_env("FOLDCP_K1_SKIP");
+    return e ? atoi(e) : 0;
+  }();
+  prm.dbg_skip = dbg_skip;
   const int grid = prm.num_tiles < dev.sm_count ? prm.num_tiles : dev.sm_count;
   const bool tanh_sig = k1_tanh_sigmoid();
   auto kern = tanh_sig ? (ab_f16 ? k1_project_kernel<true, true> : k1_project_kernel<true, false>)

@@ -18,9 +18,10 @@ __device__ __forceinline__ void split3(float x, uint32_t (&p)[3]) {
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     if constexpr (kF16) {
-      const __half h = __float2half_rn(x);
-      p[i] = static_cast<uint32_t>(__half_as_ushort(h));
-      x -= __half2float(h);
+      // saturating: a value beyond fp16's range (outside the documented preconditions) stays finite
+      const uint32_t h2 = ptx::pack_f16x2(x, 0.f);
+      p[i] = h2 & 0xffffu;
+      x -= __half2float(__ushort_as_half(static_cast<unsigned short>(h2 & 0xffffu)));
     } else {
       const __nv_bfloat16 h = __float2bfloat16_rn(x);
       p[i] = static_cast<uint32_t>(__bfloat16_as_ushort(h));
