@@ -68,9 +68,15 @@ constexpr int kThreads = (4 + kLnWarps + 4 * kTeams) * 32;
 static_assert(kTeams == 2 || kTeams == 4, "two or four epilogue teams");
 constexpr int kHalfBox = 128 * 64 * 2;          // 16 KB: one TMA box, 128 rows x 64 bf16
 constexpr int kMatBytes = 2 * kHalfBox;         // 32 KB: a 128 x 128 16-bit tile (two k-halves)
-constexpr int kZStages = 4;
+#ifndef FOLDCP_K1_ZSTAGES
+#define FOLDCP_K1_ZSTAGES 4
+#endif
+constexpr int kZStages = FOLDCP_K1_ZSTAGES;      // 4 (with 4 staging buffers) or 2 (with 8)
 constexpr int kMaskSlots = 8;                   // >= kZStages + 3 (see the epilogue), power of 2
-constexpr int kOutBufs = 4;                     // staging buffers [128 ch][64 pairs], two per team
+// staging buffers [128 ch][64 pairs]: (tensor, 64-pair group) of a tile, and with a 2-deep z ring a
+// second set so that the stores of two tiles are in flight
+constexpr int kOutSets = kZStages == 2 ? 2 : 1;
+constexpr int kOutBufs = 4 * kOutSets;
 
 constexpr int kOffZ = 0;                                   // z ring
 constexpr int kOffOut = kOffZ + kZStages * kMatBytes;      // staging buffers
@@ -81,7 +87,7 @@ constexpr int kRingDepth = 8;
 constexpr int kOffRing = kOffBar + 256;
 constexpr int kSmemBytes = kOffRing + TileRing<kRingDepth>::kBytes;
 static_assert(kSmemBytes <= 232448, "K1 shared memory exceeds 227 KB");
-static_assert((3 * kZStages + 18) * 8 <= 256, "barrier region too small");
+static_assert((3 * kZStages + 10 + 2 * kOutBufs) * 8 <= 256, "barrier region too small");
 
 constexpr int kTmemW = 0;        // columns 0..255: four weight matrices, 64 columns each
 constexpr int kTmemAcc = 256;    // columns 256..511: four slots of (projection 32 | gate 32)
@@ -144,7 +150,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
   const uint32_t tmem_slot = bar + 8u * (3 * kZStages + 8);
   const uint32_t wready = bar + 8u * (3 * kZStages + 9);   // weights are in TMEM
   auto ofull = [&](int b) { return bar + 8u * (3 * kZStages + 10 + b); };    // staging buffer b
-  auto oempty = [&](int b) { return bar + 8u * (3 * kZStages + 14 + b); };   // (tensor, group)
+  auto oempty = [&](int b) { return bar + 8u * (3 * kZStages + 10 + kOutBufs + b); };   // (set, tensor, group)
   const TileRing<kRingDepth> ring{smem + kOffRing};
   constexpr uint32_t kRingConsumers = 2 + 1 + kLnWarps + 4 * kTeams;   // 2 MMA, store, LN, epilogue
 
@@ -277,9 +283,9 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         for (int g = 0; g < 2; ++g) {
 #pragma unroll
           for (int u = 0; u < 2; ++u) {
-            const int b = 2 * u + g;
+            const int b = (it % kOutSets) * 4 + 2 * u + g;
             K1_PROBE_T0(t1);
-            ptx::mbar_wait(ofull(b), it & 1);
+            ptx::mbar_wait(ofull(b), (it / kOutSets) & 1);
             K1_PROBE_ADD(sw_f, t1);
             if (!K1_DBG_SKIP(4))
               ptx::tma_store_2d(u == 0 ? &tmap_a : &tmap_b, smem + kOffOut + b * kHalfBox,
@@ -469,7 +475,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         const int g = pq >> 1;                                            // 64-pair group
         const uint32_t slot = static_cast<uint32_t>(2 * h + (pq & 1));
         const uint32_t use = static_cast<uint32_t>(it * 2 + g);          // per-slot use count
-        const int b = 2 * h + g;                                          // staging buffer
+        const int b = (it % kOutSets) * 4 + 2 * h + g;                    // staging buffer
         K1_PROBE_T0(t1);
         ptx::mbar_wait(tfull(slot), use & 1u);
         K1_PROBE_ADD(ew_t, t1);
@@ -489,7 +495,7 @@ k1_project_kernel(const __grid_constant__ CUtensorMap tmap_z,
         ptx::tmem_ld_32x16(taddr + 32, vg[0]);
         // first write of this team into buffer b for this tile: last tile's store has read it
         K1_PROBE_T0(t2);
-        if (kPar == 2 || (pq & 1) == 0) ptx::mbar_wait(oempty(b), (it & 1) ^ 1u);
+        if (kPar == 2 || (pq & 1) == 0) ptx::mbar_wait(oempty(b), ((it / kOutSets) & 1) ^ 1u);
         K1_PROBE_ADD(ew_o, t2);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
