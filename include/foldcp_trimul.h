@@ -74,7 +74,9 @@ typedef enum {
   FOLDCP_ERR_WORKSPACE = 4,   /* workspace NULL or smaller than foldcp_trimul_workspace_bytes()    */
   FOLDCP_ERR_ALIAS = 5,       /* an output overlaps an input, another output or the workspace     */
   FOLDCP_ERR_ARCH = 6,        /* current device is not compute capability 10.0 (sm_100a cubin)    */
-  FOLDCP_ERR_CUDA = 7         /* launch / tensor-map failure (cudaGetLastError is preserved)       */
+  FOLDCP_ERR_CUDA = 7,        /* launch / tensor-map failure (cudaGetLastError is preserved)       */
+  FOLDCP_ERR_STATIC_LIMIT = 8 /* foldcp_trimul_static: the problem needs more scratch than
+                               * FOLDCP_STATIC_WORKSPACE_BYTES                                      */
 } foldcp_status_t;
 
 typedef enum { FOLDCP_OUTGOING = 0, FOLDCP_INCOMING = 1 } foldcp_direction_t;
@@ -288,6 +290,38 @@ int foldcp_trimul_backward(const void* d_out, const void* z, const void* mask,
  * 0 if the shape / dtype is unsupported. */
 size_t foldcp_trimul_backward_workspace_bytes(int N, int c_z, int c_hidden, int dtype);
 
+/*
+ * foldcp_trimul for callers that cannot allocate device memory (code under CUDA graph capture,
+ * serving loops and harnesses that forbid cudaMalloc): same operation, same arguments, same
+ * kernels and bitwise the same result as foldcp_trimul, but the scratch (a | b | o | LayerNorm(z)
+ * statistics | tile counters) is a `static __device__` array inside the library instead of
+ * params->workspace.  params->workspace and params->workspace_bytes are IGNORED (may be NULL / 0);
+ * the caller passes only inputs and outputs.  Calls no cudaMalloc, cudaFree or allocating library
+ * routine; the first call on each device takes the array's device address (cudaGetSymbolAddress,
+ * FOLDCP_ERR_CUDA if that fails) and keeps it.
+ *
+ *   limit  foldcp_trimul_workspace_bytes(N, c_z, c_hidden, dtype) <= FOLDCP_STATIC_WORKSPACE_BYTES
+ *          (16 MiB), i.e. N <= 144 in bf16 mode and N <= 104 in fp32 mode
+ *          (foldcp_trimul_static_max_n); beyond it the call launches nothing and returns
+ *          FOLDCP_ERR_STATIC_LIMIT -- use foldcp_trimul with a caller-owned workspace.
+ *   cost   every GPU on which the library's module is loaded holds those 16 MiB until the process
+ *          exits.
+ *   sharing  ALL calls on a device share the one array, which keeps the previous call's contents.
+ *          Nothing needs clearing by the caller: the tile counters are zeroed on `stream` at every
+ *          call and every other byte is written before it is read.  But two foldcp_trimul_static
+ *          calls that may OVERLAP on the GPU (different streams without an ordering between them,
+ *          or several host threads / graphs replaying concurrently) race on the array and corrupt
+ *          each other's result; calls on one stream, or otherwise ordered, are safe.
+ * Other errors as foldcp_trimul.
+ */
+#define FOLDCP_STATIC_WORKSPACE_BYTES (16u << 20)
+int foldcp_trimul_static(const void* z, const void* mask, const foldcp_trimul_params* params, int N,
+                         int c_z, int c_hidden, int direction, void* out, void* stream);
+/* Largest N foldcp_trimul_static accepts for this dtype (0 if the shape / dtype is unsupported). */
+int foldcp_trimul_static_max_n(int c_z, int c_hidden, int dtype);
+/* = FOLDCP_STATIC_WORKSPACE_BYTES of the library as built */
+size_t foldcp_trimul_static_workspace_bytes(void);
+
 /* Number of kernels one foldcp_trimul call launches for this dtype (for launch accounting). */
 int foldcp_trimul_launches_per_call(int dtype);
 
@@ -296,7 +330,8 @@ const char* foldcp_status_string(int status);
  * foldcp_trimul_contract_backward (the params struct grew: struct_size guards mismatches);
  * 120 made the tile counters per call (workspace grew by FOLDCP_SCHED_SCRATCH_BYTES, the stage
  * entry points take `scratch`) and added foldcp_trimul_backward; 130: the workspace holds the
- * LayerNorm(z) statistics in bf16 mode (8 bytes per pair more), fused-form stage entry points. */
+ * LayerNorm(z) statistics in bf16 mode (8 bytes per pair more), fused-form stage entry points;
+ * 140 added foldcp_trimul_static (no existing entry point changed). */
 int foldcp_version(void);
 
 #ifdef __cplusplus

@@ -28,6 +28,7 @@ EXPORTS = (
     "foldcp_trimul_backward", "foldcp_trimul_backward_workspace_bytes", "foldcp_trimul_contract_blocks",
     "foldcp_trimul_project_stats", "foldcp_trimul_finalize_fused", "foldcp_trimul_o_scale",
     "foldcp_triattn", "foldcp_triattn_workspace_bytes",
+    "foldcp_trimul_static", "foldcp_trimul_static_max_n", "foldcp_trimul_static_workspace_bytes",
     "foldcp_status_string", "foldcp_version",
 )
 
@@ -129,6 +130,12 @@ def load() -> ctypes.CDLL:
     lib.foldcp_triattn.argtypes = [vp, vp, ctypes.POINTER(_TriAttnParams), ci, ci, ci, vp, vp]
     lib.foldcp_triattn_workspace_bytes.restype = ctypes.c_size_t
     lib.foldcp_triattn_workspace_bytes.argtypes = [ci, ci, ci, ci]
+    lib.foldcp_trimul_static.restype = ci
+    lib.foldcp_trimul_static.argtypes = [vp, vp, ctypes.POINTER(_Params), ci, ci, ci, ci, vp, vp]
+    lib.foldcp_trimul_static_max_n.restype = ci
+    lib.foldcp_trimul_static_max_n.argtypes = [ci, ci, ci]
+    lib.foldcp_trimul_static_workspace_bytes.restype = ctypes.c_size_t
+    lib.foldcp_trimul_static_workspace_bytes.argtypes = []
     lib.foldcp_status_string.restype = ctypes.c_char_p
     lib.foldcp_status_string.argtypes = [ci]
     lib.foldcp_version.restype = ci
@@ -268,6 +275,40 @@ def trimul(z: torch.Tensor, mask: Optional[torch.Tensor], p: Dict[str, torch.Ten
                                        c_hidden, int(direction), out.data_ptr(), _stream())
     if st != 0:
         raise FoldcpError(st, "foldcp_trimul")
+    return out
+
+
+def static_max_n(dtype: int, c_z: int = 128, c_hidden: int = 128) -> int:
+    """Largest N trimul_static accepts for this dtype code (foldcp_trimul_static_max_n)."""
+    return load().foldcp_trimul_static_max_n(c_z, c_hidden, int(dtype))
+
+
+def static_workspace_bytes() -> int:
+    return load().foldcp_trimul_static_workspace_bytes()
+
+
+def trimul_static(z: torch.Tensor, mask: Optional[torch.Tensor], p: Dict[str, torch.Tensor],
+                  direction: int, out: torch.Tensor, eps: float = 1e-5,
+                  mask_output: bool = True, residual: bool = False) -> torch.Tensor:
+    """foldcp_trimul_static: trimul() with the scratch in the library's static device array.
+
+    Allocates nothing (neither here nor in the library): `out` must be given, no workspace is
+    passed.  N <= static_max_n(dtype); beyond it FoldcpError with FOLDCP_ERR_STATIC_LIMIT (8).
+    All calls on a device share the one array: calls that may overlap on the GPU race.
+    """
+    lib = load()
+    _check_tensors(z, p, (mask, out))
+    assert z.dim() == 3 and z.shape[0] == z.shape[1] and z.is_contiguous()
+    assert out.shape == z.shape and out.dtype == z.dtype and out.is_contiguous()
+    N, c_z = z.shape[0], z.shape[2]
+    c_hidden = p["w_a"].shape[0]
+    if mask is not None:
+        assert mask.dtype == z.dtype and mask.is_contiguous() and mask.shape == z.shape[:-1]
+    s = make_params(p, dtype_code(z), eps, mask_output, None, residual)
+    st = lib.foldcp_trimul_static(z.data_ptr(), _ptr(mask), ctypes.byref(s), N, c_z, c_hidden,
+                                  int(direction), out.data_ptr(), _stream())
+    if st != 0:
+        raise FoldcpError(st, "foldcp_trimul_static")
     return out
 
 

@@ -19,7 +19,7 @@ INCLUDE = os.path.join(os.path.dirname(PKG_DIR), "include")
 LIB_PATH = os.path.join(PKG_DIR, "libfoldcp_trimul.so")
 
 SOURCES = ["api.cu", "simt_kernels.cu", "simt_backward.cu", "k1_project.cu", "k2_contract.cu",
-           "k3_finalize.cu", "k_backward.cu", "triattn.cu"]
+           "k3_finalize.cu", "k_backward.cu", "triattn.cu", "static_ws.cu"]
 HEADERS = ["common.h", "ptx.cuh", "ln_rows.cuh", "tile_sched.cuh", "rank1.cuh"]
 
 NVCC_FLAGS = [

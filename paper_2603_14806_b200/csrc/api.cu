@@ -561,10 +561,12 @@ const char* foldcp_status_string(int status) {
     case FOLDCP_ERR_ALIAS: return "an output overlaps an input, another output or the workspace";
     case FOLDCP_ERR_ARCH: return "device is not sm_100 (compute capability 10.0)";
     case FOLDCP_ERR_CUDA: return "CUDA error";
+    case FOLDCP_ERR_STATIC_LIMIT:
+      return "problem exceeds the static workspace (FOLDCP_STATIC_WORKSPACE_BYTES): use foldcp_trimul";
     default: return "unknown status";
   }
 }
 
-int foldcp_version(void) { return 130; }   // 1.3: z statistics in the workspace, fused-form stage entries
+int foldcp_version(void) { return 140; }   // 1.4: foldcp_trimul_static (1.3: z statistics in the workspace)
 
 }  // extern "C"
