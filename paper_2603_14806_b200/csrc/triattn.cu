@@ -199,14 +199,22 @@ ta_attention_kernel(const float* __restrict__ q, const float* __restrict__ k,
 // strides and the transposed bias -- no data is moved.
 // ---------------------------------------------------------------------------------------------
 constexpr int kTcThreads = 160;                   // warp 0: TMA + MMA issue; warps 1-4: softmax
-constexpr int kTcOffT = 0;                        // bias tile  [128 q][128 k] fp16, two SW128 boxes
-constexpr int kTcOffP = 32768;                    // P tile     [128 q][128 k] fp16, two SW128 boxes
-constexpr int kTcOffV = 65536;                    // V tile     unswizzled core matrices, 8 KB
-constexpr int kTcOffQ = 73728;                    // Q tile     unswizzled core matrices, 8 KB
-constexpr int kTcOffK = 81920;                    // K tile
-constexpr int kTcOffM = 90112;                    // key mask bias, 128 floats
-constexpr int kTcOffBar = 90624;
+// Shared memory and tensor memory are sized for THREE CTAs per SM (the chain load -> S -> softmax ->
+// P V -> running output is serial inside a CTA; co-resident CTAs are what overlaps it): the P tile
+// overwrites the bias tile in place (a thread turns its own row's 16-byte chunks of t into p, same
+// swizzle), and the P V result lands in the first 32 of S's 128 TMEM columns (S is dead once P is
+// written), so a CTA needs 57 KB and 128 columns.
+constexpr int kTcOffT = 0;                        // bias tile [128 q][128 k] fp16, two SW128 boxes; then P
+constexpr int kTcOffP = kTcOffT;
+constexpr int kTcOffV = 32768;                    // V tile     unswizzled core matrices, 8 KB
+constexpr int kTcOffQ = 40960;                    // Q tile     unswizzled core matrices, 8 KB
+constexpr int kTcOffK = 49152;                    // K tile
+constexpr int kTcOffM = 57344;                    // key mask bias, 128 floats
+constexpr int kTcOffBar = 57856;
 constexpr int kTcSmem = kTcOffBar + 64;
+constexpr int kTcTmemCols = 128;
+// p = exp2(x - m) is stored as fp16: x - m may reach this before the block is redone with its own maximum
+constexpr float kTcMaxExp = 15.0f;
 
 struct TcAttnParams {
   const __half* g;       // [N*N][128]  sigmoid gate
@@ -216,7 +224,7 @@ struct TcAttnParams {
   long long ls, xs;      // pair (line, x) = line * ls + x * xs
 };
 
-__global__ void __launch_bounds__(kTcThreads)
+__global__ void __launch_bounds__(kTcThreads, 3)
 ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
                        const __grid_constant__ CUtensorMap tmap_k,
                        const __grid_constant__ CUtensorMap tmap_v,
@@ -242,14 +250,14 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       ptx::fence_mbar_init();
     }
     __syncwarp();
-    ptx::tmem_alloc<1>(tmem_slot, 256);
+    ptx::tmem_alloc<1>(tmem_slot, kTcTmemCols);
   }
   ptx::tc_fence_before();
   __syncthreads();
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-  const uint32_t tm_s = tmem_base, tm_o = tmem_base + 128;
+  const uint32_t tm_s = tmem_base, tm_o = tmem_base;   // O block over S's first 32 columns
 
   if (warp == 0) {
     if (ptx::elect_one()) {
@@ -319,6 +327,25 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       ptx::named_bar_sync(1, 128);
       ptx::mbar_wait(bar_s, b & 1);
       ptx::tc_fence_after();
+      // no mask tensor and all 128 keys of the block exist: the per-key term is zero (uniform branch)
+      const bool has_mb = prm.mask != nullptr || k0 + 128 > N;
+      // x = s + t (+ mask bias) for 8 keys: one 16-byte chunk of the bias tile
+      auto logits8 = [&](const uint32_t (&sv)[32], int c, int i, const uint32_t (&tw)[4], float (&x)[8]) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
+          x[2 * e] = __uint_as_float(sv[i * 8 + e * 2]) + tf.x;
+          x[2 * e + 1] = __uint_as_float(sv[i * 8 + e * 2 + 1]) + tf.y;
+        }
+        if (has_mb) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + (c * 32 + i * 8 + e * 2) * 4);
+            x[2 * e] += mb.x;
+            x[2 * e + 1] += mb.y;
+          }
+        }
+      };
       // pass 1: the block's row maximum
       float bmax = -INFINITY;
 #pragma unroll 1
@@ -329,21 +356,17 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           uint32_t tw[4];
+          float x[8];
           ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + ((static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4), tw);
+          logits8(sv, c, i, tw, x);
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
-            const int kk = c * 32 + i * 8 + e * 2;
-            const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + kk * 4);
-            bmax = fmaxf(bmax, __uint_as_float(sv[i * 8 + e * 2]) + tf.x + mb.x);
-            bmax = fmaxf(bmax, __uint_as_float(sv[i * 8 + e * 2 + 1]) + tf.y + mb.y);
-          }
+          for (int e = 0; e < 4; ++e) bmax = ptx::fmax3(bmax, x[2 * e], x[2 * e + 1]);
         }
       }
       const float m_new = fmaxf(m, bmax);
       const float m_use = m_new == -INFINITY ? 0.f : m_new;     // a row with no key yet: p = 0 everywhere
       const float resc = ptx::ex2_approx(m - m_use);              // 0 on the first block
-      // pass 2: p = exp2(s - m_new), row sum, P tile
+      // pass 2: p = exp2(x - m_new), row sum; p replaces t in place (this thread's own chunks)
       float lsum = 0.f;
 #pragma unroll 1
       for (int c = 0; c < 4; ++c) {
@@ -353,15 +376,14 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           uint32_t tw[4], pw[4];
+          float x[8];
           const uint32_t chunk = (static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4;
           ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + chunk, tw);
+          logits8(sv, c, i, tw, x);
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
-            const int kk = c * 32 + i * 8 + e * 2;
-            const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + kk * 4);
-            const float p0 = ptx::ex2_approx(__uint_as_float(sv[i * 8 + e * 2]) + tf.x + mb.x - m_use);
-            const float p1 = ptx::ex2_approx(__uint_as_float(sv[i * 8 + e * 2 + 1]) + tf.y + mb.y - m_use);
+            const float p0 = ptx::ex2_approx(x[2 * e] - m_use);
+            const float p1 = ptx::ex2_approx(x[2 * e + 1] - m_use);
             lsum += p0 + p1;
             pw[e] = ptx::pack_f16x2(p0, p1);
           }
@@ -405,7 +427,7 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
   }
   ptx::tc_fence_before();
   __syncthreads();
-  if (warp == 0) ptx::tmem_dealloc<1>(tmem_base, 256);
+  if (warp == 0) ptx::tmem_dealloc<1>(tmem_base, kTcTmemCols);
 }
 
 
