@@ -210,7 +210,8 @@ constexpr int kTcOffV = 32768;                    // V tile     unswizzled core 
 constexpr int kTcOffQ = 40960;                    // Q tile     unswizzled core matrices, 8 KB
 constexpr int kTcOffK = 49152;                    // K tile
 constexpr int kTcOffM = 57344;                    // key mask bias, 128 floats
-constexpr int kTcOffBar = 57856;
+constexpr int kTcOffMh = 57856;                   // the same as 128 halves (pass 1 works on half pairs)
+constexpr int kTcOffBar = 58112;
 constexpr int kTcSmem = kTcOffBar + 64;
 constexpr int kTcTmemCols = 128;
 // p = exp2(x - m) is stored as fp16: x - m may reach this before the block is redone with its own maximum
@@ -323,6 +324,7 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
           mb = -1.0e9f * kLog2e * (1.0f - mv);
         }
         reinterpret_cast<float*>(smem_raw + kTcOffM)[st] = mb;
+        reinterpret_cast<__half*>(smem_raw + kTcOffMh)[st] = __float2half_rn(fmaxf(mb, -60000.0f));
       }
       ptx::named_bar_sync(1, 128);
       ptx::mbar_wait(bar_s, b & 1);
@@ -346,8 +348,11 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
         }
       };
-      // pass 1: the block's row maximum
-      float bmax = -INFINITY;
+      // pass 1: the block's row maximum, on half pairs.  The maximum is only the reference point of
+      // the exponentials (p and the row sum use the same one), so fp16 accuracy -- a few hundredths
+      // at |x| < 100 -- is plenty: p <= 2^0.1.  A masked key is -60000 here (finite: a block with
+      // masked keys only still yields a finite reference).
+      __half2 hm = __half2half2(__ushort_as_half(static_cast<unsigned short>(0xFC00)));   // -inf
 #pragma unroll 1
       for (int c = 0; c < 4; ++c) {
         uint32_t sv[32];
@@ -355,14 +360,19 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
         ptx::tmem_ld_wait();
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          uint32_t tw[4];
-          float x[8];
+          uint32_t tw[4], mw[4];
           ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + ((static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4), tw);
-          logits8(sv, c, i, tw, x);
+          if (has_mb) ptx::lds128(smem + kTcOffMh + (c * 32 + i * 8) * 2, mw);
 #pragma unroll
-          for (int e = 0; e < 4; ++e) bmax = ptx::fmax3(bmax, x[2 * e], x[2 * e + 1]);
+          for (int e = 0; e < 4; ++e) {
+            __half2 xh = __floats2half2_rn(__uint_as_float(sv[i * 8 + e * 2]), __uint_as_float(sv[i * 8 + e * 2 + 1]));
+            xh = __hadd2(xh, *reinterpret_cast<const __half2*>(&tw[e]));
+            if (has_mb) xh = __hadd2(xh, *reinterpret_cast<const __half2*>(&mw[e]));
+            hm = __hmax2(hm, xh);
+          }
         }
       }
+      const float bmax = fmaxf(__low2float(hm), __high2float(hm));
       const float m_new = fmaxf(m, bmax);
       const float m_use = m_new == -INFINITY ? 0.f : m_new;     // a row with no key yet: p = 0 everywhere
       const float resc = ptx::ex2_approx(m - m_use);              // 0 on the first block
@@ -409,7 +419,8 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       if (lane == 0) ptx::mbar_arrive(bar_free);
     }
     if (active) {
-      const float inv = 1.0f / l;
+      // l = 0: a row without any unmasked key (outside the documented precondition) gives zeros
+      const float inv = l > 0.f ? 1.0f / l : 0.f;
       const long long a = (static_cast<long long>(line) * prm.ls + static_cast<long long>(pos) * prm.xs) * C + h * kHead;
 #pragma unroll
       for (int d = 0; d < kHead; d += 8) {
