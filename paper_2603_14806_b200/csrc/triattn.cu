@@ -17,6 +17,13 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
+// The attention kernel's issuing warp waits for the softmax warps most of the time, and it shares an
+// SM partition with one softmax warp of every co-resident CTA: without a suspend-time hint its
+// try_wait loop was a third of all executed instructions (ncu source page) and slowed exactly the
+// warps it was waiting for.
+#ifndef FOLDCP_MBAR_HINT_NS
+#define FOLDCP_MBAR_HINT_NS 2000
+#endif
 #include "../../include/foldcp_triattn.h"
 #include "common.h"
 #include "ln_rows.cuh"
@@ -214,8 +221,6 @@ constexpr int kTcOffMh = 57856;                   // the same as 128 halves (pas
 constexpr int kTcOffBar = 58112;
 constexpr int kTcSmem = kTcOffBar + 64;
 constexpr int kTcTmemCols = 128;
-// p = exp2(x - m) is stored as fp16: x - m may reach this before the block is redone with its own maximum
-constexpr float kTcMaxExp = 15.0f;
 
 struct TcAttnParams {
   const __half* g;       // [N*N][128]  sigmoid gate
@@ -331,41 +336,34 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       ptx::tc_fence_after();
       // no mask tensor and all 128 keys of the block exist: the per-key term is zero (uniform branch)
       const bool has_mb = prm.mask != nullptr || k0 + 128 > N;
-      // x = s + t (+ mask bias) for 8 keys: one 16-byte chunk of the bias tile
-      auto logits8 = [&](const uint32_t (&sv)[32], int c, int i, const uint32_t (&tw)[4], float (&x)[8]) {
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
-          x[2 * e] = __uint_as_float(sv[i * 8 + e * 2]) + tf.x;
-          x[2 * e + 1] = __uint_as_float(sv[i * 8 + e * 2 + 1]) + tf.y;
-        }
-        if (has_mb) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + (c * 32 + i * 8 + e * 2) * 4);
-            x[2 * e] += mb.x;
-            x[2 * e + 1] += mb.y;
-          }
-        }
+      // this row's 16-byte chunk of the bias / P tile that holds keys kk0 .. kk0 + 7
+      auto tchunk = [&](int kk0) -> uint32_t {
+        return smem + kTcOffT + (kk0 >> 6) * 16384 + r * 128 + ((static_cast<uint32_t>((kk0 >> 3) & 7) ^ sw) << 4);
       };
+      // Both passes read S in eight pieces of 16 columns, the next piece's tcgen05.ld in flight while
+      // the current one is worked on (three warps per SM partition cannot hide that latency otherwise).
       // pass 1: the block's row maximum, on half pairs.  The maximum is only the reference point of
       // the exponentials (p and the row sum use the same one), so fp16 accuracy -- a few hundredths
       // at |x| < 100 -- is plenty: p <= 2^0.1.  A masked key is -60000 here (finite: a block with
       // masked keys only still yields a finite reference).
       __half2 hm = __half2half2(__ushort_as_half(static_cast<unsigned short>(0xFC00)));   // -inf
-#pragma unroll 1
-      for (int c = 0; c < 4; ++c) {
-        uint32_t sv[32];
-        ptx::tmem_ld_32x32(tm_s + lane_addr + c * 32, sv);
-        ptx::tmem_ld_wait();
+      uint32_t sv[2][16];
+      ptx::tmem_ld_32x16(tm_s + lane_addr, sv[0]);
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+      for (int c = 0; c < 8; ++c) {
+        ptx::tmem_ld_wait();
+        // the last piece's prefetch is pass 2's first piece
+        ptx::tmem_ld_32x16(tm_s + lane_addr + ((c + 1) & 7) * 16, sv[(c + 1) & 1]);
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+          const int kk0 = c * 16 + i * 8;
           uint32_t tw[4], mw[4];
-          ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + ((static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4), tw);
-          if (has_mb) ptx::lds128(smem + kTcOffMh + (c * 32 + i * 8) * 2, mw);
+          ptx::lds128(tchunk(kk0), tw);
+          if (has_mb) ptx::lds128(smem + kTcOffMh + kk0 * 2, mw);
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            __half2 xh = __floats2half2_rn(__uint_as_float(sv[i * 8 + e * 2]), __uint_as_float(sv[i * 8 + e * 2 + 1]));
+            __half2 xh = __floats2half2_rn(__uint_as_float(sv[c & 1][i * 8 + e * 2]),
+                                           __uint_as_float(sv[c & 1][i * 8 + e * 2 + 1]));
             xh = __hadd2(xh, *reinterpret_cast<const __half2*>(&tw[e]));
             if (has_mb) xh = __hadd2(xh, *reinterpret_cast<const __half2*>(&mw[e]));
             hm = __hmax2(hm, xh);
@@ -377,29 +375,37 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const float m_use = m_new == -INFINITY ? 0.f : m_new;     // a row with no key yet: p = 0 everywhere
       const float resc = ptx::ex2_approx(m - m_use);              // 0 on the first block
       // pass 2: p = exp2(x - m_new), row sum; p replaces t in place (this thread's own chunks)
-      float lsum = 0.f;
-#pragma unroll 1
-      for (int c = 0; c < 4; ++c) {
-        uint32_t sv[32];
-        ptx::tmem_ld_32x32(tm_s + lane_addr + c * 32, sv);
-        ptx::tmem_ld_wait();
+      float lsum0 = 0.f, lsum1 = 0.f;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+      for (int c = 0; c < 8; ++c) {
+        ptx::tmem_ld_wait();
+        if (c + 1 < 8) ptx::tmem_ld_32x16(tm_s + lane_addr + (c + 1) * 16, sv[(c + 1) & 1]);
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+          const int kk0 = c * 16 + i * 8;
           uint32_t tw[4], pw[4];
-          float x[8];
-          const uint32_t chunk = (static_cast<uint32_t>((c & 1) * 4 + i) ^ sw) << 4;
-          ptx::lds128(smem + kTcOffT + (c >> 1) * 16384 + r * 128 + chunk, tw);
-          logits8(sv, c, i, tw, x);
+          const uint32_t addr = tchunk(kk0);
+          ptx::lds128(addr, tw);
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            const float p0 = ptx::ex2_approx(x[2 * e] - m_use);
-            const float p1 = ptx::ex2_approx(x[2 * e + 1] - m_use);
-            lsum += p0 + p1;
+            const float2 tf = __half22float2(*reinterpret_cast<const __half2*>(&tw[e]));
+            float x0 = __uint_as_float(sv[c & 1][i * 8 + e * 2]) + tf.x;
+            float x1 = __uint_as_float(sv[c & 1][i * 8 + e * 2 + 1]) + tf.y;
+            if (has_mb) {
+              const float2 mb = *reinterpret_cast<const float2*>(smem_raw + kTcOffM + (kk0 + e * 2) * 4);
+              x0 += mb.x;
+              x1 += mb.y;
+            }
+            const float p0 = ptx::ex2_approx(x0 - m_use);
+            const float p1 = ptx::ex2_approx(x1 - m_use);
+            lsum0 += p0;
+            lsum1 += p1;
             pw[e] = ptx::pack_f16x2(p0, p1);
           }
-          ptx::sts128(smem + kTcOffP + (c >> 1) * 16384 + r * 128 + chunk, pw[0], pw[1], pw[2], pw[3]);
+          ptx::sts128(addr, pw[0], pw[1], pw[2], pw[3]);
         }
       }
+      const float lsum = lsum0 + lsum1;
       l = l * resc + lsum;
       m = m_new;
       ptx::tc_fence_before();
