@@ -206,20 +206,22 @@ ta_attention_kernel(const float* __restrict__ q, const float* __restrict__ k,
 // strides and the transposed bias -- no data is moved.
 // ---------------------------------------------------------------------------------------------
 constexpr int kTcThreads = 160;                   // warp 0: TMA + MMA issue; warps 1-4: softmax
-// Shared memory and tensor memory are sized for THREE CTAs per SM (the chain load -> S -> softmax ->
-// P V -> running output is serial inside a CTA; co-resident CTAs are what overlaps it): the P tile
-// overwrites the bias tile in place (a thread turns its own row's 16-byte chunks of t into p, same
-// swizzle), and the P V result lands in the first 32 of S's 128 TMEM columns (S is dead once P is
-// written), so a CTA needs 57 KB and 128 columns.
+// Shared memory, tensor memory and registers are sized for FOUR CTAs per SM (the chain load -> S ->
+// softmax -> P V -> running output is serial inside a CTA, and the kernel's speed follows the number
+// of resident softmax warps): the P tile overwrites the bias tile in place (a thread turns its own
+// row's 16-byte chunks of t into p, same swizzle), the P V result lands in the first 32 of S's 128 TMEM
+// columns (S is dead once P is written), and the V tile is loaded into the K tile's buffer once
+// S = Q K^T has retired (under the softmax, which takes far longer) -- 49 KB and 128 columns per CTA.
 constexpr int kTcOffT = 0;                        // bias tile [128 q][128 k] fp16, two SW128 boxes; then P
 constexpr int kTcOffP = kTcOffT;
-constexpr int kTcOffV = 32768;                    // V tile     unswizzled core matrices, 8 KB
+constexpr int kTcOffK = 32768;                    // K tile, then V tile: unswizzled core matrices, 8 KB
+constexpr int kTcOffV = kTcOffK;
 constexpr int kTcOffQ = 40960;                    // Q tile     unswizzled core matrices, 8 KB
-constexpr int kTcOffK = 49152;                    // K tile
-constexpr int kTcOffM = 57344;                    // key mask bias, 128 floats
-constexpr int kTcOffMh = 57856;                   // the same as 128 halves (pass 1 works on half pairs)
-constexpr int kTcOffBar = 58112;
+constexpr int kTcOffM = 49152;                    // key mask bias, 128 floats
+constexpr int kTcOffMh = 49664;                   // the same as 128 halves (pass 1 works on half pairs)
+constexpr int kTcOffBar = 49920;
 constexpr int kTcSmem = kTcOffBar + 64;
+constexpr int kTcCtasPerSm = 4;
 constexpr int kTcTmemCols = 128;
 
 struct TcAttnParams {
@@ -230,7 +232,7 @@ struct TcAttnParams {
   long long ls, xs;      // pair (line, x) = line * ls + x * xs
 };
 
-__global__ void __launch_bounds__(kTcThreads, 3)
+__global__ void __launch_bounds__(kTcThreads, kTcCtasPerSm)
 ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
                        const __grid_constant__ CUtensorMap tmap_k,
                        const __grid_constant__ CUtensorMap tmap_v,
@@ -239,7 +241,7 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
   const uint32_t smem = ptx::smem_u32(smem_raw);
   const uint32_t bar = smem + kTcOffBar;
   const uint32_t bar_q = bar, bar_kv = bar + 8, bar_s = bar + 16, bar_p = bar + 24, bar_o = bar + 32,
-                 bar_free = bar + 40, tmem_slot = bar + 48;
+                 bar_free = bar + 40, bar_v = bar + 48, tmem_slot = bar + 56;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int N = prm.N;
   const int pos0 = blockIdx.x * 128, line = blockIdx.y, h = blockIdx.z;
@@ -253,6 +255,7 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       ptx::mbar_init(bar_p, 4);
       ptx::mbar_init(bar_o, 1);
       ptx::mbar_init(bar_free, 4);
+      ptx::mbar_init(bar_v, 1);
       ptx::fence_mbar_init();
     }
     __syncwarp();
@@ -276,9 +279,8 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
       for (int b = 0; b < nblocks; ++b) {
         const int k0 = b * 128;
         if (b > 0) ptx::mbar_wait(bar_free, (b - 1) & 1);
-        ptx::mbar_arrive_expect_tx(bar_kv, 8192 + 8192 + 32768);
+        ptx::mbar_arrive_expect_tx(bar_kv, 8192 + 32768);
         ptx::tma_load_5d(smem + kTcOffK, &tmap_k, bar_kv, 0, 0, h * 4, k0 / 8, line);
-        ptx::tma_load_5d(smem + kTcOffV, &tmap_v, bar_kv, 0, 0, h * 4, k0 / 8, line);
         ptx::tma_load_2d(smem + kTcOffT, &tmap_t, bar_kv, k0, h * N + pos0);
         ptx::tma_load_2d(smem + kTcOffT + 16384, &tmap_t, bar_kv, k0 + 64, h * N + pos0);
         ptx::mbar_wait(bar_kv, b & 1);
@@ -289,7 +291,12 @@ ta_attention_tc_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             ptx::make_smem_desc_noswizzle(smem + kTcOffK + ks * 256, 128, 512), idesc_s,
                             ks ? 1u : 0u);
         ptx::umma_commit<1>(bar_s);
+        // S has retired: the K tile is dead, its buffer takes the V tile while the softmax runs
+        ptx::mbar_wait(bar_s, b & 1);
+        ptx::mbar_arrive_expect_tx(bar_v, 8192);
+        ptx::tma_load_5d(smem + kTcOffV, &tmap_v, bar_v, 0, 0, h * 4, k0 / 8, line);
         ptx::mbar_wait(bar_p, b & 1);
+        ptx::mbar_wait(bar_v, b & 1);
         ptx::tc_fence_after();
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {     // K = 128 keys
